@@ -1,0 +1,513 @@
+// splotch_api.cu -- host side of the C ABI declared in include/splotch.h.
+// Argument checking, camera constants, workspace layout and the per-frame kernel sequence.  No compute happens on
+// the host: every stage of the path is one of the kernels in splotch_kernels.cuh.
+#include "splotch_kernels.cuh"
+#include "../../include/splotch.h"
+
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+#include <new>
+
+using namespace splotch;
+
+namespace {
+
+constexpr int kStages = 6;
+constexpr int kProfRing = 256;              // frames of per-stage events kept while profiling
+const char *kStageNames[kStages] = {"count", "colscan", "binscan", "scatter", "splat", "compose"};
+
+struct Layout {
+    size_t counts, cls_counts, bin_count, bin_start, chunk_start, stats, desc, partials, records, staging, total;
+    unsigned long long capacity, max_chunks;
+    int nrows;
+};
+
+}  // namespace
+
+struct splotch_ctx {
+    int device = 0, width = 0, height = 0;
+    unsigned long long max_particles = 0;
+    int n_sm = 0, smem_optin = 0;
+    bool camera_set = false;
+    float cam[16] = {0};
+    float4 *lut = nullptr;                   // device, [kMaxSpecies][kMaxLut]
+    int lut_n[kMaxSpecies] = {0};
+    bool profiling = false;
+    cudaEvent_t (*ev_ring)[kStages + 1] = nullptr;   // [kProfRing][kStages + 1], created when profiling is first enabled
+    cudaEvent_t *ev = nullptr;                       // slot of the frame being recorded
+    unsigned long long prof_frames = 0;              // frames recorded since profiling was (re)enabled
+    // last frame
+    bool have_frame = false;
+    char *ws = nullptr;
+    Layout lay{};
+    FrameParams fp{};
+    unsigned long long last_n = 0;
+    cudaStream_t last_stream = nullptr;
+    int splat_blocks_per_sm[3] = {0, 0, 0};  // T = 8, 16, 32
+    char err[512] = {0};
+};
+
+namespace {
+
+char g_create_err[512] = "";               // last splotch_create failure (there is no context to hold it)
+
+int fail(splotch_ctx *c, int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(c ? c->err : g_create_err, sizeof g_create_err, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CU_TRY(ctx, expr)                                                                               \
+    do {                                                                                                \
+        cudaError_t e_ = (expr);                                                                        \
+        if (e_ != cudaSuccess)                                                                          \
+            return fail(ctx, SPLOTCH_ECUDA, "%s failed: %s", #expr, cudaGetErrorString(e_));           \
+    } while (0)
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+int tile_shift(int T) { return T == 8 ? 3 : T == 16 ? 4 : T == 32 ? 5 : -1; }
+
+size_t hist_bytes(int W, int H, int T)
+{
+    const int ntx = (W + T - 1) / T, nty = (H + T - 1) / T;
+    const int S = T << kSuperShift;
+    const int nsx = (W + S - 1) / S, nsy = (H + S - 1) / S;
+    return sizeof(unsigned int) * ((size_t)ntx * nty + (size_t)nsx * nsy);
+}
+
+int bin_rows(const splotch_ctx *c, int T)
+{
+    // two resident blocks per SM while two private histograms fit in shared memory, else one
+    return c->n_sm * (2 * (hist_bytes(c->width, c->height, T) + 1024) <= (size_t)c->smem_optin ? 2 : 1);
+}
+
+// Workspace layout.  Either `capacity` is given (sizing query) or derived from `bytes` (render).
+bool make_layout(const splotch_ctx *c, unsigned long long n, int T, unsigned long long capacity, size_t bytes,
+                 bool staging, Layout *L)
+{
+    const int ntx = (c->width + T - 1) / T, nty = (c->height + T - 1) / T;
+    const size_t n_tiles = (size_t)ntx * nty;
+    const size_t nbins = hist_bytes(c->width, c->height, T) / sizeof(unsigned int);
+    const size_t partial_bytes = sizeof(float4) * (size_t)T * T;
+    L->nrows = bin_rows(c, T);
+    size_t off = 0;
+    L->counts = off;      off = align_up(off + sizeof(unsigned int) * nbins * L->nrows, 256);
+    L->cls_counts = off;  off = align_up(off + sizeof(unsigned int) * 4 * L->nrows, 256);
+    L->bin_count = off;   off = align_up(off + sizeof(unsigned int) * nbins, 256);
+    L->bin_start = off;   off = align_up(off + sizeof(unsigned int) * (nbins + 1), 256);
+    L->chunk_start = off; off = align_up(off + sizeof(unsigned int) * (n_tiles + 1), 256);
+    L->stats = off;       off = align_up(off + sizeof(DeviceStats), 256);
+    L->staging = off;
+    if (staging) {
+        off = align_up(off + 6 * align_up(sizeof(float) * n, 256), 256);
+        off = align_up(off + sizeof(float) * 3 * (size_t)c->width * c->height, 256);
+    }
+    const size_t fixed = off;
+    if (capacity == 0) {
+        // derive from bytes: capacity * 32 + (n_tiles + capacity / kChunk + 1) * (partial + 8) <= bytes - fixed
+        const size_t per_chunk = partial_bytes + sizeof(uint2);
+        const size_t need0 = fixed + (n_tiles + 2) * per_chunk + 8192;
+        if (bytes < need0) return false;
+        const double avail = (double)(bytes - need0);
+        capacity = (unsigned long long)(avail / (32.0 + (double)per_chunk / kChunk));
+        if (capacity > 0xfffffff0ull) capacity = 0xfffffff0ull;
+    }
+    L->capacity = capacity;
+    L->max_chunks = n_tiles + capacity / kChunk + 1;
+    L->desc = off;     off = align_up(off + sizeof(uint2) * L->max_chunks, 256);
+    L->partials = off; off = align_up(off + partial_bytes * L->max_chunks, 256);
+    L->records = off;  off = align_up(off + 32ull * capacity, 256);
+    L->total = off;
+    return bytes == 0 || off <= bytes;
+}
+
+template <int T>
+int query_splat_occupancy(splotch_ctx *c, int *out)
+{
+    CU_TRY(c, cudaFuncSetAttribute(k_splat<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SplatCfg<T>::kSmemBytes));
+    CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, k_splat<T>, SplatCfg<T>::kWarps * 32, SplatCfg<T>::kSmemBytes));
+    if (*out < 1) *out = 1;
+    return SPLOTCH_OK;
+}
+
+int check_params(splotch_ctx *c, const splotch_particles *p, unsigned long long n, const splotch_params *q,
+                 FrameParams *fp)
+{
+    if (!p || !q) return fail(c, SPLOTCH_EINVAL, "null particles or params");
+    if (n > c->max_particles) return fail(c, SPLOTCH_EINVAL, "n = %llu exceeds max_particles = %llu", n, c->max_particles);
+    if (n > 0 && (!p->x || !p->y || !p->z || !p->h || !p->I || !p->scalar))
+        return fail(c, SPLOTCH_EINVAL, "null particle field");
+    if (!c->camera_set) return fail(c, SPLOTCH_ESTATE, "camera not set");
+    const int ts = tile_shift(q->tile);
+    if (ts < 0) return fail(c, SPLOTCH_EINVAL, "tile must be 8, 16 or 32 (got %d)", q->tile);
+    if (!(q->chi > 0.0f) || !(q->r_small >= 0.0f) || !(q->r_small < q->r_large))
+        return fail(c, SPLOTCH_EINVAL, "need chi > 0 and 0 <= r_small < r_large");
+    if (hist_bytes(c->width, c->height, q->tile) + 1024 > (size_t)c->smem_optin)
+        return fail(c, SPLOTCH_EINVAL, "tile %d gives too many tiles for a %dx%d image (per-block histogram exceeds shared memory); use a larger tile",
+                    q->tile, c->width, c->height);
+    if (!q->additive) return fail(c, SPLOTCH_EINVAL, "ordered (E != A) mode is not built yet");
+    const int ns = p->species_offsets ? p->n_species : 1;
+    if (ns < 1 || ns > kMaxSpecies) return fail(c, SPLOTCH_EINVAL, "n_species must be 1..%d", kMaxSpecies);
+    if (!q->species) return fail(c, SPLOTCH_EINVAL, "null species parameters");
+    memset(fp, 0, sizeof *fp);
+    memcpy(fp->cam, c->cam, sizeof fp->cam);
+    fp->chi = q->chi; fp->r_small = q->r_small; fp->r_large = q->r_large; fp->z_near = q->z_near;
+    fp->W = c->width; fp->H = c->height; fp->fW = (float)c->width; fp->fH = (float)c->height;
+    fp->csmall = (float)(3.14159265358979323846 * (1.0 - exp(-(double)q->chi * (double)q->chi)));
+    fp->T = q->tile; fp->tshift = ts;
+    fp->ntx = (c->width + q->tile - 1) / q->tile; fp->nty = (c->height + q->tile - 1) / q->tile;
+    fp->n_tiles = fp->ntx * fp->nty;
+    fp->sshift = ts + kSuperShift;
+    const int S = 1 << fp->sshift;
+    fp->nsx = (c->width + S - 1) / S; fp->nsy = (c->height + S - 1) / S;
+    fp->n_super = fp->nsx * fp->nsy;
+    fp->nbins = fp->n_tiles + fp->n_super;
+    fp->additive = q->additive ? 1 : 0;
+    fp->apply_transfer = q->apply_transfer ? 1 : 0;
+    fp->n_species = ns;
+    fp->lut = c->lut;
+    for (int s = 0; s <= ns; ++s) {
+        const unsigned long long o = p->species_offsets ? p->species_offsets[s] : (s == 0 ? 0ull : n);
+        if ((s == 0 && o != 0) || (s == ns && o != n) || (s > 0 && o < fp->sp_begin[s - 1]))
+            return fail(c, SPLOTCH_EINVAL, "species_offsets must ascend from 0 to n");
+        fp->sp_begin[s] = o;
+    }
+    for (int s = 0; s < ns; ++s) {
+        const splotch_species_params &sp = q->species[s];
+        SpeciesDev &d = fp->sp[s];
+        d.brightness = sp.brightness; d.absorb = sp.absorb;
+        d.fixed_r = sp.fixed_rgb[0]; d.fixed_g = sp.fixed_rgb[1]; d.fixed_b = sp.fixed_rgb[2];
+        d.use_colormap = sp.use_colormap ? 1 : 0; d.use_log10 = sp.scalar_log10 ? 1 : 0;
+        d.smin = sp.scalar_min; d.range = sp.scalar_max - sp.scalar_min;
+        d.lut_n = c->lut_n[s];
+        if (d.use_colormap) {
+            if (d.lut_n < 2) return fail(c, SPLOTCH_ESTATE, "species %d uses a colour map but none was set", s);
+            if (!(sp.scalar_max != sp.scalar_min)) return fail(c, SPLOTCH_EINVAL, "species %d: scalar_min == scalar_max", s);
+        }
+    }
+    return SPLOTCH_OK;
+}
+
+bool aligned16(const splotch_particles *p)
+{
+    const uintptr_t m = (uintptr_t)p->x | (uintptr_t)p->y | (uintptr_t)p->z | (uintptr_t)p->h | (uintptr_t)p->I |
+                        (uintptr_t)p->scalar;
+    return (m & 15u) == 0;
+}
+
+template <int T>
+int launch_render_tail(splotch_ctx *c, const Layout &L, char *ws, const FrameParams &fp, float *image, cudaStream_t st)
+{
+    const int ti = T == 8 ? 0 : T == 16 ? 1 : 2;
+    const int grid = c->n_sm * c->splat_blocks_per_sm[ti];
+    k_splat<T><<<grid, SplatCfg<T>::kWarps * 32, SplatCfg<T>::kSmemBytes, st>>>(
+        (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.bin_start), (const uint2 *)(ws + L.desc),
+        (DeviceStats *)(ws + L.stats), (float4 *)(ws + L.partials), fp);
+    if (c->profiling) cudaEventRecord(c->ev[5], st);
+    k_compose<T><<<fp.n_tiles, 256, 0, st>>>((const float4 *)(ws + L.partials), (const unsigned int *)(ws + L.chunk_start),
+                                             (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.bin_start),
+                                             (const DeviceStats *)(ws + L.stats), fp, image);
+    if (c->profiling) cudaEventRecord(c->ev[6], st);
+    return SPLOTCH_OK;
+}
+
+int render_device(splotch_ctx *c, const splotch_particles *p, unsigned long long n, const FrameParams &fp,
+                  const Layout &L, float *image, char *ws, cudaStream_t st)
+{
+    const bool al = aligned16(p);
+    const size_t hbytes = sizeof(unsigned int) * (size_t)fp.nbins;
+    unsigned long long per = (n + L.nrows - 1) / L.nrows;
+    per = (per + 3) / 4 * 4;
+    if (per == 0) per = 4;
+    unsigned int *counts = (unsigned int *)(ws + L.counts);
+    unsigned int *cls_counts = (unsigned int *)(ws + L.cls_counts);
+    unsigned int *bin_count = (unsigned int *)(ws + L.bin_count);
+    unsigned int *bin_start = (unsigned int *)(ws + L.bin_start);
+    unsigned int *chunk_start = (unsigned int *)(ws + L.chunk_start);
+    DeviceStats *stats = (DeviceStats *)(ws + L.stats);
+    if (c->profiling) {
+        c->ev = c->ev_ring[c->prof_frames % kProfRing];
+        cudaEventRecord(c->ev[0], st);
+    }
+    if (al) k_count<true><<<L.nrows, kBinThreads, hbytes, st>>>(p->x, p->y, p->z, p->h, n, per, fp, counts, cls_counts);
+    else    k_count<false><<<L.nrows, kBinThreads, hbytes, st>>>(p->x, p->y, p->z, p->h, n, per, fp, counts, cls_counts);
+    if (c->profiling) cudaEventRecord(c->ev[1], st);
+    k_colscan<<<(fp.nbins + 255) / 256, 256, 0, st>>>(counts, L.nrows, fp.nbins, bin_count);
+    if (c->profiling) cudaEventRecord(c->ev[2], st);
+    k_binscan<<<1, 1024, 0, st>>>(bin_count, fp.n_tiles, fp.nbins, bin_start, chunk_start, (uint2 *)(ws + L.desc),
+                                  cls_counts, L.nrows, L.capacity, L.max_chunks, stats);
+    if (c->profiling) cudaEventRecord(c->ev[3], st);
+    if (al) k_scatter<true><<<L.nrows, kBinThreads, hbytes, st>>>(p->x, p->y, p->z, p->h, p->I, p->scalar, n, per, fp, counts,
+                                                                  bin_start, stats, (float4 *)(ws + L.records));
+    else    k_scatter<false><<<L.nrows, kBinThreads, hbytes, st>>>(p->x, p->y, p->z, p->h, p->I, p->scalar, n, per, fp, counts,
+                                                                   bin_start, stats, (float4 *)(ws + L.records));
+    if (c->profiling) cudaEventRecord(c->ev[4], st);
+    int rc;
+    if (fp.T == 8) rc = launch_render_tail<8>(c, L, ws, fp, image, st);
+    else if (fp.T == 16) rc = launch_render_tail<16>(c, L, ws, fp, image, st);
+    else rc = launch_render_tail<32>(c, L, ws, fp, image, st);
+    if (rc != SPLOTCH_OK) return rc;
+    CU_TRY(c, cudaGetLastError());
+    c->have_frame = true; c->ws = ws; c->lay = L; c->fp = fp; c->last_n = n; c->last_stream = st;
+    if (c->profiling) ++c->prof_frames;
+    return SPLOTCH_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *splotch_version(void) { return "splotch-b200 0.1 (sm_100a)"; }
+
+const char *splotch_stage_name(int s) { return (s >= 0 && s < kStages) ? kStageNames[s] : ""; }
+
+const char *splotch_last_error(const splotch_ctx *c) { return c ? c->err : g_create_err; }
+
+int splotch_create(splotch_ctx **out, int device, int width, int height, uint64_t max_particles)
+{
+    if (!out) return SPLOTCH_EINVAL;
+    *out = nullptr;
+    if (width <= 0 || height <= 0 || width > 32768 || height > 32768 || max_particles > 0xfffffff0ull)
+        return fail(nullptr, SPLOTCH_EINVAL, "bad image size or max_particles");
+    int ndev = 0;
+    CU_TRY(nullptr, cudaGetDeviceCount(&ndev));
+    if (device < 0 || device >= ndev) return fail(nullptr, SPLOTCH_ECUDA, "no CUDA device %d (%d visible)", device, ndev);
+    cudaDeviceProp prop;
+    CU_TRY(nullptr, cudaGetDeviceProperties(&prop, device));
+    if (prop.major != 10) return fail(nullptr, SPLOTCH_EDEVICE, "device %d is sm_%d%d, need sm_100", device, prop.major, prop.minor);
+    CU_TRY(nullptr, cudaSetDevice(device));
+    splotch_ctx *c = new (std::nothrow) splotch_ctx();
+    if (!c) return fail(nullptr, SPLOTCH_ENOMEM, "host allocation failed");
+    c->device = device; c->width = width; c->height = height; c->max_particles = max_particles;
+    c->n_sm = prop.multiProcessorCount;
+    c->smem_optin = (int)prop.sharedMemPerBlockOptin;
+    const int hb = c->smem_optin - 1024;      // dynamic shared memory the binning kernels may ask for
+    int rc = [&]() -> int {
+        CU_TRY(c, cudaMalloc(&c->lut, sizeof(float4) * kMaxSpecies * kMaxLut));
+        CU_TRY(c, cudaMemset(c->lut, 0, sizeof(float4) * kMaxSpecies * kMaxLut));
+        CU_TRY(c, cudaFuncSetAttribute(k_count<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb));
+        CU_TRY(c, cudaFuncSetAttribute(k_count<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb));
+        CU_TRY(c, cudaFuncSetAttribute(k_scatter<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb));
+        CU_TRY(c, cudaFuncSetAttribute(k_scatter<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb));
+        int r = query_splat_occupancy<8>(c, &c->splat_blocks_per_sm[0]);
+        if (r == SPLOTCH_OK) r = query_splat_occupancy<16>(c, &c->splat_blocks_per_sm[1]);
+        if (r == SPLOTCH_OK) r = query_splat_occupancy<32>(c, &c->splat_blocks_per_sm[2]);
+        return r;
+    }();
+    if (rc != SPLOTCH_OK) {
+        snprintf(g_create_err, sizeof g_create_err, "%s", c->err);
+        splotch_destroy(c);
+        return rc;
+    }
+    *out = c;
+    return SPLOTCH_OK;
+}
+
+int splotch_destroy(splotch_ctx *c)
+{
+    if (!c) return SPLOTCH_EINVAL;
+    cudaSetDevice(c->device);
+    if (c->lut) cudaFree(c->lut);
+    if (c->ev_ring) {
+        for (int f = 0; f < kProfRing; ++f)
+            for (int i = 0; i <= kStages; ++i)
+                if (c->ev_ring[f][i]) cudaEventDestroy(c->ev_ring[f][i]);
+        delete[] c->ev_ring;
+    }
+    delete c;
+    return SPLOTCH_OK;
+}
+
+// Camera constants: double arithmetic on the float inputs, one rounding to float32 (C1 "host constants").
+int splotch_set_camera(splotch_ctx *c, const float eye[3], const float lookat[3], const float up[3], float fov_deg)
+{
+    if (!c) return SPLOTCH_EINVAL;
+    if (!eye || !lookat || !up) return fail(c, SPLOTCH_EINVAL, "null camera vector");
+    if (!(fov_deg > 0.0f) || !(fov_deg < 180.0f)) return fail(c, SPLOTCH_EINVAL, "fov must be in (0, 180) degrees");
+    double fwd[3], rgt[3], upp[3];
+    for (int k = 0; k < 3; ++k) fwd[k] = (double)lookat[k] - (double)eye[k];
+    const double nf = sqrt(fwd[0] * fwd[0] + fwd[1] * fwd[1] + fwd[2] * fwd[2]);
+    if (!(nf > 0.0)) return fail(c, SPLOTCH_EINVAL, "eye == lookat");
+    for (int k = 0; k < 3; ++k) fwd[k] /= nf;
+    rgt[0] = fwd[1] * (double)up[2] - fwd[2] * (double)up[1];
+    rgt[1] = fwd[2] * (double)up[0] - fwd[0] * (double)up[2];
+    rgt[2] = fwd[0] * (double)up[1] - fwd[1] * (double)up[0];
+    const double nr = sqrt(rgt[0] * rgt[0] + rgt[1] * rgt[1] + rgt[2] * rgt[2]);
+    if (!(nr > 0.0)) return fail(c, SPLOTCH_EINVAL, "up is parallel to the view direction");
+    for (int k = 0; k < 3; ++k) rgt[k] /= nr;
+    upp[0] = rgt[1] * fwd[2] - rgt[2] * fwd[1];
+    upp[1] = rgt[2] * fwd[0] - rgt[0] * fwd[2];
+    upp[2] = rgt[0] * fwd[1] - rgt[1] * fwd[0];
+    for (int k = 0; k < 3; ++k) {
+        c->cam[k] = (float)rgt[k]; c->cam[3 + k] = (float)upp[k]; c->cam[6 + k] = (float)fwd[k]; c->cam[9 + k] = eye[k];
+    }
+    const double half = 0.5 * ((double)fov_deg * (3.14159265358979323846 / 180.0));
+    c->cam[12] = (float)(0.5 * (double)c->width / tan(half));
+    c->cam[13] = (float)(0.5 * (double)c->width);
+    c->cam[14] = (float)(0.5 * (double)c->height);
+    c->cam[15] = 0.0f;
+    c->camera_set = true;
+    return SPLOTCH_OK;
+}
+
+int splotch_get_camera_constants(const splotch_ctx *c, float out[16])
+{
+    if (!c || !out) return SPLOTCH_EINVAL;
+    if (!c->camera_set) return SPLOTCH_ESTATE;
+    memcpy(out, c->cam, sizeof c->cam);
+    return SPLOTCH_OK;
+}
+
+int splotch_set_colormap(splotch_ctx *c, int species, const float *rgb, int n_entries)
+{
+    if (!c) return SPLOTCH_EINVAL;
+    if (species < 0 || species >= kMaxSpecies || !rgb || n_entries < 2 || n_entries > kMaxLut)
+        return fail(c, SPLOTCH_EINVAL, "bad colour map (species 0..%d, 2..%d entries)", kMaxSpecies - 1, kMaxLut);
+    float4 *tmp = new (std::nothrow) float4[n_entries];
+    if (!tmp) return fail(c, SPLOTCH_ENOMEM, "host allocation failed");
+    for (int i = 0; i < n_entries; ++i) tmp[i] = make_float4(rgb[3 * i], rgb[3 * i + 1], rgb[3 * i + 2], 0.0f);
+    cudaSetDevice(c->device);
+    const cudaError_t e = cudaMemcpy(c->lut + species * kMaxLut, tmp, sizeof(float4) * n_entries, cudaMemcpyHostToDevice);
+    delete[] tmp;
+    if (e != cudaSuccess) return fail(c, SPLOTCH_ECUDA, "colour map upload failed: %s", cudaGetErrorString(e));
+    c->lut_n[species] = n_entries;
+    return SPLOTCH_OK;
+}
+
+int splotch_set_profiling(splotch_ctx *c, int enabled)
+{
+    if (!c) return SPLOTCH_EINVAL;
+    if (enabled && !c->ev_ring) {
+        CU_TRY(c, cudaSetDevice(c->device));
+        c->ev_ring = new (std::nothrow) cudaEvent_t[kProfRing][kStages + 1]();
+        if (!c->ev_ring) return fail(c, SPLOTCH_ENOMEM, "host allocation failed");
+        for (int f = 0; f < kProfRing; ++f)
+            for (int i = 0; i <= kStages; ++i) CU_TRY(c, cudaEventCreate(&c->ev_ring[f][i]));
+    }
+    c->profiling = enabled != 0;
+    c->prof_frames = 0;
+    return SPLOTCH_OK;
+}
+
+size_t splotch_workspace_bytes(const splotch_ctx *c, uint64_t n, int tile, uint64_t pair_capacity, int with_host_staging)
+{
+    if (!c || tile_shift(tile) < 0 || n > c->max_particles) return 0;
+    if (hist_bytes(c->width, c->height, tile) + 1024 > (size_t)c->smem_optin) return 0;
+    if (pair_capacity == 0) pair_capacity = 2ull * n + (1ull << 20);
+    if (pair_capacity > 0xfffffff0ull) return 0;
+    Layout L;
+    make_layout(c, n, tile, pair_capacity, 0, with_host_staging != 0, &L);
+    return L.total + 4096;
+}
+
+int splotch_render(splotch_ctx *c, const splotch_particles *p, uint64_t n, const splotch_params *q, float *image_out,
+                   void *workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    if (!c) return SPLOTCH_EINVAL;
+    FrameParams fp;
+    int rc = check_params(c, p, n, q, &fp);
+    if (rc != SPLOTCH_OK) return rc;
+    if (!image_out || !workspace) return fail(c, SPLOTCH_EINVAL, "null image or workspace");
+    if (((uintptr_t)workspace & 255u) != 0) return fail(c, SPLOTCH_EINVAL, "workspace must be 256-byte aligned");
+    Layout L;
+    if (!make_layout(c, n, q->tile, 0, workspace_bytes, false, &L))
+        return fail(c, SPLOTCH_ENOMEM, "workspace of %zu bytes is below the fixed minimum; ask splotch_workspace_bytes", workspace_bytes);
+    CU_TRY(c, cudaSetDevice(c->device));
+    return render_device(c, p, n, fp, L, image_out, (char *)workspace, (cudaStream_t)cuda_stream);
+}
+
+int splotch_render_host(splotch_ctx *c, const splotch_particles *hp, uint64_t n, const splotch_params *q,
+                        float *host_image_out, void *workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    if (!c) return SPLOTCH_EINVAL;
+    FrameParams fp;
+    int rc = check_params(c, hp, n, q, &fp);
+    if (rc != SPLOTCH_OK) return rc;
+    if (!host_image_out || !workspace) return fail(c, SPLOTCH_EINVAL, "null image or workspace");
+    if (((uintptr_t)workspace & 255u) != 0) return fail(c, SPLOTCH_EINVAL, "workspace must be 256-byte aligned");
+    Layout L;
+    if (!make_layout(c, n, q->tile, 0, workspace_bytes, true, &L))
+        return fail(c, SPLOTCH_ENOMEM, "workspace of %zu bytes is below the fixed minimum (with host staging)", workspace_bytes);
+    CU_TRY(c, cudaSetDevice(c->device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    char *ws = (char *)workspace;
+    const size_t fstride = align_up(sizeof(float) * n, 256);
+    const float *src[6] = {hp->x, hp->y, hp->z, hp->h, hp->I, hp->scalar};
+    float *dst[6];
+    for (int k = 0; k < 6; ++k) {
+        dst[k] = (float *)(ws + L.staging + k * fstride);
+        if (n) CU_TRY(c, cudaMemcpyAsync(dst[k], src[k], sizeof(float) * n, cudaMemcpyHostToDevice, st));
+    }
+    float *dimg = (float *)(ws + L.staging + align_up(6 * fstride, 256));
+    splotch_particles dp = *hp;
+    dp.x = dst[0]; dp.y = dst[1]; dp.z = dst[2]; dp.h = dst[3]; dp.I = dst[4]; dp.scalar = dst[5];
+    rc = render_device(c, &dp, n, fp, L, dimg, ws, st);
+    if (rc != SPLOTCH_OK) return rc;
+    CU_TRY(c, cudaMemcpyAsync(host_image_out, dimg, sizeof(float) * 3 * (size_t)c->width * c->height, cudaMemcpyDeviceToHost, st));
+    CU_TRY(c, cudaStreamSynchronize(st));
+    return SPLOTCH_OK;
+}
+
+int splotch_get_stats(splotch_ctx *c, splotch_stats *out)
+{
+    if (!c || !out) return SPLOTCH_EINVAL;
+    if (!c->have_frame) return fail(c, SPLOTCH_ESTATE, "no frame rendered yet");
+    CU_TRY(c, cudaSetDevice(c->device));
+    CU_TRY(c, cudaStreamSynchronize(c->last_stream));
+    DeviceStats ds;
+    CU_TRY(c, cudaMemcpy(&ds, c->ws + c->lay.stats, sizeof ds, cudaMemcpyDeviceToHost));
+    memset(out, 0, sizeof *out);
+    out->n = c->last_n;
+    for (int k = 0; k < 4; ++k) out->count[k] = ds.count[k];
+    out->pairs = ds.pairs; out->large_pairs = ds.large_pairs; out->chunks = ds.chunks;
+    out->pair_capacity = ds.capacity; out->overflow = (int32_t)ds.overflow;
+    if (c->profiling && c->prof_frames > 0) {
+        // mean per frame over the frames recorded since profiling was enabled (at most the last kProfRing)
+        const unsigned long long nf = c->prof_frames < kProfRing ? c->prof_frames : kProfRing;
+        out->n_stages = kStages;
+        for (int s = 0; s < kStages; ++s) {
+            double sum = 0.0;
+            for (unsigned long long f = 0; f < nf; ++f) {
+                float ms = 0.0f;
+                CU_TRY(c, cudaEventElapsedTime(&ms, c->ev_ring[f][s], c->ev_ring[f][s + 1]));
+                sum += ms;
+            }
+            out->stage_ms[s] = (float)(sum / (double)nf);
+        }
+    }
+    return SPLOTCH_OK;
+}
+
+int splotch_debug_geometry(splotch_ctx *c, const splotch_particles *p, uint64_t n, const splotch_params *q, int8_t *cls,
+                           float *px, float *py, float *sp, float *rp, float *zc, int32_t *pbox, int32_t *tbox,
+                           int32_t *ilabel, void *cuda_stream)
+{
+    if (!c) return SPLOTCH_EINVAL;
+    FrameParams fp;
+    const int rc = check_params(c, p, n, q, &fp);
+    if (rc != SPLOTCH_OK) return rc;
+    if (n == 0) return SPLOTCH_OK;
+    CU_TRY(c, cudaSetDevice(c->device));
+    k_debug_geometry<<<(unsigned int)((n + 255) / 256), 256, 0, (cudaStream_t)cuda_stream>>>(
+        p->x, p->y, p->z, p->h, n, fp, cls, px, py, sp, rp, zc, (int4 *)pbox, (int4 *)tbox, ilabel);
+    CU_TRY(c, cudaGetLastError());
+    return SPLOTCH_OK;
+}
+
+int splotch_debug_tile_counts(splotch_ctx *c, uint32_t *out, void *cuda_stream)
+{
+    if (!c || !out) return SPLOTCH_EINVAL;
+    if (!c->have_frame) return fail(c, SPLOTCH_ESTATE, "no frame rendered yet");
+    CU_TRY(c, cudaSetDevice(c->device));
+    CU_TRY(c, cudaMemcpyAsync(out, c->ws + c->lay.bin_count, sizeof(uint32_t) * (size_t)c->fp.n_tiles,
+                              cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
+    return SPLOTCH_OK;
+}
+
+}  // extern "C"

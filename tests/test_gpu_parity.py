@@ -1,0 +1,270 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Acceptance (BASELINE.json north_star): image relative L2 error <= 1e-5 and max per-pixel absolute error
+<= 1e-4 * image max, in float32; class labels, pixel / tile boxes, the paper's tile index i(p), the float32
+screen geometry and per-tile pair counts bit-exact.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import splotch_oracle as so
+from paper_1309_1114_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+REL_L2 = 1e-5
+MAX_ABS = 1e-4
+
+
+def _binding():
+    from paper_1309_1114_b200 import binding
+    return binding
+
+
+def to_dev(fields):
+    return {k: v.cuda().contiguous() for k, v in fields.items()}
+
+
+def to_np(fields):
+    return {k: v.cpu().numpy() for k, v in fields.items()}
+
+
+def luts_for(species, lut):
+    return [lut if s.use_colormap else None for s in species]
+
+
+def oracle_frame(w, lut, tile, window=None):
+    return so.render(to_np(w.fields), w.species, luts_for(w.species, lut.numpy()), w.camera, w.width, w.height,
+                     chi=w.chi, r_small=w.r_small, r_large=w.r_large, z_near=w.z_near, tile=tile,
+                     additive=w.additive, apply_transfer=w.apply_transfer, window=window, return_geometry=True)
+
+
+def gpu_frame(w, lut, tile, fields_dev=None, pair_capacity=0):
+    b = _binding()
+    r = b.Renderer(w.width, w.height, max(w.n, 1))
+    r.set_camera(w.camera)
+    for s, sp in enumerate(w.species):
+        if sp.use_colormap:
+            r.set_colormap(s, lut)
+    f = fields_dev if fields_dev is not None else to_dev(w.fields)
+    kw = dict(chi=w.chi, r_small=w.r_small, r_large=w.r_large, z_near=w.z_near, tile=tile, additive=w.additive,
+              apply_transfer=w.apply_transfer)
+    img = r.render(f, w.species, pair_capacity=pair_capacity, **kw)
+    torch.cuda.synchronize()
+    return r, f, kw, img
+
+
+def assert_image_close(gpu_img, ref, what=""):
+    g = gpu_img.double().cpu().numpy()
+    assert np.isfinite(g).all(), what
+    mx = ref.max()
+    if mx == 0:
+        assert (g == 0).all(), what
+        return
+    rel = np.linalg.norm(g - ref) / np.linalg.norm(ref)
+    mab = np.abs(g - ref).max() / mx
+    assert rel <= REL_L2, f"{what}: relative L2 {rel:.3e}"
+    assert mab <= MAX_ABS, f"{what}: max abs / max {mab:.3e}"
+
+
+def assert_geometry_exact(r, f, w, kw, g, cam):
+    assert np.array_equal(np.asarray(r.camera_constants(), np.float32), cam)
+    d = r.debug_geometry(f, w.species, **kw)
+    torch.cuda.synchronize()
+    for k in ("cls", "pbox", "tbox", "ilabel"):
+        assert np.array_equal(d[k].cpu().numpy(), g[k]), k
+    for k in ("px", "py", "sp", "rp", "zc"):          # bit-exact float32
+        a, b_ = d[k].cpu().numpy(), g[k]
+        act = g["cls"] != so.CULLED if k != "zc" else ~np.isnan(g[k])        # NaN payload bits are not compared
+        assert np.array_equal(a[act].view(np.uint32), b_[act].view(np.uint32)), k
+        assert np.array_equal(np.isnan(a), np.isnan(b_)) or k != "zc"
+
+
+def assert_counts_exact(r, w, tile, g):
+    st = r.stats()
+    assert st["overflow"] == 0
+    assert st["count"] == [int((g["cls"] == c).sum()) for c in range(4)]
+    oc = so.tile_counts(g, w.width, w.height, tile)
+    gc = r.debug_tile_counts(tile).cpu().numpy()
+    assert np.array_equal(gc.astype(np.int64), oc.astype(np.int64))
+    assert st["pairs"] == int(oc.sum())
+    return st
+
+
+def full_check(w, tile, lut=None):
+    lut = wl.palette() if lut is None else lut
+    ref, g, cam = oracle_frame(w, lut, tile)
+    r, f, kw, img = gpu_frame(w, lut, tile)
+    assert_geometry_exact(r, f, w, kw, g, cam)
+    st = assert_counts_exact(r, w, tile, g)
+    assert_image_close(img, ref, w.name)
+    r.close()
+    return st, g
+
+
+@pytest.mark.parametrize("tile", [8, 16, 32])
+def test_cfg0_full(tile):
+    w = wl.make_config(0)
+    st, g = full_check(w, tile)
+    assert st["count"][wl_MEDIUM] > 90_000
+
+
+wl_SMALL, wl_MEDIUM, wl_LARGE = 1, 2, 3
+
+
+def test_cfg1_reduced_ragged_tiles():
+    w = wl.make_config(1, n=1_000_000, size=(800, 600))         # 600 / 16 = 37.5: ragged last tile row
+    st, g = full_check(w, 16)
+    assert st["count"][wl_SMALL] > 100_000 and st["count"][wl_MEDIUM] > 100_000
+
+
+def test_cfg2_reduced_two_species():
+    w = wl.make_config(2, n=600_000, eta=0.04)                  # 1920 x 1080, 1080 / 16 = 67.5; eta keeps the S/M mix
+    st, g = full_check(w, 16)
+    assert st["count"][wl_SMALL] > 0 and st["count"][wl_MEDIUM] > 0
+
+
+@pytest.mark.parametrize("tile,r_large", [(16, 12.0), (32, 24.0), (16, 64.0)])
+def test_cfg3_reduced_large_particles(tile, r_large):
+    w = wl.make_config(3, n=150_000, size=(512, 384))
+    w.r_large = r_large
+    st, g = full_check(w, tile)
+    assert st["count"][wl_LARGE] > 1000
+    assert st["large_pairs"] >= st["count"][wl_LARGE]
+
+
+def test_apply_transfer():
+    w = wl.make_config(0, n=30_000)
+    w.apply_transfer = True
+    for k in w.fields:
+        pass
+    w.fields["I"] = w.fields["I"] * 40.0                        # make 1 - exp(-S) differ visibly from S
+    full_check(w, 16)
+
+
+@pytest.mark.parametrize("n", [0, 1, 3, 5, 33, 1027])
+def test_tiny_and_ragged_particle_counts(n):
+    w = wl.make_config(0, n=max(n, 1), size=(64, 48))
+    if n == 0:
+        w.fields = {k: v[:0] for k, v in w.fields.items()}
+        w.n = 0
+        w.species[0].end = 0
+    full_check(w, 16)
+
+
+def test_unaligned_field_pointers_take_the_scalar_path():
+    w = wl.make_config(0, n=20_001, size=(128, 128))
+    lut = wl.palette()
+    base = {k: torch.cat([torch.zeros(1), v]).cuda() for k, v in w.fields.items()}
+    f = {k: v[1:] for k, v in base.items()}                     # 4-byte offset: not 16-byte aligned
+    assert f["x"].data_ptr() % 16 != 0
+    ref, g, cam = oracle_frame(w, lut, 16)
+    r, f, kw, img = gpu_frame(w, lut, 16, fields_dev=f)
+    assert_counts_exact(r, w, 16, g)
+    assert_image_close(img, ref)
+
+
+def test_degenerate_inputs_nan_inf_behind_camera():
+    w = wl.make_config(0, n=4096, size=(96, 96))
+    x = w.fields["x"]
+    x[::7] = float("nan")
+    w.fields["h"][1::11] = float("inf")
+    w.fields["h"][2::13] = -1.0
+    w.fields["z"][3::5] = 9.0                                   # behind the camera (eye at z = 2.5 looking at -z)
+    w.fields["h"][4::17] = 0.0
+    st, g = full_check(w, 16)
+    assert st["count"][0] > 1000
+
+
+def test_all_culled_gives_a_zero_image():
+    w = wl.make_config(0, n=5000, size=(64, 64))
+    w.fields["z"] = w.fields["z"] + 100.0
+    st, g = full_check(w, 16)
+    assert st["count"][0] == 5000 and st["pairs"] == 0
+
+
+def test_single_heavy_pixel_and_heavy_tile():
+    """Many particles on one pixel / one tile: long same-pixel chains and several chunks of one tile."""
+    n = 60_000
+    w = wl.make_config(0, n=n, size=(64, 64))
+    w.fields["x"] = 0.5 + 1e-4 * (w.fields["x"] - 0.5)
+    w.fields["y"] = 0.5 + 1e-4 * (w.fields["y"] - 0.5)
+    w.fields["h"][: n // 2] = 1e-5                               # half SMALL on ~one pixel, half MEDIUM
+    st, g = full_check(w, 16)
+    assert st["chunks"] >= 4
+
+
+def test_pair_overflow_is_reported_and_image_is_zero():
+    w = wl.make_config(0, n=50_000, size=(128, 128))
+    lut = wl.palette()
+    r, f, kw, img = gpu_frame(w, lut, 16, pair_capacity=1000)
+    st = r.stats()
+    assert st["overflow"] == 1 and st["pairs"] > 1000
+    assert float(img.abs().max()) == 0.0
+    # a larger workspace on the same context renders the frame
+    img2 = r.render(f, w.species, pair_capacity=200_000, **kw)
+    assert r.stats()["overflow"] == 0 and float(img2.max()) > 0
+
+
+def test_render_host_matches_device_render():
+    w = wl.make_config(0, n=40_000, size=(160, 120))
+    lut = wl.palette()
+    r, f, kw, img = gpu_frame(w, lut, 16)
+    host = {k: v.contiguous().pin_memory() for k, v in w.fields.items()}
+    out = torch.empty((w.height, w.width, 3), dtype=torch.float32).pin_memory()
+    r.render_host(host, w.species, out, **kw)
+    ref, g, cam = oracle_frame(w, lut, 16)
+    assert_image_close(out, ref)
+    assert_image_close(img, ref)
+
+
+def test_errors_are_reported_not_raised_from_c():
+    b = _binding()
+    r = b.Renderer(64, 64, 1000)
+    w = wl.make_config(0, n=100, size=(64, 64))
+    f = to_dev(w.fields)
+    with pytest.raises(b.SplotchError) as e:
+        r.render(f, w.species)                                   # camera not set
+    assert e.value.code == b.SPLOTCH_ESTATE
+    r.set_camera(w.camera)
+    with pytest.raises(b.SplotchError) as e:
+        r.render(f, w.species)                                   # colour map not set
+    assert e.value.code == b.SPLOTCH_ESTATE
+    r.set_colormap(0, wl.palette())
+    with pytest.raises(b.SplotchError) as e:
+        r.render(f, w.species, tile=12)
+    assert e.value.code == b.SPLOTCH_EINVAL
+    with pytest.raises(b.SplotchError):
+        r.set_camera(wl.Camera((0, 0, 0), (0, 0, 0), (0, 1, 0), 45.0))
+    with pytest.raises(b.SplotchError):
+        r.set_camera(wl.Camera((0, 0, 1), (0, 0, 0), (0, 0, 2), 45.0))
+    big = wl.make_config(0, n=2000, size=(64, 64))
+    with pytest.raises(b.SplotchError):
+        r.render(to_dev(big.fields), big.species)                # n > max_particles
+    r.render(f, w.species)
+
+
+def test_permutation_invariance_on_gpu():
+    w = wl.make_config(0, n=50_000, size=(128, 128))
+    lut = wl.palette()
+    r, f, kw, img = gpu_frame(w, lut, 16)
+    perm = torch.randperm(w.n, generator=torch.Generator().manual_seed(1)).cuda()
+    f2 = {k: v[perm].contiguous() for k, v in f.items()}
+    img2 = r.render(f2, w.species, **kw).clone()
+    torch.cuda.synchronize()
+    a, b_ = img.double().cpu().numpy(), img2.double().cpu().numpy()
+    assert np.linalg.norm(a - b_) <= 2e-6 * np.linalg.norm(a)
+
+
+def test_cfg1_full_size_bench_configuration():
+    """BASELINE configs[1] at full size (10M particles, 800 x 800), the launch configuration bench.py times."""
+    w = wl.make_config(1, device="cuda")
+    lut = wl.palette()
+    fdev = {k: v.contiguous() for k, v in w.fields.items()}
+    w.fields = {k: v.cpu() for k, v in fdev.items()}
+    ref, g, cam = oracle_frame(w, lut, 16)
+    r, f, kw, img = gpu_frame(w, lut, 16, fields_dev=fdev)
+    assert_geometry_exact(r, f, w, kw, g, cam)
+    assert_counts_exact(r, w, 16, g)
+    assert_image_close(img, ref, "cfg1 full")
