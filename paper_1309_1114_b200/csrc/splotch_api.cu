@@ -19,7 +19,7 @@ constexpr int kProfRing = 256;              // frames of per-stage events kept w
 const char *kStageNames[kStages] = {"count", "colscan", "binscan", "scatter", "splat", "compose"};
 
 struct Layout {
-    size_t counts, cls_counts, bin_count, bin_start, chunk_start, stats, desc, partials, records, staging, total;
+    size_t counts, cls_counts, bin_count, bin_start, seg_start, stats, chunk_tile, partials, records, staging, total;
     unsigned long long capacity, max_chunks;
     int nrows;
 };
@@ -81,10 +81,13 @@ size_t hist_bytes(int W, int H, int T)
     return sizeof(unsigned int) * ((size_t)ntx * nty + (size_t)nsx * nsy);
 }
 
+// dynamic shared memory of k_count / k_scatter: the block's histogram / cursors plus room for the colour tables
+size_t bin_smem_bytes(int W, int H, int T) { return hist_bytes(W, H, T) + 16 + sizeof(float4) * kLutSmemMax; }
+
 int bin_rows(const splotch_ctx *c, int T)
 {
     // two resident blocks per SM while two private histograms fit in shared memory, else one
-    return c->n_sm * (2 * (hist_bytes(c->width, c->height, T) + 1024) <= (size_t)c->smem_optin ? 2 : 1);
+    return c->n_sm * (2 * (bin_smem_bytes(c->width, c->height, T) + 1024) <= (size_t)c->smem_optin ? 2 : 1);
 }
 
 // Workspace layout.  Either `capacity` is given (sizing query) or derived from `bytes` (render).
@@ -94,14 +97,14 @@ bool make_layout(const splotch_ctx *c, unsigned long long n, int T, unsigned lon
     const int ntx = (c->width + T - 1) / T, nty = (c->height + T - 1) / T;
     const size_t n_tiles = (size_t)ntx * nty;
     const size_t nbins = hist_bytes(c->width, c->height, T) / sizeof(unsigned int);
-    const size_t partial_bytes = sizeof(float4) * (size_t)T * T;
+    const size_t partial_bytes = sizeof(long long) * 3 * (size_t)T * T;     // one segment's framebuffer
     L->nrows = bin_rows(c, T);
     size_t off = 0;
     L->counts = off;      off = align_up(off + sizeof(unsigned int) * nbins * L->nrows, 256);
     L->cls_counts = off;  off = align_up(off + sizeof(unsigned int) * 4 * L->nrows, 256);
     L->bin_count = off;   off = align_up(off + sizeof(unsigned int) * nbins, 256);
     L->bin_start = off;   off = align_up(off + sizeof(unsigned int) * (nbins + 1), 256);
-    L->chunk_start = off; off = align_up(off + sizeof(unsigned int) * (n_tiles + 1), 256);
+    L->seg_start = off;   off = align_up(off + sizeof(unsigned int) * (n_tiles + 1), 256);
     L->stats = off;       off = align_up(off + sizeof(DeviceStats), 256);
     L->staging = off;
     if (staging) {
@@ -109,19 +112,21 @@ bool make_layout(const splotch_ctx *c, unsigned long long n, int T, unsigned lon
         off = align_up(off + sizeof(float) * 3 * (size_t)c->width * c->height, 256);
     }
     const size_t fixed = off;
+    // chunks <= max(32 per SM, capacity / kChunkMax) + 2 (k_binscan's choice of the chunk size); segments <= tiles + chunks
+    const size_t per_chunk = partial_bytes + sizeof(unsigned int);
+    const size_t min_chunks = (size_t)c->n_sm * 32 + 2;
     if (capacity == 0) {
-        // derive from bytes: capacity * 32 + (n_tiles + capacity / kChunk + 1) * (partial + 8) <= bytes - fixed
-        const size_t per_chunk = partial_bytes + sizeof(uint2);
-        const size_t need0 = fixed + (n_tiles + 2) * per_chunk + 8192;
+        // derive from bytes: capacity * 32 + (n_tiles + chunks) * partial + chunks * 4 <= bytes - fixed
+        const size_t need0 = fixed + n_tiles * partial_bytes + min_chunks * per_chunk + 8192;
         if (bytes < need0) return false;
         const double avail = (double)(bytes - need0);
-        capacity = (unsigned long long)(avail / (32.0 + (double)per_chunk / kChunk));
+        capacity = (unsigned long long)(avail / (32.0 + (double)per_chunk / kChunkMax));
         if (capacity > 0xfffffff0ull) capacity = 0xfffffff0ull;
     }
     L->capacity = capacity;
-    L->max_chunks = n_tiles + capacity / kChunk + 1;
-    L->desc = off;     off = align_up(off + sizeof(uint2) * L->max_chunks, 256);
-    L->partials = off; off = align_up(off + partial_bytes * L->max_chunks, 256);
+    L->max_chunks = (capacity / kChunkMax + 2 > min_chunks) ? capacity / kChunkMax + 2 : min_chunks;
+    L->chunk_tile = off; off = align_up(off + sizeof(unsigned int) * L->max_chunks, 256);
+    L->partials = off;   off = align_up(off + partial_bytes * (n_tiles + L->max_chunks), 256);
     L->records = off;  off = align_up(off + 32ull * capacity, 256);
     L->total = off;
     return bytes == 0 || off <= bytes;
@@ -131,7 +136,7 @@ template <int T>
 int query_splat_occupancy(splotch_ctx *c, int *out)
 {
     CU_TRY(c, cudaFuncSetAttribute(k_splat<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SplatCfg<T>::kSmemBytes));
-    CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, k_splat<T>, SplatCfg<T>::kWarps * 32, SplatCfg<T>::kSmemBytes));
+    CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, k_splat<T>, kSplatThreads, SplatCfg<T>::kSmemBytes));
     if (*out < 1) *out = 1;
     return SPLOTCH_OK;
 }
@@ -148,7 +153,7 @@ int check_params(splotch_ctx *c, const splotch_particles *p, unsigned long long 
     if (ts < 0) return fail(c, SPLOTCH_EINVAL, "tile must be 8, 16 or 32 (got %d)", q->tile);
     if (!(q->chi > 0.0f) || !(q->r_small >= 0.0f) || !(q->r_small < q->r_large))
         return fail(c, SPLOTCH_EINVAL, "need chi > 0 and 0 <= r_small < r_large");
-    if (hist_bytes(c->width, c->height, q->tile) + 1024 > (size_t)c->smem_optin)
+    if (bin_smem_bytes(c->width, c->height, q->tile) + 1024 > (size_t)c->smem_optin)
         return fail(c, SPLOTCH_EINVAL, "tile %d gives too many tiles for a %dx%d image (per-block histogram exceeds shared memory); use a larger tile",
                     q->tile, c->width, c->height);
     if (!q->additive) return fail(c, SPLOTCH_EINVAL, "ordered (E != A) mode is not built yet");
@@ -176,8 +181,9 @@ int check_params(splotch_ctx *c, const splotch_particles *p, unsigned long long 
         const unsigned long long o = p->species_offsets ? p->species_offsets[s] : (s == 0 ? 0ull : n);
         if ((s == 0 && o != 0) || (s == ns && o != n) || (s > 0 && o < fp->sp_begin[s - 1]))
             return fail(c, SPLOTCH_EINVAL, "species_offsets must ascend from 0 to n");
-        fp->sp_begin[s] = o;
+        fp->sp_begin[s] = (unsigned int)o;
     }
+    int lut_total = 0;
     for (int s = 0; s < ns; ++s) {
         const splotch_species_params &sp = q->species[s];
         SpeciesDev &d = fp->sp[s];
@@ -186,11 +192,14 @@ int check_params(splotch_ctx *c, const splotch_particles *p, unsigned long long 
         d.use_colormap = sp.use_colormap ? 1 : 0; d.use_log10 = sp.scalar_log10 ? 1 : 0;
         d.smin = sp.scalar_min; d.range = sp.scalar_max - sp.scalar_min;
         d.lut_n = c->lut_n[s];
+        d.lut_off = lut_total;
+        if (d.use_colormap) lut_total += d.lut_n;
         if (d.use_colormap) {
             if (d.lut_n < 2) return fail(c, SPLOTCH_ESTATE, "species %d uses a colour map but none was set", s);
             if (!(sp.scalar_max != sp.scalar_min)) return fail(c, SPLOTCH_EINVAL, "species %d: scalar_min == scalar_max", s);
         }
     }
+    fp->lut_total = lut_total <= kLutSmemMax ? lut_total : 0;      // larger tables are read from global memory
     return SPLOTCH_OK;
 }
 
@@ -206,11 +215,11 @@ int launch_render_tail(splotch_ctx *c, const Layout &L, char *ws, const FramePar
 {
     const int ti = T == 8 ? 0 : T == 16 ? 1 : 2;
     const int grid = c->n_sm * c->splat_blocks_per_sm[ti];
-    k_splat<T><<<grid, SplatCfg<T>::kWarps * 32, SplatCfg<T>::kSmemBytes, st>>>(
-        (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.bin_start), (const uint2 *)(ws + L.desc),
-        (DeviceStats *)(ws + L.stats), (float4 *)(ws + L.partials), fp);
+    k_splat<T><<<grid, kSplatThreads, SplatCfg<T>::kSmemBytes, st>>>(
+        (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.bin_start), (const unsigned int *)(ws + L.seg_start),
+        (const unsigned int *)(ws + L.chunk_tile), (DeviceStats *)(ws + L.stats), (long long *)(ws + L.partials), fp);
     if (c->profiling) cudaEventRecord(c->ev[5], st);
-    k_compose<T><<<fp.n_tiles, 256, 0, st>>>((const float4 *)(ws + L.partials), (const unsigned int *)(ws + L.chunk_start),
+    k_compose<T><<<fp.n_tiles, 256, 0, st>>>((const long long *)(ws + L.partials), (const unsigned int *)(ws + L.seg_start),
                                              (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.bin_start),
                                              (const DeviceStats *)(ws + L.stats), fp, image);
     if (c->profiling) cudaEventRecord(c->ev[6], st);
@@ -221,7 +230,7 @@ int render_device(splotch_ctx *c, const splotch_particles *p, unsigned long long
                   const Layout &L, float *image, char *ws, cudaStream_t st)
 {
     const bool al = aligned16(p);
-    const size_t hbytes = sizeof(unsigned int) * (size_t)fp.nbins;
+    const size_t hbytes = bin_smem_bytes(fp.W, fp.H, fp.T);
     unsigned long long per = (n + L.nrows - 1) / L.nrows;
     per = (per + 3) / 4 * 4;
     if (per == 0) per = 4;
@@ -229,7 +238,7 @@ int render_device(splotch_ctx *c, const splotch_particles *p, unsigned long long
     unsigned int *cls_counts = (unsigned int *)(ws + L.cls_counts);
     unsigned int *bin_count = (unsigned int *)(ws + L.bin_count);
     unsigned int *bin_start = (unsigned int *)(ws + L.bin_start);
-    unsigned int *chunk_start = (unsigned int *)(ws + L.chunk_start);
+    unsigned int *seg_start = (unsigned int *)(ws + L.seg_start);
     DeviceStats *stats = (DeviceStats *)(ws + L.stats);
     if (c->profiling) {
         c->ev = c->ev_ring[c->prof_frames % kProfRing];
@@ -240,8 +249,8 @@ int render_device(splotch_ctx *c, const splotch_particles *p, unsigned long long
     if (c->profiling) cudaEventRecord(c->ev[1], st);
     k_colscan<<<(fp.nbins + 255) / 256, 256, 0, st>>>(counts, L.nrows, fp.nbins, bin_count);
     if (c->profiling) cudaEventRecord(c->ev[2], st);
-    k_binscan<<<1, 1024, 0, st>>>(bin_count, fp.n_tiles, fp.nbins, bin_start, chunk_start, (uint2 *)(ws + L.desc),
-                                  cls_counts, L.nrows, L.capacity, L.max_chunks, stats);
+    k_binscan<<<1, 1024, 0, st>>>(bin_count, fp.n_tiles, fp.nbins, bin_start, seg_start, (unsigned int *)(ws + L.chunk_tile),
+                                  cls_counts, L.nrows, L.capacity, L.max_chunks, c->n_sm, stats);
     if (c->profiling) cudaEventRecord(c->ev[3], st);
     if (al) k_scatter<true><<<L.nrows, kBinThreads, hbytes, st>>>(p->x, p->y, p->z, p->h, p->I, p->scalar, n, per, fp, counts,
                                                                   bin_start, stats, (float4 *)(ws + L.records));
@@ -398,7 +407,7 @@ int splotch_set_profiling(splotch_ctx *c, int enabled)
 size_t splotch_workspace_bytes(const splotch_ctx *c, uint64_t n, int tile, uint64_t pair_capacity, int with_host_staging)
 {
     if (!c || tile_shift(tile) < 0 || n > c->max_particles) return 0;
-    if (hist_bytes(c->width, c->height, tile) + 1024 > (size_t)c->smem_optin) return 0;
+    if (bin_smem_bytes(c->width, c->height, tile) + 1024 > (size_t)c->smem_optin) return 0;
     if (pair_capacity == 0) pair_capacity = 2ull * n + (1ull << 20);
     if (pair_capacity > 0xfffffff0ull) return 0;
     Layout L;

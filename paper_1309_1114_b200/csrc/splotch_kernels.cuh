@@ -3,13 +3,16 @@
 // Stage map (paper passages in PAPER.md):
 //   k_count    A1+A3+A4a  roto-translate, project, classify (:76, :138, :156-173) and count (particle, bin) pairs
 //   k_colscan  A4b        per-bin exclusive scan over the count matrix rows (replaces thrust::reduce_by_key, :203)
-//   k_binscan  A4c        exclusive scan over bins, chunk table, frame statistics (replaces inclusive_scan, :205)
-//   k_scatter  A1-A3+A2+A4d  recompute geometry, colourise (:76, :85), write render records in bin order
+//   k_binscan  A4c        exclusive scan over bins, chunk/segment tables, frame statistics (replaces inclusive_scan, :205)
+//   k_scatter  A1-A3+A2+A4d  recompute geometry, colourise (:76, :85), write 32-byte render records in bin order
 //                            (replaces copy_if + sort_by_key, :196-202)
-//   k_splat    A5         small + medium particles of one chunk of one tile into warp-private shared-memory
-//                         framebuffers (the paper's medium-particle kernel, :183, :224-228, without its halo copies)
-//   k_compose  A6+A8      per tile: sum chunk partials, gather the LARGE particles of the tile's super-tile
-//                         (the paper renders these on the CPU, :232-238), optional 1-exp(-S), write the image
+//   k_splat    A5         SMALL + MEDIUM records of one chunk: all fragments of 32 records are spread over the 32 lanes
+//                         of a warp and accumulated into the tile's 64-bit fixed-point framebuffer in shared memory
+//                         with native integer atomics (the paper's medium-particle kernel, :183, :224-228, without
+//                         its halo copies and without idle threads for small footprints)
+//   k_compose  A6+A8      per tile: sum segment partials (exact integer sums), gather the LARGE particles of the
+//                         tile's super-tile (the paper renders these on the CPU, :232-238), optional 1-exp(-S),
+//                         write the image once
 //
 // Canonical float32 geometry: every operation that decides an integer (class, pixel box, tile box, the inside
 // test) is written with round-to-nearest intrinsics (__fmul_rn, __fmaf_rn, __fdiv_rn ...) which nvcc never
@@ -22,10 +25,13 @@ namespace splotch {
 
 constexpr int kMaxSpecies   = 8;
 constexpr int kMaxLut       = 1024;
-constexpr int kChunk        = 4096;   // records per work item of k_splat
-constexpr int kSplatWarps   = 8;
+constexpr int kChunkMax     = 4096;   // records per work item of k_splat (upper bound; the frame picks its own)
+constexpr int kChunkMin     = 512;
+constexpr int kSplatThreads = 256;
 constexpr int kBinThreads   = 512;    // k_count / k_scatter block size
 constexpr int kSuperShift   = 3;      // super-tile = 8 x 8 tiles (LARGE particles are binned to super-tiles)
+constexpr int kLutSmemMax   = 1024;   // colour-table entries (all species together) staged in shared memory by k_scatter
+constexpr int kFixedBits    = 30;     // the largest record amplitude maps to [2^29, 2^30) fixed-point units
 
 enum { CULLED = 0, SMALL = 1, MEDIUM = 2, LARGE = 3 };
 
@@ -33,7 +39,7 @@ struct SpeciesDev {
     float brightness, absorb;
     float fixed_r, fixed_g, fixed_b;
     float smin, range;
-    int   use_colormap, use_log10, lut_n, pad;
+    int   use_colormap, use_log10, lut_n, lut_off;   // lut_off: first entry in the packed shared-memory table
 };
 
 struct FrameParams {
@@ -45,16 +51,16 @@ struct FrameParams {
     int   ntx, nty, n_tiles;
     int   sshift, nsx, nsy, n_super, nbins;
     int   additive, apply_transfer;
-    int   n_species;
-    unsigned long long sp_begin[kMaxSpecies + 1];
+    int   n_species, lut_total;  // lut_total: packed entries of all colour-mapped species, 0 = read tables from global
+    unsigned int sp_begin[kMaxSpecies + 1];
     SpeciesDev sp[kMaxSpecies];
     const float4 *lut;           // [kMaxSpecies][kMaxLut] rgb0
 };
 
-struct DeviceStats {             // written by k_binscan, read back by splotch_get_stats
+struct DeviceStats {             // written by k_binscan / k_scatter, read back by splotch_get_stats
     unsigned long long count[4];
-    unsigned long long pairs, large_pairs, chunks, capacity;
-    unsigned int overflow, work_counter, pad0, pad1;
+    unsigned long long pairs, large_pairs, chunks, capacity, segments;
+    unsigned int overflow, work_counter, chunk_size, amax_bits;
 };
 
 struct Geo {
@@ -69,6 +75,8 @@ __device__ __forceinline__ float dot3(const float *a, float dx, float dy, float 
 }
 
 // C1 of DESIGN.md: the canonical float32 sequence (PAPER.md:76 projection, Eq. 7 :138 radius, :156-160 classes).
+// Written without branches (every lane evaluates both the SMALL and the box formulas and selects): the warps of
+// the streaming kernels stay converged whatever the mix of classes.
 __device__ __forceinline__ Geo geometry(float x, float y, float z, float h, const FrameParams &fp)
 {
     Geo g;
@@ -76,36 +84,28 @@ __device__ __forceinline__ Geo geometry(float x, float y, float z, float h, cons
     const float xc = dot3(fp.cam + 0, dx, dy, dz);
     const float yc = dot3(fp.cam + 3, dx, dy, dz);
     g.zc = dot3(fp.cam + 6, dx, dy, dz);
-    g.cls = CULLED;
-    g.px = g.py = g.sp = g.rp = 0.0f;
-    g.x0 = g.y0 = 0;
-    g.x1 = g.y1 = -1;
-    if (g.zc > fp.z_near) {
-        const float k = __fdiv_rn(fp.cam[12], g.zc);
-        g.px = __fmaf_rn(xc, k, fp.cam[13]);
-        g.py = __fmaf_rn(-yc, k, fp.cam[14]);
-        g.sp = __fmul_rn(h, k);
-        g.rp = __fmul_rn(fp.chi, g.sp);
-        if (g.rp >= 0.0f && g.rp <= 3.0e38f) {
-            if (g.rp <= fp.r_small) {
-                if (g.px >= 0.0f && g.px < fp.fW && g.py >= 0.0f && g.py < fp.fH) {
-                    g.cls = SMALL;
-                    g.x0 = g.x1 = (int)floorf(g.px);
-                    g.y0 = g.y1 = (int)floorf(g.py);
-                }
-            } else {
-                const float fx0 = fmaxf(ceilf(__fsub_rn(__fsub_rn(g.px, g.rp), 0.5f)), 0.0f);
-                const float fx1 = fmaxf(fminf(floorf(__fsub_rn(__fadd_rn(g.px, g.rp), 0.5f)), __fsub_rn(fp.fW, 1.0f)), -1.0f);
-                const float fy0 = fmaxf(ceilf(__fsub_rn(__fsub_rn(g.py, g.rp), 0.5f)), 0.0f);
-                const float fy1 = fmaxf(fminf(floorf(__fsub_rn(__fadd_rn(g.py, g.rp), 0.5f)), __fsub_rn(fp.fH, 1.0f)), -1.0f);
-                if (fx0 <= fx1 && fy0 <= fy1) {
-                    g.cls = (g.rp <= fp.r_large) ? MEDIUM : LARGE;
-                    g.x0 = (int)fx0; g.x1 = (int)fx1;
-                    g.y0 = (int)fy0; g.y1 = (int)fy1;
-                }
-            }
-        }
-    }
+    bool ok = g.zc > fp.z_near;
+    const float k = __fdiv_rn(fp.cam[12], g.zc);
+    g.px = __fmaf_rn(xc, k, fp.cam[13]);
+    g.py = __fmaf_rn(-yc, k, fp.cam[14]);
+    g.sp = __fmul_rn(h, k);
+    g.rp = __fmul_rn(fp.chi, g.sp);
+    ok = ok && g.rp >= 0.0f && g.rp <= 3.0e38f;
+    const bool small = g.rp <= fp.r_small;
+    const bool s_ok = g.px >= 0.0f && g.px < fp.fW && g.py >= 0.0f && g.py < fp.fH;
+    const float fx0 = fmaxf(ceilf(__fsub_rn(__fsub_rn(g.px, g.rp), 0.5f)), 0.0f);
+    const float fx1 = fmaxf(fminf(floorf(__fsub_rn(__fadd_rn(g.px, g.rp), 0.5f)), __fsub_rn(fp.fW, 1.0f)), -1.0f);
+    const float fy0 = fmaxf(ceilf(__fsub_rn(__fsub_rn(g.py, g.rp), 0.5f)), 0.0f);
+    const float fy1 = fmaxf(fminf(floorf(__fsub_rn(__fadd_rn(g.py, g.rp), 0.5f)), __fsub_rn(fp.fH, 1.0f)), -1.0f);
+    const bool b_ok = fx0 <= fx1 && fy0 <= fy1;
+    const int big = (g.rp <= fp.r_large) ? MEDIUM : LARGE;
+    g.cls = ok ? (small ? (s_ok ? SMALL : CULLED) : (b_ok ? big : CULLED)) : CULLED;
+    const bool act = g.cls != CULLED;
+    const int ipx = __float2int_rz(g.px), ipy = __float2int_rz(g.py);          // px, py >= 0 when SMALL: truncation is floor
+    g.x0 = act ? (small ? ipx : __float2int_rz(fx0)) : 0;
+    g.x1 = act ? (small ? ipx : __float2int_rz(fx1)) : -1;
+    g.y0 = act ? (small ? ipy : __float2int_rz(fy0)) : 0;
+    g.y1 = act ? (small ? ipy : __float2int_rz(fy1)) : -1;
     return g;
 }
 
@@ -120,26 +120,23 @@ __device__ __forceinline__ int paper_label(const Geo &g, const FrameParams &fp)
     return ((int)cy >> fp.tshift) * fp.ntx + ((int)cx >> fp.tshift);
 }
 
-// Visit every bin a particle is assigned to: its tile (SMALL), the tiles of its pixel box (MEDIUM) or the
-// super-tiles of its pixel box (LARGE, bins n_tiles ...).  k_count and k_scatter share this traversal.
-template <class F>
-__device__ __forceinline__ void for_each_bin(const Geo &g, const FrameParams &fp, F &&f)
+// Bin box of an active particle: tiles of its pixel box (SMALL, MEDIUM) or super-tiles (LARGE, bins n_tiles ...).
+// k_count and k_scatter share this traversal: bins are base + by * pitch + bx for bx in [bx0, bx1], by in [by0, by1].
+struct BinBox { int bx0, bx1, by0, by1, pitch, base, n; };      // n = number of bins (0 for CULLED)
+
+__device__ __forceinline__ BinBox bin_box(const Geo &g, const FrameParams &fp)
 {
-    if (g.cls == CULLED) return;
-    if (g.cls == LARGE) {
-        const int sx0 = g.x0 >> fp.sshift, sx1 = g.x1 >> fp.sshift;
-        const int sy0 = g.y0 >> fp.sshift, sy1 = g.y1 >> fp.sshift;
-        for (int sy = sy0; sy <= sy1; ++sy)
-            for (int sx = sx0; sx <= sx1; ++sx) f(fp.n_tiles + sy * fp.nsx + sx);
-        return;
-    }
-    const int tx0 = g.x0 >> fp.tshift, tx1 = g.x1 >> fp.tshift;
-    const int ty0 = g.y0 >> fp.tshift, ty1 = g.y1 >> fp.tshift;
-    for (int ty = ty0; ty <= ty1; ++ty)
-        for (int tx = tx0; tx <= tx1; ++tx) f(ty * fp.ntx + tx);
+    BinBox b;
+    const int sh = (g.cls == LARGE) ? fp.sshift : fp.tshift;
+    b.bx0 = g.x0 >> sh; b.bx1 = g.x1 >> sh;
+    b.by0 = g.y0 >> sh; b.by1 = g.y1 >> sh;
+    b.pitch = (g.cls == LARGE) ? fp.nsx : fp.ntx;
+    b.base = (g.cls == LARGE) ? fp.n_tiles : 0;
+    b.n = (g.cls == CULLED) ? 0 : (b.bx1 - b.bx0 + 1) * (b.by1 - b.by0 + 1);
+    return b;
 }
 
-// ---- streaming loads: four consecutive particles of one field ------------------------------------------------
+// ---- streaming loads / stores ----------------------------------------------------------------------------------
 __device__ __forceinline__ float4 ldg_stream4(const float *p)
 {
     float4 v;
@@ -148,66 +145,89 @@ __device__ __forceinline__ float4 ldg_stream4(const float *p)
     return v;
 }
 
-template <bool ALIGNED>
-__device__ __forceinline__ void load4(const float *__restrict__ a, unsigned long long i, unsigned long long hi, float (&v)[4])
+// one 32-byte render record, one request (256-bit global access, sm_100)
+__device__ __forceinline__ void st_record(float4 *rec, unsigned int slot, const float4 &a, const float4 &b)
 {
-    if (ALIGNED && i + 4 <= hi) {
+    asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                 :: "l"(rec + 2ull * slot), "f"(a.x), "f"(a.y), "f"(a.z), "f"(a.w), "f"(b.x), "f"(b.y), "f"(b.z), "f"(b.w)
+                 : "memory");
+}
+
+__device__ __forceinline__ void ld_record(const float4 *rec, unsigned int slot, float4 &a, float4 &b)
+{
+    asm volatile("ld.global.nc.L1::no_allocate.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=f"(a.x), "=f"(a.y), "=f"(a.z), "=f"(a.w), "=f"(b.x), "=f"(b.y), "=f"(b.z), "=f"(b.w)
+                 : "l"(rec + 2ull * slot));
+}
+
+template <bool ALIGNED>
+__device__ __forceinline__ void load4(const float *__restrict__ a, unsigned int i, unsigned int len, float (&v)[4])
+{
+    if (ALIGNED && i + 4 <= len) {
         const float4 q = ldg_stream4(a + i);
         v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w;
     } else {
 #pragma unroll
-        for (int j = 0; j < 4; ++j) v[j] = (i + j < hi) ? __ldg(a + i + j) : 0.0f;
+        for (int j = 0; j < 4; ++j) v[j] = (i + j < len) ? __ldg(a + i + j) : 0.0f;
     }
 }
 
 __device__ __forceinline__ unsigned int warp_sum(unsigned int v)
 {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
+    return __reduce_add_sync(0xffffffffu, v);
 }
 
 // ---- A1 + A3 + A4a: classify and count ------------------------------------------------------------------------
 // Block b owns the particle range [b*per, (b+1)*per) and a private histogram over all bins in shared memory;
 // row b of `counts` receives it, so the count stage needs no global atomics and is deterministic.
 template <bool ALIGNED>
-__global__ void __launch_bounds__(kBinThreads)
+__global__ void __launch_bounds__(kBinThreads, 2)
 k_count(const float *__restrict__ x, const float *__restrict__ y, const float *__restrict__ z,
         const float *__restrict__ h, unsigned long long n, unsigned long long per, const __grid_constant__ FrameParams fp,
         unsigned int *__restrict__ counts, unsigned int *__restrict__ cls_counts)
 {
     extern __shared__ unsigned int hist[];
     __shared__ unsigned int s_cls[4];
-    for (int i = threadIdx.x; i < fp.nbins; i += blockDim.x) hist[i] = 0u;
+    for (int i = threadIdx.x; i < fp.nbins; i += kBinThreads) hist[i] = 0u;
     if (threadIdx.x < 4) s_cls[threadIdx.x] = 0u;
     __syncthreads();
     const unsigned long long lo = (unsigned long long)blockIdx.x * per;
-    const unsigned long long hi = min(n, lo + per);
-    unsigned int c1 = 0, c2 = 0, c3 = 0, call = 0;
-    for (unsigned long long i = lo + 4ull * threadIdx.x; i < hi; i += 4ull * blockDim.x) {
+    const unsigned int len = lo < n ? (unsigned int)min(n - lo, per) : 0u;
+    x += lo; y += lo; z += lo; h += lo;
+    unsigned int c1 = 0, c2 = 0, c3 = 0, c0 = 0;
+    // the loop bound is the same for the 32 lanes of a warp (lanes past the end idle), so warps stay converged
+    const unsigned int lane4 = 4u * (threadIdx.x & 31u);
+    for (unsigned int iw = 4u * (threadIdx.x & ~31u); iw < len; iw += 4u * kBinThreads) {
+        const unsigned int i = iw + lane4;
         float xs[4], ys[4], zs[4], hs[4];
-        load4<ALIGNED>(x, i, hi, xs);
-        load4<ALIGNED>(y, i, hi, ys);
-        load4<ALIGNED>(z, i, hi, zs);
-        load4<ALIGNED>(h, i, hi, hs);
+        load4<ALIGNED>(x, i, len, xs);
+        load4<ALIGNED>(y, i, len, ys);
+        load4<ALIGNED>(z, i, len, zs);
+        load4<ALIGNED>(h, i, len, hs);
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            if (i + j < hi) {
-                const Geo g = geometry(xs[j], ys[j], zs[j], hs[j], fp);
-                ++call;
-                c1 += (g.cls == SMALL); c2 += (g.cls == MEDIUM); c3 += (g.cls == LARGE);
-                for_each_bin(g, fp, [&](int bin) { atomicAdd(&hist[bin], 1u); });
+            Geo g = geometry(xs[j], ys[j], zs[j], hs[j], fp);
+            const bool live = i + j < len;
+            if (!live) g.cls = CULLED;
+            c0 += (live && g.cls == CULLED); c1 += (g.cls == SMALL); c2 += (g.cls == MEDIUM); c3 += (g.cls == LARGE);
+            const BinBox b = bin_box(g, fp);
+            const int nmax = __reduce_max_sync(0xffffffffu, b.n);
+            int bx = b.bx0, by = b.by0;
+            for (int t = 0; t < nmax; ++t) {
+                if (t < b.n) atomicAdd(&hist[b.base + by * b.pitch + bx], 1u);
+                const bool wrap = bx == b.bx1;
+                bx = wrap ? b.bx0 : bx + 1;
+                by += wrap;
             }
         }
     }
-    c1 = warp_sum(c1); c2 = warp_sum(c2); c3 = warp_sum(c3); call = warp_sum(call);
+    c0 = warp_sum(c0); c1 = warp_sum(c1); c2 = warp_sum(c2); c3 = warp_sum(c3);
     if ((threadIdx.x & 31) == 0) {
-        atomicAdd(&s_cls[0], call - c1 - c2 - c3);
-        atomicAdd(&s_cls[1], c1); atomicAdd(&s_cls[2], c2); atomicAdd(&s_cls[3], c3);
+        atomicAdd(&s_cls[0], c0); atomicAdd(&s_cls[1], c1); atomicAdd(&s_cls[2], c2); atomicAdd(&s_cls[3], c3);
     }
     __syncthreads();
     unsigned int *row = counts + (size_t)blockIdx.x * fp.nbins;
-    for (int i = threadIdx.x; i < fp.nbins; i += blockDim.x) row[i] = hist[i];
+    for (int i = threadIdx.x; i < fp.nbins; i += kBinThreads) row[i] = hist[i];
     if (threadIdx.x < 4) cls_counts[blockIdx.x * 4 + threadIdx.x] = s_cls[threadIdx.x];
 }
 
@@ -234,7 +254,7 @@ k_colscan(unsigned int *__restrict__ counts, int nrows, int nbins, unsigned int 
     bin_count[bin] = run;
 }
 
-// ---- A4c: scan over bins, chunk table, statistics (one block) ------------------------------------------------
+// ---- A4c: scan over bins, segment table, statistics (one block) ------------------------------------------------
 __device__ __forceinline__ unsigned long long block_excl_scan_1024(unsigned long long v, unsigned long long *s_warp,
                                                                    unsigned long long *total)
 {
@@ -263,42 +283,59 @@ __device__ __forceinline__ unsigned long long block_excl_scan_1024(unsigned long
     return r;
 }
 
+// The tile part of the record array, [0, pairs), is cut into chunks of `chunk_size` consecutive records (the work
+// items of k_splat).  A segment is the overlap of one chunk with one tile; tile t owns the partial-framebuffer
+// slots seg_start[t] .. seg_start[t+1]-1, one per chunk it overlaps, in chunk order.  chunk_tile[c] is the tile
+// that holds the first record of chunk c.
 __global__ void __launch_bounds__(1024)
 k_binscan(const unsigned int *__restrict__ bin_count, int n_tiles, int nbins, unsigned int *__restrict__ bin_start,
-          unsigned int *__restrict__ chunk_start, uint2 *__restrict__ chunk_desc,
+          unsigned int *__restrict__ seg_start, unsigned int *__restrict__ chunk_tile,
           const unsigned int *__restrict__ cls_counts, int nrows, unsigned long long capacity,
-          unsigned long long max_chunks, DeviceStats *__restrict__ stats)
+          unsigned long long max_chunks, int n_sm, DeviceStats *__restrict__ stats)
 {
     __shared__ unsigned long long s_warp[32];
-    __shared__ unsigned long long s_tot_pairs, s_tot_all, s_tot_chunks;
+    __shared__ unsigned long long s_tot_pairs, s_tot_all, s_tot_segs;
     const int per = (nbins + 1023) / 1024;
     const int b0 = min(nbins, (int)threadIdx.x * per), b1 = min(nbins, b0 + per);
-    unsigned long long sum_all = 0, sum_tiles = 0, sum_chunks = 0;
+    unsigned long long sum_all = 0, sum_tiles = 0;
     for (int b = b0; b < b1; ++b) {
         const unsigned int c = bin_count[b];
         sum_all += c;
-        if (b < n_tiles) { sum_tiles += c; sum_chunks += (c + kChunk - 1) / kChunk; }
+        if (b < n_tiles) sum_tiles += c;
     }
     const unsigned long long off_all = block_excl_scan_1024(sum_all, s_warp, &s_tot_all);
-    const unsigned long long off_chunks = block_excl_scan_1024(sum_chunks, s_warp, &s_tot_chunks);
     (void)block_excl_scan_1024(sum_tiles, s_warp, &s_tot_pairs);
-    const bool overflow = s_tot_all > capacity || s_tot_chunks > max_chunks;
-    unsigned long long run = off_all, crun = off_chunks;
+    // chunk size of this frame: about 32 chunks per SM, between kChunkMin and kChunkMax, a multiple of 256
+    unsigned long long cs = (s_tot_pairs + (unsigned long long)n_sm * 32 - 1) / ((unsigned long long)n_sm * 32);
+    cs = (cs + 255) / 256 * 256;
+    cs = min((unsigned long long)kChunkMax, max((unsigned long long)kChunkMin, cs));
+    const unsigned int K = (unsigned int)cs;
+    unsigned long long run = off_all, nseg = 0;
+    for (int b = b0; b < b1; ++b) {
+        const unsigned int c = bin_count[b];
+        if (b < n_tiles && c > 0) nseg += (run + c - 1) / K - run / K + 1;
+        run += c;
+    }
+    const unsigned long long off_seg = block_excl_scan_1024(nseg, s_warp, &s_tot_segs);
+    const bool overflow = s_tot_all > capacity || (s_tot_pairs + K - 1) / K > max_chunks;
+    run = off_all;
+    unsigned long long srun = off_seg;
     for (int b = b0; b < b1; ++b) {
         const unsigned int c = bin_count[b];
         bin_start[b] = (unsigned int)run;
         if (b < n_tiles) {
-            chunk_start[b] = (unsigned int)crun;
-            const unsigned int nc = (c + kChunk - 1) / kChunk;
-            if (!overflow)
-                for (unsigned int k = 0; k < nc; ++k) chunk_desc[crun + k] = make_uint2((unsigned int)b, k);
-            crun += nc;
+            seg_start[b] = (unsigned int)srun;
+            if (c > 0) {
+                srun += (run + c - 1) / K - run / K + 1;
+                if (!overflow)      // chunks whose first record lies in this tile
+                    for (unsigned long long cc = (run + K - 1) / K; cc * K < run + c; ++cc) chunk_tile[cc] = (unsigned int)b;
+            }
         }
         run += c;
     }
     if (threadIdx.x == 1023) {
         bin_start[nbins] = (unsigned int)s_tot_all;
-        chunk_start[n_tiles] = (unsigned int)s_tot_chunks;
+        seg_start[n_tiles] = (unsigned int)s_tot_segs;
     }
     if (threadIdx.x < 4) {
         unsigned long long c = 0;
@@ -308,15 +345,18 @@ k_binscan(const unsigned int *__restrict__ bin_count, int n_tiles, int nbins, un
     if (threadIdx.x == 0) {
         stats->pairs = s_tot_pairs;
         stats->large_pairs = s_tot_all - s_tot_pairs;
-        stats->chunks = overflow ? 0ull : s_tot_chunks;
+        stats->chunks = overflow ? 0ull : (s_tot_pairs + K - 1) / K;
+        stats->segments = overflow ? 0ull : s_tot_segs;
         stats->capacity = capacity;
         stats->overflow = overflow ? 1u : 0u;
         stats->work_counter = 0u;
+        stats->chunk_size = K;
+        stats->amax_bits = 0u;
     }
 }
 
 // ---- A2: colour + amplitude (PAPER.md:76 normalisation/log, :85 look-up table) -------------------------------
-__device__ __forceinline__ int species_of(unsigned long long i, const FrameParams &fp)
+__device__ __forceinline__ int species_of(unsigned int i, const FrameParams &fp)
 {
     int s = 0;
 #pragma unroll
@@ -324,9 +364,9 @@ __device__ __forceinline__ int species_of(unsigned long long i, const FrameParam
     return s;
 }
 
-__device__ __forceinline__ float3 amplitude(float I, float scalar, float h, int s, const FrameParams &fp)
+// lut: the species' table (shared or global memory), lut_n entries
+__device__ __forceinline__ float3 amplitude(float I, float scalar, float h, const SpeciesDev &S, const float4 *lut)
 {
-    const SpeciesDev &S = fp.sp[s];
     float r = S.fixed_r, g = S.fixed_g, b = S.fixed_b;
     if (S.use_colormap) {
         float v = scalar;
@@ -335,10 +375,10 @@ __device__ __forceinline__ float3 amplitude(float I, float scalar, float h, int 
         t = (t > 0.0f) ? t : 0.0f;                 // NaN clamps to 0
         t = fminf(t, 1.0f);
         const float u = t * (float)(S.lut_n - 1);
-        const int i0 = min((int)floorf(u), S.lut_n - 2);
+        const int i0 = min((int)u, S.lut_n - 2);
         const float fr = u - (float)i0;
-        const float4 a = __ldg(fp.lut + s * kMaxLut + i0);
-        const float4 c = __ldg(fp.lut + s * kMaxLut + i0 + 1);
+        const float4 a = lut[i0];
+        const float4 c = lut[i0 + 1];
         r = fmaf(fr, c.x - a.x, a.x);
         g = fmaf(fr, c.y - a.y, a.y);
         b = fmaf(fr, c.z - a.z, a.z);
@@ -349,59 +389,83 @@ __device__ __forceinline__ float3 amplitude(float I, float scalar, float h, int 
 
 // Render record, 32 bytes: {px, py, c = -log2(e)/sp^2, rp | -1 for SMALL} {aR, aG, aB, zc}
 // MEDIUM / LARGE: a = E * col.   SMALL: a = E * col * pi sp^2 (1 - exp(-chi^2)) (the whole clipped flux).
-__device__ __forceinline__ void st_record(float4 *rec, unsigned int slot, float4 a, float4 b)
-{
-    rec[2ull * slot] = a;
-    rec[2ull * slot + 1] = b;
-}
-
+// A record whose amplitude is not finite (I or scalar = Inf / NaN) carries amplitude 0.
 template <bool ALIGNED>
-__global__ void __launch_bounds__(kBinThreads)
+__global__ void __launch_bounds__(kBinThreads, 2)
 k_scatter(const float *__restrict__ x, const float *__restrict__ y, const float *__restrict__ z,
           const float *__restrict__ h, const float *__restrict__ I, const float *__restrict__ scalar,
           unsigned long long n, unsigned long long per, const __grid_constant__ FrameParams fp,
           const unsigned int *__restrict__ counts, const unsigned int *__restrict__ bin_start,
-          const DeviceStats *__restrict__ stats, float4 *__restrict__ records)
+          DeviceStats *__restrict__ stats, float4 *__restrict__ records)
 {
-    extern __shared__ unsigned int cursor[];
+    extern __shared__ unsigned int cursor[];                 // nbins cursors, then the packed colour tables
+    __shared__ float s_amax[kBinThreads / 32];
     if (stats->overflow) return;
+    float4 *s_lut = reinterpret_cast<float4 *>(cursor + ((fp.nbins + 3) & ~3));
     const unsigned int *row = counts + (size_t)blockIdx.x * fp.nbins;
-    for (int i = threadIdx.x; i < fp.nbins; i += blockDim.x) cursor[i] = bin_start[i] + row[i];
+    for (int i = threadIdx.x; i < fp.nbins; i += kBinThreads) cursor[i] = bin_start[i] + row[i];
+    if (fp.lut_total > 0) {
+        for (int s = 0; s < fp.n_species; ++s)
+            if (fp.sp[s].use_colormap)
+                for (int i = threadIdx.x; i < fp.sp[s].lut_n; i += kBinThreads)
+                    s_lut[fp.sp[s].lut_off + i] = fp.lut[s * kMaxLut + i];
+    }
     __syncthreads();
     const unsigned long long lo = (unsigned long long)blockIdx.x * per;
-    const unsigned long long hi = min(n, lo + per);
-    for (unsigned long long i = lo + 4ull * threadIdx.x; i < hi; i += 4ull * blockDim.x) {
+    const unsigned int len = lo < n ? (unsigned int)min(n - lo, per) : 0u;
+    const unsigned int lo32 = (unsigned int)lo;
+    x += lo; y += lo; z += lo; h += lo; I += lo; scalar += lo;
+    // species of the block's first and last particle: most blocks lie inside one species
+    const int s_first = species_of(lo32, fp), s_last = species_of(lo32 + (len ? len - 1 : 0), fp);
+    float amax = 0.0f;
+    const bool one_species = s_first == s_last;
+    const unsigned int lane4 = 4u * (threadIdx.x & 31u);
+    for (unsigned int iw = 4u * (threadIdx.x & ~31u); iw < len; iw += 4u * kBinThreads) {
+        const unsigned int i = iw + lane4;
         float xs[4], ys[4], zs[4], hs[4], Is[4], ss[4];
-        load4<ALIGNED>(x, i, hi, xs);
-        load4<ALIGNED>(y, i, hi, ys);
-        load4<ALIGNED>(z, i, hi, zs);
-        load4<ALIGNED>(h, i, hi, hs);
-        load4<ALIGNED>(I, i, hi, Is);
-        load4<ALIGNED>(scalar, i, hi, ss);
+        load4<ALIGNED>(x, i, len, xs);
+        load4<ALIGNED>(y, i, len, ys);
+        load4<ALIGNED>(z, i, len, zs);
+        load4<ALIGNED>(h, i, len, hs);
+        load4<ALIGNED>(I, i, len, Is);
+        load4<ALIGNED>(scalar, i, len, ss);
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            if (i + j < hi) {
-                const Geo g = geometry(xs[j], ys[j], zs[j], hs[j], fp);
-                if (g.cls != CULLED) {
-                    float3 a = amplitude(Is[j], ss[j], hs[j], species_of(i + j, fp), fp);
-                    float4 ra, rb;
-                    ra.x = g.px; ra.y = g.py;
-                    if (g.cls == SMALL) {
-                        const float w = fp.csmall * (g.sp * g.sp);
-                        a.x *= w; a.y *= w; a.z *= w;
-                        ra.z = 0.0f; ra.w = -1.0f;
-                    } else {
-                        ra.z = __fdiv_rn(-1.4426950408889634f, __fmul_rn(g.sp, g.sp));
-                        ra.w = g.rp;
-                    }
-                    rb = make_float4(a.x, a.y, a.z, g.zc);
-                    for_each_bin(g, fp, [&](int bin) {
-                        const unsigned int slot = atomicAdd(&cursor[bin], 1u);
-                        st_record(records, slot, ra, rb);
-                    });
-                }
+            Geo g = geometry(xs[j], ys[j], zs[j], hs[j], fp);
+            if (!(i + j < len)) g.cls = CULLED;
+            const int s = one_species ? s_first : species_of(min(lo32 + i + j, lo32 + len - 1), fp);
+            const SpeciesDev &S = fp.sp[s];
+            const float4 *lut = fp.lut_total > 0 ? s_lut + S.lut_off : fp.lut + s * kMaxLut;
+            float3 a = amplitude(Is[j], ss[j], hs[j], S, lut);
+            const bool small = g.cls == SMALL;
+            const float w = small ? fp.csmall * (g.sp * g.sp) : 1.0f;
+            a.x *= w; a.y *= w; a.z *= w;
+            float4 ra, rb;
+            ra.x = g.px; ra.y = g.py;
+            ra.z = small ? 0.0f : __fdiv_rn(-1.4426950408889634f, __fmul_rn(g.sp, g.sp));
+            ra.w = small ? -1.0f : g.rp;
+            const float am = fmaxf(fabsf(a.x), fmaxf(fabsf(a.y), fabsf(a.z)));
+            if (!(am <= 3.0e38f)) a = make_float3(0.0f, 0.0f, 0.0f);             // Inf / NaN amplitude
+            else if (g.cls == SMALL || g.cls == MEDIUM) amax = fmaxf(amax, am);
+            rb = make_float4(a.x, a.y, a.z, g.zc);
+            const BinBox b = bin_box(g, fp);
+            const int nmax = __reduce_max_sync(0xffffffffu, b.n);
+            int bx = b.bx0, by = b.by0;
+            for (int t = 0; t < nmax; ++t) {
+                if (t < b.n) st_record(records, atomicAdd(&cursor[b.base + by * b.pitch + bx], 1u), ra, rb);
+                const bool wrap = bx == b.bx1;
+                bx = wrap ? b.bx0 : bx + 1;
+                by += wrap;
             }
         }
+    }
+    // largest SMALL / MEDIUM record amplitude of the frame: fixes the fixed-point scale of k_splat
+    amax = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(amax)));   // amax >= 0: bit order = value order
+    if ((threadIdx.x & 31) == 0) s_amax[threadIdx.x >> 5] = amax;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < kBinThreads / 32; ++w) amax = fmaxf(amax, s_amax[w]);
+        if (amax > 0.0f) atomicMax(&stats->amax_bits, __float_as_uint(amax));
     }
 }
 
@@ -413,138 +477,176 @@ __device__ __forceinline__ float ex2_approx(float x)
     return y;
 }
 
+__device__ __forceinline__ float rcp_approx(float x)
+{
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+__device__ __forceinline__ float pow2i(int e) { return __int_as_float((e + 127) << 23); }   // -126 <= e <= 127
+
+// Fixed-point exponent of the frame: contributions are accumulated in units of 2^-e, with the largest record
+// amplitude in [2^(kFixedBits-1), 2^kFixedBits).  Integer sums are exact and independent of the summation order.
+__device__ __forceinline__ int fixed_exponent(unsigned int amax_bits)
+{
+    if (amax_bits == 0u) return 0;
+    int ex = (int)(amax_bits >> 23) - 126;              // amax = m 2^ex, m in [0.5, 1) (subnormals: ex = -126, fine)
+    return kFixedBits - ex;
+}
+
 template <int T> struct SplatCfg {
-    static constexpr int kStride = T + 3;                       // float4 per framebuffer row (bank spreading)
-    static constexpr int kFbElems = T * kStride;                // float4 per warp-private framebuffer
-    static constexpr int kWarps = (T == 32) ? 4 : kSplatWarps;
-    static constexpr size_t kSmemBytes = sizeof(float4) * (size_t)kFbElems * kWarps;
+    static constexpr int kPix = T * T;
+    static constexpr int kWarps = kSplatThreads / 32;
+    static constexpr size_t kSmemBytes = sizeof(unsigned int) * 6 * kPix + sizeof(float4) * 2 * 32 * kWarps;
 };
 
-// One work item = up to kChunk consecutive records of one tile.  Every warp owns a private T x T RGB
-// framebuffer in shared memory and walks its share of the records: SMALL records are deposited one lane per
-// particle (lanes that hit the same pixel take turns), MEDIUM records one particle at a time with the lanes
-// spread over the pixels of its box, so there is never a concurrent update of one pixel and no atomics.
-// The warps' framebuffers are summed into the chunk's partial tile.
+// add the signed 32-bit value v to the 64-bit accumulator (lo, hi): one native shared-memory atomic, a second one
+// only on a carry / borrow out of the low word
+__device__ __forceinline__ void fixed_add(unsigned int *lo, unsigned int *hi, int v)
+{
+    if (v == 0) return;
+    const unsigned int uv = (unsigned int)v;
+    const unsigned int old = atomicAdd(lo, uv);
+    const int up = (v >> 31) + (int)((unsigned int)(old + uv) < uv);
+    if (up != 0) atomicAdd(hi, (unsigned int)up);
+}
+
+// One work item = chunk_size consecutive records; the chunk is cut into segments at tile boundaries.  For each
+// segment the CTA clears the tile framebuffer (64-bit fixed point, shared memory), every warp takes batches of 32
+// records, lays the fragments (pixels of the clipped boxes) of the batch end to end and hands 32 consecutive
+// fragments to its 32 lanes per step, so lanes stay busy whatever the footprint (1 pixel for SMALL records).
+// The segment's framebuffer goes to its partial slot; k_compose adds the slots of a tile.
 template <int T>
-__global__ void __launch_bounds__(SplatCfg<T>::kWarps * 32)
+__global__ void __launch_bounds__(kSplatThreads)
 k_splat(const float4 *__restrict__ records, const unsigned int *__restrict__ bin_start,
-        const uint2 *__restrict__ chunk_desc, DeviceStats *__restrict__ stats, float4 *__restrict__ partials,
-        const __grid_constant__ FrameParams fp)
+        const unsigned int *__restrict__ seg_start, const unsigned int *__restrict__ chunk_tile,
+        DeviceStats *__restrict__ stats, long long *__restrict__ partials, const __grid_constant__ FrameParams fp)
 {
     using Cfg = SplatCfg<T>;
-    constexpr int kStride = Cfg::kStride, kWarps = Cfg::kWarps, kThreads = kWarps * 32;
-    extern __shared__ float4 fb_all[];
+    constexpr int kPix = Cfg::kPix;
+    extern __shared__ __align__(16) unsigned int smem_u[];
+    unsigned int *fb_lo = smem_u, *fb_hi = smem_u + 3 * kPix;
+    float4 *stage_all = reinterpret_cast<float4 *>(smem_u + 6 * kPix);
     __shared__ unsigned int s_chunk;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    float4 *fb = fb_all + warp * Cfg::kFbElems;
+    float4 *stage = stage_all + warp * 64;
+    const unsigned int lane_lt = (1u << lane) - 1u, lane_le = 0xffffffffu >> (31 - lane);
     const unsigned int total = (unsigned int)stats->chunks;
+    const unsigned int K = stats->chunk_size;
+    const unsigned int pairs = (unsigned int)stats->pairs;
+    const int e = fixed_exponent(stats->amax_bits);
+    const float sc1 = pow2i(e / 2), sc2 = pow2i(e - e / 2);
     for (;;) {
+        __syncthreads();
         if (threadIdx.x == 0) s_chunk = atomicAdd(&stats->work_counter, 1u);
-        for (int i = threadIdx.x; i < Cfg::kFbElems * kWarps; i += kThreads) fb_all[i] = make_float4(0.f, 0.f, 0.f, 0.f);
         __syncthreads();
         const unsigned int chunk = s_chunk;
         if (chunk >= total) break;
-        const uint2 d = chunk_desc[chunk];
-        const int tile = (int)d.x;
-        const unsigned int begin = bin_start[tile] + d.y * kChunk;
-        const unsigned int end = min(begin + (unsigned int)kChunk, bin_start[tile + 1]);
-        const int tx0 = (tile % fp.ntx) * T, ty0 = (tile / fp.ntx) * T;
-        const float ftx0 = (float)tx0, fty0 = (float)ty0;
-        const float ftx1 = (float)min(tx0 + T - 1, fp.W - 1), fty1 = (float)min(ty0 + T - 1, fp.H - 1);
-        for (unsigned int base = begin + warp * 32; base < end; base += kThreads) {
-            const unsigned int idx = base + lane;
-            const bool valid = idx < end;
-            float4 ra = make_float4(0.f, 0.f, 0.f, 0.f), rb = ra;
-            if (valid) { ra = __ldg(records + 2ull * idx); rb = __ldg(records + 2ull * idx + 1); }
-            const bool is_small = valid && ra.w < 0.0f;
-            // ---- SMALL: one lane per particle; equal pixels within the warp take turns
-            if (__any_sync(0xffffffffu, is_small)) {
-                const int pix = is_small ? ((int)floorf(ra.y) - ty0) * kStride + ((int)floorf(ra.x) - tx0)
-                                         : (0x100000 + lane);
-                unsigned int grp = __match_any_sync(0xffffffffu, pix);
-                bool pending = is_small;
-                while (__any_sync(0xffffffffu, pending)) {
-                    const int leader = __ffs(grp) - 1;            // lowest lane of my pixel group still waiting
-                    if (pending && lane == leader) {
-                        float4 v = fb[pix];
-                        v.x += rb.x; v.y += rb.y; v.z += rb.z;
-                        fb[pix] = v;
-                        pending = false;
+        const unsigned int r0 = chunk * K, r1 = min(r0 + K, pairs);
+        int tile = (int)chunk_tile[chunk];
+        unsigned int tb = bin_start[tile], te = bin_start[tile + 1];
+        for (;;) {
+            // ---- segment = [max(tb, r0), min(te, r1)) of `tile`
+            const unsigned int begin = max(tb, r0), end = min(te, r1);
+            for (int i = threadIdx.x; i < 6 * kPix; i += kSplatThreads) smem_u[i] = 0u;
+            __syncthreads();
+            const int tx0 = (tile % fp.ntx) * T, ty0 = (tile / fp.ntx) * T;
+            const float ftx0 = (float)tx0, fty0 = (float)ty0;
+            const float ftx1 = (float)min(tx0 + T - 1, fp.W - 1), fty1 = (float)min(ty0 + T - 1, fp.H - 1);
+            for (unsigned int base = begin + warp * 32; base < end; base += kSplatThreads) {
+                const unsigned int idx = base + lane;
+                const bool valid = idx < end;
+                float4 ra = make_float4(0.f, 0.f, 0.f, 0.f), rb = ra;
+                if (valid) ld_record(records, idx, ra, rb);
+                const bool is_small = ra.w < 0.0f;
+                int bx0 = 0, by0 = 0, bw = 0, bh = 0;
+                if (valid) {
+                    if (is_small) {
+                        bx0 = (int)ra.x - tx0; by0 = (int)ra.y - ty0; bw = bh = 1;
+                    } else {        // clip the pixel box to the tile (same float32 formulas as the classification stage)
+                        const float fx0 = fmaxf(ceilf(__fsub_rn(__fsub_rn(ra.x, ra.w), 0.5f)), ftx0);
+                        const float fx1 = fminf(floorf(__fsub_rn(__fadd_rn(ra.x, ra.w), 0.5f)), ftx1);
+                        const float fy0 = fmaxf(ceilf(__fsub_rn(__fsub_rn(ra.y, ra.w), 0.5f)), fty0);
+                        const float fy1 = fminf(floorf(__fsub_rn(__fadd_rn(ra.y, ra.w), 0.5f)), fty1);
+                        if (fx0 <= fx1 && fy0 <= fy1) {
+                            bx0 = (int)fx0 - tx0; by0 = (int)fy0 - ty0;
+                            bw = (int)fx1 - (int)fx0 + 1; bh = (int)fy1 - (int)fy0 + 1;
+                        }
                     }
-                    grp &= grp - 1u;                              // drop that lane (no-op once the group is empty)
-                    __syncwarp();
                 }
-            }
-            // ---- MEDIUM: clip the pixel box to the tile (same float32 formulas as the classification stage)
-            int bx0 = 0, by0 = 0, bw = 0, bh = 0;
-            if (valid && !is_small) {
-                const float fx0 = fmaxf(ceilf(__fsub_rn(__fsub_rn(ra.x, ra.w), 0.5f)), ftx0);
-                const float fx1 = fminf(floorf(__fsub_rn(__fadd_rn(ra.x, ra.w), 0.5f)), ftx1);
-                const float fy0 = fmaxf(ceilf(__fsub_rn(__fsub_rn(ra.y, ra.w), 0.5f)), fty0);
-                const float fy1 = fminf(floorf(__fsub_rn(__fadd_rn(ra.y, ra.w), 0.5f)), fty1);
-                if (fx0 <= fx1 && fy0 <= fy1) {
-                    bx0 = (int)fx0; by0 = (int)fy0;
-                    bw = (int)fx1 - bx0 + 1; bh = (int)fy1 - by0 + 1;
+                const int nfrag = bw * bh;
+                int incl = nfrag;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int t = __shfl_up_sync(0xffffffffu, incl, o);
+                    if (lane >= o) incl += t;
                 }
-            }
-            const int packed = (bx0 - tx0) | ((by0 - ty0) << 8) | (bw << 16) | (bh << 24);
-            unsigned int med = __ballot_sync(0xffffffffu, bw > 0);
-            while (med) {
-                const int src = __ffs(med) - 1;
-                med &= med - 1;
-                const float ppx = __shfl_sync(0xffffffffu, ra.x, src);
-                const float ppy = __shfl_sync(0xffffffffu, ra.y, src);
-                const float pc = __shfl_sync(0xffffffffu, ra.z, src);
-                const float prp = __shfl_sync(0xffffffffu, ra.w, src);
-                const float aR = __shfl_sync(0xffffffffu, rb.x, src);
-                const float aG = __shfl_sync(0xffffffffu, rb.y, src);
-                const float aB = __shfl_sync(0xffffffffu, rb.z, src);
-                const int pk = __shfl_sync(0xffffffffu, packed, src);
-                const int lx0 = pk & 0xff, ly0 = (pk >> 8) & 0xff, w = (pk >> 16) & 0xff, hgt = (pk >> 24) & 0xff;
-                const int npx = w * hgt;
-                const float inv_w = 1.0f / (float)w;
-                const float r2 = __fmul_rn(prp, prp);
-                for (int k = lane; k < npx; k += 32) {
-                    const int j = (int)(((float)k + 0.5f) * inv_w);
-                    const int i = k - j * w;
-                    const int lx = lx0 + i, ly = ly0 + j;
-                    const float dxf = __fsub_rn(__fadd_rn((float)(tx0 + lx), 0.5f), ppx);
-                    const float dyf = __fsub_rn(__fadd_rn((float)(ty0 + ly), 0.5f), ppy);
-                    const float d2 = __fmaf_rn(dxf, dxf, __fmul_rn(dyf, dyf));
-                    if (d2 <= r2) {
-                        const float wgt = ex2_approx(d2 * pc);
-                        float4 *q = fb + ly * kStride + lx;
-                        float4 v = *q;
-                        v.x = fmaf(aR, wgt, v.x); v.y = fmaf(aG, wgt, v.y); v.z = fmaf(aB, wgt, v.z);
-                        *q = v;
+                const int start = incl - nfrag;
+                const int F = __shfl_sync(0xffffffffu, incl, 31);
+                const bool nonempty = nfrag > 0;
+                const unsigned int ne_mask = __ballot_sync(0xffffffffu, nonempty);
+                if (nonempty) {
+                    const int slot = __popc(ne_mask & lane_lt);
+                    const unsigned int pack = (unsigned int)start | ((unsigned int)bx0 << 15) | ((unsigned int)by0 << 20) |
+                                              ((unsigned int)(bw - 1) << 25) | (is_small ? 0x40000000u : 0u);
+                    stage[2 * slot] = make_float4(ra.x, ra.y, ra.z, __fmul_rn(ra.w, ra.w));
+                    stage[2 * slot + 1] = make_float4(rb.x * sc1 * sc2, rb.y * sc1 * sc2, rb.z * sc1 * sc2, __uint_as_float(pack));
+                }
+                __syncwarp();
+                for (int f0 = 0; f0 < F; f0 += 32) {
+                    const int rel = start - f0;
+                    const unsigned int m = __reduce_or_sync(0xffffffffu, (nonempty && rel >= 0 && rel < 32) ? (1u << rel) : 0u);
+                    const int nb = __popc(__ballot_sync(0xffffffffu, nonempty && rel < 0));
+                    const int f = f0 + lane;
+                    if (f < F) {
+                        const int s = nb - 1 + __popc(m & lane_le);
+                        const float4 A = stage[2 * s], B = stage[2 * s + 1];
+                        const unsigned int pack = __float_as_uint(B.w);
+                        const int k = f - (int)(pack & 0x7fffu);
+                        const int w = (int)((pack >> 25) & 31u) + 1;
+                        const int j = (int)(((float)k + 0.5f) * rcp_approx((float)w));
+                        const int lx = (int)((pack >> 15) & 31u) + (k - j * w), ly = (int)((pack >> 20) & 31u) + j;
+                        float wgt = 1.0f;
+                        bool inside = true;
+                        if (!(pack & 0x40000000u)) {
+                            const float dxf = __fsub_rn(__fadd_rn((float)(tx0 + lx), 0.5f), A.x);
+                            const float dyf = __fsub_rn(__fadd_rn((float)(ty0 + ly), 0.5f), A.y);
+                            const float d2 = __fmaf_rn(dxf, dxf, __fmul_rn(dyf, dyf));
+                            inside = d2 <= A.w;
+                            wgt = ex2_approx(d2 * A.z);
+                        }
+                        if (inside) {
+                            const int p = ly * T + lx;
+                            fixed_add(fb_lo + p, fb_hi + p, __float2int_rn(B.x * wgt));
+                            fixed_add(fb_lo + kPix + p, fb_hi + kPix + p, __float2int_rn(B.y * wgt));
+                            fixed_add(fb_lo + 2 * kPix + p, fb_hi + 2 * kPix + p, __float2int_rn(B.z * wgt));
+                        }
                     }
                 }
                 __syncwarp();
             }
+            __syncthreads();
+            // ---- flush the segment's framebuffer to its partial slot
+            const unsigned int seg = seg_start[tile] + (chunk - tb / K);
+            long long *out = partials + (size_t)seg * (3 * kPix);
+            for (int i = threadIdx.x; i < 3 * kPix; i += kSplatThreads)
+                out[i] = (long long)(((unsigned long long)fb_hi[i] << 32) | fb_lo[i]);
+            if (te >= r1) break;
+            // ---- next non-empty tile
+            do { ++tile; tb = te; te = bin_start[tile + 1]; } while (te == tb);
+            __syncthreads();
         }
-        __syncthreads();
-        float4 *out = partials + (size_t)chunk * (T * T);
-        for (int p = threadIdx.x; p < T * T; p += kThreads) {
-            const int yy = p / T, xx = p % T;
-            float4 s = fb_all[yy * kStride + xx];
-#pragma unroll
-            for (int w = 1; w < kWarps; ++w) {
-                const float4 v = fb_all[w * Cfg::kFbElems + yy * kStride + xx];
-                s.x += v.x; s.y += v.y; s.z += v.z;
-            }
-            out[p] = s;
-        }
-        __syncthreads();
     }
 }
 
 // ---- A6 + A8: compose one tile ----------------------------------------------------------------------------------
-// Thread t owns pixels t, t+256, ... of the tile (registers).  Sums the chunk partials in chunk order, then
-// gathers the LARGE records of the tile's super-tile (each record is tested against the tile, survivors are
-// staged in shared memory and evaluated by every pixel owner), in two-level float32 accumulation.
+// Thread t owns pixels t, t+256, ... of the tile (registers).  Adds the tile's segment partials (64-bit integers,
+// exact), then gathers the LARGE records of the tile's super-tile (each record is tested against the tile,
+// survivors are staged in shared memory and evaluated by every pixel owner), in two-level float32 accumulation.
 template <int T>
 __global__ void __launch_bounds__(256)
-k_compose(const float4 *__restrict__ partials, const unsigned int *__restrict__ chunk_start,
+k_compose(const long long *__restrict__ partials, const unsigned int *__restrict__ seg_start,
           const float4 *__restrict__ records, const unsigned int *__restrict__ bin_start,
           const DeviceStats *__restrict__ stats, const __grid_constant__ FrameParams fp,
           float *__restrict__ image)
@@ -557,10 +659,12 @@ k_compose(const float4 *__restrict__ partials, const unsigned int *__restrict__ 
     const int tx = tile % fp.ntx, ty = tile / fp.ntx;
     const int tx0 = tx * T, ty0 = ty * T;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    long long fix[kPpt][3];
     float acc[kPpt][3], sub[kPpt][3], fxc[kPpt], fyc[kPpt];
 #pragma unroll
     for (int k = 0; k < kPpt; ++k) {
         const int p = threadIdx.x + k * 256;
+        fix[k][0] = fix[k][1] = fix[k][2] = 0ll;
         acc[k][0] = acc[k][1] = acc[k][2] = 0.0f;
         sub[k][0] = sub[k][1] = sub[k][2] = 0.0f;
         fxc[k] = __fadd_rn((float)(tx0 + p % T), 0.5f);
@@ -568,14 +672,15 @@ k_compose(const float4 *__restrict__ partials, const unsigned int *__restrict__ 
     }
     const bool ok = stats->overflow == 0u;
     if (ok) {
-        const unsigned int c0 = chunk_start[tile], c1 = chunk_start[tile + 1];
-        for (unsigned int ch = c0; ch < c1; ++ch) {
+        const unsigned int s0 = seg_start[tile], s1 = seg_start[tile + 1];
+        for (unsigned int sg = s0; sg < s1; ++sg) {
 #pragma unroll
             for (int k = 0; k < kPpt; ++k) {
                 const int p = threadIdx.x + k * 256;
                 if (p < kPix) {
-                    const float4 v = __ldg(partials + (size_t)ch * kPix + p);
-                    acc[k][0] += v.x; acc[k][1] += v.y; acc[k][2] += v.z;
+                    const long long *q = partials + (size_t)sg * (3 * kPix) + p;
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) fix[k][c] += __ldg(q + c * kPix);
                 }
             }
         }
@@ -589,8 +694,7 @@ k_compose(const float4 *__restrict__ partials, const unsigned int *__restrict__ 
             bool hit = false;
             float4 ra, rb;
             if (idx < le) {
-                ra = __ldg(records + 2ull * idx);
-                rb = __ldg(records + 2ull * idx + 1);
+                ld_record(records, idx, ra, rb);
                 const float fx0 = ceilf(__fsub_rn(__fsub_rn(ra.x, ra.w), 0.5f));
                 const float fx1 = floorf(__fsub_rn(__fadd_rn(ra.x, ra.w), 0.5f));
                 const float fy0 = ceilf(__fsub_rn(__fsub_rn(ra.y, ra.w), 0.5f));
@@ -640,6 +744,7 @@ k_compose(const float4 *__restrict__ partials, const unsigned int *__restrict__ 
 #pragma unroll
             for (int c = 0; c < 3; ++c) acc[k][c] += sub[k][c];
     }
+    const double unit = ldexp(1.0, -fixed_exponent(stats->amax_bits));       // one fixed-point unit
 #pragma unroll
     for (int k = 0; k < kPpt; ++k) {
         const int p = threadIdx.x + k * 256;
@@ -647,7 +752,10 @@ k_compose(const float4 *__restrict__ partials, const unsigned int *__restrict__ 
         if (p < kPix && ix < fp.W && iy < fp.H) {
             float *o = image + 3ull * ((size_t)iy * fp.W + ix);
 #pragma unroll
-            for (int c = 0; c < 3; ++c) o[c] = fp.apply_transfer ? -expm1f(-acc[k][c]) : acc[k][c];
+            for (int c = 0; c < 3; ++c) {
+                const float v = (float)((double)fix[k][c] * unit + (double)acc[k][c]);
+                o[c] = fp.apply_transfer ? -expm1f(-v) : v;
+            }
         }
     }
 }
