@@ -97,7 +97,7 @@ bool make_layout(const splotch_ctx *c, unsigned long long n, int T, unsigned lon
     const int ntx = (c->width + T - 1) / T, nty = (c->height + T - 1) / T;
     const size_t n_tiles = (size_t)ntx * nty;
     const size_t nbins = hist_bytes(c->width, c->height, T) / sizeof(unsigned int);
-    const size_t partial_bytes = sizeof(long long) * 3 * (size_t)T * T;     // one segment's framebuffer
+    const size_t partial_bytes = sizeof(unsigned int) * 6 * (size_t)T * T;  // one segment's framebuffer (lo, hi planes x RGB)
     L->nrows = bin_rows(c, T);
     size_t off = 0;
     L->counts = off;      off = align_up(off + sizeof(unsigned int) * nbins * L->nrows, 256);
@@ -164,6 +164,7 @@ int check_params(splotch_ctx *c, const splotch_particles *p, unsigned long long 
     memcpy(fp->cam, c->cam, sizeof fp->cam);
     fp->chi = q->chi; fp->r_small = q->r_small; fp->r_large = q->r_large; fp->z_near = q->z_near;
     fp->W = c->width; fp->H = c->height; fp->fW = (float)c->width; fp->fH = (float)c->height;
+    fp->fWm1 = (float)(c->width - 1); fp->fHm1 = (float)(c->height - 1);
     fp->csmall = (float)(3.14159265358979323846 * (1.0 - exp(-(double)q->chi * (double)q->chi)));
     fp->T = q->tile; fp->tshift = ts;
     fp->ntx = (c->width + q->tile - 1) / q->tile; fp->nty = (c->height + q->tile - 1) / q->tile;
@@ -190,8 +191,10 @@ int check_params(splotch_ctx *c, const splotch_particles *p, unsigned long long 
         d.brightness = sp.brightness; d.absorb = sp.absorb;
         d.fixed_r = sp.fixed_rgb[0]; d.fixed_g = sp.fixed_rgb[1]; d.fixed_b = sp.fixed_rgb[2];
         d.use_colormap = sp.use_colormap ? 1 : 0; d.use_log10 = sp.scalar_log10 ? 1 : 0;
-        d.smin = sp.scalar_min; d.range = sp.scalar_max - sp.scalar_min;
+        d.smin = sp.scalar_min;
+        d.inv_range = (float)(1.0 / ((double)sp.scalar_max - (double)sp.scalar_min));
         d.lut_n = c->lut_n[s];
+        d.lut_nm1 = (float)(d.lut_n - 1); d.lut_nm2 = (float)(d.lut_n - 2);
         d.lut_off = lut_total;
         if (d.use_colormap) lut_total += d.lut_n;
         if (d.use_colormap) {
@@ -217,9 +220,9 @@ int launch_render_tail(splotch_ctx *c, const Layout &L, char *ws, const FramePar
     const int grid = c->n_sm * c->splat_blocks_per_sm[ti];
     k_splat<T><<<grid, kSplatThreads, SplatCfg<T>::kSmemBytes, st>>>(
         (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.bin_start), (const unsigned int *)(ws + L.seg_start),
-        (const unsigned int *)(ws + L.chunk_tile), (DeviceStats *)(ws + L.stats), (long long *)(ws + L.partials), fp);
+        (const unsigned int *)(ws + L.chunk_tile), (DeviceStats *)(ws + L.stats), (unsigned int *)(ws + L.partials), fp);
     if (c->profiling) cudaEventRecord(c->ev[5], st);
-    k_compose<T><<<fp.n_tiles, 256, 0, st>>>((const long long *)(ws + L.partials), (const unsigned int *)(ws + L.seg_start),
+    k_compose<T><<<fp.n_tiles, 256, 0, st>>>((const unsigned int *)(ws + L.partials), (const unsigned int *)(ws + L.seg_start),
                                              (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.bin_start),
                                              (const DeviceStats *)(ws + L.stats), fp, image);
     if (c->profiling) cudaEventRecord(c->ev[6], st);

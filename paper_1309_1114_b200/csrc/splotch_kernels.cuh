@@ -7,9 +7,10 @@
 //   k_scatter  A1-A3+A2+A4d  recompute geometry, colourise (:76, :85), write 32-byte render records in bin order
 //                            (replaces copy_if + sort_by_key, :196-202)
 //   k_splat    A5         SMALL + MEDIUM records of one chunk: all fragments of 32 records are spread over the 32 lanes
-//                         of a warp and accumulated into the tile's 64-bit fixed-point framebuffer in shared memory
-//                         with native integer atomics (the paper's medium-particle kernel, :183, :224-228, without
-//                         its halo copies and without idle threads for small footprints)
+//                         of a warp and accumulated into the tile's fixed-point framebuffer in shared memory (two
+//                         32-bit planes per channel, native integer atomics without return; the paper's
+//                         medium-particle kernel, :183, :224-228, without its halo copies and without idle threads
+//                         for small footprints)
 //   k_compose  A6+A8      per tile: sum segment partials (exact integer sums), gather the LARGE particles of the
 //                         tile's super-tile (the paper renders these on the CPU, :232-238), optional 1-exp(-S),
 //                         write the image once
@@ -17,6 +18,9 @@
 // Canonical float32 geometry: every operation that decides an integer (class, pixel box, tile box, the inside
 // test) is written with round-to-nearest intrinsics (__fmul_rn, __fmaf_rn, __fdiv_rn ...) which nvcc never
 // contracts or reorders, so the values equal those of any IEEE-754 binary32 implementation of the same sequence.
+// floor / ceil / float->int of the (clamped) box bounds are taken with the 1.5 * 2^23 addition trick: exact for
+// arguments in [-1, 32768], and on the FMA / ALU pipes instead of the quarter-rate conversion pipe (FRND, F2I),
+// which bounded the first version of every kernel here (profiles/r1_step1_*).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -25,7 +29,7 @@ namespace splotch {
 
 constexpr int kMaxSpecies   = 8;
 constexpr int kMaxLut       = 1024;
-constexpr int kChunkMax     = 4096;   // records per work item of k_splat (upper bound; the frame picks its own)
+constexpr int kChunkMax     = 32768;  // records per work item of k_splat (upper bound; the frame picks its own)
 constexpr int kChunkMin     = 512;
 constexpr int kSplatThreads = 256;
 constexpr int kBinThreads   = 512;    // k_count / k_scatter block size
@@ -38,14 +42,15 @@ enum { CULLED = 0, SMALL = 1, MEDIUM = 2, LARGE = 3 };
 struct SpeciesDev {
     float brightness, absorb;
     float fixed_r, fixed_g, fixed_b;
-    float smin, range;
+    float smin, inv_range;                           // t = (v - smin) * inv_range
+    float lut_nm1, lut_nm2;                          // (float)(lut_n - 1), (float)(lut_n - 2)
     int   use_colormap, use_log10, lut_n, lut_off;   // lut_off: first entry in the packed shared-memory table
 };
 
 struct FrameParams {
     float cam[16];               // r[3] u[3] f[3] eye[3] s cx cy 0
     float chi, r_small, r_large, z_near;
-    float fW, fH;
+    float fW, fH, fWm1, fHm1;
     float csmall;                // pi (1 - exp(-chi^2)): flux of the clipped unit Gaussian per sigma_px^2
     int   W, H, T, tshift;
     int   ntx, nty, n_tiles;
@@ -74,9 +79,26 @@ __device__ __forceinline__ float dot3(const float *a, float dx, float dy, float 
     return __fmaf_rn(a[2], dz, __fmaf_rn(a[1], dy, __fmul_rn(a[0], dx)));
 }
 
+constexpr float kMagic     = 12582912.0f;     // 1.5 * 2^23: v + kMagic has ulp 1 for |v| < 2^22
+constexpr int   kMagicBits = 0x4B400000;
+
+// round-to-nearest-even integer of v in [-1, 32768] and the float it came from: r = rint(v), i = (int)r
+__device__ __forceinline__ int rint_small(float v, float &r)
+{
+    const float t = __fadd_rn(v, kMagic);
+    r = __fsub_rn(t, kMagic);
+    return __float_as_int(t) - kMagicBits;
+}
+__device__ __forceinline__ int floor_small(float v) { float r; const int i = rint_small(v, r); return i - (r > v ? 1 : 0); }
+__device__ __forceinline__ int ceil_small(float v)  { float r; const int i = rint_small(v, r); return i + (r < v ? 1 : 0); }
+
 // C1 of DESIGN.md: the canonical float32 sequence (PAPER.md:76 projection, Eq. 7 :138 radius, :156-160 classes).
 // Written without branches (every lane evaluates both the SMALL and the box formulas and selects): the warps of
-// the streaming kernels stay converged whatever the mix of classes.
+// the streaming kernels stay converged whatever the mix of classes.  The box bounds are clamped to the screen
+// BEFORE rounding, which gives the same integers as C1's "round, then clamp" (floor and ceil are monotonic, the
+// clamp limits are integers, fminf / fmaxf drop a NaN operand on both sides) and keeps the rounding argument in
+// the range where the addition trick is exact; a lower bound beyond the screen becomes W (H): the box is empty
+// either way.
 __device__ __forceinline__ Geo geometry(float x, float y, float z, float h, const FrameParams &fp)
 {
     Geo g;
@@ -93,19 +115,26 @@ __device__ __forceinline__ Geo geometry(float x, float y, float z, float h, cons
     ok = ok && g.rp >= 0.0f && g.rp <= 3.0e38f;
     const bool small = g.rp <= fp.r_small;
     const bool s_ok = g.px >= 0.0f && g.px < fp.fW && g.py >= 0.0f && g.py < fp.fH;
-    const float fx0 = fmaxf(ceilf(__fsub_rn(__fsub_rn(g.px, g.rp), 0.5f)), 0.0f);
-    const float fx1 = fmaxf(fminf(floorf(__fsub_rn(__fadd_rn(g.px, g.rp), 0.5f)), __fsub_rn(fp.fW, 1.0f)), -1.0f);
-    const float fy0 = fmaxf(ceilf(__fsub_rn(__fsub_rn(g.py, g.rp), 0.5f)), 0.0f);
-    const float fy1 = fmaxf(fminf(floorf(__fsub_rn(__fadd_rn(g.py, g.rp), 0.5f)), __fsub_rn(fp.fH, 1.0f)), -1.0f);
-    const bool b_ok = fx0 <= fx1 && fy0 <= fy1;
+    // lower bounds: SMALL floor(p), else ceil((p - rp) - 0.5); one rounding serves both
+    const float ax = small ? g.px : __fsub_rn(__fsub_rn(g.px, g.rp), 0.5f);
+    const float ay = small ? g.py : __fsub_rn(__fsub_rn(g.py, g.rp), 0.5f);
+    const float axc = fminf(fmaxf(ax, 0.0f), fp.fW), ayc = fminf(fmaxf(ay, 0.0f), fp.fH);
+    float rx, ry;
+    const int ix = rint_small(axc, rx), iy = rint_small(ayc, ry);
+    const int x0 = ix + (small ? -(int)(rx > axc) : (int)(rx < axc));
+    const int y0 = iy + (small ? -(int)(ry > ayc) : (int)(ry < ayc));
+    // upper bounds: floor((p + rp) - 0.5) clamped to [-1, W - 1]
+    const float bxc = fmaxf(fminf(__fsub_rn(__fadd_rn(g.px, g.rp), 0.5f), fp.fWm1), -1.0f);
+    const float byc = fmaxf(fminf(__fsub_rn(__fadd_rn(g.py, g.rp), 0.5f), fp.fHm1), -1.0f);
+    const int x1 = floor_small(bxc), y1 = floor_small(byc);
+    const bool b_ok = x0 <= x1 && y0 <= y1;
     const int big = (g.rp <= fp.r_large) ? MEDIUM : LARGE;
     g.cls = ok ? (small ? (s_ok ? SMALL : CULLED) : (b_ok ? big : CULLED)) : CULLED;
     const bool act = g.cls != CULLED;
-    const int ipx = __float2int_rz(g.px), ipy = __float2int_rz(g.py);          // px, py >= 0 when SMALL: truncation is floor
-    g.x0 = act ? (small ? ipx : __float2int_rz(fx0)) : 0;
-    g.x1 = act ? (small ? ipx : __float2int_rz(fx1)) : -1;
-    g.y0 = act ? (small ? ipy : __float2int_rz(fy0)) : 0;
-    g.y1 = act ? (small ? ipy : __float2int_rz(fy1)) : -1;
+    g.x0 = act ? x0 : 0;
+    g.x1 = act ? (small ? x0 : x1) : -1;
+    g.y0 = act ? y0 : 0;
+    g.y1 = act ? (small ? y0 : y1) : -1;
     return g;
 }
 
@@ -194,7 +223,7 @@ k_count(const float *__restrict__ x, const float *__restrict__ y, const float *_
     const unsigned long long lo = (unsigned long long)blockIdx.x * per;
     const unsigned int len = lo < n ? (unsigned int)min(n - lo, per) : 0u;
     x += lo; y += lo; z += lo; h += lo;
-    unsigned int c1 = 0, c2 = 0, c3 = 0, c0 = 0;
+    unsigned int c1 = 0, c2 = 0, c3 = 0;          // per-warp class counts (every lane holds the same value)
     // the loop bound is the same for the 32 lanes of a warp (lanes past the end idle), so warps stay converged
     const unsigned int lane4 = 4u * (threadIdx.x & 31u);
     for (unsigned int iw = 4u * (threadIdx.x & ~31u); iw < len; iw += 4u * kBinThreads) {
@@ -207,27 +236,31 @@ k_count(const float *__restrict__ x, const float *__restrict__ y, const float *_
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             Geo g = geometry(xs[j], ys[j], zs[j], hs[j], fp);
-            const bool live = i + j < len;
-            if (!live) g.cls = CULLED;
-            c0 += (live && g.cls == CULLED); c1 += (g.cls == SMALL); c2 += (g.cls == MEDIUM); c3 += (g.cls == LARGE);
+            if (!(i + j < len)) { g.cls = CULLED; g.x1 = -1; g.y1 = -1; g.x0 = 0; g.y0 = 0; }
+            c1 += __popc(__ballot_sync(0xffffffffu, g.cls == SMALL));
+            c2 += __popc(__ballot_sync(0xffffffffu, g.cls == MEDIUM));
+            c3 += __popc(__ballot_sync(0xffffffffu, g.cls == LARGE));
             const BinBox b = bin_box(g, fp);
-            const int nmax = __reduce_max_sync(0xffffffffu, b.n);
-            int bx = b.bx0, by = b.by0;
-            for (int t = 0; t < nmax; ++t) {
-                if (t < b.n) atomicAdd(&hist[b.base + by * b.pitch + bx], 1u);
-                const bool wrap = bx == b.bx1;
-                bx = wrap ? b.bx0 : bx + 1;
-                by += wrap;
+            // most particles cover one bin: one atomic for everybody, the walk over the rest only where needed
+            if (b.n > 0) atomicAdd(&hist[b.base + b.by0 * b.pitch + b.bx0], 1u);
+            if (__any_sync(0xffffffffu, b.n > 1)) {
+                const int nmax = __reduce_max_sync(0xffffffffu, b.n);
+                int bx = b.bx0, by = b.by0;
+                for (int t = 1; t < nmax; ++t) {
+                    const bool wrap = bx == b.bx1;
+                    bx = wrap ? b.bx0 : bx + 1;
+                    by += wrap;
+                    if (t < b.n) atomicAdd(&hist[b.base + by * b.pitch + bx], 1u);
+                }
             }
         }
     }
-    c0 = warp_sum(c0); c1 = warp_sum(c1); c2 = warp_sum(c2); c3 = warp_sum(c3);
-    if ((threadIdx.x & 31) == 0) {
-        atomicAdd(&s_cls[0], c0); atomicAdd(&s_cls[1], c1); atomicAdd(&s_cls[2], c2); atomicAdd(&s_cls[3], c3);
-    }
+    if ((threadIdx.x & 31) == 0) { atomicAdd(&s_cls[1], c1); atomicAdd(&s_cls[2], c2); atomicAdd(&s_cls[3], c3); }
     __syncthreads();
     unsigned int *row = counts + (size_t)blockIdx.x * fp.nbins;
     for (int i = threadIdx.x; i < fp.nbins; i += kBinThreads) row[i] = hist[i];
+    if (threadIdx.x == 0) s_cls[0] = len - s_cls[1] - s_cls[2] - s_cls[3];
+    __syncthreads();
     if (threadIdx.x < 4) cls_counts[blockIdx.x * 4 + threadIdx.x] = s_cls[threadIdx.x];
 }
 
@@ -364,19 +397,24 @@ __device__ __forceinline__ int species_of(unsigned int i, const FrameParams &fp)
     return s;
 }
 
-// lut: the species' table (shared or global memory), lut_n entries
+// lut: the species' table (shared or global memory), lut_n entries.  Colour and amplitude are continuous in the
+// inputs (no integer is decided here beyond the table cell), so plain float32 with a reciprocal range is enough.
 __device__ __forceinline__ float3 amplitude(float I, float scalar, float h, const SpeciesDev &S, const float4 *lut)
 {
     float r = S.fixed_r, g = S.fixed_g, b = S.fixed_b;
     if (S.use_colormap) {
         float v = scalar;
         if (S.use_log10) v = log10f(v);
-        float t = (v - S.smin) / S.range;
+        float t = (v - S.smin) * S.inv_range;
         t = (t > 0.0f) ? t : 0.0f;                 // NaN clamps to 0
         t = fminf(t, 1.0f);
-        const float u = t * (float)(S.lut_n - 1);
-        const int i0 = min((int)u, S.lut_n - 2);
-        const float fr = u - (float)i0;
+        const float u = t * S.lut_nm1;             // 0 <= u <= lut_n - 1 <= 1023
+        float ru;
+        int i0 = rint_small(u, ru);
+        const bool up = ru > u;                    // rint rounded up: floor is one below
+        i0 = min(i0 - (up ? 1 : 0), S.lut_n - 2);
+        const float f0 = fminf(ru - (up ? 1.0f : 0.0f), S.lut_nm2);
+        const float fr = u - f0;
         const float4 a = lut[i0];
         const float4 c = lut[i0 + 1];
         r = fmaf(fr, c.x - a.x, a.x);
@@ -387,9 +425,26 @@ __device__ __forceinline__ float3 amplitude(float I, float scalar, float h, cons
     return make_float3(r * col, g * col, b * col);
 }
 
-// Render record, 32 bytes: {px, py, c = -log2(e)/sp^2, rp | -1 for SMALL} {aR, aG, aB, zc}
-// MEDIUM / LARGE: a = E * col.   SMALL: a = E * col * pi sp^2 (1 - exp(-chi^2)) (the whole clipped flux).
+// Render record, 32 bytes: {px, py, c, r2} {aR, aG, aB, box}
+//   MEDIUM / LARGE: c = -log2(e) / sp^2, r2 = rp^2 (float32, the C1 inside test compares d2 with it), a = E * col.
+//   SMALL: c = 0 and r2 = +inf, so the one pixel of its box passes the inside test with weight exp2(0) = 1;
+//          a = E * col * pi sp^2 (1 - exp(-chi^2)) (the whole clipped flux).
+//   box: the particle's pixel box clipped to the bin it is filed under, relative to the bin's origin.  Tile bins
+//        (SMALL, MEDIUM): x0 | y0 << 5 | (x1 - x0) << 10 | (y1 - y0) << 15.  Super-tile bins (LARGE):
+//        x0 | y0 << 8 | x1 << 16 | y1 << 24.  The renderers never round a float again.
 // A record whose amplitude is not finite (I or scalar = Inf / NaN) carries amplitude 0.
+__device__ __forceinline__ unsigned int pack_box(const Geo &g, int cls, int bx, int by, const FrameParams &fp)
+{
+    if (cls == LARGE) {
+        const int ox = bx << fp.sshift, oy = by << fp.sshift, m = (1 << fp.sshift) - 1;
+        const int cx0 = max(g.x0 - ox, 0), cx1 = min(g.x1 - ox, m), cy0 = max(g.y0 - oy, 0), cy1 = min(g.y1 - oy, m);
+        return (unsigned int)cx0 | ((unsigned int)cy0 << 8) | ((unsigned int)cx1 << 16) | ((unsigned int)cy1 << 24);
+    }
+    const int ox = bx << fp.tshift, oy = by << fp.tshift, m = fp.T - 1;
+    const int cx0 = max(g.x0 - ox, 0), cx1 = min(g.x1 - ox, m), cy0 = max(g.y0 - oy, 0), cy1 = min(g.y1 - oy, m);
+    return (unsigned int)cx0 | ((unsigned int)cy0 << 5) | ((unsigned int)(cx1 - cx0) << 10) | ((unsigned int)(cy1 - cy0) << 15);
+}
+
 template <bool ALIGNED>
 __global__ void __launch_bounds__(kBinThreads, 2)
 k_scatter(const float *__restrict__ x, const float *__restrict__ y, const float *__restrict__ z,
@@ -432,30 +487,40 @@ k_scatter(const float *__restrict__ x, const float *__restrict__ y, const float 
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             Geo g = geometry(xs[j], ys[j], zs[j], hs[j], fp);
-            if (!(i + j < len)) g.cls = CULLED;
+            if (!(i + j < len)) { g.cls = CULLED; g.x1 = -1; g.y1 = -1; g.x0 = 0; g.y0 = 0; }
             const int s = one_species ? s_first : species_of(min(lo32 + i + j, lo32 + len - 1), fp);
             const SpeciesDev &S = fp.sp[s];
             const float4 *lut = fp.lut_total > 0 ? s_lut + S.lut_off : fp.lut + s * kMaxLut;
             float3 a = amplitude(Is[j], ss[j], hs[j], S, lut);
             const bool small = g.cls == SMALL;
-            const float w = small ? fp.csmall * (g.sp * g.sp) : 1.0f;
+            const float sp2 = __fmul_rn(g.sp, g.sp);
+            const float w = small ? fp.csmall * sp2 : 1.0f;
             a.x *= w; a.y *= w; a.z *= w;
             float4 ra, rb;
             ra.x = g.px; ra.y = g.py;
-            ra.z = small ? 0.0f : __fdiv_rn(-1.4426950408889634f, __fmul_rn(g.sp, g.sp));
-            ra.w = small ? -1.0f : g.rp;
+            ra.z = small ? 0.0f : __fdividef(-1.4426950408889634f, sp2);
+            ra.w = small ? __int_as_float(0x7f800000) : __fmul_rn(g.rp, g.rp);
             const float am = fmaxf(fabsf(a.x), fmaxf(fabsf(a.y), fabsf(a.z)));
             if (!(am <= 3.0e38f)) a = make_float3(0.0f, 0.0f, 0.0f);             // Inf / NaN amplitude
             else if (g.cls == SMALL || g.cls == MEDIUM) amax = fmaxf(amax, am);
-            rb = make_float4(a.x, a.y, a.z, g.zc);
+            rb = make_float4(a.x, a.y, a.z, 0.0f);
             const BinBox b = bin_box(g, fp);
-            const int nmax = __reduce_max_sync(0xffffffffu, b.n);
-            int bx = b.bx0, by = b.by0;
-            for (int t = 0; t < nmax; ++t) {
-                if (t < b.n) st_record(records, atomicAdd(&cursor[b.base + by * b.pitch + bx], 1u), ra, rb);
-                const bool wrap = bx == b.bx1;
-                bx = wrap ? b.bx0 : bx + 1;
-                by += wrap;
+            if (b.n > 0) {
+                rb.w = __uint_as_float(pack_box(g, g.cls, b.bx0, b.by0, fp));
+                st_record(records, atomicAdd(&cursor[b.base + b.by0 * b.pitch + b.bx0], 1u), ra, rb);
+            }
+            if (__any_sync(0xffffffffu, b.n > 1)) {
+                const int nmax = __reduce_max_sync(0xffffffffu, b.n);
+                int bx = b.bx0, by = b.by0;
+                for (int t = 1; t < nmax; ++t) {
+                    const bool wrap = bx == b.bx1;
+                    bx = wrap ? b.bx0 : bx + 1;
+                    by += wrap;
+                    if (t < b.n) {
+                        rb.w = __uint_as_float(pack_box(g, g.cls, bx, by, fp));
+                        st_record(records, atomicAdd(&cursor[b.base + by * b.pitch + bx], 1u), ra, rb);
+                    }
+                }
             }
         }
     }
@@ -477,13 +542,6 @@ __device__ __forceinline__ float ex2_approx(float x)
     return y;
 }
 
-__device__ __forceinline__ float rcp_approx(float x)
-{
-    float y;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-}
-
 __device__ __forceinline__ float pow2i(int e) { return __int_as_float((e + 127) << 23); }   // -126 <= e <= 127
 
 // Fixed-point exponent of the frame: contributions are accumulated in units of 2^-e, with the largest record
@@ -495,43 +553,48 @@ __device__ __forceinline__ int fixed_exponent(unsigned int amax_bits)
     return kFixedBits - ex;
 }
 
+// Framebuffer of a tile in shared memory: per channel a low plane (sums of the low 16 bits of each contribution,
+// unsigned) and a high plane (sums of the signed upper bits).  value = hi * 65536 + lo.  A segment holds at most
+// kChunkMax = 32768 records and a record touches a pixel once, so neither plane can wrap.  Both updates are native
+// 32-bit shared-memory atomics without a return value (64-bit and float atomics on shared memory are CAS loops).
 template <int T> struct SplatCfg {
     static constexpr int kPix = T * T;
     static constexpr int kWarps = kSplatThreads / 32;
     static constexpr size_t kSmemBytes = sizeof(unsigned int) * 6 * kPix + sizeof(float4) * 2 * 32 * kWarps;
 };
 
-// add the signed 32-bit value v to the 64-bit accumulator (lo, hi): one native shared-memory atomic, a second one
-// only on a carry / borrow out of the low word
-__device__ __forceinline__ void fixed_add(unsigned int *lo, unsigned int *hi, int v)
+__device__ __forceinline__ void fixed_add(unsigned int *lo, unsigned int *hi, float value)
 {
-    if (v == 0) return;
-    const unsigned int uv = (unsigned int)v;
-    const unsigned int old = atomicAdd(lo, uv);
-    const int up = (v >> 31) + (int)((unsigned int)(old + uv) < uv);
+    const int v = __float2int_rn(value);                // |v| <= 2^kFixedBits
+    atomicAdd(lo, (unsigned int)v & 0xffffu);
+    const int up = v >> 16;
     if (up != 0) atomicAdd(hi, (unsigned int)up);
 }
 
 // One work item = chunk_size consecutive records; the chunk is cut into segments at tile boundaries.  For each
-// segment the CTA clears the tile framebuffer (64-bit fixed point, shared memory), every warp takes batches of 32
-// records, lays the fragments (pixels of the clipped boxes) of the batch end to end and hands 32 consecutive
-// fragments to its 32 lanes per step, so lanes stay busy whatever the footprint (1 pixel for SMALL records).
+// segment the CTA clears the tile framebuffer, every warp takes batches of 32 records, lays the fragments (pixels
+// of the records' boxes, which k_scatter already clipped to the tile) of the batch end to end and hands 32
+// consecutive fragments to its 32 lanes per step, so lanes stay busy whatever the footprint (1 pixel for SMALL
+// records).  Per fragment: locate the record (ballot / popc), decode the pixel (multiply-shift division), C1 inside
+// test, one ex2, three fixed-point adds.  The only conversion-pipe work per fragment is the ex2 and three F2I.
 // The segment's framebuffer goes to its partial slot; k_compose adds the slots of a tile.
 template <int T>
 __global__ void __launch_bounds__(kSplatThreads)
 k_splat(const float4 *__restrict__ records, const unsigned int *__restrict__ bin_start,
         const unsigned int *__restrict__ seg_start, const unsigned int *__restrict__ chunk_tile,
-        DeviceStats *__restrict__ stats, long long *__restrict__ partials, const __grid_constant__ FrameParams fp)
+        DeviceStats *__restrict__ stats, unsigned int *__restrict__ partials, const __grid_constant__ FrameParams fp)
 {
     using Cfg = SplatCfg<T>;
     constexpr int kPix = Cfg::kPix;
     extern __shared__ __align__(16) unsigned int smem_u[];
-    unsigned int *fb_lo = smem_u, *fb_hi = smem_u + 3 * kPix;
+    unsigned int *fb = smem_u;                                            // lo R G B, hi R G B
     float4 *stage_all = reinterpret_cast<float4 *>(smem_u + 6 * kPix);
     __shared__ unsigned int s_chunk;
+    __shared__ unsigned int s_inv[32];                                    // 65536 / w + 1: k / w = (k * inv) >> 16 for k < 1024
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    float4 *stage = stage_all + warp * 64;
-    const unsigned int lane_lt = (1u << lane) - 1u, lane_le = 0xffffffffu >> (31 - lane);
+    float4 *stA = stage_all + warp * 64, *stB = stA + 32;
+    const unsigned int lane_le = 0xffffffffu >> (31 - lane);
+    if (threadIdx.x < 32) s_inv[threadIdx.x] = 65536u / (threadIdx.x + 1u) + 1u;
     const unsigned int total = (unsigned int)stats->chunks;
     const unsigned int K = stats->chunk_size;
     const unsigned int pairs = (unsigned int)stats->pairs;
@@ -549,33 +612,20 @@ k_splat(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
         for (;;) {
             // ---- segment = [max(tb, r0), min(te, r1)) of `tile`
             const unsigned int begin = max(tb, r0), end = min(te, r1);
-            for (int i = threadIdx.x; i < 6 * kPix; i += kSplatThreads) smem_u[i] = 0u;
+            for (int i = threadIdx.x; i < 6 * kPix; i += kSplatThreads) fb[i] = 0u;
             __syncthreads();
             const int tx0 = (tile % fp.ntx) * T, ty0 = (tile / fp.ntx) * T;
-            const float ftx0 = (float)tx0, fty0 = (float)ty0;
-            const float ftx1 = (float)min(tx0 + T - 1, fp.W - 1), fty1 = (float)min(ty0 + T - 1, fp.H - 1);
+            // (float)(tx0 + lx) + 0.5 = int_as_float(0x4B000000 | lx) + ox, exactly (ox = tx0 + 0.5 - 2^23)
+            const float ox = __fsub_rn(__fadd_rn((float)tx0, 0.5f), 8388608.0f);
+            const float oy = __fsub_rn(__fadd_rn((float)ty0, 0.5f), 8388608.0f);
             for (unsigned int base = begin + warp * 32; base < end; base += kSplatThreads) {
                 const unsigned int idx = base + lane;
                 const bool valid = idx < end;
                 float4 ra = make_float4(0.f, 0.f, 0.f, 0.f), rb = ra;
                 if (valid) ld_record(records, idx, ra, rb);
-                const bool is_small = ra.w < 0.0f;
-                int bx0 = 0, by0 = 0, bw = 0, bh = 0;
-                if (valid) {
-                    if (is_small) {
-                        bx0 = (int)ra.x - tx0; by0 = (int)ra.y - ty0; bw = bh = 1;
-                    } else {        // clip the pixel box to the tile (same float32 formulas as the classification stage)
-                        const float fx0 = fmaxf(ceilf(__fsub_rn(__fsub_rn(ra.x, ra.w), 0.5f)), ftx0);
-                        const float fx1 = fminf(floorf(__fsub_rn(__fadd_rn(ra.x, ra.w), 0.5f)), ftx1);
-                        const float fy0 = fmaxf(ceilf(__fsub_rn(__fsub_rn(ra.y, ra.w), 0.5f)), fty0);
-                        const float fy1 = fminf(floorf(__fsub_rn(__fadd_rn(ra.y, ra.w), 0.5f)), fty1);
-                        if (fx0 <= fx1 && fy0 <= fy1) {
-                            bx0 = (int)fx0 - tx0; by0 = (int)fy0 - ty0;
-                            bw = (int)fx1 - (int)fx0 + 1; bh = (int)fy1 - (int)fy0 + 1;
-                        }
-                    }
-                }
-                const int nfrag = bw * bh;
+                const unsigned int box = __float_as_uint(rb.w);
+                const int bw = (int)((box >> 10) & 31u) + 1, bh = (int)((box >> 15) & 31u) + 1;
+                const int nfrag = valid ? bw * bh : 0;
                 int incl = nfrag;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) {
@@ -584,43 +634,32 @@ k_splat(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
                 }
                 const int start = incl - nfrag;
                 const int F = __shfl_sync(0xffffffffu, incl, 31);
-                const bool nonempty = nfrag > 0;
-                const unsigned int ne_mask = __ballot_sync(0xffffffffu, nonempty);
-                if (nonempty) {
-                    const int slot = __popc(ne_mask & lane_lt);
-                    const unsigned int pack = (unsigned int)start | ((unsigned int)bx0 << 15) | ((unsigned int)by0 << 20) |
-                                              ((unsigned int)(bw - 1) << 25) | (is_small ? 0x40000000u : 0u);
-                    stage[2 * slot] = make_float4(ra.x, ra.y, ra.z, __fmul_rn(ra.w, ra.w));
-                    stage[2 * slot + 1] = make_float4(rb.x * sc1 * sc2, rb.y * sc1 * sc2, rb.z * sc1 * sc2, __uint_as_float(pack));
-                }
+                stA[lane] = ra;
+                stB[lane] = make_float4(rb.x * sc1 * sc2, rb.y * sc1 * sc2, rb.z * sc1 * sc2,
+                                        __uint_as_float((unsigned int)start | ((box & 0x3ffu) << 15) | ((box & 0x7c00u) << 15)));
                 __syncwarp();
                 for (int f0 = 0; f0 < F; f0 += 32) {
                     const int rel = start - f0;
-                    const unsigned int m = __reduce_or_sync(0xffffffffu, (nonempty && rel >= 0 && rel < 32) ? (1u << rel) : 0u);
-                    const int nb = __popc(__ballot_sync(0xffffffffu, nonempty && rel < 0));
+                    const unsigned int m = __reduce_or_sync(0xffffffffu, (valid && rel >= 0 && rel < 32) ? (1u << rel) : 0u);
+                    const int nb = __popc(__ballot_sync(0xffffffffu, valid && rel < 0));
                     const int f = f0 + lane;
                     if (f < F) {
                         const int s = nb - 1 + __popc(m & lane_le);
-                        const float4 A = stage[2 * s], B = stage[2 * s + 1];
-                        const unsigned int pack = __float_as_uint(B.w);
-                        const int k = f - (int)(pack & 0x7fffu);
-                        const int w = (int)((pack >> 25) & 31u) + 1;
-                        const int j = (int)(((float)k + 0.5f) * rcp_approx((float)w));
-                        const int lx = (int)((pack >> 15) & 31u) + (k - j * w), ly = (int)((pack >> 20) & 31u) + j;
-                        float wgt = 1.0f;
-                        bool inside = true;
-                        if (!(pack & 0x40000000u)) {
-                            const float dxf = __fsub_rn(__fadd_rn((float)(tx0 + lx), 0.5f), A.x);
-                            const float dyf = __fsub_rn(__fadd_rn((float)(ty0 + ly), 0.5f), A.y);
-                            const float d2 = __fmaf_rn(dxf, dxf, __fmul_rn(dyf, dyf));
-                            inside = d2 <= A.w;
-                            wgt = ex2_approx(d2 * A.z);
-                        }
-                        if (inside) {
-                            const int p = ly * T + lx;
-                            fixed_add(fb_lo + p, fb_hi + p, __float2int_rn(B.x * wgt));
-                            fixed_add(fb_lo + kPix + p, fb_hi + kPix + p, __float2int_rn(B.y * wgt));
-                            fixed_add(fb_lo + 2 * kPix + p, fb_hi + 2 * kPix + p, __float2int_rn(B.z * wgt));
+                        const float4 A = stA[s], B = stB[s];
+                        const unsigned int pk = __float_as_uint(B.w);
+                        const unsigned int k = (unsigned int)f - (pk & 0x7fffu);
+                        const unsigned int wm1 = pk >> 25;
+                        const unsigned int j = (k * s_inv[wm1]) >> 16;
+                        const unsigned int lx = ((pk >> 15) & 31u) + (k - j * (wm1 + 1u)), ly = ((pk >> 20) & 31u) + j;
+                        const float dxf = __fsub_rn(__fadd_rn(__uint_as_float(0x4B000000u | lx), ox), A.x);
+                        const float dyf = __fsub_rn(__fadd_rn(__uint_as_float(0x4B000000u | ly), oy), A.y);
+                        const float d2 = __fmaf_rn(dxf, dxf, __fmul_rn(dyf, dyf));
+                        if (d2 <= A.w) {
+                            const float wgt = ex2_approx(d2 * A.z);
+                            unsigned int *q = fb + ly * T + lx;
+                            fixed_add(q, q + 3 * kPix, B.x * wgt);
+                            fixed_add(q + kPix, q + 4 * kPix, B.y * wgt);
+                            fixed_add(q + 2 * kPix, q + 5 * kPix, B.z * wgt);
                         }
                     }
                 }
@@ -629,9 +668,8 @@ k_splat(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
             __syncthreads();
             // ---- flush the segment's framebuffer to its partial slot
             const unsigned int seg = seg_start[tile] + (chunk - tb / K);
-            long long *out = partials + (size_t)seg * (3 * kPix);
-            for (int i = threadIdx.x; i < 3 * kPix; i += kSplatThreads)
-                out[i] = (long long)(((unsigned long long)fb_hi[i] << 32) | fb_lo[i]);
+            unsigned int *out = partials + (size_t)seg * (6 * kPix);
+            for (int i = threadIdx.x; i < 6 * kPix; i += kSplatThreads) out[i] = fb[i];
             if (te >= r1) break;
             // ---- next non-empty tile
             do { ++tile; tb = te; te = bin_start[tile + 1]; } while (te == tb);
@@ -641,12 +679,12 @@ k_splat(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
 }
 
 // ---- A6 + A8: compose one tile ----------------------------------------------------------------------------------
-// Thread t owns pixels t, t+256, ... of the tile (registers).  Adds the tile's segment partials (64-bit integers,
-// exact), then gathers the LARGE records of the tile's super-tile (each record is tested against the tile,
+// Thread t owns pixels t, t+256, ... of the tile (registers).  Adds the tile's segment partials (integers, exact),
+// then gathers the LARGE records of the tile's super-tile (each record's box is tested against the tile,
 // survivors are staged in shared memory and evaluated by every pixel owner), in two-level float32 accumulation.
 template <int T>
 __global__ void __launch_bounds__(256)
-k_compose(const long long *__restrict__ partials, const unsigned int *__restrict__ seg_start,
+k_compose(const unsigned int *__restrict__ partials, const unsigned int *__restrict__ seg_start,
           const float4 *__restrict__ records, const unsigned int *__restrict__ bin_start,
           const DeviceStats *__restrict__ stats, const __grid_constant__ FrameParams fp,
           float *__restrict__ image)
@@ -673,21 +711,34 @@ k_compose(const long long *__restrict__ partials, const unsigned int *__restrict
     const bool ok = stats->overflow == 0u;
     if (ok) {
         const unsigned int s0 = seg_start[tile], s1 = seg_start[tile + 1];
-        for (unsigned int sg = s0; sg < s1; ++sg) {
+        // four segments per round: 6 * 4 independent loads per pixel in flight (heavy tiles own hundreds of segments)
+        for (unsigned int sg = s0; sg < s1; sg += 4) {
 #pragma unroll
             for (int k = 0; k < kPpt; ++k) {
                 const int p = threadIdx.x + k * 256;
                 if (p < kPix) {
-                    const long long *q = partials + (size_t)sg * (3 * kPix) + p;
+                    unsigned int v[4][6];
 #pragma unroll
-                    for (int c = 0; c < 3; ++c) fix[k][c] += __ldg(q + c * kPix);
+                    for (int u = 0; u < 4; ++u) {
+                        const unsigned int *q = partials + (size_t)min(sg + u, s1 - 1) * (6 * kPix) + p;
+#pragma unroll
+                        for (int c = 0; c < 6; ++c) v[u][c] = __ldg(q + c * kPix);
+                    }
+#pragma unroll
+                    for (int u = 0; u < 4; ++u)
+                        if (sg + u < s1) {
+#pragma unroll
+                            for (int c = 0; c < 3; ++c)
+                                fix[k][c] += (long long)(int)v[u][3 + c] * 65536ll + (long long)v[u][c];
+                        }
                 }
             }
         }
         const int sbin = fp.n_tiles + (ty >> kSuperShift) * fp.nsx + (tx >> kSuperShift);
         const unsigned int lb = bin_start[sbin], le = bin_start[sbin + 1];
-        const float ftx0 = (float)tx0, fty0 = (float)ty0;
-        const float ftx1 = (float)min(tx0 + T - 1, fp.W - 1), fty1 = (float)min(ty0 + T - 1, fp.H - 1);
+        // the tile inside its super-tile, in pixels
+        const int qx0 = (tx & ((1 << kSuperShift) - 1)) * T, qy0 = (ty & ((1 << kSuperShift) - 1)) * T;
+        const int qx1 = qx0 + T - 1, qy1 = qy0 + T - 1;
         int batch = 0;
         for (unsigned int base = lb; base < le; base += 256, ++batch) {
             const unsigned int idx = base + threadIdx.x;
@@ -695,11 +746,10 @@ k_compose(const long long *__restrict__ partials, const unsigned int *__restrict
             float4 ra, rb;
             if (idx < le) {
                 ld_record(records, idx, ra, rb);
-                const float fx0 = ceilf(__fsub_rn(__fsub_rn(ra.x, ra.w), 0.5f));
-                const float fx1 = floorf(__fsub_rn(__fadd_rn(ra.x, ra.w), 0.5f));
-                const float fy0 = ceilf(__fsub_rn(__fsub_rn(ra.y, ra.w), 0.5f));
-                const float fy1 = floorf(__fsub_rn(__fadd_rn(ra.y, ra.w), 0.5f));
-                hit = fx0 <= ftx1 && fx1 >= ftx0 && fy0 <= fty1 && fy1 >= fty0;
+                const unsigned int box = __float_as_uint(rb.w);
+                const int bx0 = (int)(box & 255u), by0 = (int)((box >> 8) & 255u);
+                const int bx1 = (int)((box >> 16) & 255u), by1 = (int)(box >> 24);
+                hit = bx0 <= qx1 && bx1 >= qx0 && by0 <= qy1 && by1 >= qy0;
             }
             const unsigned int bal = __ballot_sync(0xffffffffu, hit);
             if (lane == 0) s_woff[warp] = __popc(bal);
@@ -718,12 +768,11 @@ k_compose(const long long *__restrict__ partials, const unsigned int *__restrict
             const int cnt = s_cnt;
             for (int m = 0; m < cnt; ++m) {
                 const float4 a = sA[m], b = sB[m];
-                const float r2 = __fmul_rn(a.w, a.w);
 #pragma unroll
                 for (int k = 0; k < kPpt; ++k) {
                     const float dxf = __fsub_rn(fxc[k], a.x), dyf = __fsub_rn(fyc[k], a.y);
                     const float d2 = __fmaf_rn(dxf, dxf, __fmul_rn(dyf, dyf));
-                    if (d2 <= r2) {
+                    if (d2 <= a.w) {
                         const float wgt = ex2_approx(d2 * a.z);
                         sub[k][0] = fmaf(b.x, wgt, sub[k][0]);
                         sub[k][1] = fmaf(b.y, wgt, sub[k][1]);
