@@ -3,7 +3,7 @@
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--impl ours|reference]
 
-A step is one whole frame (count -> scans -> scatter -> splat -> compose) of BASELINE configs[1]
+A step is one whole frame (count -> scan -> scatter -> splat -> compose) of BASELINE configs[1]
 (10M particles, 50 Plummer halos + 20 % background, 800 x 800, additive mode) with the particles
 already resident in HBM.  One JSON line is printed by rank 0.  `e2e` is the same frame through
 splotch_render_host: pinned HOST particle arrays in, HOST image out, copies inside the timed region.
@@ -30,7 +30,7 @@ import torch  # noqa: E402
 from paper_1309_1114_b200 import workloads as wl  # noqa: E402
 
 TILE = 16
-KERNELS_PER_FRAME = 6        # k_count, k_colscan, k_binscan, k_scatter, k_splat, k_compose
+KERNELS_PER_FRAME = 5        # k_count, k_scan, k_scatter, k_splat, k_compose (+ one memset node)
 FLOP_PER_FRAGMENT = 8        # 2 FMA (d^2) + compare + scale + exp2 + 3 FMA, FMA counted once
 
 
@@ -205,7 +205,7 @@ def run_ours(args):
     for k in ("count", "scatter"):
         gbs = bytes_by_stage[k] / (stage[k] * 1e-3) / 1e9
         stage_roof[k] = {"ms": stage[k], "GB/s": gbs, "frac_hbm": gbs / hbm_gbs}
-    for k in ("colscan", "binscan", "splat", "compose"):
+    for k in ("scan", "splat", "compose"):
         stage_roof[k] = {"ms": stage[k]}
     stage_roof["splat"]["Gfragments/s"] = frags / (stage["splat"] * 1e-3) / 1e9
     # sum of per-stage lower bounds: HBM terms + ALU term

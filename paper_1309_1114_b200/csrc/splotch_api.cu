@@ -14,13 +14,13 @@ using namespace splotch;
 
 namespace {
 
-constexpr int kStages = 6;
+constexpr int kStages = 5;
 constexpr int kProfRing = 256;              // frames of per-stage events kept while profiling
-const char *kStageNames[kStages] = {"count", "colscan", "binscan", "scatter", "splat", "compose"};
+const char *kStageNames[kStages] = {"count", "scan", "scatter", "splat", "compose"};
 
 struct Layout {
-    size_t counts, cls_counts, bin_count, bin_start, seg_start, stats, chunk_tile, partials, records, staging, total;
-    unsigned long long capacity, max_chunks;
+    size_t counts, cls_counts, bin_count, bin_start, stats, accum, accum_bytes, records, staging, total;
+    unsigned long long capacity;
     int nrows;
 };
 
@@ -97,36 +97,31 @@ bool make_layout(const splotch_ctx *c, unsigned long long n, int T, unsigned lon
     const int ntx = (c->width + T - 1) / T, nty = (c->height + T - 1) / T;
     const size_t n_tiles = (size_t)ntx * nty;
     const size_t nbins = hist_bytes(c->width, c->height, T) / sizeof(unsigned int);
-    const size_t partial_bytes = sizeof(unsigned int) * 6 * (size_t)T * T;  // one segment's framebuffer (lo, hi planes x RGB)
     L->nrows = bin_rows(c, T);
     size_t off = 0;
     L->counts = off;      off = align_up(off + sizeof(unsigned int) * nbins * L->nrows, 256);
     L->cls_counts = off;  off = align_up(off + sizeof(unsigned int) * 4 * L->nrows, 256);
     L->bin_count = off;   off = align_up(off + sizeof(unsigned int) * nbins, 256);
     L->bin_start = off;   off = align_up(off + sizeof(unsigned int) * (nbins + 1), 256);
-    L->seg_start = off;   off = align_up(off + sizeof(unsigned int) * (n_tiles + 1), 256);
+    // DeviceStats and the tiles' 64-bit sums sit together: one memset clears both before every frame
     L->stats = off;       off = align_up(off + sizeof(DeviceStats), 256);
+    L->accum = off;
+    L->accum_bytes = sizeof(unsigned long long) * 3 * (size_t)T * T * n_tiles;
+    off = align_up(off + L->accum_bytes, 256);
     L->staging = off;
     if (staging) {
         off = align_up(off + 6 * align_up(sizeof(float) * n, 256), 256);
         off = align_up(off + sizeof(float) * 3 * (size_t)c->width * c->height, 256);
     }
     const size_t fixed = off;
-    // chunks <= max(32 per SM, capacity / kChunkMax) + 2 (k_binscan's choice of the chunk size); segments <= tiles + chunks
-    const size_t per_chunk = partial_bytes + sizeof(unsigned int);
-    const size_t min_chunks = (size_t)c->n_sm * 32 + 2;
     if (capacity == 0) {
-        // derive from bytes: capacity * 32 + (n_tiles + chunks) * partial + chunks * 4 <= bytes - fixed
-        const size_t need0 = fixed + n_tiles * partial_bytes + min_chunks * per_chunk + 8192;
+        // derive from bytes: capacity * 32 <= bytes - fixed
+        const size_t need0 = fixed + 8192;
         if (bytes < need0) return false;
-        const double avail = (double)(bytes - need0);
-        capacity = (unsigned long long)(avail / (32.0 + (double)per_chunk / kChunkMax));
+        capacity = (unsigned long long)((bytes - need0) / 32);
         if (capacity > 0xfffffff0ull) capacity = 0xfffffff0ull;
     }
     L->capacity = capacity;
-    L->max_chunks = (capacity / kChunkMax + 2 > min_chunks) ? capacity / kChunkMax + 2 : min_chunks;
-    L->chunk_tile = off; off = align_up(off + sizeof(unsigned int) * L->max_chunks, 256);
-    L->partials = off;   off = align_up(off + partial_bytes * (n_tiles + L->max_chunks), 256);
     L->records = off;  off = align_up(off + 32ull * capacity, 256);
     L->total = off;
     return bytes == 0 || off <= bytes;
@@ -136,7 +131,7 @@ template <int T>
 int query_splat_occupancy(splotch_ctx *c, int *out)
 {
     CU_TRY(c, cudaFuncSetAttribute(k_splat<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SplatCfg<T>::kSmemBytes));
-    CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, k_splat<T>, kSplatThreads, SplatCfg<T>::kSmemBytes));
+    CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, k_splat<T>, SplatCfg<T>::kThreads, SplatCfg<T>::kSmemBytes));
     if (*out < 1) *out = 1;
     return SPLOTCH_OK;
 }
@@ -218,14 +213,13 @@ int launch_render_tail(splotch_ctx *c, const Layout &L, char *ws, const FramePar
 {
     const int ti = T == 8 ? 0 : T == 16 ? 1 : 2;
     const int grid = c->n_sm * c->splat_blocks_per_sm[ti];
-    k_splat<T><<<grid, kSplatThreads, SplatCfg<T>::kSmemBytes, st>>>(
-        (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.bin_start), (const unsigned int *)(ws + L.seg_start),
-        (const unsigned int *)(ws + L.chunk_tile), (DeviceStats *)(ws + L.stats), (unsigned int *)(ws + L.partials), fp);
+    k_splat<T><<<grid, SplatCfg<T>::kThreads, SplatCfg<T>::kSmemBytes, st>>>(
+        (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.bin_start), (DeviceStats *)(ws + L.stats), (unsigned long long *)(ws + L.accum), fp);
+    if (c->profiling) cudaEventRecord(c->ev[4], st);
+    k_compose<T><<<fp.n_tiles, 256, 0, st>>>((const unsigned long long *)(ws + L.accum), (const float4 *)(ws + L.records),
+                                             (const unsigned int *)(ws + L.bin_start), (const DeviceStats *)(ws + L.stats),
+                                             fp, image);
     if (c->profiling) cudaEventRecord(c->ev[5], st);
-    k_compose<T><<<fp.n_tiles, 256, 0, st>>>((const unsigned int *)(ws + L.partials), (const unsigned int *)(ws + L.seg_start),
-                                             (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.bin_start),
-                                             (const DeviceStats *)(ws + L.stats), fp, image);
-    if (c->profiling) cudaEventRecord(c->ev[6], st);
     return SPLOTCH_OK;
 }
 
@@ -241,25 +235,23 @@ int render_device(splotch_ctx *c, const splotch_particles *p, unsigned long long
     unsigned int *cls_counts = (unsigned int *)(ws + L.cls_counts);
     unsigned int *bin_count = (unsigned int *)(ws + L.bin_count);
     unsigned int *bin_start = (unsigned int *)(ws + L.bin_start);
-    unsigned int *seg_start = (unsigned int *)(ws + L.seg_start);
     DeviceStats *stats = (DeviceStats *)(ws + L.stats);
     if (c->profiling) {
         c->ev = c->ev_ring[c->prof_frames % kProfRing];
         cudaEventRecord(c->ev[0], st);
     }
+    cudaMemsetAsync(ws + L.stats, 0, (L.accum - L.stats) + L.accum_bytes, st);      // DeviceStats + the tiles' sums
     if (al) k_count<true><<<L.nrows, kBinThreads, hbytes, st>>>(p->x, p->y, p->z, p->h, n, per, fp, counts, cls_counts);
     else    k_count<false><<<L.nrows, kBinThreads, hbytes, st>>>(p->x, p->y, p->z, p->h, n, per, fp, counts, cls_counts);
     if (c->profiling) cudaEventRecord(c->ev[1], st);
-    k_colscan<<<(fp.nbins + 255) / 256, 256, 0, st>>>(counts, L.nrows, fp.nbins, bin_count);
+    k_scan<<<(fp.nbins + 31) / 32, kScanThreads, 0, st>>>(counts, L.nrows, fp.nbins, fp.n_tiles, bin_count, bin_start, cls_counts, L.capacity,
+                                                          c->n_sm, stats);
     if (c->profiling) cudaEventRecord(c->ev[2], st);
-    k_binscan<<<1, 1024, 0, st>>>(bin_count, fp.n_tiles, fp.nbins, bin_start, seg_start, (unsigned int *)(ws + L.chunk_tile),
-                                  cls_counts, L.nrows, L.capacity, L.max_chunks, c->n_sm, stats);
-    if (c->profiling) cudaEventRecord(c->ev[3], st);
     if (al) k_scatter<true><<<L.nrows, kBinThreads, hbytes, st>>>(p->x, p->y, p->z, p->h, p->I, p->scalar, n, per, fp, counts,
                                                                   bin_start, stats, (float4 *)(ws + L.records));
     else    k_scatter<false><<<L.nrows, kBinThreads, hbytes, st>>>(p->x, p->y, p->z, p->h, p->I, p->scalar, n, per, fp, counts,
                                                                    bin_start, stats, (float4 *)(ws + L.records));
-    if (c->profiling) cudaEventRecord(c->ev[4], st);
+    if (c->profiling) cudaEventRecord(c->ev[3], st);
     int rc;
     if (fp.T == 8) rc = launch_render_tail<8>(c, L, ws, fp, image, st);
     else if (fp.T == 16) rc = launch_render_tail<16>(c, L, ws, fp, image, st);

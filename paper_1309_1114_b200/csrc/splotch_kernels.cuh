@@ -2,8 +2,9 @@
 //
 // Stage map (paper passages in PAPER.md):
 //   k_count    A1+A3+A4a  roto-translate, project, classify (:76, :138, :156-173) and count (particle, bin) pairs
-//   k_colscan  A4b        per-bin exclusive scan over the count matrix rows (replaces thrust::reduce_by_key, :203)
-//   k_binscan  A4c        exclusive scan over bins, chunk/segment tables, frame statistics (replaces inclusive_scan, :205)
+//   k_scan     A4b+A4c    per-bin exclusive scan down the rows of the count matrix (replaces thrust::reduce_by_key,
+//                         :203); the last block to finish scans over the bins, builds the chunk table and the frame
+//                         statistics (replaces inclusive_scan, :205)
 //   k_scatter  A1-A3+A2+A4d  recompute geometry, colourise (:76, :85), write 32-byte render records in bin order
 //                            (replaces copy_if + sort_by_key, :196-202)
 //   k_splat    A5         SMALL + MEDIUM records of one chunk: all fragments of 32 records are spread over the 32 lanes
@@ -11,9 +12,9 @@
 //                         32-bit planes per channel, native integer atomics without return; the paper's
 //                         medium-particle kernel, :183, :224-228, without its halo copies and without idle threads
 //                         for small footprints)
-//   k_compose  A6+A8      per tile: sum segment partials (exact integer sums), gather the LARGE particles of the
-//                         tile's super-tile (the paper renders these on the CPU, :232-238), optional 1-exp(-S),
-//                         write the image once
+//   k_compose  A6+A8      per tile: read the tile's fixed-point sums, gather the LARGE particles of the tile's
+//                         super-tile (the paper renders these on the CPU, :232-238), optional 1-exp(-S), write the
+//                         image once
 //
 // Canonical float32 geometry: every operation that decides an integer (class, pixel box, tile box, the inside
 // test) is written with round-to-nearest intrinsics (__fmul_rn, __fmaf_rn, __fdiv_rn ...) which nvcc never
@@ -31,7 +32,6 @@ constexpr int kMaxSpecies   = 8;
 constexpr int kMaxLut       = 1024;
 constexpr int kChunkMax     = 32768;  // records per work item of k_splat (upper bound; the frame picks its own)
 constexpr int kChunkMin     = 512;
-constexpr int kSplatThreads = 256;
 constexpr int kBinThreads   = 512;    // k_count / k_scatter block size
 constexpr int kSuperShift   = 3;      // super-tile = 8 x 8 tiles (LARGE particles are binned to super-tiles)
 constexpr int kLutSmemMax   = 1024;   // colour-table entries (all species together) staged in shared memory by k_scatter
@@ -62,10 +62,10 @@ struct FrameParams {
     const float4 *lut;           // [kMaxSpecies][kMaxLut] rgb0
 };
 
-struct DeviceStats {             // written by k_binscan / k_scatter, read back by splotch_get_stats
+struct DeviceStats {             // cleared before every frame; written by k_scan / k_scatter, read back by splotch_get_stats
     unsigned long long count[4];
-    unsigned long long pairs, large_pairs, chunks, capacity, segments;
-    unsigned int overflow, work_counter, chunk_size, amax_bits;
+    unsigned long long pairs, large_pairs, chunks, capacity;
+    unsigned int overflow, work_counter, chunk_size, amax_bits, scan_done, pad;
 };
 
 struct Geo {
@@ -241,16 +241,22 @@ k_count(const float *__restrict__ x, const float *__restrict__ y, const float *_
             c2 += __popc(__ballot_sync(0xffffffffu, g.cls == MEDIUM));
             c3 += __popc(__ballot_sync(0xffffffffu, g.cls == LARGE));
             const BinBox b = bin_box(g, fp);
-            // most particles cover one bin: one atomic for everybody, the walk over the rest only where needed
-            if (b.n > 0) atomicAdd(&hist[b.base + b.by0 * b.pitch + b.bx0], 1u);
-            if (__any_sync(0xffffffffu, b.n > 1)) {
-                const int nmax = __reduce_max_sync(0xffffffffu, b.n);
+            // a box covers at most 2 x 2 bins unless it is wider than a tile: four predicated atomics, no loop
+            const bool any = b.n > 0, w2 = b.bx1 > b.bx0, h2 = b.by1 > b.by0;
+            unsigned int *h00 = hist + (b.base + b.by0 * b.pitch + b.bx0);
+            if (any) atomicAdd(h00, 1u);
+            if (any && w2) atomicAdd(h00 + 1, 1u);
+            if (any && h2) atomicAdd(h00 + b.pitch, 1u);
+            if (any && w2 && h2) atomicAdd(h00 + b.pitch + 1, 1u);
+            const bool big = any && (b.bx1 - b.bx0 > 1 || b.by1 - b.by0 > 1);
+            if (__any_sync(0xffffffffu, big)) {          // the bins beyond the first 2 x 2
+                const int nmax = __reduce_max_sync(0xffffffffu, big ? b.n : 0);
                 int bx = b.bx0, by = b.by0;
-                for (int t = 1; t < nmax; ++t) {
+                for (int t = 0; t < nmax; ++t) {
+                    if (big && t < b.n && (bx - b.bx0 > 1 || by - b.by0 > 1)) atomicAdd(&hist[b.base + by * b.pitch + bx], 1u);
                     const bool wrap = bx == b.bx1;
                     bx = wrap ? b.bx0 : bx + 1;
                     by += wrap;
-                    if (t < b.n) atomicAdd(&hist[b.base + by * b.pitch + bx], 1u);
                 }
             }
         }
@@ -264,32 +270,11 @@ k_count(const float *__restrict__ x, const float *__restrict__ y, const float *_
     if (threadIdx.x < 4) cls_counts[blockIdx.x * 4 + threadIdx.x] = s_cls[threadIdx.x];
 }
 
-// ---- A4b: per bin, exclusive scan down the rows of the count matrix -----------------------------------------
-__global__ void __launch_bounds__(256)
-k_colscan(unsigned int *__restrict__ counts, int nrows, int nbins, unsigned int *__restrict__ bin_count)
-{
-    const int bin = blockIdx.x * blockDim.x + threadIdx.x;
-    if (bin >= nbins) return;
-    unsigned int run = 0;
-    int b = 0;
-    for (; b + 8 <= nrows; b += 8) {
-        unsigned int c[8];
-#pragma unroll
-        for (int k = 0; k < 8; ++k) c[k] = counts[(size_t)(b + k) * nbins + bin];
-#pragma unroll
-        for (int k = 0; k < 8; ++k) { counts[(size_t)(b + k) * nbins + bin] = run; run += c[k]; }
-    }
-    for (; b < nrows; ++b) {
-        const unsigned int c = counts[(size_t)b * nbins + bin];
-        counts[(size_t)b * nbins + bin] = run;
-        run += c;
-    }
-    bin_count[bin] = run;
-}
+// ---- A4b + A4c: scans ----------------------------------------------------------------------------------------------
+constexpr int kScanThreads = 256;
 
-// ---- A4c: scan over bins, segment table, statistics (one block) ------------------------------------------------
-__device__ __forceinline__ unsigned long long block_excl_scan_1024(unsigned long long v, unsigned long long *s_warp,
-                                                                   unsigned long long *total)
+__device__ __forceinline__ unsigned long long block_excl_scan_256(unsigned long long v, unsigned long long *s_warp,
+                                                                  unsigned long long *total)
 {
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     unsigned long long inc = v;
@@ -300,15 +285,10 @@ __device__ __forceinline__ unsigned long long block_excl_scan_1024(unsigned long
     }
     if (lane == 31) s_warp[w] = inc;
     __syncthreads();
-    if (w == 0) {
-        unsigned long long ws = s_warp[lane], winc = ws;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const unsigned long long t = __shfl_up_sync(0xffffffffu, winc, o);
-            if (lane >= o) winc += t;
-        }
-        s_warp[lane] = winc - ws;
-        if (lane == 31) *total = winc;
+    if (threadIdx.x == 0) {
+        unsigned long long run = 0;
+        for (int k = 0; k < kScanThreads / 32; ++k) { const unsigned long long c = s_warp[k]; s_warp[k] = run; run += c; }
+        *total = run;
     }
     __syncthreads();
     const unsigned long long r = s_warp[w] + inc - v;
@@ -316,75 +296,120 @@ __device__ __forceinline__ unsigned long long block_excl_scan_1024(unsigned long
     return r;
 }
 
-// The tile part of the record array, [0, pairs), is cut into chunks of `chunk_size` consecutive records (the work
-// items of k_splat).  A segment is the overlap of one chunk with one tile; tile t owns the partial-framebuffer
-// slots seg_start[t] .. seg_start[t+1]-1, one per chunk it overlaps, in chunk order.  chunk_tile[c] is the tile
-// that holds the first record of chunk c.
-__global__ void __launch_bounds__(1024)
-k_binscan(const unsigned int *__restrict__ bin_count, int n_tiles, int nbins, unsigned int *__restrict__ bin_start,
-          unsigned int *__restrict__ seg_start, unsigned int *__restrict__ chunk_tile,
-          const unsigned int *__restrict__ cls_counts, int nrows, unsigned long long capacity,
-          unsigned long long max_chunks, int n_sm, DeviceStats *__restrict__ stats)
+// Phase 1, every block: 32 bins x 8 row groups.  Thread (bin, g) sums its rows of the count matrix (independent
+// loads, bins of neighbouring lanes are neighbours in memory), the groups are combined through shared memory, and
+// the rows are rewritten as exclusive prefixes: counts[b][bin] becomes the offset of block b inside the bin.
+// Phase 2, the last block to finish (a counter in DeviceStats, cleared with it before every frame): exclusive scan
+// over the bins -> bin_start, frame statistics, and the chunk size: the tile part of the record array, [0, pairs),
+// is cut into chunks of chunk_size consecutive records, the work items of k_splat.
+__global__ void __launch_bounds__(kScanThreads)
+k_scan(unsigned int *__restrict__ counts, int nrows, int nbins, int n_tiles, unsigned int *__restrict__ bin_count,
+       unsigned int *__restrict__ bin_start, const unsigned int *__restrict__ cls_counts, unsigned long long capacity, int n_sm,
+       DeviceStats *__restrict__ stats)
 {
-    __shared__ unsigned long long s_warp[32];
-    __shared__ unsigned long long s_tot_pairs, s_tot_all, s_tot_segs;
-    const int per = (nbins + 1023) / 1024;
+    __shared__ unsigned int s_part[8][32];
+    __shared__ unsigned long long s_warp[kScanThreads / 32];
+    __shared__ unsigned long long s_tot_pairs, s_tot_all;
+    __shared__ unsigned int s_ticket, s_cls[4];
+    {
+        const int bin = blockIdx.x * 32 + (threadIdx.x & 31), g = threadIdx.x >> 5;
+        const int rpg = (nrows + 7) / 8;
+        const int rb = min(nrows, g * rpg), re = min(nrows, rb + rpg);
+        unsigned int sum = 0;
+        if (bin < nbins) {
+            int r = rb;
+            for (; r + 8 <= re; r += 8) {
+                unsigned int c[8];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) c[k] = counts[(size_t)(r + k) * nbins + bin];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) sum += c[k];
+            }
+            for (; r < re; ++r) sum += counts[(size_t)r * nbins + bin];
+        }
+        s_part[g][threadIdx.x & 31] = sum;
+        __syncthreads();
+        unsigned int run = 0;
+        for (int k = 0; k < g; ++k) run += s_part[k][threadIdx.x & 31];
+        if (bin < nbins) {
+            if (g == 7) bin_count[bin] = run + sum;
+            int r = rb;
+            for (; r + 8 <= re; r += 8) {
+                unsigned int c[8];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) c[k] = counts[(size_t)(r + k) * nbins + bin];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) { counts[(size_t)(r + k) * nbins + bin] = run; run += c[k]; }
+            }
+            for (; r < re; ++r) {
+                const unsigned int c = counts[(size_t)r * nbins + bin];
+                counts[(size_t)r * nbins + bin] = run;
+                run += c;
+            }
+        }
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_ticket = atomicAdd(&stats->scan_done, 1u);
+    __syncthreads();
+    if (s_ticket != gridDim.x - 1) return;
+    __threadfence();
+    // ---- phase 2: one block
+    const int per = (nbins + kScanThreads - 1) / kScanThreads;
     const int b0 = min(nbins, (int)threadIdx.x * per), b1 = min(nbins, b0 + per);
     unsigned long long sum_all = 0, sum_tiles = 0;
-    for (int b = b0; b < b1; ++b) {
-        const unsigned int c = bin_count[b];
-        sum_all += c;
-        if (b < n_tiles) sum_tiles += c;
+    for (int bb = b0; bb < b1; bb += 8) {
+        unsigned int c8[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) c8[k] = (bb + k < b1) ? __ldcg(bin_count + bb + k) : 0u;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) { sum_all += c8[k]; if (bb + k < n_tiles) sum_tiles += c8[k]; }
     }
-    const unsigned long long off_all = block_excl_scan_1024(sum_all, s_warp, &s_tot_all);
-    (void)block_excl_scan_1024(sum_tiles, s_warp, &s_tot_pairs);
+    if (threadIdx.x < 4) s_cls[threadIdx.x] = 0u;
+    __syncthreads();
+    {   // class counts: every thread sums a strided share of the per-block counts
+        unsigned int c[4] = {0u, 0u, 0u, 0u};
+        for (int r = threadIdx.x; r < nrows; r += kScanThreads) {
+            const uint4 v = *reinterpret_cast<const uint4 *>(cls_counts + 4 * r);
+            c[0] += v.x; c[1] += v.y; c[2] += v.z; c[3] += v.w;
+        }
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const unsigned int t = __reduce_add_sync(0xffffffffu, c[k]);
+            if ((threadIdx.x & 31) == 0 && t) atomicAdd(&s_cls[k], t);
+        }
+    }
+    const unsigned long long off_all = block_excl_scan_256(sum_all, s_warp, &s_tot_all);
+    (void)block_excl_scan_256(sum_tiles, s_warp, &s_tot_pairs);
     // chunk size of this frame: about 32 chunks per SM, between kChunkMin and kChunkMax, a multiple of 256
     unsigned long long cs = (s_tot_pairs + (unsigned long long)n_sm * 32 - 1) / ((unsigned long long)n_sm * 32);
     cs = (cs + 255) / 256 * 256;
     cs = min((unsigned long long)kChunkMax, max((unsigned long long)kChunkMin, cs));
     const unsigned int K = (unsigned int)cs;
-    unsigned long long run = off_all, nseg = 0;
-    for (int b = b0; b < b1; ++b) {
-        const unsigned int c = bin_count[b];
-        if (b < n_tiles && c > 0) nseg += (run + c - 1) / K - run / K + 1;
-        run += c;
-    }
-    const unsigned long long off_seg = block_excl_scan_1024(nseg, s_warp, &s_tot_segs);
-    const bool overflow = s_tot_all > capacity || (s_tot_pairs + K - 1) / K > max_chunks;
-    run = off_all;
-    unsigned long long srun = off_seg;
-    for (int b = b0; b < b1; ++b) {
-        const unsigned int c = bin_count[b];
-        bin_start[b] = (unsigned int)run;
-        if (b < n_tiles) {
-            seg_start[b] = (unsigned int)srun;
-            if (c > 0) {
-                srun += (run + c - 1) / K - run / K + 1;
-                if (!overflow)      // chunks whose first record lies in this tile
-                    for (unsigned long long cc = (run + K - 1) / K; cc * K < run + c; ++cc) chunk_tile[cc] = (unsigned int)b;
-            }
+    const bool overflow = s_tot_all > capacity;
+    unsigned long long run = off_all;
+    for (int bb = b0; bb < b1; bb += 8) {            // eight independent loads per round (this block is latency bound)
+        unsigned int c8[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) c8[k] = (bb + k < b1) ? __ldcg(bin_count + bb + k) : 0u;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            if (bb + k < b1) bin_start[bb + k] = (unsigned int)run;
+            run += c8[k];
         }
-        run += c;
     }
-    if (threadIdx.x == 1023) {
-        bin_start[nbins] = (unsigned int)s_tot_all;
-        seg_start[n_tiles] = (unsigned int)s_tot_segs;
-    }
-    if (threadIdx.x < 4) {
-        unsigned long long c = 0;
-        for (int r = 0; r < nrows; ++r) c += cls_counts[r * 4 + threadIdx.x];
-        stats->count[threadIdx.x] = c;
-    }
+    if (threadIdx.x == kScanThreads - 1) bin_start[nbins] = (unsigned int)s_tot_all;
+    if (threadIdx.x < 4) stats->count[threadIdx.x] = s_cls[threadIdx.x];      // block scans above synchronised
     if (threadIdx.x == 0) {
         stats->pairs = s_tot_pairs;
         stats->large_pairs = s_tot_all - s_tot_pairs;
         stats->chunks = overflow ? 0ull : (s_tot_pairs + K - 1) / K;
-        stats->segments = overflow ? 0ull : s_tot_segs;
         stats->capacity = capacity;
         stats->overflow = overflow ? 1u : 0u;
         stats->work_counter = 0u;
         stats->chunk_size = K;
         stats->amax_bits = 0u;
+        stats->scan_done = 0u;
     }
 }
 
@@ -553,48 +578,74 @@ __device__ __forceinline__ int fixed_exponent(unsigned int amax_bits)
     return kFixedBits - ex;
 }
 
-// Framebuffer of a tile in shared memory: per channel a low plane (sums of the low 16 bits of each contribution,
-// unsigned) and a high plane (sums of the signed upper bits).  value = hi * 65536 + lo.  A segment holds at most
-// kChunkMax = 32768 records and a record touches a pixel once, so neither plane can wrap.  Both updates are native
-// 32-bit shared-memory atomics without a return value (64-bit and float atomics on shared memory are CAS loops).
-template <int T> struct SplatCfg {
-    static constexpr int kPix = T * T;
-    static constexpr int kWarps = kSplatThreads / 32;
-    static constexpr size_t kSmemBytes = sizeof(unsigned int) * 6 * kPix + sizeof(float4) * 2 * 32 * kWarps;
-};
+// ---- packed float32 pairs (Blackwell FADD2 / FMUL2 / FFMA2: two IEEE round-to-nearest results per issue slot) ----
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk2(float a, float b) { f32x2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
+__device__ __forceinline__ void upk2(f32x2 v, float &a, float &b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
+__device__ __forceinline__ f32x2 fadd2(f32x2 a, f32x2 b) { f32x2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2 fmul2(f32x2 a, f32x2 b) { f32x2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2 ffma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
 
+// Framebuffer of a tile in shared memory, fixed point: per channel a low plane (sums of the low 16 bits of each
+// contribution, unsigned) and a high plane (sums of the signed upper bits).  value = hi * 65536 + lo, in units of
+// 2^-e.  A segment holds at most kChunkMax = 32768 records and a record touches a pixel once, so neither plane can
+// wrap.  Updates are native 32-bit shared-memory atomics without a return value (64-bit and float atomics on shared
+// memory are CAS loops on sm_100).  Integer sums are exact and independent of the order.
 __device__ __forceinline__ void fixed_add(unsigned int *lo, unsigned int *hi, float value)
 {
     const int v = __float2int_rn(value);                // |v| <= 2^kFixedBits
-    atomicAdd(lo, (unsigned int)v & 0xffffu);
     const int up = v >> 16;
-    if (up != 0) atomicAdd(hi, (unsigned int)up);
+    const unsigned int alo = (unsigned int)__cvta_generic_to_shared(lo), ahi = (unsigned int)__cvta_generic_to_shared(hi);
+    asm volatile("{\n\t.reg .pred p;\n\tred.shared.add.u32 [%0], %2;\n\tsetp.ne.s32 p, %3, 0;\n\t@p red.shared.add.u32 [%1], %3;\n\t}"
+                 :: "r"(alo), "r"(ahi), "r"((unsigned int)v & 0xffffu), "r"(up) : "memory");
 }
 
-// One work item = chunk_size consecutive records; the chunk is cut into segments at tile boundaries.  For each
-// segment the CTA clears the tile framebuffer, every warp takes batches of 32 records, lays the fragments (pixels
-// of the records' boxes, which k_scatter already clipped to the tile) of the batch end to end and hands 32
-// consecutive fragments to its 32 lanes per step, so lanes stay busy whatever the footprint (1 pixel for SMALL
-// records).  Per fragment: locate the record (ballot / popc), decode the pixel (multiply-shift division), C1 inside
-// test, one ex2, three fixed-point adds.  The only conversion-pipe work per fragment is the ex2 and three F2I.
-// The segment's framebuffer goes to its partial slot; k_compose adds the slots of a tile.
+// Geometry of the tile renderer: a warp owns a strip of 64 pixels (16 x 4, or 8 x 8 for T = 8), a lane owns two
+// horizontally adjacent pixels of it and keeps their RGB sums in registers as packed pairs.
+template <int T> struct SplatCfg {
+    static constexpr int kPix = T * T;
+    static constexpr int kSW = T >= 16 ? 16 : 8;         // strip width
+    static constexpr int kSH = 64 / kSW;                 // strip height
+    static constexpr int kStripsX = T / kSW, kStripsY = T / kSH;
+    static constexpr int kWarps = kStripsX * kStripsY;   // 1, 4, 16 for T = 8, 16, 32
+    static constexpr int kThreads = 32 * kWarps;         // one record per thread and batch
+    static constexpr int kFoldBatches = 1024 / kThreads > 0 ? 1024 / kThreads : 1;   // fold the sub-sums every ~1024 records
+    static constexpr size_t kSmemBytes = sizeof(unsigned int) * 6 * kPix + (sizeof(float4) * 2 + sizeof(unsigned int)) * kThreads;
+};
+
+// One work item = chunk_size consecutive records of the bin-sorted array; the chunk is cut into segments at tile
+// boundaries.  Per segment the CTA clears the tile's fixed-point planes and its register sums, then takes batches
+// of one record per thread:
+//   * records whose box is at most 2 x 2 pixels (every SMALL record, the smallest MEDIUM ones) are splatted by the
+//     thread that loaded them, pixel by pixel, into the fixed-point planes (shared-memory integer atomics);
+//   * all other records are staged in shared memory with the set of strips their box touches; every warp walks the
+//     records that touch its strip and evaluates each for its 64 pixels at once: the C1 inside test and the Gaussian
+//     weight in packed float32 pairs (FADD2 / FFMA2 / FMUL2), two ex2, three packed FMAs into registers.  No atomics,
+//     no conversions, no per-fragment index arithmetic; this is the paper's "one pixel per thread, particles in
+//     sequence" scheme (:226) with the block replaced by a 64-pixel warp strip and a box test in front.
+// Register sums are two-level (folded every ~1024 records) so a pixel that receives thousands of contributions in a
+// segment keeps float32 sums accurate to ~1e-6.  At the end of the segment each lane converts its sums to fixed
+// point and adds them to the planes of its own pixels; the planes are then added to the tile's 64-bit sums in global
+// memory (`accum`, cleared before every frame), which k_compose turns into the image.
 template <int T>
-__global__ void __launch_bounds__(kSplatThreads)
-k_splat(const float4 *__restrict__ records, const unsigned int *__restrict__ bin_start,
-        const unsigned int *__restrict__ seg_start, const unsigned int *__restrict__ chunk_tile,
-        DeviceStats *__restrict__ stats, unsigned int *__restrict__ partials, const __grid_constant__ FrameParams fp)
+__global__ void __launch_bounds__(SplatCfg<T>::kThreads)
+k_splat(const float4 *__restrict__ records, const unsigned int *__restrict__ bin_start, DeviceStats *__restrict__ stats,
+        unsigned long long *__restrict__ accum, const __grid_constant__ FrameParams fp)
 {
     using Cfg = SplatCfg<T>;
-    constexpr int kPix = Cfg::kPix;
+    constexpr int kPix = Cfg::kPix, kThreads = Cfg::kThreads;
     extern __shared__ __align__(16) unsigned int smem_u[];
     unsigned int *fb = smem_u;                                            // lo R G B, hi R G B
-    float4 *stage_all = reinterpret_cast<float4 *>(smem_u + 6 * kPix);
+    float4 *stA = reinterpret_cast<float4 *>(smem_u + 6 * kPix);
+    float4 *stB = stA + kThreads;
+    unsigned int *stM = reinterpret_cast<unsigned int *>(stB + kThreads);  // strips touched: x mask << 16 | y mask (0: not staged)
     __shared__ unsigned int s_chunk;
-    __shared__ unsigned int s_inv[32];                                    // 65536 / w + 1: k / w = (k * inv) >> 16 for k < 1024
+    __shared__ int s_tile;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    float4 *stA = stage_all + warp * 64, *stB = stA + 32;
-    const unsigned int lane_le = 0xffffffffu >> (31 - lane);
-    if (threadIdx.x < 32) s_inv[threadIdx.x] = 65536u / (threadIdx.x + 1u) + 1u;
+    // this lane's pixel pair inside the tile
+    const int sx = warp % Cfg::kStripsX, sy = warp / Cfg::kStripsX;
+    const int lx = sx * Cfg::kSW + 2 * (lane % (Cfg::kSW / 2)), ly = sy * Cfg::kSH + lane / (Cfg::kSW / 2);
+    const unsigned int my_strip = (1u << (16 + sx)) | (1u << sy);
     const unsigned int total = (unsigned int)stats->chunks;
     const unsigned int K = stats->chunk_size;
     const unsigned int pairs = (unsigned int)stats->pairs;
@@ -602,74 +653,134 @@ k_splat(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
     const float sc1 = pow2i(e / 2), sc2 = pow2i(e - e / 2);
     for (;;) {
         __syncthreads();
-        if (threadIdx.x == 0) s_chunk = atomicAdd(&stats->work_counter, 1u);
+        if (warp == 0) {
+            // next chunk, and the tile that holds its first record: the last tile t with bin_start[t] <= r0, found
+            // by a 32-way search over bin_start (three or four rounds of 32 probes)
+            unsigned int c = 0u;
+            if (lane == 0) c = atomicAdd(&stats->work_counter, 1u);
+            c = __shfl_sync(0xffffffffu, c, 0);
+            if (c < total) {
+                const unsigned int r = c * K;
+                int lo = 0, n = fp.n_tiles;                       // answer in [lo, lo + n)
+                while (n > 1) {
+                    const int step = (n + 31) / 32;
+                    const int t = lo + lane * step;
+                    const bool le = t < lo + n && __ldg(bin_start + t) <= r;
+                    const int k = __popc(__ballot_sync(0xffffffffu, le)) - 1;     // lane 0 always qualifies
+                    lo += k * step;
+                    n = min(step, n - k * step);
+                }
+                if (lane == 0) s_tile = lo;
+            }
+            if (lane == 0) s_chunk = c;
+        }
         __syncthreads();
         const unsigned int chunk = s_chunk;
         if (chunk >= total) break;
         const unsigned int r0 = chunk * K, r1 = min(r0 + K, pairs);
-        int tile = (int)chunk_tile[chunk];
+        int tile = s_tile;
         unsigned int tb = bin_start[tile], te = bin_start[tile + 1];
         for (;;) {
             // ---- segment = [max(tb, r0), min(te, r1)) of `tile`
             const unsigned int begin = max(tb, r0), end = min(te, r1);
-            for (int i = threadIdx.x; i < 6 * kPix; i += kSplatThreads) fb[i] = 0u;
+            for (int i = threadIdx.x; i < 6 * kPix; i += kThreads) fb[i] = 0u;
             __syncthreads();
             const int tx0 = (tile % fp.ntx) * T, ty0 = (tile / fp.ntx) * T;
-            // (float)(tx0 + lx) + 0.5 = int_as_float(0x4B000000 | lx) + ox, exactly (ox = tx0 + 0.5 - 2^23)
-            const float ox = __fsub_rn(__fadd_rn((float)tx0, 0.5f), 8388608.0f);
-            const float oy = __fsub_rn(__fadd_rn((float)ty0, 0.5f), 8388608.0f);
-            for (unsigned int base = begin + warp * 32; base < end; base += kSplatThreads) {
-                const unsigned int idx = base + lane;
-                const bool valid = idx < end;
+            const float fx = __fadd_rn((float)(tx0 + lx), 0.5f), fy = __fadd_rn((float)(ty0 + ly), 0.5f);
+            const f32x2 fxp = pk2(fx, __fadd_rn(fx, 1.0f));
+            f32x2 accR = 0ull, accG = 0ull, accB = 0ull, subR = 0ull, subG = 0ull, subB = 0ull;   // +0.0f pairs
+            int fold = 0;
+            for (unsigned int base = begin; base < end; base += kThreads) {
+                const unsigned int idx = base + threadIdx.x;
                 float4 ra = make_float4(0.f, 0.f, 0.f, 0.f), rb = ra;
-                if (valid) ld_record(records, idx, ra, rb);
-                const unsigned int box = __float_as_uint(rb.w);
-                const int bw = (int)((box >> 10) & 31u) + 1, bh = (int)((box >> 15) & 31u) + 1;
-                const int nfrag = valid ? bw * bh : 0;
-                int incl = nfrag;
+                unsigned int touch = 0u;
+                if (idx < end) {
+                    ld_record(records, idx, ra, rb);
+                    const unsigned int box = __float_as_uint(rb.w);
+                    const int bx0 = (int)(box & 31u), by0 = (int)((box >> 5) & 31u);
+                    const int bw1 = (int)((box >> 10) & 31u), bh1 = (int)((box >> 15) & 31u);     // width - 1, height - 1
+                    if (bw1 <= 1 && bh1 <= 1) {
+                        // ---- direct path: at most 2 x 2 pixels, fixed point
+                        const float ax = rb.x * sc1 * sc2, ay = rb.y * sc1 * sc2, az = rb.z * sc1 * sc2;
+                        const float fx0 = __fadd_rn((float)(tx0 + bx0), 0.5f), fy0 = __fadd_rn((float)(ty0 + by0), 0.5f);
 #pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const int t = __shfl_up_sync(0xffffffffu, incl, o);
-                    if (lane >= o) incl += t;
-                }
-                const int start = incl - nfrag;
-                const int F = __shfl_sync(0xffffffffu, incl, 31);
-                stA[lane] = ra;
-                stB[lane] = make_float4(rb.x * sc1 * sc2, rb.y * sc1 * sc2, rb.z * sc1 * sc2,
-                                        __uint_as_float((unsigned int)start | ((box & 0x3ffu) << 15) | ((box & 0x7c00u) << 15)));
-                __syncwarp();
-                for (int f0 = 0; f0 < F; f0 += 32) {
-                    const int rel = start - f0;
-                    const unsigned int m = __reduce_or_sync(0xffffffffu, (valid && rel >= 0 && rel < 32) ? (1u << rel) : 0u);
-                    const int nb = __popc(__ballot_sync(0xffffffffu, valid && rel < 0));
-                    const int f = f0 + lane;
-                    if (f < F) {
-                        const int s = nb - 1 + __popc(m & lane_le);
-                        const float4 A = stA[s], B = stB[s];
-                        const unsigned int pk = __float_as_uint(B.w);
-                        const unsigned int k = (unsigned int)f - (pk & 0x7fffu);
-                        const unsigned int wm1 = pk >> 25;
-                        const unsigned int j = (k * s_inv[wm1]) >> 16;
-                        const unsigned int lx = ((pk >> 15) & 31u) + (k - j * (wm1 + 1u)), ly = ((pk >> 20) & 31u) + j;
-                        const float dxf = __fsub_rn(__fadd_rn(__uint_as_float(0x4B000000u | lx), ox), A.x);
-                        const float dyf = __fsub_rn(__fadd_rn(__uint_as_float(0x4B000000u | ly), oy), A.y);
-                        const float d2 = __fmaf_rn(dxf, dxf, __fmul_rn(dyf, dyf));
-                        if (d2 <= A.w) {
-                            const float wgt = ex2_approx(d2 * A.z);
-                            unsigned int *q = fb + ly * T + lx;
-                            fixed_add(q, q + 3 * kPix, B.x * wgt);
-                            fixed_add(q + kPix, q + 4 * kPix, B.y * wgt);
-                            fixed_add(q + 2 * kPix, q + 5 * kPix, B.z * wgt);
+                        for (int q = 0; q < 4; ++q) {
+                            const int qx = q & 1, qy = q >> 1;
+                            if (qx <= bw1 && qy <= bh1) {
+                                const float dxf = __fsub_rn(qx ? __fadd_rn(fx0, 1.0f) : fx0, ra.x);
+                                const float dyf = __fsub_rn(qy ? __fadd_rn(fy0, 1.0f) : fy0, ra.y);
+                                const float d2 = __fmaf_rn(dxf, dxf, __fmul_rn(dyf, dyf));
+                                if (d2 <= ra.w) {
+                                    const float wgt = ex2_approx(d2 * ra.z);
+                                    unsigned int *q0 = fb + (by0 + qy) * T + bx0 + qx;
+                                    fixed_add(q0, q0 + 3 * kPix, ax * wgt);
+                                    fixed_add(q0 + kPix, q0 + 4 * kPix, ay * wgt);
+                                    fixed_add(q0 + 2 * kPix, q0 + 5 * kPix, az * wgt);
+                                }
+                            }
                         }
+                    } else {
+                        const int x1 = bx0 + bw1, y1 = by0 + bh1;
+                        const unsigned int xm = (2u << (x1 / Cfg::kSW)) - (1u << (bx0 / Cfg::kSW));
+                        const unsigned int ym = (2u << (y1 / Cfg::kSH)) - (1u << (by0 / Cfg::kSH));
+                        touch = (xm << 16) | ym;
                     }
                 }
-                __syncwarp();
+                __syncthreads();                         // previous batch fully consumed
+                stA[threadIdx.x] = ra; stB[threadIdx.x] = rb; stM[threadIdx.x] = touch;
+                __syncthreads();
+#pragma unroll 1
+                for (int g = 0; g < kThreads; g += 32) {
+                    const unsigned int t = stM[g + lane];
+                    unsigned int m = __ballot_sync(0xffffffffu, (t & my_strip & 0xffff0000u) && (t & my_strip & 0xffffu));
+                    while (m) {
+                        const int r = g + __ffs(m) - 1;
+                        m &= m - 1;
+                        const float4 A = stA[r], B = stB[r];
+                        const float dyf = __fsub_rn(fy, A.y);
+                        const f32x2 dx = fadd2(fxp, pk2(-A.x, -A.x));
+                        const float t2 = __fmul_rn(dyf, dyf);
+                        const f32x2 d2 = ffma2(dx, dx, pk2(t2, t2));
+                        const f32x2 arg = fmul2(d2, pk2(A.z, A.z));
+                        float d20, d21, a0, a1;
+                        upk2(d2, d20, d21); upk2(arg, a0, a1);
+                        const float w0 = d20 <= A.w ? ex2_approx(a0) : 0.0f;
+                        const float w1 = d21 <= A.w ? ex2_approx(a1) : 0.0f;
+                        const f32x2 w = pk2(w0, w1);
+                        subR = ffma2(pk2(B.x, B.x), w, subR);
+                        subG = ffma2(pk2(B.y, B.y), w, subG);
+                        subB = ffma2(pk2(B.z, B.z), w, subB);
+                    }
+                }
+                if (++fold == Cfg::kFoldBatches) {
+                    fold = 0;
+                    accR = fadd2(accR, subR); accG = fadd2(accG, subG); accB = fadd2(accB, subB);
+                    subR = subG = subB = 0ull;
+                }
+            }
+            accR = fadd2(accR, subR); accG = fadd2(accG, subG); accB = fadd2(accB, subB);
+            __syncthreads();                             // all direct-path atomics of the segment have landed
+            {   // register sums -> fixed point, added to this lane's own two pixels (no other thread touches them now)
+                float v[6];
+                upk2(accR, v[0], v[1]); upk2(accG, v[2], v[3]); upk2(accB, v[4], v[5]);
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+#pragma unroll
+                    for (int q = 0; q < 2; ++q) {
+                        const long long f = __float2ll_rn(v[2 * c + q] * sc1 * sc2);
+                        unsigned int *q0 = fb + c * kPix + ly * T + lx + q;
+                        q0[0] += (unsigned int)(f & 0xffffll);
+                        q0[3 * kPix] += (unsigned int)(int)(f >> 16);
+                    }
             }
             __syncthreads();
-            // ---- flush the segment's framebuffer to its partial slot
-            const unsigned int seg = seg_start[tile] + (chunk - tb / K);
-            unsigned int *out = partials + (size_t)seg * (6 * kPix);
-            for (int i = threadIdx.x; i < 6 * kPix; i += kSplatThreads) out[i] = fb[i];
+            // ---- add the segment's planes to the tile's sums in global memory (64-bit integer reductions in L2:
+            //      exact and commutative, so the order in which the segments of a heavy tile arrive does not matter)
+            unsigned long long *out = accum + (size_t)tile * (3 * kPix);
+            for (int i = threadIdx.x; i < 3 * kPix; i += kThreads) {
+                const long long v = (long long)(int)fb[3 * kPix + i] * 65536ll + (long long)fb[i];
+                if (v != 0ll) atomicAdd(out + i, (unsigned long long)v);
+            }
             if (te >= r1) break;
             // ---- next non-empty tile
             do { ++tile; tb = te; te = bin_start[tile + 1]; } while (te == tb);
@@ -679,15 +790,14 @@ k_splat(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
 }
 
 // ---- A6 + A8: compose one tile ----------------------------------------------------------------------------------
-// Thread t owns pixels t, t+256, ... of the tile (registers).  Adds the tile's segment partials (integers, exact),
-// then gathers the LARGE records of the tile's super-tile (each record's box is tested against the tile,
-// survivors are staged in shared memory and evaluated by every pixel owner), in two-level float32 accumulation.
+// Thread t owns pixels t, t+256, ... of the tile (registers).  Reads the tile's fixed-point sums, then gathers the
+// LARGE records of the tile's super-tile (each record's box is tested against the tile, survivors are staged in
+// shared memory and evaluated by every pixel owner), in two-level float32 accumulation.
 template <int T>
 __global__ void __launch_bounds__(256)
-k_compose(const unsigned int *__restrict__ partials, const unsigned int *__restrict__ seg_start,
-          const float4 *__restrict__ records, const unsigned int *__restrict__ bin_start,
-          const DeviceStats *__restrict__ stats, const __grid_constant__ FrameParams fp,
-          float *__restrict__ image)
+k_compose(const unsigned long long *__restrict__ accum, const float4 *__restrict__ records,
+          const unsigned int *__restrict__ bin_start, const DeviceStats *__restrict__ stats,
+          const __grid_constant__ FrameParams fp, float *__restrict__ image)
 {
     constexpr int kPix = T * T;
     constexpr int kPpt = (kPix + 255) / 256;
@@ -710,28 +820,13 @@ k_compose(const unsigned int *__restrict__ partials, const unsigned int *__restr
     }
     const bool ok = stats->overflow == 0u;
     if (ok) {
-        const unsigned int s0 = seg_start[tile], s1 = seg_start[tile + 1];
-        // four segments per round: 6 * 4 independent loads per pixel in flight (heavy tiles own hundreds of segments)
-        for (unsigned int sg = s0; sg < s1; sg += 4) {
 #pragma unroll
-            for (int k = 0; k < kPpt; ++k) {
-                const int p = threadIdx.x + k * 256;
-                if (p < kPix) {
-                    unsigned int v[4][6];
+        for (int k = 0; k < kPpt; ++k) {
+            const int p = threadIdx.x + k * 256;
+            if (p < kPix) {
+                const unsigned long long *q = accum + (size_t)tile * (3 * kPix) + p;
 #pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        const unsigned int *q = partials + (size_t)min(sg + u, s1 - 1) * (6 * kPix) + p;
-#pragma unroll
-                        for (int c = 0; c < 6; ++c) v[u][c] = __ldg(q + c * kPix);
-                    }
-#pragma unroll
-                    for (int u = 0; u < 4; ++u)
-                        if (sg + u < s1) {
-#pragma unroll
-                            for (int c = 0; c < 3; ++c)
-                                fix[k][c] += (long long)(int)v[u][3 + c] * 65536ll + (long long)v[u][c];
-                        }
-                }
+                for (int c = 0; c < 3; ++c) fix[k][c] = (long long)__ldg(q + c * kPix);
             }
         }
         const int sbin = fp.n_tiles + (ty >> kSuperShift) * fp.nsx + (tx >> kSuperShift);
