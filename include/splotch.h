@@ -86,13 +86,15 @@ typedef struct {
 typedef struct {
     uint64_t n;                      /* particles of the last frame                                         */
     uint64_t count[4];               /* per class, indexed by SPLOTCH_CULLED .. SPLOTCH_LARGE               */
-    uint64_t pairs;                  /* (particle, tile) pairs of SMALL + MEDIUM particles                  */
+    uint64_t pairs;                  /* (particle, tile) pairs of SMALL + MEDIUM particles (ordered mode:
+                                        of all active particles, LARGE ones are binned to tiles as well)    */
     uint64_t large_pairs;            /* (particle, super-tile) pairs of LARGE particles                     */
     uint64_t chunks;                 /* work items of the tile renderer                                     */
     uint64_t pair_capacity;          /* records the workspace could hold                                    */
     int32_t  overflow;               /* 1: pairs + large_pairs > pair_capacity, the image is all zero       */
     int32_t  n_stages;               /* number of valid entries in stage_ms (0 unless profiling is on)      */
-    float    stage_ms[8];            /* count, scan, scatter, splat, compose, ... (see splotch_stage_name)  */
+    float    stage_ms[8];            /* additive: count, scan, scatter, splat, compose; ordered: count, scan,
+                                        pairs, sort, bounds, render, combine (see splotch_stage_name)        */
 } splotch_stats;
 
 /* Create a context for images of width x height on CUDA device `device`; at most max_particles per frame.
@@ -144,7 +146,7 @@ int splotch_render_host(splotch_ctx *ctx, const splotch_particles *host_particle
 
 /* Statistics of the last frame.  Synchronises the stream of that frame.  HOST out. */
 int splotch_get_stats(splotch_ctx *ctx, splotch_stats *out);
-const char *splotch_stage_name(int stage);
+const char *splotch_stage_name(int additive, int stage);   /* stage names of an additive / ordered frame */
 
 /* Test hooks: the per-particle results of the classification stage, written to DEVICE arrays of length n
  * (any may be NULL): cls int8; px, py (screen centre), sp (sigma in px), rp (r(p)), zc (camera depth)
@@ -154,7 +156,7 @@ int splotch_debug_geometry(splotch_ctx *ctx, const splotch_particles *particles,
                            const splotch_params *params, int8_t *cls, float *px, float *py, float *sp,
                            float *rp, float *zc, int32_t *pbox, int32_t *tbox, int32_t *ilabel,
                            void *cuda_stream);
-/* Per-tile pair counts of the last frame: DEVICE out, nty x ntx uint32. */
+/* Per-tile pair counts of the last frame: DEVICE out, nty x ntx uint32 (SMALL + MEDIUM; ordered mode: all). */
 int splotch_debug_tile_counts(splotch_ctx *ctx, uint32_t *out, void *cuda_stream);
 
 const char *splotch_last_error(const splotch_ctx *ctx);

@@ -82,7 +82,7 @@ def load() -> C.CDLL:
     lib.splotch_render.argtypes = [vp, C.POINTER(SplotchParticles), u64, C.POINTER(SplotchParams), vp, vp, C.c_size_t, vp]
     lib.splotch_render_host.argtypes = lib.splotch_render.argtypes
     lib.splotch_get_stats.argtypes = [vp, C.POINTER(SplotchStats)]
-    lib.splotch_stage_name.argtypes = [i32]
+    lib.splotch_stage_name.argtypes = [i32, i32]
     lib.splotch_stage_name.restype = C.c_char_p
     lib.splotch_debug_geometry.argtypes = [vp, C.POINTER(SplotchParticles), u64, C.POINTER(SplotchParams)] + [vp] * 10
     lib.splotch_debug_tile_counts.argtypes = [vp, vp, vp]
@@ -240,7 +240,8 @@ class Renderer:
         _check(self.ctx, self.lib.splotch_get_stats(self.ctx, C.byref(st)))
         d = {"n": st.n, "count": list(st.count), "pairs": st.pairs, "large_pairs": st.large_pairs,
              "chunks": st.chunks, "pair_capacity": st.pair_capacity, "overflow": st.overflow,
-             "stage_ms": {self.lib.splotch_stage_name(i).decode(): st.stage_ms[i] for i in range(st.n_stages)}}
+             "stage_ms": {self.lib.splotch_stage_name(int(st.n_stages <= 5), i).decode(): st.stage_ms[i]
+                          for i in range(st.n_stages)}}
         return d
 
     def debug_geometry(self, fields: Dict[str, torch.Tensor], species: Sequence, **params) -> Dict[str, torch.Tensor]:

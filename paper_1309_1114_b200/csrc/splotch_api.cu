@@ -2,6 +2,7 @@
 // Argument checking, camera constants, workspace layout and the per-frame kernel sequence.  No compute happens on
 // the host: every stage of the path is one of the kernels in splotch_kernels.cuh.
 #include "splotch_kernels.cuh"
+#include "splotch_ordered.cuh"
 #include "../../include/splotch.h"
 
 #include <math.h>
@@ -14,14 +15,20 @@ using namespace splotch;
 
 namespace {
 
-constexpr int kStages = 5;
+constexpr int kStages = 7;                  // most stages a frame has (ordered mode); additive frames have 5
+constexpr int kStagesAdditive = 5, kStagesOrdered = 7;
 constexpr int kProfRing = 256;              // frames of per-stage events kept while profiling
-const char *kStageNames[kStages] = {"count", "scan", "scatter", "splat", "compose"};
+const char *kStageNamesAdditive[kStagesAdditive] = {"count", "scan", "scatter", "splat", "compose"};
+const char *kStageNamesOrdered[kStagesOrdered] = {"count", "scan", "pairs", "sort", "bounds", "render", "combine"};
 
 struct Layout {
     size_t counts, cls_counts, bin_count, bin_start, stats, accum, accum_bytes, records, staging, total;
     unsigned long long capacity;
     int nrows;
+    // ordered mode
+    size_t blk_pairs, tile_start, rec, keys[2], vals[2], hist, sums, seg;
+    int nblk_o, nblk_rs, n_sums;
+    unsigned int m_hist;
 };
 
 }  // namespace
@@ -44,8 +51,11 @@ struct splotch_ctx {
     Layout lay{};
     FrameParams fp{};
     unsigned long long last_n = 0;
+    bool last_additive = true;
+    int prof_stages = kStagesAdditive;              // stages of the frames recorded since profiling was enabled
     cudaStream_t last_stream = nullptr;
     int splat_blocks_per_sm[3] = {0, 0, 0};  // T = 8, 16, 32
+    int orender_blocks_per_sm[3] = {0, 0, 0};
     char err[512] = {0};
 };
 
@@ -127,6 +137,52 @@ bool make_layout(const splotch_ctx *c, unsigned long long n, int T, unsigned lon
     return bytes == 0 || off <= bytes;
 }
 
+// Workspace layout of the ordered mode for a given pair capacity.
+void make_layout_ordered(const splotch_ctx *c, unsigned long long n, int T, unsigned long long capacity, bool staging, Layout *L)
+{
+    const int ntx = (c->width + T - 1) / T, nty = (c->height + T - 1) / T;
+    const size_t n_tiles = (size_t)ntx * nty;
+    L->capacity = capacity;
+    L->nblk_o = (int)((n + kOBlockParticles - 1) / kOBlockParticles);
+    L->nblk_rs = (int)((capacity + kRsTile - 1) / kRsTile);
+    if (L->nblk_rs < 1) L->nblk_rs = 1;
+    L->m_hist = 256u * (unsigned int)L->nblk_rs;
+    L->n_sums = (int)((L->m_hist + kScTile - 1) / kScTile);
+    size_t off = 0;
+    L->stats = off;       off = align_up(off + sizeof(DeviceStats), 256);
+    L->blk_pairs = off;   off = align_up(off + sizeof(unsigned int) * (size_t)(L->nblk_o + 1), 256);
+    L->tile_start = off;  off = align_up(off + sizeof(unsigned int) * (n_tiles + 1), 256);
+    L->hist = off;        off = align_up(off + sizeof(unsigned int) * (size_t)L->m_hist, 256);
+    L->sums = off;        off = align_up(off + sizeof(unsigned int) * (size_t)L->n_sums, 256);
+    L->rec = off;         off = align_up(off + 32ull * n, 256);
+    L->staging = off;
+    if (staging) {
+        off = align_up(off + 6 * align_up(sizeof(float) * n, 256), 256);
+        off = align_up(off + sizeof(float) * 3 * (size_t)c->width * c->height, 256);
+    }
+    for (int k = 0; k < 2; ++k) { L->keys[k] = off; off = align_up(off + 8ull * capacity, 256); }
+    for (int k = 0; k < 2; ++k) { L->vals[k] = off; off = align_up(off + 4ull * capacity, 256); }
+    // one (t, c_R, c_G, c_B) per pixel and segment; segment slot = chunk + tile, chunks <= ceil(capacity / kOChunkMin)
+    L->seg = off;
+    off = align_up(off + sizeof(float4) * (size_t)T * T * ((capacity + kOChunkMin - 1) / kOChunkMin + n_tiles + 1), 256);
+    L->total = off;
+}
+
+// Largest capacity whose ordered layout fits in `bytes` (0 if not even an empty frame fits).
+bool fit_layout_ordered(const splotch_ctx *c, unsigned long long n, int T, size_t bytes, bool staging, Layout *L)
+{
+    make_layout_ordered(c, n, T, 0, staging, L);
+    if (L->total + 8192 > bytes) return false;
+    unsigned long long lo = 0, hi = 0xfffffff0ull;
+    while (lo < hi) {
+        const unsigned long long mid = lo + (hi - lo + 1) / 2;
+        make_layout_ordered(c, n, T, mid, staging, L);
+        if (L->total + 8192 <= bytes) lo = mid; else hi = mid - 1;
+    }
+    make_layout_ordered(c, n, T, lo, staging, L);
+    return true;
+}
+
 template <int T>
 int query_splat_occupancy(splotch_ctx *c, int *out)
 {
@@ -151,7 +207,9 @@ int check_params(splotch_ctx *c, const splotch_particles *p, unsigned long long 
     if (bin_smem_bytes(c->width, c->height, q->tile) + 1024 > (size_t)c->smem_optin)
         return fail(c, SPLOTCH_EINVAL, "tile %d gives too many tiles for a %dx%d image (per-block histogram exceeds shared memory); use a larger tile",
                     q->tile, c->width, c->height);
-    if (!q->additive) return fail(c, SPLOTCH_EINVAL, "ordered (E != A) mode is not built yet");
+    if (!q->additive)
+        for (int s = 0; s < (p->species_offsets ? p->n_species : 1) && s < kMaxSpecies && q->species; ++s)
+            if (!(q->species[s].absorb >= 0.0f)) return fail(c, SPLOTCH_EINVAL, "species %d: absorb must be >= 0", s);
     const int ns = p->species_offsets ? p->n_species : 1;
     if (ns < 1 || ns > kMaxSpecies) return fail(c, SPLOTCH_EINVAL, "n_species must be 1..%d", kMaxSpecies);
     if (!q->species) return fail(c, SPLOTCH_EINVAL, "null species parameters");
@@ -258,8 +316,91 @@ int render_device(splotch_ctx *c, const splotch_particles *p, unsigned long long
     else rc = launch_render_tail<32>(c, L, ws, fp, image, st);
     if (rc != SPLOTCH_OK) return rc;
     CU_TRY(c, cudaGetLastError());
-    c->have_frame = true; c->ws = ws; c->lay = L; c->fp = fp; c->last_n = n; c->last_stream = st;
-    if (c->profiling) ++c->prof_frames;
+    c->have_frame = true; c->ws = ws; c->lay = L; c->fp = fp; c->last_n = n; c->last_stream = st; c->last_additive = true;
+    if (c->profiling) { ++c->prof_frames; c->prof_stages = kStagesAdditive; }
+    return SPLOTCH_OK;
+}
+
+template <int T>
+void launch_ordered_tail(splotch_ctx *c, const Layout &L, char *ws, const FrameParams &fp, const unsigned long long *keys,
+                         const unsigned int *vals, float *image, cudaStream_t st)
+{
+    const int ti = T == 8 ? 0 : T == 16 ? 1 : 2;
+    DeviceStats *stats = (DeviceStats *)(ws + L.stats);
+    const unsigned int *tile_start = (const unsigned int *)(ws + L.tile_start);
+    k_orender<T><<<c->n_sm * c->orender_blocks_per_sm[ti], SplatCfg<T>::kThreads, 0, st>>>(
+        (const float4 *)(ws + L.rec), keys, vals, tile_start, stats, (float4 *)(ws + L.seg), fp);
+    if (c->profiling) cudaEventRecord(c->ev[6], st);
+    k_ocombine<T><<<fp.n_tiles, 256, 0, st>>>((const float4 *)(ws + L.seg), tile_start, stats, fp, image);
+    if (c->profiling) cudaEventRecord(c->ev[7], st);
+}
+
+// Ordered (E != A) frame: count -> scan -> pairs -> radix sort -> bounds -> render -> combine, all on `st`.
+int render_ordered(splotch_ctx *c, const splotch_particles *p, unsigned long long n, const FrameParams &fp,
+                   const Layout &L, float *image, char *ws, cudaStream_t st)
+{
+    const bool al = aligned16(p);
+    DeviceStats *stats = (DeviceStats *)(ws + L.stats);
+    unsigned int *blk = (unsigned int *)(ws + L.blk_pairs);
+    unsigned int *hist = (unsigned int *)(ws + L.hist), *sums = (unsigned int *)(ws + L.sums);
+    unsigned long long *keys[2] = {(unsigned long long *)(ws + L.keys[0]), (unsigned long long *)(ws + L.keys[1])};
+    unsigned int *vals[2] = {(unsigned int *)(ws + L.vals[0]), (unsigned int *)(ws + L.vals[1])};
+    if (c->profiling) {
+        c->ev = c->ev_ring[c->prof_frames % kProfRing];
+        cudaEventRecord(c->ev[0], st);
+    }
+    cudaMemsetAsync(stats, 0, sizeof(DeviceStats), st);
+    if (L.nblk_o > 0) {
+        if (al) k_ocount<true><<<L.nblk_o, kOThreads, 0, st>>>(p->x, p->y, p->z, p->h, n, fp, blk, stats);
+        else    k_ocount<false><<<L.nblk_o, kOThreads, 0, st>>>(p->x, p->y, p->z, p->h, n, fp, blk, stats);
+    }
+    if (c->profiling) cudaEventRecord(c->ev[1], st);
+    k_oscan<<<1, kOScanThreads, 0, st>>>(blk, L.nblk_o, n, L.capacity, c->n_sm, stats);
+    if (c->profiling) cudaEventRecord(c->ev[2], st);
+    if (L.nblk_o > 0) {
+        const size_t lsm = sizeof(float4) * kLutSmemMax;
+        if (al) k_opairs<true><<<L.nblk_o, kOThreads, lsm, st>>>(p->x, p->y, p->z, p->h, p->I, p->scalar, n, fp, blk, stats,
+                                                                 (float4 *)(ws + L.rec), keys[0], vals[0]);
+        else    k_opairs<false><<<L.nblk_o, kOThreads, lsm, st>>>(p->x, p->y, p->z, p->h, p->I, p->scalar, n, fp, blk, stats,
+                                                                  (float4 *)(ws + L.rec), keys[0], vals[0]);
+    }
+    if (c->profiling) cudaEventRecord(c->ev[3], st);
+    // radix passes: 4 bytes of depth, then the bytes of the tile index
+    int tile_bytes = 1;
+    while (tile_bytes < 4 && (fp.n_tiles - 1) >> (8 * tile_bytes)) ++tile_bytes;
+    int cur = 0;
+    for (int pass = 0; pass < 4 + tile_bytes; ++pass) {
+        const int shift = 8 * pass;
+        k_rs_count<<<L.nblk_rs, kRsThreads, 0, st>>>(keys[cur], stats, shift, L.nblk_rs, hist);
+        k_sc_reduce<<<L.n_sums, kScThreads, 0, st>>>(hist, L.m_hist, sums);
+        k_sc_top<<<1, 1024, 0, st>>>(sums, L.n_sums);
+        k_sc_apply<<<L.n_sums, kScThreads, 0, st>>>(hist, L.m_hist, sums);
+        k_rs_scatter<<<L.nblk_rs, kRsThreads, sizeof(RsSmem), st>>>(keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], stats, shift,
+                                                                     L.nblk_rs, hist);
+        cur ^= 1;
+    }
+    if (c->profiling) cudaEventRecord(c->ev[4], st);
+    {
+        const unsigned long long work = L.capacity > (unsigned long long)fp.n_tiles + 1 ? L.capacity : (unsigned long long)fp.n_tiles + 1;
+        k_obounds<<<(unsigned int)((work + 255) / 256), 256, 0, st>>>(keys[cur], stats, fp.n_tiles, (unsigned int *)(ws + L.tile_start));
+    }
+    if (c->profiling) cudaEventRecord(c->ev[5], st);
+    if (fp.T == 8) launch_ordered_tail<8>(c, L, ws, fp, keys[cur], vals[cur], image, st);
+    else if (fp.T == 16) launch_ordered_tail<16>(c, L, ws, fp, keys[cur], vals[cur], image, st);
+    else launch_ordered_tail<32>(c, L, ws, fp, keys[cur], vals[cur], image, st);
+    CU_TRY(c, cudaGetLastError());
+    c->have_frame = true; c->ws = ws; c->lay = L; c->fp = fp; c->last_n = n; c->last_stream = st; c->last_additive = false;
+    if (c->profiling) { ++c->prof_frames; c->prof_stages = kStagesOrdered; }
+    return SPLOTCH_OK;
+}
+
+// Layout of a frame from the caller's workspace; ENOMEM message on failure.
+int frame_layout(splotch_ctx *c, unsigned long long n, const splotch_params *q, size_t bytes, bool staging, Layout *L)
+{
+    const bool ok = q->additive ? make_layout(c, n, q->tile, 0, bytes, staging, L)
+                                : fit_layout_ordered(c, n, q->tile, bytes, staging, L);
+    if (!ok) return fail(c, SPLOTCH_ENOMEM, "workspace of %zu bytes is below the fixed minimum%s; ask splotch_workspace_bytes",
+                         bytes, staging ? " (with host staging)" : "");
     return SPLOTCH_OK;
 }
 
@@ -269,7 +410,11 @@ extern "C" {
 
 const char *splotch_version(void) { return "splotch-b200 0.1 (sm_100a)"; }
 
-const char *splotch_stage_name(int s) { return (s >= 0 && s < kStages) ? kStageNames[s] : ""; }
+const char *splotch_stage_name(int additive, int s)
+{
+    if (additive) return (s >= 0 && s < kStagesAdditive) ? kStageNamesAdditive[s] : "";
+    return (s >= 0 && s < kStagesOrdered) ? kStageNamesOrdered[s] : "";
+}
 
 const char *splotch_last_error(const splotch_ctx *c) { return c ? c->err : g_create_err; }
 
@@ -302,6 +447,12 @@ int splotch_create(splotch_ctx **out, int device, int width, int height, uint64_
         int r = query_splat_occupancy<8>(c, &c->splat_blocks_per_sm[0]);
         if (r == SPLOTCH_OK) r = query_splat_occupancy<16>(c, &c->splat_blocks_per_sm[1]);
         if (r == SPLOTCH_OK) r = query_splat_occupancy<32>(c, &c->splat_blocks_per_sm[2]);
+        if (r != SPLOTCH_OK) return r;
+        CU_TRY(c, cudaFuncSetAttribute(k_rs_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(RsSmem)));
+        CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->orender_blocks_per_sm[0], k_orender<8>, SplatCfg<8>::kThreads, 0));
+        CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->orender_blocks_per_sm[1], k_orender<16>, SplatCfg<16>::kThreads, 0));
+        CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->orender_blocks_per_sm[2], k_orender<32>, SplatCfg<32>::kThreads, 0));
+        for (int k = 0; k < 3; ++k) if (c->orender_blocks_per_sm[k] < 1) c->orender_blocks_per_sm[k] = 1;
         return r;
     }();
     if (rc != SPLOTCH_OK) {
@@ -405,9 +556,10 @@ size_t splotch_workspace_bytes(const splotch_ctx *c, uint64_t n, int tile, uint6
     if (bin_smem_bytes(c->width, c->height, tile) + 1024 > (size_t)c->smem_optin) return 0;
     if (pair_capacity == 0) pair_capacity = 2ull * n + (1ull << 20);
     if (pair_capacity > 0xfffffff0ull) return 0;
-    Layout L;
+    Layout L, Lo;
     make_layout(c, n, tile, pair_capacity, 0, with_host_staging != 0, &L);
-    return L.total + 4096;
+    make_layout_ordered(c, n, tile, pair_capacity, with_host_staging != 0, &Lo);       // either mode must fit
+    return (L.total > Lo.total + 8192 ? L.total : Lo.total + 8192) + 4096;
 }
 
 int splotch_render(splotch_ctx *c, const splotch_particles *p, uint64_t n, const splotch_params *q, float *image_out,
@@ -420,9 +572,10 @@ int splotch_render(splotch_ctx *c, const splotch_particles *p, uint64_t n, const
     if (!image_out || !workspace) return fail(c, SPLOTCH_EINVAL, "null image or workspace");
     if (((uintptr_t)workspace & 255u) != 0) return fail(c, SPLOTCH_EINVAL, "workspace must be 256-byte aligned");
     Layout L;
-    if (!make_layout(c, n, q->tile, 0, workspace_bytes, false, &L))
-        return fail(c, SPLOTCH_ENOMEM, "workspace of %zu bytes is below the fixed minimum; ask splotch_workspace_bytes", workspace_bytes);
+    rc = frame_layout(c, n, q, workspace_bytes, false, &L);
+    if (rc != SPLOTCH_OK) return rc;
     CU_TRY(c, cudaSetDevice(c->device));
+    if (!q->additive) return render_ordered(c, p, n, fp, L, image_out, (char *)workspace, (cudaStream_t)cuda_stream);
     return render_device(c, p, n, fp, L, image_out, (char *)workspace, (cudaStream_t)cuda_stream);
 }
 
@@ -436,8 +589,8 @@ int splotch_render_host(splotch_ctx *c, const splotch_particles *hp, uint64_t n,
     if (!host_image_out || !workspace) return fail(c, SPLOTCH_EINVAL, "null image or workspace");
     if (((uintptr_t)workspace & 255u) != 0) return fail(c, SPLOTCH_EINVAL, "workspace must be 256-byte aligned");
     Layout L;
-    if (!make_layout(c, n, q->tile, 0, workspace_bytes, true, &L))
-        return fail(c, SPLOTCH_ENOMEM, "workspace of %zu bytes is below the fixed minimum (with host staging)", workspace_bytes);
+    rc = frame_layout(c, n, q, workspace_bytes, true, &L);
+    if (rc != SPLOTCH_OK) return rc;
     CU_TRY(c, cudaSetDevice(c->device));
     cudaStream_t st = (cudaStream_t)cuda_stream;
     char *ws = (char *)workspace;
@@ -451,7 +604,7 @@ int splotch_render_host(splotch_ctx *c, const splotch_particles *hp, uint64_t n,
     float *dimg = (float *)(ws + L.staging + align_up(6 * fstride, 256));
     splotch_particles dp = *hp;
     dp.x = dst[0]; dp.y = dst[1]; dp.z = dst[2]; dp.h = dst[3]; dp.I = dst[4]; dp.scalar = dst[5];
-    rc = render_device(c, &dp, n, fp, L, dimg, ws, st);
+    rc = q->additive ? render_device(c, &dp, n, fp, L, dimg, ws, st) : render_ordered(c, &dp, n, fp, L, dimg, ws, st);
     if (rc != SPLOTCH_OK) return rc;
     CU_TRY(c, cudaMemcpyAsync(host_image_out, dimg, sizeof(float) * 3 * (size_t)c->width * c->height, cudaMemcpyDeviceToHost, st));
     CU_TRY(c, cudaStreamSynchronize(st));
@@ -474,8 +627,8 @@ int splotch_get_stats(splotch_ctx *c, splotch_stats *out)
     if (c->profiling && c->prof_frames > 0) {
         // mean per frame over the frames recorded since profiling was enabled (at most the last kProfRing)
         const unsigned long long nf = c->prof_frames < kProfRing ? c->prof_frames : kProfRing;
-        out->n_stages = kStages;
-        for (int s = 0; s < kStages; ++s) {
+        out->n_stages = c->prof_stages;
+        for (int s = 0; s < c->prof_stages; ++s) {
             double sum = 0.0;
             for (unsigned long long f = 0; f < nf; ++f) {
                 float ms = 0.0f;
@@ -509,8 +662,14 @@ int splotch_debug_tile_counts(splotch_ctx *c, uint32_t *out, void *cuda_stream)
     if (!c || !out) return SPLOTCH_EINVAL;
     if (!c->have_frame) return fail(c, SPLOTCH_ESTATE, "no frame rendered yet");
     CU_TRY(c, cudaSetDevice(c->device));
-    CU_TRY(c, cudaMemcpyAsync(out, c->ws + c->lay.bin_count, sizeof(uint32_t) * (size_t)c->fp.n_tiles,
-                              cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
+    if (c->last_additive) {
+        CU_TRY(c, cudaMemcpyAsync(out, c->ws + c->lay.bin_count, sizeof(uint32_t) * (size_t)c->fp.n_tiles,
+                                  cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
+    } else {
+        k_odiff<<<(c->fp.n_tiles + 255) / 256, 256, 0, (cudaStream_t)cuda_stream>>>((const unsigned int *)(c->ws + c->lay.tile_start),
+                                                                                     c->fp.n_tiles, out);
+        CU_TRY(c, cudaGetLastError());
+    }
     return SPLOTCH_OK;
 }
 

@@ -65,6 +65,7 @@ struct FrameParams {
 struct DeviceStats {             // cleared before every frame; written by k_scan / k_scatter, read back by splotch_get_stats
     unsigned long long count[4];
     unsigned long long pairs, large_pairs, chunks, capacity;
+    unsigned long long sort_n;   // ordered mode: pairs the sort and the renderer work on (0 on overflow)
     unsigned int overflow, work_counter, chunk_size, amax_bits, scan_done, pad;
 };
 
@@ -424,7 +425,7 @@ __device__ __forceinline__ int species_of(unsigned int i, const FrameParams &fp)
 
 // lut: the species' table (shared or global memory), lut_n entries.  Colour and amplitude are continuous in the
 // inputs (no integer is decided here beyond the table cell), so plain float32 with a reciprocal range is enough.
-__device__ __forceinline__ float3 amplitude(float I, float scalar, float h, const SpeciesDev &S, const float4 *lut)
+__device__ __forceinline__ float3 colour_of(float scalar, const SpeciesDev &S, const float4 *lut)
 {
     float r = S.fixed_r, g = S.fixed_g, b = S.fixed_b;
     if (S.use_colormap) {
@@ -446,8 +447,15 @@ __device__ __forceinline__ float3 amplitude(float I, float scalar, float h, cons
         g = fmaf(fr, c.y - a.y, a.y);
         b = fmaf(fr, c.z - a.z, a.z);
     }
+    return make_float3(r, g, b);
+}
+
+// E_p * (column constant) = b_s * colour * sqrt(pi) h I (R12, R13)
+__device__ __forceinline__ float3 amplitude(float I, float scalar, float h, const SpeciesDev &S, const float4 *lut)
+{
+    const float3 c = colour_of(scalar, S, lut);
     const float col = S.brightness * (1.7724538509055160273f * h * I);   // b_s * sqrt(pi) h I
-    return make_float3(r * col, g * col, b * col);
+    return make_float3(c.x * col, c.y * col, c.z * col);
 }
 
 // Render record, 32 bytes: {px, py, c, r2} {aR, aG, aB, box}

@@ -1,0 +1,623 @@
+// splotch_ordered.cuh -- device code of the ordered (E_p != A_p) mode, step A7 of DESIGN.md (sm_100a).
+//
+// Eq. 1 for one particle is linear in I: crossing particle p maps I -> I + (E_p/A_p - I)(1 - exp(-A_p tau_p)),
+// tau_p = rho_0 sqrt(pi) sigma w_p(pixel) from Eq. 2 (:83).  With E_p != A_p the result depends on the order in which
+// the particles are crossed (:85 sets that case aside; reading R15 of DESIGN.md: far to near by the float32 camera
+// depth z_c, ties by lower particle index first).  The additive path's unordered binning cannot give that order, so
+// this mode has its own pipeline:
+//   k_ocount    A1+A3      classify, count the (particle, tile) pairs of every block of 2048 particles
+//   k_oscan     A4         exclusive scan of the block totals, frame statistics
+//   k_opairs    A1-A3+A2   one 32-byte record per particle (index order) and its pairs, in index order:
+//                          key = tile << 32 | ~bits(z_c), value = particle index
+//   k_rs_*      A4/A7      stable least-significant-digit radix sort of the pairs, 8 bits per pass (4 passes for the
+//                          depth, 1-3 for the tile); equal keys keep index order, which is the tie rule of R15.
+//                          Replaces thrust::sort_by_key (:201); hand-written: histogram, one linear scan of the
+//                          digit-major count matrix, rank by warp match + shared-memory reordering
+//   k_obounds   A4         tile start offsets from the sorted keys (replaces reduce_by_key + inclusive_scan, :203-205)
+//   k_orender   A7         a CTA walks a chunk of the sorted pairs tile by tile; per pixel it composes the particles'
+//                          affine maps I -> t I + c in order, into one (t, c_R, c_G, c_B) per pixel and segment
+//   k_ocombine  A7+A8      per tile: fold the segments' maps in order from I = 0 (composition is associative), write
+//                          the image
+#pragma once
+#include "splotch_kernels.cuh"
+
+namespace splotch {
+
+constexpr int kOThreads = 512;                 // k_ocount / k_opairs: 4 consecutive particles per thread
+constexpr int kOBlockParticles = 4 * kOThreads;
+constexpr int kRsThreads = 512;                // radix sort: 8 elements per thread
+constexpr int kRsItems = 8;
+constexpr int kRsTile = kRsThreads * kRsItems; // 4096 elements per block and pass
+constexpr int kRsWarps = kRsThreads / 32;
+constexpr int kOChunkMin = 4096;               // records per work item of k_orender (lower bound)
+
+__device__ __forceinline__ int tile_pairs(const Geo &g, const FrameParams &fp)
+{
+    if (g.cls == CULLED) return 0;
+    return ((g.x1 >> fp.tshift) - (g.x0 >> fp.tshift) + 1) * ((g.y1 >> fp.tshift) - (g.y0 >> fp.tshift) + 1);
+}
+
+// ---- classify and count pairs per block -------------------------------------------------------------------------
+template <bool ALIGNED>
+__global__ void __launch_bounds__(kOThreads)
+k_ocount(const float *__restrict__ x, const float *__restrict__ y, const float *__restrict__ z, const float *__restrict__ h,
+         unsigned long long n, const __grid_constant__ FrameParams fp, unsigned int *__restrict__ blk_pairs,
+         DeviceStats *__restrict__ stats)
+{
+    __shared__ unsigned int s_sum[4];
+    if (threadIdx.x < 4) s_sum[threadIdx.x] = 0u;
+    __syncthreads();
+    const unsigned long long lo = (unsigned long long)blockIdx.x * kOBlockParticles;
+    const unsigned int len = (unsigned int)min(n - lo, (unsigned long long)kOBlockParticles);
+    x += lo; y += lo; z += lo; h += lo;
+    const unsigned int i = 4u * threadIdx.x;
+    float xs[4], ys[4], zs[4], hs[4];
+    load4<ALIGNED>(x, i, len, xs);
+    load4<ALIGNED>(y, i, len, ys);
+    load4<ALIGNED>(z, i, len, zs);
+    load4<ALIGNED>(h, i, len, hs);
+    unsigned int pairs = 0u, c1 = 0u, c2 = 0u, c3 = 0u;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        Geo g = geometry(xs[j], ys[j], zs[j], hs[j], fp);
+        if (!(i + j < len)) g.cls = CULLED;
+        pairs += (unsigned int)tile_pairs(g, fp);
+        c1 += g.cls == SMALL; c2 += g.cls == MEDIUM; c3 += g.cls == LARGE;
+    }
+    pairs = warp_sum(pairs);
+    const unsigned int cc = warp_sum(c1 | (c2 << 10) | (c3 << 20));        // at most 128 per field and warp
+    if ((threadIdx.x & 31) == 0) {
+        atomicAdd(&s_sum[0], pairs);
+        atomicAdd(&s_sum[1], cc & 1023u); atomicAdd(&s_sum[2], (cc >> 10) & 1023u); atomicAdd(&s_sum[3], cc >> 20);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) blk_pairs[blockIdx.x] = s_sum[0];
+    if (threadIdx.x >= 1 && threadIdx.x < 4 && s_sum[threadIdx.x]) atomicAdd(&stats->count[threadIdx.x], (unsigned long long)s_sum[threadIdx.x]);
+}
+
+// ---- exclusive scan of the block totals (one block) ---------------------------------------------------------------
+constexpr int kOScanThreads = 1024;
+
+__global__ void __launch_bounds__(kOScanThreads)
+k_oscan(unsigned int *__restrict__ blk_pairs, int nblk, unsigned long long n, unsigned long long capacity, int n_sm,
+        DeviceStats *__restrict__ stats)
+{
+    __shared__ unsigned long long s_warp[kOScanThreads / 32];
+    __shared__ unsigned long long s_total;
+    const int per = (nblk + kOScanThreads - 1) / kOScanThreads;
+    const int b0 = min(nblk, (int)threadIdx.x * per), b1 = min(nblk, b0 + per);
+    unsigned long long sum = 0;
+    for (int b = b0; b < b1; ++b) sum += blk_pairs[b];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    unsigned long long inc = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const unsigned long long t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) s_warp[w] = inc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned long long run = 0;
+        for (int k = 0; k < kOScanThreads / 32; ++k) { const unsigned long long c = s_warp[k]; s_warp[k] = run; run += c; }
+        s_total = run;
+    }
+    __syncthreads();
+    unsigned long long run = s_warp[w] + inc - sum;
+    const unsigned long long total = s_total;
+    const bool overflow = total > capacity;
+    for (int b = b0; b < b1; ++b) { const unsigned int c = blk_pairs[b]; blk_pairs[b] = (unsigned int)run; run += c; }
+    if (threadIdx.x == 0) {
+        unsigned long long cs = (total + (unsigned long long)n_sm * 32 - 1) / ((unsigned long long)n_sm * 32);
+        cs = (cs + 255) / 256 * 256;
+        cs = min((unsigned long long)kChunkMax, max((unsigned long long)kOChunkMin, cs));
+        stats->pairs = total;
+        stats->large_pairs = 0ull;
+        stats->sort_n = overflow ? 0ull : total;         // the sort and the renderers see an empty frame on overflow
+        stats->chunks = overflow ? 0ull : (total + cs - 1) / cs;
+        stats->capacity = capacity;
+        stats->overflow = overflow ? 1u : 0u;
+        stats->work_counter = 0u;
+        stats->chunk_size = (unsigned int)cs;
+        stats->count[0] = n - stats->count[1] - stats->count[2] - stats->count[3];
+    }
+}
+
+// ---- records and pairs in index order -----------------------------------------------------------------------------
+// Ordered-mode record, 32 bytes, one per particle: {px, py, c, r2 | flag} {q_R, q_G, q_B, ak}
+//   MEDIUM / LARGE: c = -log2(e) / sp^2, r2 = rp^2 (the C1 inside test).  SMALL: (px, py) = the centre of its pixel,
+//   c = 0, r2 = 0.25: only that pixel passes the inside test, with weight exp2(0) = 1.
+//   kappa > 0: q = E / kappa (the fixed point of Eq. 1 inside the particle), ak = kappa * col [* pi sp^2 (1 - e^-chi^2)
+//   for SMALL], so that 1 - exp(-A tau) = 1 - exp(-ak w).   kappa == 0 (flag = sign bit of r2): q = E * col [* ...],
+//   I += q w.  Non-finite amplitudes give a record without effect.
+template <bool ALIGNED>
+__global__ void __launch_bounds__(kOThreads)
+k_opairs(const float *__restrict__ x, const float *__restrict__ y, const float *__restrict__ z, const float *__restrict__ h,
+         const float *__restrict__ I, const float *__restrict__ scalar, unsigned long long n,
+         const __grid_constant__ FrameParams fp, const unsigned int *__restrict__ blk_off, const DeviceStats *__restrict__ stats,
+         float4 *__restrict__ rec, unsigned long long *__restrict__ keys, unsigned int *__restrict__ vals)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float4 *s_lut = reinterpret_cast<float4 *>(smem_raw);
+    __shared__ unsigned int s_w[kOThreads / 32];
+    if (stats->overflow) return;
+    if (fp.lut_total > 0) {
+        for (int s = 0; s < fp.n_species; ++s)
+            if (fp.sp[s].use_colormap)
+                for (int i = threadIdx.x; i < fp.sp[s].lut_n; i += kOThreads)
+                    s_lut[fp.sp[s].lut_off + i] = fp.lut[s * kMaxLut + i];
+    }
+    const unsigned long long lo = (unsigned long long)blockIdx.x * kOBlockParticles;
+    const unsigned int len = (unsigned int)min(n - lo, (unsigned long long)kOBlockParticles);
+    const unsigned int lo32 = (unsigned int)lo;
+    x += lo; y += lo; z += lo; h += lo; I += lo; scalar += lo;
+    const unsigned int i = 4u * threadIdx.x;
+    float xs[4], ys[4], zs[4], hs[4], Is[4], ss[4];
+    load4<ALIGNED>(x, i, len, xs);
+    load4<ALIGNED>(y, i, len, ys);
+    load4<ALIGNED>(z, i, len, zs);
+    load4<ALIGNED>(h, i, len, hs);
+    load4<ALIGNED>(I, i, len, Is);
+    load4<ALIGNED>(scalar, i, len, ss);
+    Geo g[4];
+    unsigned int cnt = 0u;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        g[j] = geometry(xs[j], ys[j], zs[j], hs[j], fp);
+        if (!(i + j < len)) g[j].cls = CULLED;
+        cnt += (unsigned int)tile_pairs(g[j], fp);
+    }
+    // position of this thread's first pair: block offset + exclusive scan over the threads (index order)
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    unsigned int inc = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const unsigned int t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) s_w[w] = inc;
+    __syncthreads();                                   // also: colour tables staged
+    unsigned int woff = 0u;
+    for (int k = 0; k < w; ++k) woff += s_w[k];
+    unsigned long long pos = (unsigned long long)blk_off[blockIdx.x] + woff + inc - cnt;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        if (g[j].cls == CULLED) continue;
+        const unsigned int idx = lo32 + i + j;
+        const int s = species_of(idx, fp);
+        const SpeciesDev &S = fp.sp[s];
+        const float4 *lut = fp.lut_total > 0 ? s_lut + S.lut_off : fp.lut + s * kMaxLut;
+        const float3 rgb = colour_of(ss[j], S, lut);
+        const float3 E = make_float3(S.brightness * rgb.x, S.brightness * rgb.y, S.brightness * rgb.z);
+        const bool small = g[j].cls == SMALL;
+        const float sp2 = __fmul_rn(g[j].sp, g[j].sp);
+        const float col = 1.7724538509055160273f * hs[j] * Is[j] * (small ? fp.csmall * sp2 : 1.0f);   // tau at weight 1
+        float4 ra, rb;
+        if (small) {
+            ra.x = __fadd_rn((float)g[j].x0, 0.5f); ra.y = __fadd_rn((float)g[j].y0, 0.5f);
+            ra.z = 0.0f; ra.w = 0.25f;
+        } else {
+            ra.x = g[j].px; ra.y = g[j].py;
+            ra.z = __fdividef(-1.4426950408889634f, sp2);
+            ra.w = __fmul_rn(g[j].rp, g[j].rp);
+        }
+        const float kappa = S.absorb;
+        if (kappa > 0.0f) {
+            const float inv = 1.0f / kappa;
+            rb = make_float4(E.x * inv, E.y * inv, E.z * inv, kappa * col);
+        } else {
+            rb = make_float4(E.x * col, E.y * col, E.z * col, 0.0f);
+            ra.w = -ra.w;                              // flag: pure emission, I += q w
+        }
+        const float am = fmaxf(fmaxf(fabsf(rb.x), fabsf(rb.y)), fmaxf(fabsf(rb.z), fabsf(rb.w)));
+        if (!(am <= 3.0e38f)) rb = make_float4(0.0f, 0.0f, 0.0f, 0.0f);   // Inf / NaN: a record without effect
+        st_record(rec, idx, ra, rb);
+        const unsigned long long zkey = (unsigned long long)(~__float_as_uint(g[j].zc));
+        const int tx0 = g[j].x0 >> fp.tshift, tx1 = g[j].x1 >> fp.tshift;
+        const int ty0 = g[j].y0 >> fp.tshift, ty1 = g[j].y1 >> fp.tshift;
+        for (int ty = ty0; ty <= ty1; ++ty)
+            for (int tx = tx0; tx <= tx1; ++tx) {
+                keys[pos] = ((unsigned long long)(unsigned int)(ty * fp.ntx + tx) << 32) | zkey;
+                vals[pos] = idx;
+                ++pos;
+            }
+    }
+}
+
+// ---- stable LSD radix sort, 8 bits per pass, 64-bit keys + 32-bit values -----------------------------------------
+__device__ __forceinline__ unsigned int rs_digit(unsigned long long key, int shift) { return (unsigned int)(key >> shift) & 255u; }
+
+// hist is digit-major: hist[d * nblk + b]; one linear exclusive scan over it gives every block's output offsets.
+__global__ void __launch_bounds__(kRsThreads)
+k_rs_count(const unsigned long long *__restrict__ keys, const DeviceStats *__restrict__ stats, int shift, int nblk,
+           unsigned int *__restrict__ hist)
+{
+    __shared__ unsigned int s_h[256];
+    if (threadIdx.x < 256) s_h[threadIdx.x] = 0u;
+    __syncthreads();
+    const unsigned long long P = stats->sort_n;
+    const unsigned long long seg = (unsigned long long)blockIdx.x * kRsTile;
+    if (seg < P) {
+        const unsigned int cnt = (unsigned int)min(P - seg, (unsigned long long)kRsTile);
+        const int lane = threadIdx.x & 31;
+#pragma unroll
+        for (int i = 0; i < kRsItems; ++i) {
+            const unsigned int p = i * kRsThreads + threadIdx.x;
+            const unsigned int d = p < cnt ? rs_digit(__ldg(keys + seg + p), shift) : 256u;
+            const unsigned int peers = __match_any_sync(0xffffffffu, d);
+            if (d < 256u && lane == __ffs(peers) - 1) atomicAdd(&s_h[d], (unsigned int)__popc(peers));
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x < 256) hist[(size_t)threadIdx.x * nblk + blockIdx.x] = s_h[threadIdx.x];
+}
+
+// exclusive scan of m unsigned ints in place, three launches: block sums, scan of the sums (one block), apply
+constexpr int kScThreads = 512, kScItems = 8, kScTile = kScThreads * kScItems;
+
+__device__ __forceinline__ unsigned int block_excl_scan_u32(unsigned int v, unsigned int *s_warp, unsigned int *total)
+{
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    unsigned int inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const unsigned int t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) s_warp[w] = inc;
+    __syncthreads();
+    if (w == 0) {
+        const unsigned int c = lane < nw ? s_warp[lane] : 0u;
+        unsigned int ci = c;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const unsigned int t = __shfl_up_sync(0xffffffffu, ci, o);
+            if (lane >= o) ci += t;
+        }
+        if (lane < nw) s_warp[lane] = ci - c;
+        if (lane == 31) *total = ci;
+    }
+    __syncthreads();
+    const unsigned int r = s_warp[w] + inc - v;
+    __syncthreads();
+    return r;
+}
+
+__global__ void __launch_bounds__(kScThreads)
+k_sc_reduce(const unsigned int *__restrict__ a, unsigned int m, unsigned int *__restrict__ sums)
+{
+    __shared__ unsigned int s_warp[32], s_total;
+    const unsigned int base = blockIdx.x * kScTile + threadIdx.x * kScItems;
+    unsigned int s = 0u;
+    if (base + kScItems <= m) {
+        const uint4 u = *reinterpret_cast<const uint4 *>(a + base), v = *reinterpret_cast<const uint4 *>(a + base + 4);
+        s = u.x + u.y + u.z + u.w + v.x + v.y + v.z + v.w;
+    } else {
+        for (int k = 0; k < kScItems; ++k) if (base + k < m) s += a[base + k];
+    }
+    (void)block_excl_scan_u32(s, s_warp, &s_total);
+    if (threadIdx.x == 0) sums[blockIdx.x] = s_total;
+}
+
+__global__ void __launch_bounds__(1024)
+k_sc_top(unsigned int *__restrict__ sums, int ng)
+{
+    __shared__ unsigned int s_warp[32], s_total;
+    const int per = (ng + 1023) / 1024;
+    const int b0 = min(ng, (int)threadIdx.x * per), b1 = min(ng, b0 + per);
+    unsigned int s = 0u;
+    for (int b = b0; b < b1; ++b) s += sums[b];
+    unsigned int run = block_excl_scan_u32(s, s_warp, &s_total);
+    for (int b = b0; b < b1; ++b) { const unsigned int c = sums[b]; sums[b] = run; run += c; }
+}
+
+__global__ void __launch_bounds__(kScThreads)
+k_sc_apply(unsigned int *__restrict__ a, unsigned int m, const unsigned int *__restrict__ sums)
+{
+    __shared__ unsigned int s_warp[32], s_total;
+    const unsigned int base = blockIdx.x * kScTile + threadIdx.x * kScItems;
+    unsigned int v[kScItems];
+    unsigned int s = 0u;
+#pragma unroll
+    for (int k = 0; k < kScItems; ++k) { v[k] = base + k < m ? a[base + k] : 0u; s += v[k]; }
+    unsigned int run = block_excl_scan_u32(s, s_warp, &s_total) + sums[blockIdx.x];
+#pragma unroll
+    for (int k = 0; k < kScItems; ++k) {
+        if (base + k < m) a[base + k] = run;
+        run += v[k];
+    }
+}
+
+struct RsSmem {
+    unsigned long long keys[kRsTile];
+    unsigned int vals[kRsTile];
+    unsigned int wcount[kRsWarps][257];
+    unsigned int dstart[256];
+    unsigned int gbase[256];
+    unsigned int warp_tmp[32];
+    unsigned int total;
+};
+
+// One block moves its 4096 elements to their places of this pass.  Element order inside the block is (warp, item,
+// lane) = position order; ranks among equal digits are taken in that order (warp match + per-warp counters, then an
+// exclusive prefix over the warps), so the pass is stable.  The elements are first reordered in shared memory, then
+// written out position by position: consecutive threads write consecutive addresses of a digit's run.
+__global__ void __launch_bounds__(kRsThreads)
+k_rs_scatter(const unsigned long long *__restrict__ keys_in, const unsigned int *__restrict__ vals_in,
+             unsigned long long *__restrict__ keys_out, unsigned int *__restrict__ vals_out,
+             const DeviceStats *__restrict__ stats, int shift, int nblk, const unsigned int *__restrict__ hist)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    RsSmem &S = *reinterpret_cast<RsSmem *>(smem_raw);
+    const unsigned long long P = stats->sort_n;
+    const unsigned long long seg = (unsigned long long)blockIdx.x * kRsTile;
+    if (seg >= P) return;
+    const unsigned int cnt = (unsigned int)min(P - seg, (unsigned long long)kRsTile);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    for (int i = threadIdx.x; i < kRsWarps * 257; i += kRsThreads) (&S.wcount[0][0])[i] = 0u;
+    unsigned long long key[kRsItems];
+    unsigned int val[kRsItems], rank[kRsItems];
+    const unsigned int wbase = w * (32 * kRsItems) + lane;
+#pragma unroll
+    for (int i = 0; i < kRsItems; ++i) {
+        const unsigned int p = wbase + i * 32;
+        key[i] = p < cnt ? __ldg(keys_in + seg + p) : ~0ull;
+        val[i] = p < cnt ? __ldg(vals_in + seg + p) : 0u;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < kRsItems; ++i) {
+        const unsigned int p = wbase + i * 32;
+        const unsigned int d = p < cnt ? rs_digit(key[i], shift) : 256u;
+        const unsigned int peers = __match_any_sync(0xffffffffu, d);
+        const int leader = __ffs(peers) - 1;
+        unsigned int old = 0u;
+        if (lane == leader) { old = S.wcount[w][d]; S.wcount[w][d] = old + (unsigned int)__popc(peers); }
+        old = __shfl_sync(0xffffffffu, old, leader);
+        rank[i] = old + (unsigned int)__popc(peers & ((1u << lane) - 1u));
+        __syncwarp();
+    }
+    __syncthreads();
+    unsigned int tot = 0u;
+    if (threadIdx.x < 256) {
+        for (int k = 0; k < kRsWarps; ++k) { const unsigned int c = S.wcount[k][threadIdx.x]; S.wcount[k][threadIdx.x] = tot; tot += c; }
+    }
+    const unsigned int ds = block_excl_scan_u32(tot, S.warp_tmp, &S.total);      // threads >= 256 contribute 0
+    if (threadIdx.x < 256) {
+        S.dstart[threadIdx.x] = ds;
+        S.gbase[threadIdx.x] = hist[(size_t)threadIdx.x * nblk + blockIdx.x] - ds;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < kRsItems; ++i) {
+        const unsigned int p = wbase + i * 32;
+        if (p < cnt) {
+            const unsigned int d = rs_digit(key[i], shift);
+            const unsigned int lp = S.dstart[d] + S.wcount[w][d] + rank[i];
+            S.keys[lp] = key[i];
+            S.vals[lp] = val[i];
+        }
+    }
+    __syncthreads();
+    for (unsigned int j = threadIdx.x; j < cnt; j += kRsThreads) {
+        const unsigned long long k = S.keys[j];
+        const unsigned int o = S.gbase[rs_digit(k, shift)] + j;
+        keys_out[o] = k;
+        vals_out[o] = S.vals[j];
+    }
+}
+
+// ---- tile start offsets from the sorted keys ----------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_obounds(const unsigned long long *__restrict__ keys, const DeviceStats *__restrict__ stats, int n_tiles,
+          unsigned int *__restrict__ tile_start)
+{
+    const unsigned long long P = stats->sort_n;
+    const unsigned long long p = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (P == 0ull) {
+        if (p <= (unsigned long long)n_tiles) tile_start[p] = 0u;
+        return;
+    }
+    if (p >= P) return;
+    const int t = (int)(keys[p] >> 32);
+    const int tp = p > 0 ? (int)(keys[p - 1] >> 32) : -1;
+    for (int u = tp + 1; u <= t; ++u) tile_start[u] = (unsigned int)p;
+    if (p == P - 1) for (int u = t + 1; u <= n_tiles; ++u) tile_start[u] = (unsigned int)P;
+}
+
+__global__ void __launch_bounds__(256)
+k_odiff(const unsigned int *__restrict__ tile_start, int n_tiles, unsigned int *__restrict__ out)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < n_tiles) out[t] = tile_start[t + 1] - tile_start[t];
+}
+
+// ---- A7: ordered compositing of one chunk -------------------------------------------------------------------------
+// a = 1 - exp(-x) and e = exp(-x) for the optical depth x of one particle at one pixel.  |x| < 0.25: a from the
+// Taylor series to x^8 (relative error < 2e-8), e = 1 - a; otherwise e = 2^(-x log2 e) (ex2.approx), a = 1 - e.
+__device__ __forceinline__ void absorb_pair(float x, float &a, float &e)
+{
+    float p = fmaf(-x, 0.125f, 1.0f);
+    p = fmaf(-x * (1.0f / 7.0f), p, 1.0f);
+    p = fmaf(-x * (1.0f / 6.0f), p, 1.0f);
+    p = fmaf(-x * 0.2f, p, 1.0f);
+    p = fmaf(-x * 0.25f, p, 1.0f);
+    p = fmaf(-x * (1.0f / 3.0f), p, 1.0f);
+    p = fmaf(-x * 0.5f, p, 1.0f);
+    const float as = x * p;
+    const float el = ex2_approx(x * -1.4426950408889634f);
+    const bool small = fabsf(x) < 0.25f;
+    a = small ? as : 1.0f - el;
+    e = small ? 1.0f - as : el;
+}
+
+// floor of v as an int, for any float (clamped to +-1e9 first; NaN gives -1e9)
+__device__ __forceinline__ int floor_clamped(float v) { return __float2int_rd(fminf(fmaxf(v, -1.0e9f), 1.0e9f)); }
+
+template <int T>
+__global__ void __launch_bounds__(SplatCfg<T>::kThreads)
+k_orender(const float4 *__restrict__ rec, const unsigned long long *__restrict__ keys, const unsigned int *__restrict__ vals,
+          const unsigned int *__restrict__ tile_start, DeviceStats *__restrict__ stats, float4 *__restrict__ seg,
+          const __grid_constant__ FrameParams fp)
+{
+    using Cfg = SplatCfg<T>;
+    constexpr int kPix = Cfg::kPix, kThreads = Cfg::kThreads;
+    __shared__ float4 stA[kThreads], stB[kThreads];
+    __shared__ unsigned int stM[kThreads];
+    __shared__ unsigned int s_chunk;
+    __shared__ int s_tile;
+    (void)keys;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int sx = warp % Cfg::kStripsX, sy = warp / Cfg::kStripsX;
+    const int lx = sx * Cfg::kSW + 2 * (lane % (Cfg::kSW / 2)), ly = sy * Cfg::kSH + lane / (Cfg::kSW / 2);
+    const unsigned int my_strip = (1u << (16 + sx)) | (1u << sy);
+    const unsigned int total = (unsigned int)stats->chunks;
+    const unsigned int K = stats->chunk_size;
+    const unsigned int pairs = (unsigned int)stats->sort_n;
+    for (;;) {
+        __syncthreads();
+        if (warp == 0) {
+            unsigned int c = 0u;
+            if (lane == 0) c = atomicAdd(&stats->work_counter, 1u);
+            c = __shfl_sync(0xffffffffu, c, 0);
+            if (c < total) {
+                const unsigned int r = c * K;
+                int lo = 0, n = fp.n_tiles;
+                while (n > 1) {
+                    const int step = (n + 31) / 32;
+                    const int t = lo + lane * step;
+                    const bool le = t < lo + n && __ldg(tile_start + t) <= r;
+                    const int k = __popc(__ballot_sync(0xffffffffu, le)) - 1;
+                    lo += k * step;
+                    n = min(step, n - k * step);
+                }
+                if (lane == 0) s_tile = lo;
+            }
+            if (lane == 0) s_chunk = c;
+        }
+        __syncthreads();
+        const unsigned int chunk = s_chunk;
+        if (chunk >= total) break;
+        const unsigned int r0 = chunk * K, r1 = min(r0 + K, pairs);
+        int tile = s_tile;
+        unsigned int tb = tile_start[tile], te = tile_start[tile + 1];
+        for (;;) {
+            const unsigned int begin = max(tb, r0), end = min(te, r1);
+            const int tx0 = (tile % fp.ntx) * T, ty0 = (tile / fp.ntx) * T;
+            const float fx0 = __fadd_rn((float)(tx0 + lx), 0.5f), fx1 = __fadd_rn(fx0, 1.0f);
+            const float fy = __fadd_rn((float)(ty0 + ly), 0.5f);
+            // running map of the segment: double outside, float32 inside runs of ~1024 records
+            double To[2] = {1.0, 1.0}, Co[2][3] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
+            float ti[2] = {1.0f, 1.0f}, ci[2][3] = {{0.0f, 0.0f, 0.0f}, {0.0f, 0.0f, 0.0f}};
+            int fold = 0;
+            for (unsigned int base = begin; base < end; base += kThreads) {
+                const unsigned int idx = base + threadIdx.x;
+                float4 ra = make_float4(0.f, 0.f, 0.f, 0.f), rb = ra;
+                unsigned int touch = 0u;
+                if (idx < end) {
+                    ld_record(rec, __ldg(vals + idx), ra, rb);
+                    // strips the clip disc may touch (conservative: one pixel of slack; the inside test decides)
+                    const float rr = sqrtf(fabsf(ra.w)) + 1.0f;
+                    const int bx0 = max(floor_clamped(ra.x - rr) - tx0, 0), bx1 = min(floor_clamped(ra.x + rr) - tx0, T - 1);
+                    const int by0 = max(floor_clamped(ra.y - rr) - ty0, 0), by1 = min(floor_clamped(ra.y + rr) - ty0, T - 1);
+                    if (bx0 <= bx1 && by0 <= by1) {
+                        const unsigned int xm = (2u << (bx1 / Cfg::kSW)) - (1u << (bx0 / Cfg::kSW));
+                        const unsigned int ym = (2u << (by1 / Cfg::kSH)) - (1u << (by0 / Cfg::kSH));
+                        touch = (xm << 16) | ym;
+                    }
+                }
+                __syncthreads();
+                stA[threadIdx.x] = ra; stB[threadIdx.x] = rb; stM[threadIdx.x] = touch;
+                __syncthreads();
+#pragma unroll 1
+                for (int g = 0; g < kThreads; g += 32) {
+                    const unsigned int t = stM[g + lane];
+                    unsigned int m = __ballot_sync(0xffffffffu, (t & my_strip & 0xffff0000u) && (t & my_strip & 0xffffu));
+                    while (m) {                                            // ascending bit order = depth order
+                        const int r = g + __ffs(m) - 1;
+                        m &= m - 1;
+                        const float4 A = stA[r], B = stB[r];
+                        const float r2 = fabsf(A.w);
+                        const bool emit_only = A.w < 0.0f;
+                        const float dyf = __fsub_rn(fy, A.y);
+                        const float t2 = __fmul_rn(dyf, dyf);
+#pragma unroll
+                        for (int q = 0; q < 2; ++q) {
+                            const float dxf = __fsub_rn(q ? fx1 : fx0, A.x);
+                            const float d2 = __fmaf_rn(dxf, dxf, t2);
+                            if (d2 <= r2) {
+                                const float wgt = ex2_approx(d2 * A.z);
+                                if (emit_only) {
+                                    ci[q][0] = fmaf(B.x, wgt, ci[q][0]);
+                                    ci[q][1] = fmaf(B.y, wgt, ci[q][1]);
+                                    ci[q][2] = fmaf(B.z, wgt, ci[q][2]);
+                                } else {
+                                    float a, e;
+                                    absorb_pair(B.w * wgt, a, e);
+                                    ci[q][0] = fmaf(B.x - ci[q][0], a, ci[q][0]);
+                                    ci[q][1] = fmaf(B.y - ci[q][1], a, ci[q][1]);
+                                    ci[q][2] = fmaf(B.z - ci[q][2], a, ci[q][2]);
+                                    ti[q] *= e;
+                                }
+                            }
+                        }
+                    }
+                }
+                if (++fold == Cfg::kFoldBatches) {
+                    fold = 0;
+#pragma unroll
+                    for (int q = 0; q < 2; ++q) {
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) { Co[q][c] = fma(Co[q][c], (double)ti[q], (double)ci[q][c]); ci[q][c] = 0.0f; }
+                        To[q] *= (double)ti[q];
+                        ti[q] = 1.0f;
+                    }
+                }
+            }
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) Co[q][c] = fma(Co[q][c], (double)ti[q], (double)ci[q][c]);
+                To[q] *= (double)ti[q];
+            }
+            // the segment's map: slot = chunk + tile (segments of a tile are consecutive chunks)
+            float4 *out = seg + ((size_t)chunk + (size_t)tile) * kPix + ly * T + lx;
+            out[0] = make_float4((float)To[0], (float)Co[0][0], (float)Co[0][1], (float)Co[0][2]);
+            out[1] = make_float4((float)To[1], (float)Co[1][0], (float)Co[1][1], (float)Co[1][2]);
+            if (te >= r1) break;
+            do { ++tile; tb = te; te = tile_start[tile + 1]; } while (te == tb);
+            __syncthreads();
+        }
+    }
+}
+
+// ---- A7 + A8: fold the segments of a tile in order, write the image -------------------------------------------------
+template <int T>
+__global__ void __launch_bounds__(256)
+k_ocombine(const float4 *__restrict__ seg, const unsigned int *__restrict__ tile_start, const DeviceStats *__restrict__ stats,
+           const __grid_constant__ FrameParams fp, float *__restrict__ image)
+{
+    constexpr int kPix = T * T;
+    const int tile = blockIdx.x;
+    const int tx0 = (tile % fp.ntx) * T, ty0 = (tile / fp.ntx) * T;
+    const unsigned int tb = tile_start[tile], te = tile_start[tile + 1];
+    const unsigned int K = stats->chunk_size;
+    const bool any = te > tb && stats->overflow == 0u;
+    const unsigned int c0 = any ? tb / K : 1u, c1 = any ? (te - 1u) / K : 0u;
+    for (int p = threadIdx.x; p < kPix; p += 256) {
+        double I[3] = {0.0, 0.0, 0.0};
+        for (unsigned int c = c0; c <= c1 && any; ++c) {
+            const float4 m = __ldg(seg + ((size_t)c + (size_t)tile) * kPix + p);
+            I[0] = fma(I[0], (double)m.x, (double)m.y);
+            I[1] = fma(I[1], (double)m.x, (double)m.z);
+            I[2] = fma(I[2], (double)m.x, (double)m.w);
+        }
+        const int ix = tx0 + p % T, iy = ty0 + p / T;
+        if (ix < fp.W && iy < fp.H) {
+            float *o = image + 3ull * ((size_t)iy * fp.W + ix);
+            o[0] = (float)I[0]; o[1] = (float)I[1]; o[2] = (float)I[2];
+        }
+    }
+}
+
+}  // namespace splotch

@@ -87,7 +87,7 @@ def make_renderer(w, lut):
     return r
 
 
-def check_integer_work(r, w, kw, tile, geometry_every=8):
+def check_integer_work(r, w, kw, tile, geometry_every=8, count_large=False):
     """Oracle C1 over all particles in chunks: class counts, per-tile counts; sampled chunks bit-exact per particle."""
     cam = so.camera_constants(w.camera.eye, w.camera.lookat, w.camera.up, w.camera.fov_deg, w.width, w.height)
     assert np.array_equal(np.asarray(r.camera_constants(), np.float32), cam)
@@ -100,7 +100,7 @@ def check_integer_work(r, w, kw, tile, geometry_every=8):
         g = so.geometry(*[fc[k].cpu().numpy() for k in ("x", "y", "z", "h")], cam, w.chi, w.r_small, w.r_large,
                         w.z_near, w.width, w.height, tile)
         counts += np.bincount(g["cls"], minlength=4)
-        tiles += so.tile_counts(g, w.width, w.height, tile)
+        tiles += so.tile_counts(g, w.width, w.height, tile, count_large=count_large)
         if ci % geometry_every == 0:
             sub = {k: w.fields[k][a:b] for k in wl.FIELD_NAMES}
             sp1 = [wl.Species(0, b - a)]
@@ -174,13 +174,12 @@ def run_fullsize(cfg, tile, n_random=3, win=32, modes=(True,), camera=None, w=No
         torch.cuda.synchronize()
         st = r.stats()
         assert st["overflow"] == 0
-        if additive or True:
-            counts, tiles = check_integer_work(r, w, kw, tile)
+        if True:
+            counts, tiles = check_integer_work(r, w, kw, tile, count_large=not additive)
             assert st["count"] == [int(c) for c in counts]
-            if additive:
-                gc = r.debug_tile_counts(tile).cpu().numpy().astype(np.int64)
-                assert np.array_equal(gc, tiles)
-                assert st["pairs"] == int(tiles.sum())
+            gc = r.debug_tile_counts(tile).cpu().numpy().astype(np.int64)
+            assert np.array_equal(gc, tiles)
+            assert st["pairs"] == int(tiles.sum())
         res[additive] = (st, check_windows(img, w, lut, kw, windows_for(img, win, n_random, 7 + cfg), additive=additive))
     r.close()
     return w, res
@@ -200,7 +199,12 @@ def test_cfg3_full_size_inside_halo_400M():
     assert st["count"][3] > 0.02 * w.n, st["count"]          # the large-particle stress BASELINE.json asks for
 
 
-def test_cfg4_orbit_frames_additive_100M():
+def test_cfg4_orbit_frames_100M_additive_and_ordered():
+    """Frames {0, 30, 60, 90, 119} of the 120-frame orbit at full size, first in additive mode, then in the ordered
+    E != A mode (kappa_gas = 0.5, kappa_star = 2.0; intensities scaled so that optical depths reach order one)."""
     w = None
     for frame in (0, 30, 60, 90, 119):
         w, res = run_fullsize(4, 16, n_random=1, camera=wl.orbit_camera(frame), w=w)
+    w.fields["I"] = w.fields["I"] * 50.0
+    for frame in (0, 30, 60, 90, 119):
+        w, res = run_fullsize(4, 16, n_random=1, camera=wl.orbit_camera(frame), w=w, modes=(False,))

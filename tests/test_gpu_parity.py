@@ -85,7 +85,7 @@ def assert_counts_exact(r, w, tile, g):
     st = r.stats()
     assert st["overflow"] == 0
     assert st["count"] == [int((g["cls"] == c).sum()) for c in range(4)]
-    oc = so.tile_counts(g, w.width, w.height, tile)
+    oc = so.tile_counts(g, w.width, w.height, tile, count_large=not w.additive)   # ordered mode bins LARGE to tiles too
     gc = r.debug_tile_counts(tile).cpu().numpy()
     assert np.array_equal(gc.astype(np.int64), oc.astype(np.int64))
     assert st["pairs"] == int(oc.sum())
@@ -268,3 +268,116 @@ def test_cfg1_full_size_bench_configuration():
     assert_geometry_exact(r, f, w, kw, g, cam)
     assert_counts_exact(r, w, 16, g)
     assert_image_close(img, ref, "cfg1 full")
+
+
+# ---- ordered (E != A) mode: step A7, reading R15 of DESIGN.md ---------------------------------------------------------
+def ordered(w, absorb=None):
+    w.additive = False
+    if absorb is not None:
+        for sp, k in zip(w.species, absorb):
+            sp.absorb = k
+    return w
+
+
+@pytest.mark.parametrize("tile", [8, 16, 32])
+def test_ordered_cfg0(tile):
+    w = ordered(wl.make_config(0, n=60_000, size=(160, 128)), absorb=[3.0])
+    w.fields["I"] = w.fields["I"] * 30.0                        # optical depths of order one: the order matters
+    full_check(w, tile)
+
+
+def test_ordered_cfg4_reduced_two_species():
+    w = ordered(wl.make_config(4, n=600_000, eta=0.04))         # kappa_gas = 0.5, kappa_star = 2.0 (workloads.py)
+    w.fields["I"] = w.fields["I"] * 200.0
+    st, g = full_check(w, 16)
+    assert st["count"][wl_SMALL] > 0 and st["count"][wl_MEDIUM] > 0
+
+
+def test_ordered_orbit_frame_and_large_particles():
+    w = ordered(wl.make_config(3, n=60_000, size=(256, 192)), absorb=[1.5])
+    w.r_large = 12.0
+    w.fields["I"] = w.fields["I"] * 3.0
+    st, g = full_check(w, 16)
+    assert st["count"][wl_LARGE] > 500
+
+
+def test_ordered_depth_ties_resolve_by_index():
+    """Many particles at exactly the same depth on the same pixels: the visiting order is the particle index."""
+    n = 20_000
+    w = ordered(wl.make_config(0, n=n, size=(64, 64)), absorb=[2.0])
+    w.fields["x"] = 0.5 + 0.02 * (w.fields["x"] - 0.5)
+    w.fields["y"] = 0.5 + 0.02 * (w.fields["y"] - 0.5)
+    w.fields["z"] = torch.full((n,), 0.5) + 0.25 * (torch.arange(n) % 3).float()     # three depth planes, huge tie groups
+    w.fields["I"] = w.fields["I"] * 20.0
+    full_check(w, 16)
+
+
+def test_ordered_heavy_tile_spans_many_chunks():
+    n = 300_000
+    w = ordered(wl.make_config(0, n=n, size=(64, 64)), absorb=[0.7])
+    w.fields["x"] = 0.5 + 0.03 * (w.fields["x"] - 0.5)
+    w.fields["y"] = 0.5 + 0.03 * (w.fields["y"] - 0.5)
+    w.fields["h"][: n // 2] = 1e-5                               # half SMALL
+    w.fields["I"] = w.fields["I"] * 0.5
+    st, g = full_check(w, 16)
+    assert st["chunks"] >= 8
+
+
+def test_ordered_zero_absorption_equals_the_additive_sum():
+    w = ordered(wl.make_config(0, n=30_000, size=(96, 96)), absorb=[0.0])
+    lut = wl.palette()
+    ref, g, cam = oracle_frame(w, lut, 16)
+    r, f, kw, img = gpu_frame(w, lut, 16)
+    assert_image_close(img, ref, "ordered, kappa = 0")
+    img_add = r.render(f, w.species, **dict(kw, additive=True))
+    torch.cuda.synchronize()
+    a, b_ = img.double().cpu().numpy(), img_add.double().cpu().numpy()
+    assert np.linalg.norm(a - b_) <= 2e-6 * np.linalg.norm(b_)
+
+
+def test_ordered_order_matters_and_permutation_of_memory_does_not():
+    """Reversing the depth order changes the image; shuffling the particles in memory (distinct depths) does not."""
+    w = ordered(wl.make_config(4, n=40_000, size=(128, 96), eta=0.1))
+    w.fields["I"] = w.fields["I"] * 300.0
+    lut = wl.palette()
+    r, f, kw, img = gpu_frame(w, lut, 16)
+    img = img.clone()
+    perm = torch.randperm(w.n, generator=torch.Generator().manual_seed(3))
+    w2 = ordered(wl.make_config(4, n=40_000, size=(128, 96), eta=0.1))
+    w2.fields = {k: v[perm].contiguous() for k, v in w.fields.items()}
+    # two species are contiguous index ranges: shuffle inside a single species instead
+    n_gas = w.species[0].end
+    perm = torch.cat([torch.randperm(n_gas, generator=torch.Generator().manual_seed(4)),
+                      n_gas + torch.randperm(w.n - n_gas, generator=torch.Generator().manual_seed(5))])
+    w2.fields = {k: v[perm].contiguous() for k, v in w.fields.items()}
+    ref2, g2, cam2 = oracle_frame(w2, lut, 16)
+    r2, f2, kw2, img2 = gpu_frame(w2, lut, 16)
+    assert_image_close(img2, ref2, "shuffled")
+    zc = g2["zc"][g2["cls"] != so.CULLED]
+    if len(np.unique(zc)) == len(zc):                             # no depth ties: the image is independent of memory order
+        a, b_ = img.double().cpu().numpy(), img2.double().cpu().numpy()
+        assert np.linalg.norm(a - b_) <= 5e-6 * np.linalg.norm(a)
+    # mirrored depth (camera on the other side would be another image; here: the additive image differs from ordered)
+    img_add = r.render(f, w.species, **dict(kw, additive=True)).double().cpu().numpy()
+    assert np.linalg.norm(img.double().cpu().numpy() - img_add) > 1e-3 * np.linalg.norm(img_add)
+
+
+def test_ordered_pair_overflow_is_reported():
+    w = ordered(wl.make_config(0, n=50_000, size=(128, 128)))
+    lut = wl.palette()
+    r, f, kw, img = gpu_frame(w, lut, 16, pair_capacity=1000)
+    st = r.stats()
+    assert st["overflow"] == 1 and st["pairs"] > 1000
+    assert float(img.abs().max()) == 0.0
+    img2 = r.render(f, w.species, pair_capacity=200_000, **kw)
+    assert r.stats()["overflow"] == 0 and float(img2.max()) > 0
+
+
+@pytest.mark.parametrize("n", [0, 1, 33, 4097])
+def test_ordered_tiny_counts(n):
+    w = ordered(wl.make_config(0, n=max(n, 1), size=(64, 48)), absorb=[1.0])
+    if n == 0:
+        w.fields = {k: v[:0] for k, v in w.fields.items()}
+        w.n = 0
+        w.species[0].end = 0
+    full_check(w, 16)
