@@ -29,9 +29,23 @@ import torch  # noqa: E402
 
 from paper_1309_1114_b200 import workloads as wl  # noqa: E402
 
-TILE = 16
-KERNELS_PER_FRAME = 5        # k_count, k_scan, k_scatter, k_splat, k_compose (+ one memset node)
+KERNELS_ADDITIVE = 5         # k_count, k_scan, k_scatter, k_splat, k_compose (+ one memset node)
+L2_FLUSH_BYTES = 256 << 20   # written between frames when a config's inputs fit in the 126 MB L2
+
+
+def tile_for(cfg: int) -> int:
+    return 32 if cfg == 3 else 16       # 4096^2 at 16 px would need a 65,536-bin per-block histogram
+
+
+def ordered_kernels_per_frame(n_tiles: int) -> int:
+    tile_bytes = 1
+    while tile_bytes < 4 and (n_tiles - 1) >> (8 * tile_bytes):
+        tile_bytes += 1
+    return 3 + 5 * (4 + tile_bytes) + 3   # count, scan, pairs; 5 launches per radix pass; bounds, render, combine
+
+
 FLOP_PER_FRAGMENT = 8        # 2 FMA (d^2) + compare + scale + exp2 + 3 FMA, FMA counted once
+FLOP_PER_FRAGMENT_ORDERED = 26   # + optical depth, 1 - exp(-x) (7-term series, exp2, selects), 3 x (sub, FMA), transmission product
 
 
 def measured_peaks():
@@ -84,6 +98,18 @@ class ClockSampler(threading.Thread):
                 "reasons": sorted(self.reasons), "samples": len(self.sm)}
 
 
+def ncu_traffic(kernel: str, workload: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed ncu --set full capture
+    (profiles/dram_traffic.csv: kernel,workload,bytes), or None."""
+    path = os.path.join(ROOT, "profiles", "dram_traffic.csv")
+    if os.path.exists(path):
+        for line in open(path).read().splitlines()[1:]:
+            k, wk, b = line.split(",")[:3]
+            if k == kernel and wk == workload:
+                return float(b)
+    return None
+
+
 def visible_index(local_rank: int) -> int:
     vis = os.environ.get("CUDA_VISIBLE_DEVICES")
     if vis:
@@ -115,6 +141,8 @@ def run_ours(args):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     w = wl.make_config(args.config, device=f"cuda:{local}")
+    TILE = tile_for(args.config)
+    additive = args.mode == "additive"
     lut = wl.palette()
     fields = {k: v.contiguous() for k, v in w.fields.items()}
     r = binding.Renderer(w.width, w.height, w.n, device=local)
@@ -122,10 +150,13 @@ def run_ours(args):
     for s, sp in enumerate(w.species):
         if sp.use_colormap:
             r.set_colormap(s, lut)
-    kw = dict(chi=w.chi, r_small=w.r_small, r_large=w.r_large, z_near=w.z_near, tile=TILE, additive=True,
+    kw = dict(chi=w.chi, r_small=w.r_small, r_large=w.r_large, z_near=w.z_near, tile=TILE, additive=additive,
               apply_transfer=False)
     image = torch.empty((w.height, w.width, 3), dtype=torch.float32, device=f"cuda:{local}")
     stream = torch.cuda.current_stream()
+    orbit = args.config == 4                 # fly-through: the camera moves 3 degrees per frame
+    flush = 24 * w.n < (126 << 20)           # inputs fit in L2: flush it between frames
+    fbuf = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=f"cuda:{local}") if flush else None
 
     def barrier():
         torch.cuda.synchronize()
@@ -133,24 +164,36 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- device-resident timing -------------------------------------------------------------------------------
-    for _ in range(max(args.warmup, 3)):
+    def frame(i):
+        if orbit:
+            r.set_camera(wl.orbit_camera(i % 120))
         r.render(fields, w.species, image=image, **kw)
+
+    # ---- device-resident timing -------------------------------------------------------------------------------
+    for i in range(max(args.warmup, 3)):
+        frame(i)
     torch.cuda.synchronize()
     st0 = r.stats()
     assert st0["overflow"] == 0, "pair capacity overflow"
     r.set_profiling(True)
     sampler = ClockSampler(visible_index(local))
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     barrier()
     sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
-    for _ in range(args.steps):
-        r.render(fields, w.species, image=image, **kw)
+    for i in range(args.steps):
+        if flush:
+            fbuf.fill_(i & 255)
+        ev[i][0].record(stream)
+        frame(i)
+        ev[i][1].record(stream)
     e1.record(stream)
     barrier()
     sampler.stop_flag = True
-    ms_total = e0.elapsed_time(e1)
+    per_frame = sorted(a.elapsed_time(b) for a, b in ev)
+    # with an L2 flush between frames the step time is the sum of the frames' own event pairs
+    ms_total = sum(per_frame) if flush else e0.elapsed_time(e1)
     st = r.stats()
     r.set_profiling(False)
     sampler.join(timeout=1.0)
@@ -158,11 +201,15 @@ def run_ours(args):
     if dist is not None:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     ms_step = float(t.item()) / args.steps
+    dist_ms = {"min": per_frame[0], "median": per_frame[len(per_frame) // 2],
+               "p95": per_frame[min(len(per_frame) - 1, int(0.95 * len(per_frame)))], "max": per_frame[-1]}
 
     # ---- end to end through the C ABI with HOST buffers ---------------------------------------------------------
     host = {k: v.cpu().pin_memory() for k, v in fields.items()}
     himg = torch.empty((w.height, w.width, 3), dtype=torch.float32).pin_memory()
-    e2e_steps = max(3, min(args.steps, 20))
+    e2e_steps = max(3, min(args.steps, 20 if w.n <= 20_000_000 else 3))
+    if orbit:
+        r.set_camera(wl.orbit_camera(0))
     r.render_host(host, w.species, himg, **kw)
     barrier()
     t0 = time.perf_counter()
@@ -184,53 +231,75 @@ def run_ours(args):
     dom = max(stage, key=stage.get)
     pairs = st["pairs"] + st["large_pairs"]
     active = st["n"] - st["count"][0]
+    if orbit:
+        r.set_camera(wl.orbit_camera((args.steps - 1) % 120))     # the camera of the frame the statistics belong to
     frags = fragments_estimate(r, fields, w.species, kw)
-    bytes_by_stage = {
-        "count": 16.0 * w.n,                                   # x y z h read once
-        "scatter": 24.0 * w.n + 32.0 * pairs,                  # six fields read, one 32-B record written per pair
-        "splat": 32.0 * pairs,                                 # records read once
-        "compose": 12.0 * w.width * w.height,                  # image written once
-    }
-    if dom in ("count", "scatter"):
+    n_tiles = (-(-w.width // TILE)) * (-(-w.height // TILE))
+    passes = (ordered_kernels_per_frame(n_tiles) - 6) // 5
+    # algorithmic bytes per stage and frame
+    if additive:
+        bytes_by_stage = {
+            "count": 16.0 * w.n,                                   # x y z h read once
+            "scatter": 24.0 * w.n + 32.0 * pairs,                  # six fields read, one 32-B record written per pair
+            "splat": 32.0 * pairs,                                 # records read once
+            "compose": 12.0 * w.width * w.height,                  # image written once
+        }
+        hbm_stages, alu_stages = ("count", "scatter"), ("splat", "compose")
+    else:
+        bytes_by_stage = {
+            "count": 16.0 * w.n,
+            "pairs": 24.0 * w.n + 32.0 * active + 12.0 * pairs,    # fields read, one record per particle, key + value per pair
+            "sort": passes * (8.0 + 12.0 + 12.0) * pairs,          # per pass: keys read (histogram), key + value read and written
+            "bounds": 8.0 * pairs,
+            "render": (4.0 + 32.0) * pairs,                        # value + gathered record per pair
+            "combine": 12.0 * w.width * w.height,
+        }
+        hbm_stages, alu_stages = ("count", "pairs", "sort"), ("render", "combine")
+    traffic = ncu_traffic("k_" + dom, w.name)
+    if dom in hbm_stages:
         ach = bytes_by_stage[dom] / (stage[dom] * 1e-3) / 1e9
         roof = {"kernel": "k_" + dom, "bound": "hbm", "achieved": ach, "peak": hbm_gbs, "unit": "GB/s",
-                "frac": ach / hbm_gbs, "traffic": None, "peak_source": peak_src + " copy bandwidth"}
+                "frac": ach / hbm_gbs, "traffic": traffic, "peak_source": peak_src + " copy bandwidth"}
     else:
+        flop = FLOP_PER_FRAGMENT if additive else FLOP_PER_FRAGMENT_ORDERED
         peak_tf = 148 * 128 * sm_max_mhz * 1e6 / 1e12          # FP32 lanes x clock, one op per lane per cycle
-        ach = frags * FLOP_PER_FRAGMENT / (stage[dom] * 1e-3) / 1e12
+        ach = frags * flop / (stage[dom] * 1e-3) / 1e12
         roof = {"kernel": "k_" + dom, "bound": "alu", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s",
-                "frac": ach / peak_tf, "traffic": None,
+                "frac": ach / peak_tf, "traffic": traffic,
                 "peak_source": "148 SM x 128 FP32 lanes x %.0f MHz, FMA = 1 op (DESIGN.md)" % sm_max_mhz}
     stage_roof = {}
-    for k in ("count", "scatter"):
-        gbs = bytes_by_stage[k] / (stage[k] * 1e-3) / 1e9
-        stage_roof[k] = {"ms": stage[k], "GB/s": gbs, "frac_hbm": gbs / hbm_gbs}
-    for k in ("scan", "splat", "compose"):
+    for k in stage:
         stage_roof[k] = {"ms": stage[k]}
-    stage_roof["splat"]["Gfragments/s"] = frags / (stage["splat"] * 1e-3) / 1e9
+        if k in hbm_stages:
+            gbs = bytes_by_stage[k] / (stage[k] * 1e-3) / 1e9
+            stage_roof[k].update({"GB/s": gbs, "frac_hbm": gbs / hbm_gbs})
+    rk = "splat" if additive else "render"
+    stage_roof[rk]["Gfragments/s"] = frags / (stage[rk] * 1e-3) / 1e9
     # sum of per-stage lower bounds: HBM terms + ALU term
-    t_min_ms = ((16.0 + 24.0) * w.n + 64.0 * pairs + 12.0 * w.width * w.height) / (hbm_gbs * 1e9) * 1e3 \
-        + frags * FLOP_PER_FRAGMENT / (148 * 128 * sm_max_mhz * 1e6) * 1e3
+    flop = FLOP_PER_FRAGMENT if additive else FLOP_PER_FRAGMENT_ORDERED
+    t_min_ms = sum(bytes_by_stage.values()) / (hbm_gbs * 1e9) * 1e3 + frags * flop / (148 * 128 * sm_max_mhz * 1e6) * 1e3
 
     # ---- CPU baseline: the oracle as it stands, one thread ---------------------------------------------------------
-    cpu = cpu_baseline_frame(w, lut, sample_n=min(w.n, args.cpu_sample))
+    cpu = cpu_baseline_frame(w, lut, min(w.n, args.cpu_sample), TILE, additive)
 
     out = {
         "metric": "particles/s rendered end-to-end per frame",
         "value": world * w.n / (ms_step * 1e-3), "unit": "particles/s", "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": w.name, "particles": w.n, "image": [w.width, w.height], "mode": "additive",
+        "config": {"workload": w.name, "particles": w.n, "image": [w.width, w.height], "mode": args.mode,
                    "tile": TILE, "chi": w.chi, "r_large": w.r_large, "parallelism": "replicas only" if world > 1 else "1 gpu",
-                   "l2": "inputs (%.0f MB) and records (%.0f MB) exceed the 126 MB L2, no flush" %
-                         (24e-6 * w.n, 32e-6 * pairs),
+                   "l2": ("256 MB written between frames (inputs fit in L2); step time = sum of per-frame event pairs" if flush else
+                          "inputs (%.0f MB) and records (%.0f MB) exceed the 126 MB L2, no flush" % (24e-6 * w.n, 32e-6 * pairs)),
+                   "camera": "orbit, 3 deg/frame" if orbit else "fixed",
                    "classes": dict(zip(("culled", "small", "medium", "large"), st["count"])), "pairs": pairs,
                    "active": active, "fragments_estimate": frags},
         "clocks": sampler.result(),
         "e2e": {"value": world * w.n / (e2e_ms * 1e-3), "unit": "particles/s", "ms_per_step": e2e_ms,
                 "h2d_bytes_per_step": 24 * w.n, "d2h_bytes_per_step": 12 * w.width * w.height, "steps": e2e_steps,
                 "api": "splotch_render_host (pinned host arrays in, host image out)"},
-        "gpu_launches": KERNELS_PER_FRAME * args.steps,
+        "gpu_launches": (KERNELS_ADDITIVE if additive else ordered_kernels_per_frame(n_tiles)) * args.steps,
+        "frame_ms": dist_ms,
         "roofline": roof,
         "stages": stage_roof,
         "frame_lower_bound_ms": t_min_ms, "frac_of_frame_roofline": t_min_ms / ms_step,
@@ -241,7 +310,7 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
-def cpu_baseline_frame(w, lut, sample_n: int):
+def cpu_baseline_frame(w, lut, sample_n: int, tile: int = 16, additive: bool = True):
     """Time the oracle (single thread, as it stands) on the first sample_n particles of the workload."""
     from oracle import splotch_oracle as so
     f = {k: v[:sample_n].cpu().numpy() for k, v in w.fields.items()}
@@ -255,7 +324,7 @@ def cpu_baseline_frame(w, lut, sample_n: int):
     so.lib()
     t0 = time.perf_counter()
     so.render(f, species, luts, w.camera, w.width, w.height, chi=w.chi, r_small=w.r_small, r_large=w.r_large,
-              z_near=w.z_near, tile=TILE)
+              z_near=w.z_near, tile=tile, additive=additive)
     dt = time.perf_counter() - t0
     return {"value": sample_n / dt, "unit": "particles/s", "cores": 1, "kind": "oracle", "seconds": dt,
             "sample": "first %d of %d particles of %s, one full frame, single thread" % (sample_n, w.n, w.name)}
@@ -271,17 +340,17 @@ def run_reference(args):
     sample_n = min(w.n, args.ref_sample, max(100_000, int(1.6e8 / (args.steps + args.warmup))))
     times = []
     for _ in range(args.warmup):
-        cpu_baseline_frame(w, lut, sample_n)
+        cpu_baseline_frame(w, lut, sample_n, tile_for(args.config), args.mode == "additive")
     for _ in range(args.steps):
-        times.append(cpu_baseline_frame(w, lut, sample_n)["seconds"])
+        times.append(cpu_baseline_frame(w, lut, sample_n, tile_for(args.config), args.mode == "additive")["seconds"])
     ms = 1e3 * sum(times) / len(times)
     val = sample_n / (ms * 1e-3)
     out = {"impl": "reference", "metric": "particles/s rendered end-to-end per frame", "value": val,
            "unit": "particles/s", "n_gpus": int(os.environ.get("WORLD_SIZE", "1")), "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "f64", "data": "synthetic",
-           "config": {"workload": w.name, "particles": w.n, "image": [w.width, w.height], "mode": "additive",
-                      "tile": TILE, "chi": w.chi, "r_large": w.r_large},
+           "config": {"workload": w.name, "particles": w.n, "image": [w.width, w.height], "mode": args.mode,
+                      "tile": tile_for(args.config), "chi": w.chi, "r_large": w.r_large},
            "cpu_baseline": {"value": val, "unit": "particles/s", "cores": 1, "kind": "oracle",
                             "sample": "each step: one frame of the first %d of %d particles, single thread" % (sample_n, w.n)},
            "e2e": {"value": val, "unit": "particles/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
@@ -294,6 +363,7 @@ def main():
     ap.add_argument("--steps", type=int, default=None)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=1)
+    ap.add_argument("--mode", default="additive", choices=["additive", "ordered"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-sample", type=int, default=10_000_000)
     ap.add_argument("--ref-sample", type=int, default=10_000_000)
