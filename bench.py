@@ -110,6 +110,19 @@ def ncu_traffic(kernel: str, workload: str):
     return None
 
 
+def max_over_ranks(ms: float, dist, device) -> float:
+    """The slowest rank's time: every multi-GPU number is the max over ranks of a device-side timing."""
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, n: int, ms_step: float) -> float:
+    """particles/s of the whole job: N replicas (weak scaling) render world * n particles per step."""
+    return world * n / (ms_step * 1e-3)
+
+
 def visible_index(local_rank: int) -> int:
     vis = os.environ.get("CUDA_VISIBLE_DEVICES")
     if vis:
@@ -197,10 +210,7 @@ def run_ours(args):
     st = r.stats()
     r.set_profiling(False)
     sampler.join(timeout=1.0)
-    t = torch.tensor([ms_total], dtype=torch.float64, device=f"cuda:{local}")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_step = float(t.item()) / args.steps
+    ms_step = max_over_ranks(ms_total, dist, f"cuda:{local}") / args.steps
     dist_ms = {"min": per_frame[0], "median": per_frame[len(per_frame) // 2],
                "p95": per_frame[min(len(per_frame) - 1, int(0.95 * len(per_frame)))], "max": per_frame[-1]}
 
@@ -216,10 +226,7 @@ def run_ours(args):
     for _ in range(e2e_steps):
         r.render_host(host, w.species, himg, **kw)          # synchronises the stream before returning
     t1 = time.perf_counter()
-    te = torch.tensor([(t1 - t0) * 1e3 / e2e_steps], dtype=torch.float64, device=f"cuda:{local}")
-    if dist is not None:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_ms = float(te.item())
+    e2e_ms = max_over_ranks((t1 - t0) * 1e3 / e2e_steps, dist, f"cuda:{local}")
 
     if rank != 0:
         if dist is not None:
@@ -256,17 +263,25 @@ def run_ours(args):
         }
         hbm_stages, alu_stages = ("count", "pairs", "sort"), ("render", "combine")
     traffic = ncu_traffic("k_" + dom, w.name)
-    if dom in hbm_stages:
+    flop = FLOP_PER_FRAGMENT if additive else FLOP_PER_FRAGMENT_ORDERED
+    peak_tf = 148 * 128 * sm_max_mhz * 1e6 / 1e12              # FP32 lanes x clock, one op per lane per cycle
+    bytes_by_stage.setdefault(dom, 0.0)
+    t_hbm = bytes_by_stage[dom] / (hbm_gbs * 1e9)
+    t_alu = frags * flop / (peak_tf * 1e12) if dom in alu_stages and dom in ("splat", "render", "compose") else 0.0
+    if dom == "compose" and additive:
+        t_alu = 0.0 if st["count"][3] == 0 else t_alu          # compose does fragment work only for LARGE particles
+    # the roofline that bounds the stage is the larger of its two lower bounds ("report both, take the larger")
+    if t_hbm >= t_alu:
         ach = bytes_by_stage[dom] / (stage[dom] * 1e-3) / 1e9
         roof = {"kernel": "k_" + dom, "bound": "hbm", "achieved": ach, "peak": hbm_gbs, "unit": "GB/s",
-                "frac": ach / hbm_gbs, "traffic": traffic, "peak_source": peak_src + " copy bandwidth"}
+                "frac": ach / hbm_gbs, "traffic": traffic, "peak_source": peak_src + " copy bandwidth",
+                "other_bound": {"bound": "alu", "lower_bound_ms": t_alu * 1e3}}
     else:
-        flop = FLOP_PER_FRAGMENT if additive else FLOP_PER_FRAGMENT_ORDERED
-        peak_tf = 148 * 128 * sm_max_mhz * 1e6 / 1e12          # FP32 lanes x clock, one op per lane per cycle
         ach = frags * flop / (stage[dom] * 1e-3) / 1e12
         roof = {"kernel": "k_" + dom, "bound": "alu", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s",
                 "frac": ach / peak_tf, "traffic": traffic,
-                "peak_source": "148 SM x 128 FP32 lanes x %.0f MHz, FMA = 1 op (DESIGN.md)" % sm_max_mhz}
+                "peak_source": "148 SM x 128 FP32 lanes x %.0f MHz, FMA = 1 op (DESIGN.md)" % sm_max_mhz,
+                "other_bound": {"bound": "hbm", "lower_bound_ms": t_hbm * 1e3}}
     stage_roof = {}
     for k in stage:
         stage_roof[k] = {"ms": stage[k]}
@@ -284,7 +299,7 @@ def run_ours(args):
 
     out = {
         "metric": "particles/s rendered end-to-end per frame",
-        "value": world * w.n / (ms_step * 1e-3), "unit": "particles/s", "n_gpus": world, "steps": args.steps,
+        "value": whole_job_value(world, w.n, ms_step), "unit": "particles/s", "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": w.name, "particles": w.n, "image": [w.width, w.height], "mode": args.mode,
@@ -295,7 +310,7 @@ def run_ours(args):
                    "classes": dict(zip(("culled", "small", "medium", "large"), st["count"])), "pairs": pairs,
                    "active": active, "fragments_estimate": frags},
         "clocks": sampler.result(),
-        "e2e": {"value": world * w.n / (e2e_ms * 1e-3), "unit": "particles/s", "ms_per_step": e2e_ms,
+        "e2e": {"value": whole_job_value(world, w.n, e2e_ms), "unit": "particles/s", "ms_per_step": e2e_ms,
                 "h2d_bytes_per_step": 24 * w.n, "d2h_bytes_per_step": 12 * w.width * w.height, "steps": e2e_steps,
                 "api": "splotch_render_host (pinned host arrays in, host image out)"},
         "gpu_launches": (KERNELS_ADDITIVE if additive else ordered_kernels_per_frame(n_tiles)) * args.steps,
