@@ -2,6 +2,7 @@
 // Argument checking, camera constants, workspace layout and the per-frame kernel sequence.  No compute happens on
 // the host: every stage of the path is one of the kernels in splotch_kernels.cuh.
 #include "splotch_kernels.cuh"
+#include "splotch_splat.cuh"
 #include "splotch_ordered.cuh"
 #include "../../include/splotch.h"
 
@@ -186,8 +187,8 @@ bool fit_layout_ordered(const splotch_ctx *c, unsigned long long n, int T, size_
 template <int T>
 int query_splat_occupancy(splotch_ctx *c, int *out)
 {
-    CU_TRY(c, cudaFuncSetAttribute(k_splat<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SplatCfg<T>::kSmemBytes));
-    CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, k_splat<T>, SplatCfg<T>::kThreads, SplatCfg<T>::kSmemBytes));
+    CU_TRY(c, cudaFuncSetAttribute(k_splat<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Splat2Cfg<T>::kSmemBytes));
+    CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, k_splat<T>, SplatCfg<T>::kThreads, Splat2Cfg<T>::kSmemBytes));
     if (*out < 1) *out = 1;
     return SPLOTCH_OK;
 }
@@ -271,7 +272,7 @@ int launch_render_tail(splotch_ctx *c, const Layout &L, char *ws, const FramePar
 {
     const int ti = T == 8 ? 0 : T == 16 ? 1 : 2;
     const int grid = c->n_sm * c->splat_blocks_per_sm[ti];
-    k_splat<T><<<grid, SplatCfg<T>::kThreads, SplatCfg<T>::kSmemBytes, st>>>(
+    k_splat<T><<<grid, SplatCfg<T>::kThreads, Splat2Cfg<T>::kSmemBytes, st>>>(
         (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.bin_start), (DeviceStats *)(ws + L.stats), (unsigned long long *)(ws + L.accum), fp);
     if (c->profiling) cudaEventRecord(c->ev[4], st);
     k_compose<T><<<fp.n_tiles, 256, 0, st>>>((const unsigned long long *)(ws + L.accum), (const float4 *)(ws + L.records),

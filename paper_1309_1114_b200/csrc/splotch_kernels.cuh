@@ -382,8 +382,9 @@ k_scan(unsigned int *__restrict__ counts, int nrows, int nbins, int n_tiles, uns
     }
     const unsigned long long off_all = block_excl_scan_256(sum_all, s_warp, &s_tot_all);
     (void)block_excl_scan_256(sum_tiles, s_warp, &s_tot_pairs);
-    // chunk size of this frame: about 32 chunks per SM, between kChunkMin and kChunkMax, a multiple of 256
-    unsigned long long cs = (s_tot_pairs + (unsigned long long)n_sm * 32 - 1) / ((unsigned long long)n_sm * 32);
+    // chunk size of this frame: about 128 chunks per SM (work items are taken from an atomic counter; many small ones
+    // keep the tail short when their costs differ), between kChunkMin and kChunkMax, a multiple of 256
+    unsigned long long cs = (s_tot_pairs + (unsigned long long)n_sm * 128 - 1) / ((unsigned long long)n_sm * 128);
     cs = (cs + 255) / 256 * 256;
     cs = min((unsigned long long)kChunkMax, max((unsigned long long)kChunkMin, cs));
     const unsigned int K = (unsigned int)cs;
@@ -621,181 +622,7 @@ template <int T> struct SplatCfg {
     static constexpr size_t kSmemBytes = sizeof(unsigned int) * 6 * kPix + (sizeof(float4) * 2 + sizeof(unsigned int)) * kThreads;
 };
 
-// One work item = chunk_size consecutive records of the bin-sorted array; the chunk is cut into segments at tile
-// boundaries.  Per segment the CTA clears the tile's fixed-point planes and its register sums, then takes batches
-// of one record per thread:
-//   * records whose box is at most 2 x 2 pixels (every SMALL record, the smallest MEDIUM ones) are splatted by the
-//     thread that loaded them, pixel by pixel, into the fixed-point planes (shared-memory integer atomics);
-//   * all other records are staged in shared memory with the set of strips their box touches; every warp walks the
-//     records that touch its strip and evaluates each for its 64 pixels at once: the C1 inside test and the Gaussian
-//     weight in packed float32 pairs (FADD2 / FFMA2 / FMUL2), two ex2, three packed FMAs into registers.  No atomics,
-//     no conversions, no per-fragment index arithmetic; this is the paper's "one pixel per thread, particles in
-//     sequence" scheme (:226) with the block replaced by a 64-pixel warp strip and a box test in front.
-// Register sums are two-level (folded every ~1024 records) so a pixel that receives thousands of contributions in a
-// segment keeps float32 sums accurate to ~1e-6.  At the end of the segment each lane converts its sums to fixed
-// point and adds them to the planes of its own pixels; the planes are then added to the tile's 64-bit sums in global
-// memory (`accum`, cleared before every frame), which k_compose turns into the image.
-template <int T>
-__global__ void __launch_bounds__(SplatCfg<T>::kThreads)
-k_splat(const float4 *__restrict__ records, const unsigned int *__restrict__ bin_start, DeviceStats *__restrict__ stats,
-        unsigned long long *__restrict__ accum, const __grid_constant__ FrameParams fp)
-{
-    using Cfg = SplatCfg<T>;
-    constexpr int kPix = Cfg::kPix, kThreads = Cfg::kThreads;
-    extern __shared__ __align__(16) unsigned int smem_u[];
-    unsigned int *fb = smem_u;                                            // lo R G B, hi R G B
-    float4 *stA = reinterpret_cast<float4 *>(smem_u + 6 * kPix);
-    float4 *stB = stA + kThreads;
-    unsigned int *stM = reinterpret_cast<unsigned int *>(stB + kThreads);  // strips touched: x mask << 16 | y mask (0: not staged)
-    __shared__ unsigned int s_chunk;
-    __shared__ int s_tile;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    // this lane's pixel pair inside the tile
-    const int sx = warp % Cfg::kStripsX, sy = warp / Cfg::kStripsX;
-    const int lx = sx * Cfg::kSW + 2 * (lane % (Cfg::kSW / 2)), ly = sy * Cfg::kSH + lane / (Cfg::kSW / 2);
-    const unsigned int my_strip = (1u << (16 + sx)) | (1u << sy);
-    const unsigned int total = (unsigned int)stats->chunks;
-    const unsigned int K = stats->chunk_size;
-    const unsigned int pairs = (unsigned int)stats->pairs;
-    const int e = fixed_exponent(stats->amax_bits);
-    const float sc1 = pow2i(e / 2), sc2 = pow2i(e - e / 2);
-    for (;;) {
-        __syncthreads();
-        if (warp == 0) {
-            // next chunk, and the tile that holds its first record: the last tile t with bin_start[t] <= r0, found
-            // by a 32-way search over bin_start (three or four rounds of 32 probes)
-            unsigned int c = 0u;
-            if (lane == 0) c = atomicAdd(&stats->work_counter, 1u);
-            c = __shfl_sync(0xffffffffu, c, 0);
-            if (c < total) {
-                const unsigned int r = c * K;
-                int lo = 0, n = fp.n_tiles;                       // answer in [lo, lo + n)
-                while (n > 1) {
-                    const int step = (n + 31) / 32;
-                    const int t = lo + lane * step;
-                    const bool le = t < lo + n && __ldg(bin_start + t) <= r;
-                    const int k = __popc(__ballot_sync(0xffffffffu, le)) - 1;     // lane 0 always qualifies
-                    lo += k * step;
-                    n = min(step, n - k * step);
-                }
-                if (lane == 0) s_tile = lo;
-            }
-            if (lane == 0) s_chunk = c;
-        }
-        __syncthreads();
-        const unsigned int chunk = s_chunk;
-        if (chunk >= total) break;
-        const unsigned int r0 = chunk * K, r1 = min(r0 + K, pairs);
-        int tile = s_tile;
-        unsigned int tb = bin_start[tile], te = bin_start[tile + 1];
-        for (;;) {
-            // ---- segment = [max(tb, r0), min(te, r1)) of `tile`
-            const unsigned int begin = max(tb, r0), end = min(te, r1);
-            for (int i = threadIdx.x; i < 6 * kPix; i += kThreads) fb[i] = 0u;
-            __syncthreads();
-            const int tx0 = (tile % fp.ntx) * T, ty0 = (tile / fp.ntx) * T;
-            const float fx = __fadd_rn((float)(tx0 + lx), 0.5f), fy = __fadd_rn((float)(ty0 + ly), 0.5f);
-            const f32x2 fxp = pk2(fx, __fadd_rn(fx, 1.0f));
-            f32x2 accR = 0ull, accG = 0ull, accB = 0ull, subR = 0ull, subG = 0ull, subB = 0ull;   // +0.0f pairs
-            int fold = 0;
-            for (unsigned int base = begin; base < end; base += kThreads) {
-                const unsigned int idx = base + threadIdx.x;
-                float4 ra = make_float4(0.f, 0.f, 0.f, 0.f), rb = ra;
-                unsigned int touch = 0u;
-                if (idx < end) {
-                    ld_record(records, idx, ra, rb);
-                    const unsigned int box = __float_as_uint(rb.w);
-                    const int bx0 = (int)(box & 31u), by0 = (int)((box >> 5) & 31u);
-                    const int bw1 = (int)((box >> 10) & 31u), bh1 = (int)((box >> 15) & 31u);     // width - 1, height - 1
-                    if (bw1 <= 1 && bh1 <= 1) {
-                        // ---- direct path: at most 2 x 2 pixels, fixed point
-                        const float ax = rb.x * sc1 * sc2, ay = rb.y * sc1 * sc2, az = rb.z * sc1 * sc2;
-                        const float fx0 = __fadd_rn((float)(tx0 + bx0), 0.5f), fy0 = __fadd_rn((float)(ty0 + by0), 0.5f);
-#pragma unroll
-                        for (int q = 0; q < 4; ++q) {
-                            const int qx = q & 1, qy = q >> 1;
-                            if (qx <= bw1 && qy <= bh1) {
-                                const float dxf = __fsub_rn(qx ? __fadd_rn(fx0, 1.0f) : fx0, ra.x);
-                                const float dyf = __fsub_rn(qy ? __fadd_rn(fy0, 1.0f) : fy0, ra.y);
-                                const float d2 = __fmaf_rn(dxf, dxf, __fmul_rn(dyf, dyf));
-                                if (d2 <= ra.w) {
-                                    const float wgt = ex2_approx(d2 * ra.z);
-                                    unsigned int *q0 = fb + (by0 + qy) * T + bx0 + qx;
-                                    fixed_add(q0, q0 + 3 * kPix, ax * wgt);
-                                    fixed_add(q0 + kPix, q0 + 4 * kPix, ay * wgt);
-                                    fixed_add(q0 + 2 * kPix, q0 + 5 * kPix, az * wgt);
-                                }
-                            }
-                        }
-                    } else {
-                        const int x1 = bx0 + bw1, y1 = by0 + bh1;
-                        const unsigned int xm = (2u << (x1 / Cfg::kSW)) - (1u << (bx0 / Cfg::kSW));
-                        const unsigned int ym = (2u << (y1 / Cfg::kSH)) - (1u << (by0 / Cfg::kSH));
-                        touch = (xm << 16) | ym;
-                    }
-                }
-                __syncthreads();                         // previous batch fully consumed
-                stA[threadIdx.x] = ra; stB[threadIdx.x] = rb; stM[threadIdx.x] = touch;
-                __syncthreads();
-#pragma unroll 1
-                for (int g = 0; g < kThreads; g += 32) {
-                    const unsigned int t = stM[g + lane];
-                    unsigned int m = __ballot_sync(0xffffffffu, (t & my_strip & 0xffff0000u) && (t & my_strip & 0xffffu));
-                    while (m) {
-                        const int r = g + __ffs(m) - 1;
-                        m &= m - 1;
-                        const float4 A = stA[r], B = stB[r];
-                        const float dyf = __fsub_rn(fy, A.y);
-                        const f32x2 dx = fadd2(fxp, pk2(-A.x, -A.x));
-                        const float t2 = __fmul_rn(dyf, dyf);
-                        const f32x2 d2 = ffma2(dx, dx, pk2(t2, t2));
-                        const f32x2 arg = fmul2(d2, pk2(A.z, A.z));
-                        float d20, d21, a0, a1;
-                        upk2(d2, d20, d21); upk2(arg, a0, a1);
-                        const float w0 = d20 <= A.w ? ex2_approx(a0) : 0.0f;
-                        const float w1 = d21 <= A.w ? ex2_approx(a1) : 0.0f;
-                        const f32x2 w = pk2(w0, w1);
-                        subR = ffma2(pk2(B.x, B.x), w, subR);
-                        subG = ffma2(pk2(B.y, B.y), w, subG);
-                        subB = ffma2(pk2(B.z, B.z), w, subB);
-                    }
-                }
-                if (++fold == Cfg::kFoldBatches) {
-                    fold = 0;
-                    accR = fadd2(accR, subR); accG = fadd2(accG, subG); accB = fadd2(accB, subB);
-                    subR = subG = subB = 0ull;
-                }
-            }
-            accR = fadd2(accR, subR); accG = fadd2(accG, subG); accB = fadd2(accB, subB);
-            __syncthreads();                             // all direct-path atomics of the segment have landed
-            {   // register sums -> fixed point, added to this lane's own two pixels (no other thread touches them now)
-                float v[6];
-                upk2(accR, v[0], v[1]); upk2(accG, v[2], v[3]); upk2(accB, v[4], v[5]);
-#pragma unroll
-                for (int c = 0; c < 3; ++c)
-#pragma unroll
-                    for (int q = 0; q < 2; ++q) {
-                        const long long f = __float2ll_rn(v[2 * c + q] * sc1 * sc2);
-                        unsigned int *q0 = fb + c * kPix + ly * T + lx + q;
-                        q0[0] += (unsigned int)(f & 0xffffll);
-                        q0[3 * kPix] += (unsigned int)(int)(f >> 16);
-                    }
-            }
-            __syncthreads();
-            // ---- add the segment's planes to the tile's sums in global memory (64-bit integer reductions in L2:
-            //      exact and commutative, so the order in which the segments of a heavy tile arrive does not matter)
-            unsigned long long *out = accum + (size_t)tile * (3 * kPix);
-            for (int i = threadIdx.x; i < 3 * kPix; i += kThreads) {
-                const long long v = (long long)(int)fb[3 * kPix + i] * 65536ll + (long long)fb[i];
-                if (v != 0ll) atomicAdd(out + i, (unsigned long long)v);
-            }
-            if (te >= r1) break;
-            // ---- next non-empty tile
-            do { ++tile; tb = te; te = bin_start[tile + 1]; } while (te == tb);
-            __syncthreads();
-        }
-    }
-}
+// k_splat itself lives in splotch_splat.cuh.
 
 // ---- A6 + A8: compose one tile ----------------------------------------------------------------------------------
 // Thread t owns pixels t, t+256, ... of the tile (registers).  Reads the tile's fixed-point sums, then gathers the
