@@ -97,8 +97,8 @@ size_t bin_smem_bytes(int W, int H, int T) { return hist_bytes(W, H, T) + 16 + s
 
 int bin_rows(const splotch_ctx *c, int T)
 {
-    // two resident blocks per SM while two private histograms fit in shared memory, else one
-    return c->n_sm * (2 * (bin_smem_bytes(c->width, c->height, T) + 1024) <= (size_t)c->smem_optin ? 2 : 1);
+    (void)T;
+    return c->n_sm;                         // one 1024-thread CTA per SM, each with a private histogram over all bins
 }
 
 // Workspace layout.  Either `capacity` is given (sizing query) or derived from `bytes` (render).

@@ -32,7 +32,7 @@ constexpr int kMaxSpecies   = 8;
 constexpr int kMaxLut       = 1024;
 constexpr int kChunkMax     = 32768;  // records per work item of k_splat (upper bound; the frame picks its own)
 constexpr int kChunkMin     = 512;
-constexpr int kBinThreads   = 512;    // k_count / k_scatter block size
+constexpr int kBinThreads   = 1024;   // k_count / k_scatter block size: one CTA per SM (fewer histogram rows and write streams than 2 x 512)
 constexpr int kSuperShift   = 3;      // super-tile = 8 x 8 tiles (LARGE particles are binned to super-tiles)
 constexpr int kLutSmemMax   = 1024;   // colour-table entries (all species together) staged in shared memory by k_scatter
 constexpr int kFixedBits    = 30;     // the largest record amplitude maps to [2^29, 2^30) fixed-point units
@@ -211,7 +211,7 @@ __device__ __forceinline__ unsigned int warp_sum(unsigned int v)
 // Block b owns the particle range [b*per, (b+1)*per) and a private histogram over all bins in shared memory;
 // row b of `counts` receives it, so the count stage needs no global atomics and is deterministic.
 template <bool ALIGNED>
-__global__ void __launch_bounds__(kBinThreads, 2)
+__global__ void __launch_bounds__(kBinThreads, 1)
 k_count(const float *__restrict__ x, const float *__restrict__ y, const float *__restrict__ z,
         const float *__restrict__ h, unsigned long long n, unsigned long long per, const __grid_constant__ FrameParams fp,
         unsigned int *__restrict__ counts, unsigned int *__restrict__ cls_counts)
@@ -480,7 +480,7 @@ __device__ __forceinline__ unsigned int pack_box(const Geo &g, int cls, int bx, 
 }
 
 template <bool ALIGNED>
-__global__ void __launch_bounds__(kBinThreads, 2)
+__global__ void __launch_bounds__(kBinThreads, 1)
 k_scatter(const float *__restrict__ x, const float *__restrict__ y, const float *__restrict__ z,
           const float *__restrict__ h, const float *__restrict__ I, const float *__restrict__ scalar,
           unsigned long long n, unsigned long long per, const __grid_constant__ FrameParams fp,
