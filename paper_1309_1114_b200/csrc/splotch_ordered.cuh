@@ -108,7 +108,7 @@ k_oscan(unsigned int *__restrict__ blk_pairs, int nblk, unsigned long long n, un
     const bool overflow = total > capacity;
     for (int b = b0; b < b1; ++b) { const unsigned int c = blk_pairs[b]; blk_pairs[b] = (unsigned int)run; run += c; }
     if (threadIdx.x == 0) {
-        unsigned long long cs = (total + (unsigned long long)n_sm * 32 - 1) / ((unsigned long long)n_sm * 32);
+        unsigned long long cs = (total + (unsigned long long)n_sm * 128 - 1) / ((unsigned long long)n_sm * 128);
         cs = (cs + 255) / 256 * 256;
         cs = min((unsigned long long)kChunkMax, max((unsigned long long)kOChunkMin, cs));
         stats->pairs = total;
@@ -462,8 +462,8 @@ k_orender(const float4 *__restrict__ rec, const unsigned long long *__restrict__
 {
     using Cfg = SplatCfg<T>;
     constexpr int kPix = Cfg::kPix, kThreads = Cfg::kThreads;
-    __shared__ float4 stA[kThreads], stB[kThreads];
-    __shared__ unsigned int stM[kThreads];
+    __shared__ float4 stA[2][kThreads], stB[2][kThreads];      // double buffered: one barrier per batch
+    __shared__ unsigned int stM[2][kThreads];
     __shared__ unsigned int s_chunk;
     __shared__ int s_tile;
     (void)keys;
@@ -510,12 +510,24 @@ k_orender(const float4 *__restrict__ rec, const unsigned long long *__restrict__
             double To[2] = {1.0, 1.0}, Co[2][3] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
             float ti[2] = {1.0f, 1.0f}, ci[2][3] = {{0.0f, 0.0f, 0.0f}, {0.0f, 0.0f, 0.0f}};
             int fold = 0;
-            for (unsigned int base = begin; base < end; base += kThreads) {
+            // The records of a batch are gathered through the sorted values.  Batch b + 1's records and batch b + 2's
+            // values are requested before batch b is composed, so the gather latency hides behind the arithmetic.
+            const unsigned int i0 = begin + threadIdx.x;
+            unsigned int vnext = i0 + kThreads < end ? __ldg(vals + i0 + kThreads) : 0u;
+            float4 nra = make_float4(0.f, 0.f, 0.f, 0.f), nrb = nra;
+            if (i0 < end) ld_record(rec, __ldg(vals + i0), nra, nrb);
+            unsigned int batch = 0u;
+            for (unsigned int base = begin; base < end; base += kThreads, ++batch) {
                 const unsigned int idx = base + threadIdx.x;
-                float4 ra = make_float4(0.f, 0.f, 0.f, 0.f), rb = ra;
+                const float4 ra = nra, rb = nrb;
+                {
+                    const unsigned int nxt = idx + kThreads;
+                    nra = make_float4(0.f, 0.f, 0.f, 0.f); nrb = nra;
+                    if (nxt < end) ld_record(rec, vnext, nra, nrb);
+                    if (nxt + kThreads < end) vnext = __ldg(vals + nxt + kThreads);
+                }
                 unsigned int touch = 0u;
                 if (idx < end) {
-                    ld_record(rec, __ldg(vals + idx), ra, rb);
                     // strips the clip disc may touch (conservative: one pixel of slack; the inside test decides)
                     const float rr = sqrtf(fabsf(ra.w)) + 1.0f;
                     const int bx0 = max(floor_clamped(ra.x - rr) - tx0, 0), bx1 = min(floor_clamped(ra.x + rr) - tx0, T - 1);
@@ -526,17 +538,18 @@ k_orender(const float4 *__restrict__ rec, const unsigned long long *__restrict__
                         touch = (xm << 16) | ym;
                     }
                 }
-                __syncthreads();
-                stA[threadIdx.x] = ra; stB[threadIdx.x] = rb; stM[threadIdx.x] = touch;
-                __syncthreads();
+                const float4 *sA = stA[batch & 1u], *sB = stB[batch & 1u];
+                const unsigned int *sM = stM[batch & 1u];
+                stA[batch & 1u][threadIdx.x] = ra; stB[batch & 1u][threadIdx.x] = rb; stM[batch & 1u][threadIdx.x] = touch;
+                __syncthreads();             // batch visible; every warp is done with the batch before the previous one
 #pragma unroll 1
                 for (int g = 0; g < kThreads; g += 32) {
-                    const unsigned int t = stM[g + lane];
+                    const unsigned int t = sM[g + lane];
                     unsigned int m = __ballot_sync(0xffffffffu, (t & my_strip & 0xffff0000u) && (t & my_strip & 0xffffu));
                     while (m) {                                            // ascending bit order = depth order
                         const int r = g + __ffs(m) - 1;
                         m &= m - 1;
-                        const float4 A = stA[r], B = stB[r];
+                        const float4 A = sA[r], B = sB[r];
                         const float r2 = fabsf(A.w);
                         const bool emit_only = A.w < 0.0f;
                         const float dyf = __fsub_rn(fy, A.y);
