@@ -29,7 +29,7 @@ import torch  # noqa: E402
 
 from paper_1309_1114_b200 import workloads as wl  # noqa: E402
 
-KERNELS_ADDITIVE = 5         # k_count, k_scan, k_scatter, k_splat, k_compose (+ one memset node)
+KERNELS_ADDITIVE = 6         # k_count, k_scan, k_scatter, k_splat, k_large, k_compose (+ one memset node)
 L2_FLUSH_BYTES = 256 << 20   # written between frames when a config's inputs fit in the 126 MB L2
 
 
@@ -140,7 +140,7 @@ def fragments_estimate(r, fields, species, kw) -> float:
     cls, rp, box = d["cls"], d["rp"].double(), d["pbox"].double()
     area = (box[:, 1] - box[:, 0] + 1) * (box[:, 3] - box[:, 2] + 1)
     disc = torch.minimum(torch.pi * rp * rp, area)
-    return float((cls == 1).sum() + disc[cls >= 2].sum())
+    return float((cls == 1).sum() + disc[cls >= 2].sum()), float(disc[cls == 3].sum())
 
 
 def run_ours(args):
@@ -240,7 +240,7 @@ def run_ours(args):
     active = st["n"] - st["count"][0]
     if orbit:
         r.set_camera(wl.orbit_camera((args.steps - 1) % 120))     # the camera of the frame the statistics belong to
-    frags = fragments_estimate(r, fields, w.species, kw)
+    frags, frags_large = fragments_estimate(r, fields, w.species, kw)
     n_tiles = (-(-w.width // TILE)) * (-(-w.height // TILE))
     passes = (ordered_kernels_per_frame(n_tiles) - 6) // 5
     # algorithmic bytes per stage and frame
@@ -248,10 +248,11 @@ def run_ours(args):
         bytes_by_stage = {
             "count": 16.0 * w.n,                                   # x y z h read once
             "scatter": 24.0 * w.n + 32.0 * pairs,                  # six fields read, one 32-B record written per pair
-            "splat": 32.0 * pairs,                                 # records read once
-            "compose": 12.0 * w.width * w.height,                  # image written once
+            "splat": 32.0 * st["pairs"],                           # records read once
+            "large": 32.0 * st["large_pairs"],                     # super-tile records read once (64 tiles share them in L2)
+            "compose": (24.0 + 12.0) * w.width * w.height,         # fixed-point sums read, image written once
         }
-        hbm_stages, alu_stages = ("count", "scatter"), ("splat", "compose")
+        hbm_stages, alu_stages = ("count", "scatter"), ("splat", "large", "compose")
     else:
         bytes_by_stage = {
             "count": 16.0 * w.n,
@@ -267,9 +268,8 @@ def run_ours(args):
     peak_tf = 148 * 128 * sm_max_mhz * 1e6 / 1e12              # FP32 lanes x clock, one op per lane per cycle
     bytes_by_stage.setdefault(dom, 0.0)
     t_hbm = bytes_by_stage[dom] / (hbm_gbs * 1e9)
-    t_alu = frags * flop / (peak_tf * 1e12) if dom in alu_stages and dom in ("splat", "render", "compose") else 0.0
-    if dom == "compose" and additive:
-        t_alu = 0.0 if st["count"][3] == 0 else t_alu          # compose does fragment work only for LARGE particles
+    dom_frags = {"splat": frags - frags_large, "large": frags_large, "render": frags}.get(dom, 0.0) if additive or dom == "render" else 0.0
+    t_alu = dom_frags * flop / (peak_tf * 1e12)
     # the roofline that bounds the stage is the larger of its two lower bounds ("report both, take the larger")
     if t_hbm >= t_alu:
         ach = bytes_by_stage[dom] / (stage[dom] * 1e-3) / 1e9
@@ -277,7 +277,7 @@ def run_ours(args):
                 "frac": ach / hbm_gbs, "traffic": traffic, "peak_source": peak_src + " copy bandwidth",
                 "other_bound": {"bound": "alu", "lower_bound_ms": t_alu * 1e3}}
     else:
-        ach = frags * flop / (stage[dom] * 1e-3) / 1e12
+        ach = dom_frags * flop / (stage[dom] * 1e-3) / 1e12
         roof = {"kernel": "k_" + dom, "bound": "alu", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s",
                 "frac": ach / peak_tf, "traffic": traffic,
                 "peak_source": "148 SM x 128 FP32 lanes x %.0f MHz, FMA = 1 op (DESIGN.md)" % sm_max_mhz,
@@ -308,7 +308,7 @@ def run_ours(args):
                           "inputs (%.0f MB) and records (%.0f MB) exceed the 126 MB L2, no flush" % (24e-6 * w.n, 32e-6 * pairs)),
                    "camera": "orbit, 3 deg/frame" if orbit else "fixed",
                    "classes": dict(zip(("culled", "small", "medium", "large"), st["count"])), "pairs": pairs,
-                   "active": active, "fragments_estimate": frags},
+                   "active": active, "fragments_estimate": frags, "fragments_large": frags_large},
         "clocks": sampler.result(),
         "e2e": {"value": whole_job_value(world, w.n, e2e_ms), "unit": "particles/s", "ms_per_step": e2e_ms,
                 "h2d_bytes_per_step": 24 * w.n, "d2h_bytes_per_step": 12 * w.width * w.height, "steps": e2e_steps,

@@ -93,7 +93,7 @@ typedef struct {
     uint64_t pair_capacity;          /* records the workspace could hold                                    */
     int32_t  overflow;               /* 1: pairs + large_pairs > pair_capacity, the image is all zero       */
     int32_t  n_stages;               /* number of valid entries in stage_ms (0 unless profiling is on)      */
-    float    stage_ms[8];            /* additive: count, scan, scatter, splat, compose; ordered: count, scan,
+    float    stage_ms[8];            /* additive: count, scan, scatter, splat, large, compose; ordered: count, scan,
                                         pairs, sort, bounds, render, combine (see splotch_stage_name)        */
 } splotch_stats;
 

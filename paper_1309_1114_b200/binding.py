@@ -240,7 +240,7 @@ class Renderer:
         _check(self.ctx, self.lib.splotch_get_stats(self.ctx, C.byref(st)))
         d = {"n": st.n, "count": list(st.count), "pairs": st.pairs, "large_pairs": st.large_pairs,
              "chunks": st.chunks, "pair_capacity": st.pair_capacity, "overflow": st.overflow,
-             "stage_ms": {self.lib.splotch_stage_name(int(st.n_stages <= 5), i).decode(): st.stage_ms[i]
+             "stage_ms": {self.lib.splotch_stage_name(int(st.n_stages < 7), i).decode(): st.stage_ms[i]
                           for i in range(st.n_stages)}}
         return d
 

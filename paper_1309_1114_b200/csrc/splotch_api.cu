@@ -3,6 +3,7 @@
 // the host: every stage of the path is one of the kernels in splotch_kernels.cuh.
 #include "splotch_kernels.cuh"
 #include "splotch_splat.cuh"
+#include "splotch_large.cuh"
 #include "splotch_ordered.cuh"
 #include "../../include/splotch.h"
 
@@ -17,9 +18,9 @@ using namespace splotch;
 namespace {
 
 constexpr int kStages = 7;                  // most stages a frame has (ordered mode); additive frames have 5
-constexpr int kStagesAdditive = 5, kStagesOrdered = 7;
+constexpr int kStagesAdditive = 6, kStagesOrdered = 7;
 constexpr int kProfRing = 256;              // frames of per-stage events kept while profiling
-const char *kStageNamesAdditive[kStagesAdditive] = {"count", "scan", "scatter", "splat", "compose"};
+const char *kStageNamesAdditive[kStagesAdditive] = {"count", "scan", "scatter", "splat", "large", "compose"};
 const char *kStageNamesOrdered[kStagesOrdered] = {"count", "scan", "pairs", "sort", "bounds", "render", "combine"};
 
 struct Layout {
@@ -57,6 +58,7 @@ struct splotch_ctx {
     cudaStream_t last_stream = nullptr;
     int splat_blocks_per_sm[3] = {0, 0, 0};  // T = 8, 16, 32
     int orender_blocks_per_sm[3] = {0, 0, 0};
+    int large_blocks_per_sm[3] = {0, 0, 0};
     char err[512] = {0};
 };
 
@@ -228,6 +230,7 @@ int check_params(splotch_ctx *c, const splotch_particles *p, unsigned long long 
     fp->nsx = (c->width + S - 1) / S; fp->nsy = (c->height + S - 1) / S;
     fp->n_super = fp->nsx * fp->nsy;
     fp->nbins = fp->n_tiles + fp->n_super;
+    if (fp->n_super > kMaxSuper) return fail(c, SPLOTCH_EINVAL, "tile %d gives %d super-tiles (at most %d); use a larger tile", q->tile, fp->n_super, kMaxSuper);
     fp->additive = q->additive ? 1 : 0;
     fp->apply_transfer = q->apply_transfer ? 1 : 0;
     fp->n_species = ns;
@@ -275,10 +278,11 @@ int launch_render_tail(splotch_ctx *c, const Layout &L, char *ws, const FramePar
     k_splat<T><<<grid, SplatCfg<T>::kThreads, Splat2Cfg<T>::kSmemBytes, st>>>(
         (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.bin_start), (DeviceStats *)(ws + L.stats), (unsigned long long *)(ws + L.accum), fp);
     if (c->profiling) cudaEventRecord(c->ev[4], st);
-    k_compose<T><<<fp.n_tiles, 256, 0, st>>>((const unsigned long long *)(ws + L.accum), (const float4 *)(ws + L.records),
-                                             (const unsigned int *)(ws + L.bin_start), (const DeviceStats *)(ws + L.stats),
-                                             fp, image);
+    k_large<T><<<c->n_sm * c->large_blocks_per_sm[ti], kLargeThreads, 0, st>>>(
+        (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.bin_start), (DeviceStats *)(ws + L.stats), (unsigned long long *)(ws + L.accum), fp);
     if (c->profiling) cudaEventRecord(c->ev[5], st);
+    k_compose<T><<<fp.n_tiles, 256, 0, st>>>((const unsigned long long *)(ws + L.accum), (const DeviceStats *)(ws + L.stats), fp, image);
+    if (c->profiling) cudaEventRecord(c->ev[6], st);
     return SPLOTCH_OK;
 }
 
@@ -454,6 +458,10 @@ int splotch_create(splotch_ctx **out, int device, int width, int height, uint64_
         CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->orender_blocks_per_sm[1], k_orender<16>, SplatCfg<16>::kThreads, 0));
         CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->orender_blocks_per_sm[2], k_orender<32>, SplatCfg<32>::kThreads, 0));
         for (int k = 0; k < 3; ++k) if (c->orender_blocks_per_sm[k] < 1) c->orender_blocks_per_sm[k] = 1;
+        CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->large_blocks_per_sm[0], k_large<8>, kLargeThreads, 0));
+        CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->large_blocks_per_sm[1], k_large<16>, kLargeThreads, 0));
+        CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->large_blocks_per_sm[2], k_large<32>, kLargeThreads, 0));
+        for (int k = 0; k < 3; ++k) if (c->large_blocks_per_sm[k] < 1) c->large_blocks_per_sm[k] = 1;
         return r;
     }();
     if (rc != SPLOTCH_OK) {

@@ -12,9 +12,9 @@
 //                         32-bit planes per channel, native integer atomics without return; the paper's
 //                         medium-particle kernel, :183, :224-228, without its halo copies and without idle threads
 //                         for small footprints)
-//   k_compose  A6+A8      per tile: read the tile's fixed-point sums, gather the LARGE particles of the tile's
-//                         super-tile (the paper renders these on the CPU, :232-238), optional 1-exp(-S), write the
-//                         image once
+//   k_large    A6         (splotch_large.cuh) LARGE particles, which the paper renders on the CPU (:232-238): items of
+//                         (chunk of a super-tile's records) x (tile), added to the same fixed-point sums
+//   k_compose  A8         per tile: fixed-point sums -> float32, optional 1-exp(-S), write the image once
 //
 // Canonical float32 geometry: every operation that decides an integer (class, pixel box, tile box, the inside
 // test) is written with round-to-nearest intrinsics (__fmul_rn, __fmaf_rn, __fdiv_rn ...) which nvcc never
@@ -66,7 +66,7 @@ struct DeviceStats {             // cleared before every frame; written by k_sca
     unsigned long long count[4];
     unsigned long long pairs, large_pairs, chunks, capacity;
     unsigned long long sort_n;   // ordered mode: pairs the sort and the renderer work on (0 on overflow)
-    unsigned int overflow, work_counter, chunk_size, amax_bits, scan_done, pad;
+    unsigned int overflow, work_counter, chunk_size, amax_bits, scan_done, large_counter;   // large_counter: work items of k_large
 };
 
 struct Geo {
@@ -536,7 +536,7 @@ k_scatter(const float *__restrict__ x, const float *__restrict__ y, const float 
             ra.w = small ? __int_as_float(0x7f800000) : __fmul_rn(g.rp, g.rp);
             const float am = fmaxf(fabsf(a.x), fmaxf(fabsf(a.y), fabsf(a.z)));
             if (!(am <= 3.0e38f)) a = make_float3(0.0f, 0.0f, 0.0f);             // Inf / NaN amplitude
-            else if (g.cls == SMALL || g.cls == MEDIUM) amax = fmaxf(amax, am);
+            else if (g.cls != CULLED) amax = fmaxf(amax, am);
             rb = make_float4(a.x, a.y, a.z, 0.0f);
             const BinBox b = bin_box(g, fp);
             if (b.n > 0) {
@@ -558,7 +558,7 @@ k_scatter(const float *__restrict__ x, const float *__restrict__ y, const float 
             }
         }
     }
-    // largest SMALL / MEDIUM record amplitude of the frame: fixes the fixed-point scale of k_splat
+    // largest record amplitude of the frame: fixes the fixed-point scale of k_splat and k_large
     amax = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(amax)));   // amax >= 0: bit order = value order
     if ((threadIdx.x & 31) == 0) s_amax[threadIdx.x >> 5] = amax;
     __syncthreads();
@@ -624,115 +624,27 @@ template <int T> struct SplatCfg {
 
 // k_splat itself lives in splotch_splat.cuh.
 
-// ---- A6 + A8: compose one tile ----------------------------------------------------------------------------------
-// Thread t owns pixels t, t+256, ... of the tile (registers).  Reads the tile's fixed-point sums, then gathers the
-// LARGE records of the tile's super-tile (each record's box is tested against the tile, survivors are staged in
-// shared memory and evaluated by every pixel owner), in two-level float32 accumulation.
+// ---- A8: epilogue -------------------------------------------------------------------------------------------------
+// One CTA per tile: the tile's 64-bit fixed-point sums (fed by k_splat and k_large) become the float32 image, S or
+// 1 - exp(-S) (the exact E = A solution); every pixel is written exactly once (:216-219, :238).
 template <int T>
 __global__ void __launch_bounds__(256)
-k_compose(const unsigned long long *__restrict__ accum, const float4 *__restrict__ records,
-          const unsigned int *__restrict__ bin_start, const DeviceStats *__restrict__ stats,
+k_compose(const unsigned long long *__restrict__ accum, const DeviceStats *__restrict__ stats,
           const __grid_constant__ FrameParams fp, float *__restrict__ image)
 {
     constexpr int kPix = T * T;
-    constexpr int kPpt = (kPix + 255) / 256;
-    __shared__ float4 sA[256], sB[256];
-    __shared__ int s_woff[8], s_cnt;
     const int tile = blockIdx.x;
-    const int tx = tile % fp.ntx, ty = tile / fp.ntx;
-    const int tx0 = tx * T, ty0 = ty * T;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    long long fix[kPpt][3];
-    float acc[kPpt][3], sub[kPpt][3], fxc[kPpt], fyc[kPpt];
-#pragma unroll
-    for (int k = 0; k < kPpt; ++k) {
-        const int p = threadIdx.x + k * 256;
-        fix[k][0] = fix[k][1] = fix[k][2] = 0ll;
-        acc[k][0] = acc[k][1] = acc[k][2] = 0.0f;
-        sub[k][0] = sub[k][1] = sub[k][2] = 0.0f;
-        fxc[k] = __fadd_rn((float)(tx0 + p % T), 0.5f);
-        fyc[k] = __fadd_rn((float)(ty0 + p / T), 0.5f);
-    }
+    const int tx0 = (tile % fp.ntx) * T, ty0 = (tile / fp.ntx) * T;
     const bool ok = stats->overflow == 0u;
-    if (ok) {
-#pragma unroll
-        for (int k = 0; k < kPpt; ++k) {
-            const int p = threadIdx.x + k * 256;
-            if (p < kPix) {
-                const unsigned long long *q = accum + (size_t)tile * (3 * kPix) + p;
-#pragma unroll
-                for (int c = 0; c < 3; ++c) fix[k][c] = (long long)__ldg(q + c * kPix);
-            }
-        }
-        const int sbin = fp.n_tiles + (ty >> kSuperShift) * fp.nsx + (tx >> kSuperShift);
-        const unsigned int lb = bin_start[sbin], le = bin_start[sbin + 1];
-        // the tile inside its super-tile, in pixels
-        const int qx0 = (tx & ((1 << kSuperShift) - 1)) * T, qy0 = (ty & ((1 << kSuperShift) - 1)) * T;
-        const int qx1 = qx0 + T - 1, qy1 = qy0 + T - 1;
-        int batch = 0;
-        for (unsigned int base = lb; base < le; base += 256, ++batch) {
-            const unsigned int idx = base + threadIdx.x;
-            bool hit = false;
-            float4 ra, rb;
-            if (idx < le) {
-                ld_record(records, idx, ra, rb);
-                const unsigned int box = __float_as_uint(rb.w);
-                const int bx0 = (int)(box & 255u), by0 = (int)((box >> 8) & 255u);
-                const int bx1 = (int)((box >> 16) & 255u), by1 = (int)(box >> 24);
-                hit = bx0 <= qx1 && bx1 >= qx0 && by0 <= qy1 && by1 >= qy0;
-            }
-            const unsigned int bal = __ballot_sync(0xffffffffu, hit);
-            if (lane == 0) s_woff[warp] = __popc(bal);
-            __syncthreads();
-            if (threadIdx.x == 0) {
-                int run = 0;
-                for (int w = 0; w < 8; ++w) { const int c = s_woff[w]; s_woff[w] = run; run += c; }
-                s_cnt = run;
-            }
-            __syncthreads();
-            if (hit) {
-                const int pos = s_woff[warp] + __popc(bal & ((1u << lane) - 1u));
-                sA[pos] = ra; sB[pos] = rb;
-            }
-            __syncthreads();
-            const int cnt = s_cnt;
-            for (int m = 0; m < cnt; ++m) {
-                const float4 a = sA[m], b = sB[m];
-#pragma unroll
-                for (int k = 0; k < kPpt; ++k) {
-                    const float dxf = __fsub_rn(fxc[k], a.x), dyf = __fsub_rn(fyc[k], a.y);
-                    const float d2 = __fmaf_rn(dxf, dxf, __fmul_rn(dyf, dyf));
-                    if (d2 <= a.w) {
-                        const float wgt = ex2_approx(d2 * a.z);
-                        sub[k][0] = fmaf(b.x, wgt, sub[k][0]);
-                        sub[k][1] = fmaf(b.y, wgt, sub[k][1]);
-                        sub[k][2] = fmaf(b.z, wgt, sub[k][2]);
-                    }
-                }
-            }
-            if ((batch & 3) == 3) {
-#pragma unroll
-                for (int k = 0; k < kPpt; ++k)
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) { acc[k][c] += sub[k][c]; sub[k][c] = 0.0f; }
-            }
-            __syncthreads();
-        }
-#pragma unroll
-        for (int k = 0; k < kPpt; ++k)
-#pragma unroll
-            for (int c = 0; c < 3; ++c) acc[k][c] += sub[k][c];
-    }
     const double unit = ldexp(1.0, -fixed_exponent(stats->amax_bits));       // one fixed-point unit
-#pragma unroll
-    for (int k = 0; k < kPpt; ++k) {
-        const int p = threadIdx.x + k * 256;
+    for (int p = threadIdx.x; p < kPix; p += 256) {
         const int ix = tx0 + p % T, iy = ty0 + p / T;
-        if (p < kPix && ix < fp.W && iy < fp.H) {
+        if (ix < fp.W && iy < fp.H) {
+            const unsigned long long *q = accum + (size_t)tile * (3 * kPix) + p;
             float *o = image + 3ull * ((size_t)iy * fp.W + ix);
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
-                const float v = (float)((double)fix[k][c] * unit + (double)acc[k][c]);
+                const float v = ok ? (float)((double)(long long)__ldg(q + c * kPix) * unit) : 0.0f;
                 o[c] = fp.apply_transfer ? -expm1f(-v) : v;
             }
         }

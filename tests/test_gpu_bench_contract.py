@@ -41,8 +41,8 @@ def test_default_line_is_config_1_additive():
     d = run_bench()
     check_common(d)
     assert d["config"]["workload"] == "cfg1_halos_10M" and d["config"]["mode"] == "additive"
-    assert d["gpu_launches"] == 5 * d["steps"]
-    assert set(d["stages"]) == {"count", "scan", "scatter", "splat", "compose"}
+    assert d["gpu_launches"] == 6 * d["steps"]
+    assert set(d["stages"]) == {"count", "scan", "scatter", "splat", "large", "compose"}
 
 
 def test_ordered_mode_line_on_the_small_config():
