@@ -39,7 +39,7 @@ k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
     __shared__ int s_woff[kLargeThreads / 32];
     __shared__ unsigned int s_item;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (stats->overflow) return;
+    if (stats->overflow || stats->large_pairs == 0ull) return;          // no LARGE particle in this frame
     // ---- item table: items of super-tile s = ceil(records / kLargeChunk) * 64, exclusive prefix over s
     const int n_super = fp.n_super;
     {
