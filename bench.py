@@ -1,9 +1,9 @@
 #!/usr/bin/env python
 """bench.py -- particles/s of the Splotch per-frame rendering path on B200 (BASELINE.json metric).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--impl ours|reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0..4] [--mode additive|ordered] [--impl ours|reference]
 
-A step is one whole frame (count -> scan -> scatter -> splat -> compose) of BASELINE configs[1]
+A step is one whole frame (count -> scan -> scatter -> splat -> large -> compose) of BASELINE configs[1]
 (10M particles, 50 Plummer halos + 20 % background, 800 x 800, additive mode) with the particles
 already resident in HBM.  One JSON line is printed by rank 0.  `e2e` is the same frame through
 splotch_render_host: pinned HOST particle arrays in, HOST image out, copies inside the timed region.
