@@ -134,6 +134,16 @@ def test_cfg3_reduced_large_particles(tile, r_large):
     assert st["large_pairs"] >= st["count"][wl_LARGE]
 
 
+def test_large_particles_with_8px_tiles_and_a_disc_covering_the_image():
+    """k_large with one pixel per thread (T = 8) and a particle whose disc contains every tile of the image."""
+    w = wl.make_config(3, n=40_000, size=(200, 136))
+    w.r_large = 6.0
+    w.fields["h"][:3] = 5.0                                      # three discs far larger than the image
+    w.fields["x"][:3] = 0.5; w.fields["y"][:3] = 0.5; w.fields["z"][:3] = 0.5
+    st, g = full_check(w, 8)
+    assert st["count"][wl_LARGE] > 1000
+
+
 def test_apply_transfer():
     w = wl.make_config(0, n=30_000)
     w.apply_transfer = True
