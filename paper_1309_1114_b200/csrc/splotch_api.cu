@@ -327,14 +327,14 @@ int render_device(splotch_ctx *c, const splotch_particles *p, unsigned long long
 }
 
 template <int T>
-void launch_ordered_tail(splotch_ctx *c, const Layout &L, char *ws, const FrameParams &fp, const unsigned long long *keys,
-                         const unsigned int *vals, float *image, cudaStream_t st)
+void launch_ordered_tail(splotch_ctx *c, const Layout &L, char *ws, const FrameParams &fp, const unsigned int *vals0,
+                         const unsigned int *vals1, float *image, cudaStream_t st)
 {
     const int ti = T == 8 ? 0 : T == 16 ? 1 : 2;
     DeviceStats *stats = (DeviceStats *)(ws + L.stats);
     const unsigned int *tile_start = (const unsigned int *)(ws + L.tile_start);
     k_orender<T><<<c->n_sm * c->orender_blocks_per_sm[ti], SplatCfg<T>::kThreads, 0, st>>>(
-        (const float4 *)(ws + L.rec), keys, vals, tile_start, stats, (float4 *)(ws + L.seg), fp);
+        (const float4 *)(ws + L.rec), vals0, vals1, tile_start, stats, (float4 *)(ws + L.seg), fp);
     if (c->profiling) cudaEventRecord(c->ev[6], st);
     k_ocombine<T><<<fp.n_tiles, 256, 0, st>>>((const float4 *)(ws + L.seg), tile_start, stats, fp, image);
     if (c->profiling) cudaEventRecord(c->ev[7], st);
@@ -360,7 +360,7 @@ int render_ordered(splotch_ctx *c, const splotch_particles *p, unsigned long lon
         else    k_ocount<false><<<L.nblk_o, kOThreads, 0, st>>>(p->x, p->y, p->z, p->h, n, fp, blk, stats);
     }
     if (c->profiling) cudaEventRecord(c->ev[1], st);
-    k_oscan<<<1, kOScanThreads, 0, st>>>(blk, L.nblk_o, n, L.capacity, c->n_sm, stats);
+    k_oscan<<<1, kOScanThreads, 0, st>>>(blk, L.nblk_o, n, L.capacity, c->n_sm, fp.n_tiles, stats);
     if (c->profiling) cudaEventRecord(c->ev[2], st);
     if (L.nblk_o > 0) {
         const size_t lsm = sizeof(float4) * kLutSmemMax;
@@ -370,16 +370,17 @@ int render_ordered(splotch_ctx *c, const splotch_particles *p, unsigned long lon
                                                                   (float4 *)(ws + L.rec), keys[0], vals[0]);
     }
     if (c->profiling) cudaEventRecord(c->ev[3], st);
-    // radix passes: 4 bytes of depth, then the bytes of the tile index
+    // radix passes: as many as the widest possible key needs (32 depth bits + the tile bits); the passes beyond the
+    // bits this frame's keys really use return at once (the key layout is decided on the device, by k_oscan)
     int tile_bytes = 1;
     while (tile_bytes < 4 && (fp.n_tiles - 1) >> (8 * tile_bytes)) ++tile_bytes;
     int cur = 0;
     for (int pass = 0; pass < 4 + tile_bytes; ++pass) {
         const int shift = 8 * pass;
         k_rs_count<<<L.nblk_rs, kRsThreads, 0, st>>>(keys[cur], stats, shift, L.nblk_rs, hist);
-        k_sc_reduce<<<L.n_sums, kScThreads, 0, st>>>(hist, L.m_hist, sums);
-        k_sc_top<<<1, 1024, 0, st>>>(sums, L.n_sums);
-        k_sc_apply<<<L.n_sums, kScThreads, 0, st>>>(hist, L.m_hist, sums);
+        k_sc_reduce<<<L.n_sums, kScThreads, 0, st>>>(hist, L.m_hist, sums, stats, shift);
+        k_sc_top<<<1, 1024, 0, st>>>(sums, L.n_sums, stats, shift);
+        k_sc_apply<<<L.n_sums, kScThreads, 0, st>>>(hist, L.m_hist, sums, stats, shift);
         k_rs_scatter<<<L.nblk_rs, kRsThreads, sizeof(RsSmem), st>>>(keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], stats, shift,
                                                                      L.nblk_rs, hist);
         cur ^= 1;
@@ -387,12 +388,12 @@ int render_ordered(splotch_ctx *c, const splotch_particles *p, unsigned long lon
     if (c->profiling) cudaEventRecord(c->ev[4], st);
     {
         const unsigned long long work = L.capacity > (unsigned long long)fp.n_tiles + 1 ? L.capacity : (unsigned long long)fp.n_tiles + 1;
-        k_obounds<<<(unsigned int)((work + 255) / 256), 256, 0, st>>>(keys[cur], stats, fp.n_tiles, (unsigned int *)(ws + L.tile_start));
+        k_obounds<<<(unsigned int)((work + 255) / 256), 256, 0, st>>>(keys[0], keys[1], stats, fp.n_tiles, (unsigned int *)(ws + L.tile_start));
     }
     if (c->profiling) cudaEventRecord(c->ev[5], st);
-    if (fp.T == 8) launch_ordered_tail<8>(c, L, ws, fp, keys[cur], vals[cur], image, st);
-    else if (fp.T == 16) launch_ordered_tail<16>(c, L, ws, fp, keys[cur], vals[cur], image, st);
-    else launch_ordered_tail<32>(c, L, ws, fp, keys[cur], vals[cur], image, st);
+    if (fp.T == 8) launch_ordered_tail<8>(c, L, ws, fp, vals[0], vals[1], image, st);
+    else if (fp.T == 16) launch_ordered_tail<16>(c, L, ws, fp, vals[0], vals[1], image, st);
+    else launch_ordered_tail<32>(c, L, ws, fp, vals[0], vals[1], image, st);
     CU_TRY(c, cudaGetLastError());
     c->have_frame = true; c->ws = ws; c->lay = L; c->fp = fp; c->last_n = n; c->last_stream = st; c->last_additive = false;
     if (c->profiling) { ++c->prof_frames; c->prof_stages = kStagesOrdered; }

@@ -66,6 +66,8 @@ struct DeviceStats {             // cleared before every frame; written by k_sca
     unsigned long long count[4];
     unsigned long long pairs, large_pairs, chunks, capacity;
     unsigned long long sort_n;   // ordered mode: pairs the sort and the renderer work on (0 on overflow)
+    // ordered mode, sort key = tile << zbits | (~bits(z_c) - zkey_min): only the bits that differ in this frame are sorted
+    unsigned int zkey_max, nzkey_max, zkey_min, zbits, key_bits, pad2;     // nzkey_max = max of ~zkey (its complement is the min)
     unsigned int overflow, work_counter, chunk_size, amax_bits, scan_done, large_counter;   // large_counter: work items of k_large
 };
 

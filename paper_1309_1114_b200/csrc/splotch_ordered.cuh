@@ -44,8 +44,9 @@ k_ocount(const float *__restrict__ x, const float *__restrict__ y, const float *
          unsigned long long n, const __grid_constant__ FrameParams fp, unsigned int *__restrict__ blk_pairs,
          DeviceStats *__restrict__ stats)
 {
-    __shared__ unsigned int s_sum[4];
+    __shared__ unsigned int s_sum[4], s_z[2];
     if (threadIdx.x < 4) s_sum[threadIdx.x] = 0u;
+    if (threadIdx.x < 2) s_z[threadIdx.x] = 0u;
     __syncthreads();
     const unsigned long long lo = (unsigned long long)blockIdx.x * kOBlockParticles;
     const unsigned int len = (unsigned int)min(n - lo, (unsigned long long)kOBlockParticles);
@@ -56,16 +57,19 @@ k_ocount(const float *__restrict__ x, const float *__restrict__ y, const float *
     load4<ALIGNED>(y, i, len, ys);
     load4<ALIGNED>(z, i, len, zs);
     load4<ALIGNED>(h, i, len, hs);
-    unsigned int pairs = 0u, c1 = 0u, c2 = 0u, c3 = 0u;
+    unsigned int pairs = 0u, c1 = 0u, c2 = 0u, c3 = 0u, zmax = 0u, nzmax = 0u;
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
         Geo g = geometry(xs[j], ys[j], zs[j], hs[j], fp);
         if (!(i + j < len)) g.cls = CULLED;
+        if (g.cls != CULLED) { const unsigned int zk = ~__float_as_uint(g.zc); zmax = max(zmax, zk); nzmax = max(nzmax, ~zk); }
         pairs += (unsigned int)tile_pairs(g, fp);
         c1 += g.cls == SMALL; c2 += g.cls == MEDIUM; c3 += g.cls == LARGE;
     }
     pairs = warp_sum(pairs);
     const unsigned int cc = warp_sum(c1 | (c2 << 10) | (c3 << 20));        // at most 128 per field and warp
+    zmax = __reduce_max_sync(0xffffffffu, zmax); nzmax = __reduce_max_sync(0xffffffffu, nzmax);
+    if ((threadIdx.x & 31) == 0 && zmax) { atomicMax(&s_z[0], zmax); atomicMax(&s_z[1], nzmax); }
     if ((threadIdx.x & 31) == 0) {
         atomicAdd(&s_sum[0], pairs);
         atomicAdd(&s_sum[1], cc & 1023u); atomicAdd(&s_sum[2], (cc >> 10) & 1023u); atomicAdd(&s_sum[3], cc >> 20);
@@ -73,6 +77,7 @@ k_ocount(const float *__restrict__ x, const float *__restrict__ y, const float *
     __syncthreads();
     if (threadIdx.x == 0) blk_pairs[blockIdx.x] = s_sum[0];
     if (threadIdx.x >= 1 && threadIdx.x < 4 && s_sum[threadIdx.x]) atomicAdd(&stats->count[threadIdx.x], (unsigned long long)s_sum[threadIdx.x]);
+    if (threadIdx.x == 4 && s_z[0]) { atomicMax(&stats->zkey_max, s_z[0]); atomicMax(&stats->nzkey_max, s_z[1]); }
 }
 
 // ---- exclusive scan of the block totals (one block) ---------------------------------------------------------------
@@ -80,7 +85,7 @@ constexpr int kOScanThreads = 1024;
 
 __global__ void __launch_bounds__(kOScanThreads)
 k_oscan(unsigned int *__restrict__ blk_pairs, int nblk, unsigned long long n, unsigned long long capacity, int n_sm,
-        DeviceStats *__restrict__ stats)
+        int n_tiles, DeviceStats *__restrict__ stats)
 {
     __shared__ unsigned long long s_warp[kOScanThreads / 32];
     __shared__ unsigned long long s_total;
@@ -120,6 +125,11 @@ k_oscan(unsigned int *__restrict__ blk_pairs, int nblk, unsigned long long n, un
         stats->work_counter = 0u;
         stats->chunk_size = (unsigned int)cs;
         stats->count[0] = n - stats->count[1] - stats->count[2] - stats->count[3];
+        // key layout of this frame: depth keys relative to the smallest one, only as many bits as their range needs
+        const unsigned int zmin = ~stats->nzkey_max, zrange = stats->zkey_max >= zmin ? stats->zkey_max - zmin : 0u;
+        const unsigned int zbits = zrange ? 32u - (unsigned int)__clz(zrange) : 0u;
+        const unsigned int tbits = n_tiles > 1 ? 32u - (unsigned int)__clz((unsigned int)n_tiles - 1u) : 0u;
+        stats->zkey_min = zmin; stats->zbits = zbits; stats->key_bits = zbits + tbits;
     }
 }
 
@@ -141,6 +151,7 @@ k_opairs(const float *__restrict__ x, const float *__restrict__ y, const float *
     float4 *s_lut = reinterpret_cast<float4 *>(smem_raw);
     __shared__ unsigned int s_w[kOThreads / 32];
     if (stats->overflow) return;
+    const unsigned int zkey_min = stats->zkey_min, zbits = stats->zbits;
     if (fp.lut_total > 0) {
         for (int s = 0; s < fp.n_species; ++s)
             if (fp.sp[s].use_colormap)
@@ -212,12 +223,12 @@ k_opairs(const float *__restrict__ x, const float *__restrict__ y, const float *
         const float am = fmaxf(fmaxf(fabsf(rb.x), fabsf(rb.y)), fmaxf(fabsf(rb.z), fabsf(rb.w)));
         if (!(am <= 3.0e38f)) rb = make_float4(0.0f, 0.0f, 0.0f, 0.0f);   // Inf / NaN: a record without effect
         st_record(rec, idx, ra, rb);
-        const unsigned long long zkey = (unsigned long long)(~__float_as_uint(g[j].zc));
+        const unsigned long long zkey = (unsigned long long)(~__float_as_uint(g[j].zc) - zkey_min);
         const int tx0 = g[j].x0 >> fp.tshift, tx1 = g[j].x1 >> fp.tshift;
         const int ty0 = g[j].y0 >> fp.tshift, ty1 = g[j].y1 >> fp.tshift;
         for (int ty = ty0; ty <= ty1; ++ty)
             for (int tx = tx0; tx <= tx1; ++tx) {
-                keys[pos] = ((unsigned long long)(unsigned int)(ty * fp.ntx + tx) << 32) | zkey;
+                keys[pos] = ((unsigned long long)(unsigned int)(ty * fp.ntx + tx) << zbits) | zkey;
                 vals[pos] = idx;
                 ++pos;
             }
@@ -233,6 +244,7 @@ k_rs_count(const unsigned long long *__restrict__ keys, const DeviceStats *__res
            unsigned int *__restrict__ hist)
 {
     __shared__ unsigned int s_h[256];
+    if ((unsigned int)shift >= stats->key_bits) return;          // this frame's keys have no bit left for this pass
     if (threadIdx.x < 256) s_h[threadIdx.x] = 0u;
     __syncthreads();
     const unsigned long long P = stats->sort_n;
@@ -284,9 +296,11 @@ __device__ __forceinline__ unsigned int block_excl_scan_u32(unsigned int v, unsi
 }
 
 __global__ void __launch_bounds__(kScThreads)
-k_sc_reduce(const unsigned int *__restrict__ a, unsigned int m, unsigned int *__restrict__ sums)
+k_sc_reduce(const unsigned int *__restrict__ a, unsigned int m, unsigned int *__restrict__ sums,
+            const DeviceStats *__restrict__ stats, int shift)
 {
     __shared__ unsigned int s_warp[32], s_total;
+    if ((unsigned int)shift >= stats->key_bits) return;
     const unsigned int base = blockIdx.x * kScTile + threadIdx.x * kScItems;
     unsigned int s = 0u;
     if (base + kScItems <= m) {
@@ -300,9 +314,10 @@ k_sc_reduce(const unsigned int *__restrict__ a, unsigned int m, unsigned int *__
 }
 
 __global__ void __launch_bounds__(1024)
-k_sc_top(unsigned int *__restrict__ sums, int ng)
+k_sc_top(unsigned int *__restrict__ sums, int ng, const DeviceStats *__restrict__ stats, int shift)
 {
     __shared__ unsigned int s_warp[32], s_total;
+    if ((unsigned int)shift >= stats->key_bits) return;
     const int per = (ng + 1023) / 1024;
     const int b0 = min(ng, (int)threadIdx.x * per), b1 = min(ng, b0 + per);
     unsigned int s = 0u;
@@ -312,9 +327,11 @@ k_sc_top(unsigned int *__restrict__ sums, int ng)
 }
 
 __global__ void __launch_bounds__(kScThreads)
-k_sc_apply(unsigned int *__restrict__ a, unsigned int m, const unsigned int *__restrict__ sums)
+k_sc_apply(unsigned int *__restrict__ a, unsigned int m, const unsigned int *__restrict__ sums,
+           const DeviceStats *__restrict__ stats, int shift)
 {
     __shared__ unsigned int s_warp[32], s_total;
+    if ((unsigned int)shift >= stats->key_bits) return;
     const unsigned int base = blockIdx.x * kScTile + threadIdx.x * kScItems;
     unsigned int v[kScItems];
     unsigned int s = 0u;
@@ -351,7 +368,7 @@ k_rs_scatter(const unsigned long long *__restrict__ keys_in, const unsigned int 
     RsSmem &S = *reinterpret_cast<RsSmem *>(smem_raw);
     const unsigned long long P = stats->sort_n;
     const unsigned long long seg = (unsigned long long)blockIdx.x * kRsTile;
-    if (seg >= P) return;
+    if (seg >= P || (unsigned int)shift >= stats->key_bits) return;
     const unsigned int cnt = (unsigned int)min(P - seg, (unsigned long long)kRsTile);
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     for (int i = threadIdx.x; i < kRsWarps * 257; i += kRsThreads) (&S.wcount[0][0])[i] = 0u;
@@ -409,8 +426,8 @@ k_rs_scatter(const unsigned long long *__restrict__ keys_in, const unsigned int 
 
 // ---- tile start offsets from the sorted keys ----------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-k_obounds(const unsigned long long *__restrict__ keys, const DeviceStats *__restrict__ stats, int n_tiles,
-          unsigned int *__restrict__ tile_start)
+k_obounds(const unsigned long long *__restrict__ keys0, const unsigned long long *__restrict__ keys1,
+          const DeviceStats *__restrict__ stats, int n_tiles, unsigned int *__restrict__ tile_start)
 {
     const unsigned long long P = stats->sort_n;
     const unsigned long long p = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -419,8 +436,11 @@ k_obounds(const unsigned long long *__restrict__ keys, const DeviceStats *__rest
         return;
     }
     if (p >= P) return;
-    const int t = (int)(keys[p] >> 32);
-    const int tp = p > 0 ? (int)(keys[p - 1] >> 32) : -1;
+    // the sorted pairs are in buffer (number of passes that ran) & 1
+    const unsigned long long *keys = (((stats->key_bits + 7u) >> 3) & 1u) ? keys1 : keys0;
+    const unsigned int zbits = stats->zbits;
+    const int t = (int)(keys[p] >> zbits);
+    const int tp = p > 0 ? (int)(keys[p - 1] >> zbits) : -1;
     for (int u = tp + 1; u <= t; ++u) tile_start[u] = (unsigned int)p;
     if (p == P - 1) for (int u = t + 1; u <= n_tiles; ++u) tile_start[u] = (unsigned int)P;
 }
@@ -456,7 +476,7 @@ __device__ __forceinline__ int floor_clamped(float v) { return __float2int_rd(fm
 
 template <int T>
 __global__ void __launch_bounds__(SplatCfg<T>::kThreads)
-k_orender(const float4 *__restrict__ rec, const unsigned long long *__restrict__ keys, const unsigned int *__restrict__ vals,
+k_orender(const float4 *__restrict__ rec, const unsigned int *__restrict__ vals0, const unsigned int *__restrict__ vals1,
           const unsigned int *__restrict__ tile_start, DeviceStats *__restrict__ stats, float4 *__restrict__ seg,
           const __grid_constant__ FrameParams fp)
 {
@@ -466,7 +486,7 @@ k_orender(const float4 *__restrict__ rec, const unsigned long long *__restrict__
     __shared__ unsigned int stM[2][kThreads];
     __shared__ unsigned int s_chunk;
     __shared__ int s_tile;
-    (void)keys;
+    const unsigned int *__restrict__ vals = (((stats->key_bits + 7u) >> 3) & 1u) ? vals1 : vals0;   // the sorted values
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int sx = warp % Cfg::kStripsX, sy = warp / Cfg::kStripsX;
     const int lx = sx * Cfg::kSW + 2 * (lane % (Cfg::kSW / 2)), ly = sy * Cfg::kSH + lane / (Cfg::kSW / 2);
