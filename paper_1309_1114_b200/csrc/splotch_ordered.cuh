@@ -252,12 +252,26 @@ k_rs_count(const unsigned long long *__restrict__ keys, const DeviceStats *__res
     if (seg < P) {
         const unsigned int cnt = (unsigned int)min(P - seg, (unsigned long long)kRsTile);
         const int lane = threadIdx.x & 31;
+        // depth digits are spread over the 256 counters: plain shared-memory atomics.  Tile digits are nearly the same
+        // for a whole block (the pairs are in index order, neighbours share tiles): aggregate equal digits in the warp
+        const bool spread = (unsigned int)shift + 8u <= stats->zbits;
+        unsigned long long k[kRsItems];
 #pragma unroll
         for (int i = 0; i < kRsItems; ++i) {
             const unsigned int p = i * kRsThreads + threadIdx.x;
-            const unsigned int d = p < cnt ? rs_digit(__ldg(keys + seg + p), shift) : 256u;
-            const unsigned int peers = __match_any_sync(0xffffffffu, d);
-            if (d < 256u && lane == __ffs(peers) - 1) atomicAdd(&s_h[d], (unsigned int)__popc(peers));
+            k[i] = p < cnt ? __ldg(keys + seg + p) : 0ull;
+        }
+        if (spread) {
+#pragma unroll
+            for (int i = 0; i < kRsItems; ++i)
+                if (i * kRsThreads + threadIdx.x < cnt) atomicAdd(&s_h[rs_digit(k[i], shift)], 1u);
+        } else {
+#pragma unroll
+            for (int i = 0; i < kRsItems; ++i) {
+                const unsigned int d = i * kRsThreads + threadIdx.x < cnt ? rs_digit(k[i], shift) : 256u;
+                const unsigned int peers = __match_any_sync(0xffffffffu, d);
+                if (d < 256u && lane == __ffs(peers) - 1) atomicAdd(&s_h[d], (unsigned int)__popc(peers));
+            }
         }
     }
     __syncthreads();
