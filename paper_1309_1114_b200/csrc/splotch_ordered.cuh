@@ -396,16 +396,20 @@ k_rs_scatter(const unsigned long long *__restrict__ keys_in, const unsigned int 
         val[i] = p < cnt ? __ldg(vals_in + seg + p) : 0u;
     }
     __syncthreads();
+    // the eight matches first (independent, their latency overlaps), then the counter rounds, which depend on each other
+    unsigned int dig[kRsItems], peers[kRsItems];
 #pragma unroll
     for (int i = 0; i < kRsItems; ++i) {
-        const unsigned int p = wbase + i * 32;
-        const unsigned int d = p < cnt ? rs_digit(key[i], shift) : 256u;
-        const unsigned int peers = __match_any_sync(0xffffffffu, d);
-        const int leader = __ffs(peers) - 1;
+        dig[i] = wbase + i * 32 < cnt ? rs_digit(key[i], shift) : 256u;
+        peers[i] = __match_any_sync(0xffffffffu, dig[i]);
+    }
+#pragma unroll
+    for (int i = 0; i < kRsItems; ++i) {
+        const int leader = __ffs(peers[i]) - 1;
         unsigned int old = 0u;
-        if (lane == leader) { old = S.wcount[w][d]; S.wcount[w][d] = old + (unsigned int)__popc(peers); }
+        if (lane == leader) { old = S.wcount[w][dig[i]]; S.wcount[w][dig[i]] = old + (unsigned int)__popc(peers[i]); }
         old = __shfl_sync(0xffffffffu, old, leader);
-        rank[i] = old + (unsigned int)__popc(peers & ((1u << lane) - 1u));
+        rank[i] = old + (unsigned int)__popc(peers[i] & ((1u << lane) - 1u));
         __syncwarp();
     }
     __syncthreads();
