@@ -204,6 +204,12 @@ __device__ __forceinline__ void load4(const float *__restrict__ a, unsigned int 
     }
 }
 
+// shared-memory reduction without a return value and with a register operand: one instruction, no branch around it
+__device__ __forceinline__ void red_add_shared(unsigned int *p, unsigned int v)
+{
+    asm volatile("red.shared.add.u32 [%0], %1;" :: "r"((unsigned int)__cvta_generic_to_shared(p)), "r"(v) : "memory");
+}
+
 __device__ __forceinline__ unsigned int warp_sum(unsigned int v)
 {
     return __reduce_add_sync(0xffffffffu, v);
@@ -240,17 +246,17 @@ k_count(const float *__restrict__ x, const float *__restrict__ y, const float *_
         for (int j = 0; j < 4; ++j) {
             Geo g = geometry(xs[j], ys[j], zs[j], hs[j], fp);
             if (!(i + j < len)) { g.cls = CULLED; g.x1 = -1; g.y1 = -1; g.x0 = 0; g.y0 = 0; }
-            c1 += __popc(__ballot_sync(0xffffffffu, g.cls == SMALL));
-            c2 += __popc(__ballot_sync(0xffffffffu, g.cls == MEDIUM));
-            c3 += __popc(__ballot_sync(0xffffffffu, g.cls == LARGE));
+            c1 += g.cls == SMALL; c2 += g.cls == MEDIUM; c3 += g.cls == LARGE;        // per thread, summed at the end
             const BinBox b = bin_box(g, fp);
-            // a box covers at most 2 x 2 bins unless it is wider than a tile: four predicated atomics, no loop
+            // a box covers at most 2 x 2 bins unless it is wider than a tile: four unconditional reductions with a 0 / 1
+            // operand (no branches; a CULLED particle adds 0 to bin 0, the +1 / +pitch neighbours of the last bin fall into
+            // the unused colour-table area behind the histogram)
             const bool any = b.n > 0, w2 = b.bx1 > b.bx0, h2 = b.by1 > b.by0;
             unsigned int *h00 = hist + (b.base + b.by0 * b.pitch + b.bx0);
-            if (any) atomicAdd(h00, 1u);
-            if (any && w2) atomicAdd(h00 + 1, 1u);
-            if (any && h2) atomicAdd(h00 + b.pitch, 1u);
-            if (any && w2 && h2) atomicAdd(h00 + b.pitch + 1, 1u);
+            red_add_shared(h00, any ? 1u : 0u);
+            red_add_shared(h00 + 1, (any && w2) ? 1u : 0u);
+            red_add_shared(h00 + b.pitch, (any && h2) ? 1u : 0u);
+            red_add_shared(h00 + b.pitch + 1, (any && w2 && h2) ? 1u : 0u);
             const bool big = any && (b.bx1 - b.bx0 > 1 || b.by1 - b.by0 > 1);
             if (__any_sync(0xffffffffu, big)) {          // the bins beyond the first 2 x 2
                 const int nmax = __reduce_max_sync(0xffffffffu, big ? b.n : 0);
@@ -264,6 +270,7 @@ k_count(const float *__restrict__ x, const float *__restrict__ y, const float *_
             }
         }
     }
+    c1 = warp_sum(c1); c2 = warp_sum(c2); c3 = warp_sum(c3);
     if ((threadIdx.x & 31) == 0) { atomicAdd(&s_cls[1], c1); atomicAdd(&s_cls[2], c2); atomicAdd(&s_cls[3], c3); }
     __syncthreads();
     unsigned int *row = counts + (size_t)blockIdx.x * fp.nbins;
