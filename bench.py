@@ -242,7 +242,7 @@ def run_ours(args):
         r.set_camera(wl.orbit_camera((args.steps - 1) % 120))     # the camera of the frame the statistics belong to
     frags, frags_large = fragments_estimate(r, fields, w.species, kw)
     n_tiles = (-(-w.width // TILE)) * (-(-w.height // TILE))
-    passes = (ordered_kernels_per_frame(n_tiles) - 6) // 5
+    passes = -(-st["sort_key_bits"] // 8) if not additive else 0      # radix passes that really ran
     # algorithmic bytes per stage and frame
     if additive:
         bytes_by_stage = {

@@ -95,6 +95,9 @@ typedef struct {
     int32_t  n_stages;               /* number of valid entries in stage_ms (0 unless profiling is on)      */
     float    stage_ms[8];            /* additive: count, scan, scatter, splat, large, compose; ordered: count, scan,
                                         pairs, sort, bounds, render, combine (see splotch_stage_name)        */
+    int32_t  sort_key_bits;          /* ordered mode: bits of the (tile, depth) sort key this frame used;
+                                        ceil(bits / 8) radix passes ran.  0 in additive mode                 */
+    int32_t  reserved;
 } splotch_stats;
 
 /* Create a context for images of width x height on CUDA device `device`; at most max_particles per frame.

@@ -49,7 +49,8 @@ class SplotchParams(C.Structure):
 class SplotchStats(C.Structure):
     _fields_ = [("n", C.c_uint64), ("count", C.c_uint64 * 4), ("pairs", C.c_uint64), ("large_pairs", C.c_uint64),
                 ("chunks", C.c_uint64), ("pair_capacity", C.c_uint64), ("overflow", C.c_int32),
-                ("n_stages", C.c_int32), ("stage_ms", C.c_float * 8)]
+                ("n_stages", C.c_int32), ("stage_ms", C.c_float * 8), ("sort_key_bits", C.c_int32),
+                ("reserved", C.c_int32)]
 
 
 class SplotchError(RuntimeError):
@@ -240,6 +241,7 @@ class Renderer:
         _check(self.ctx, self.lib.splotch_get_stats(self.ctx, C.byref(st)))
         d = {"n": st.n, "count": list(st.count), "pairs": st.pairs, "large_pairs": st.large_pairs,
              "chunks": st.chunks, "pair_capacity": st.pair_capacity, "overflow": st.overflow,
+             "sort_key_bits": st.sort_key_bits,
              "stage_ms": {self.lib.splotch_stage_name(int(st.n_stages < 7), i).decode(): st.stage_ms[i]
                           for i in range(st.n_stages)}}
         return d

@@ -634,6 +634,7 @@ int splotch_get_stats(splotch_ctx *c, splotch_stats *out)
     for (int k = 0; k < 4; ++k) out->count[k] = ds.count[k];
     out->pairs = ds.pairs; out->large_pairs = ds.large_pairs; out->chunks = ds.chunks;
     out->pair_capacity = ds.capacity; out->overflow = (int32_t)ds.overflow;
+    out->sort_key_bits = c->last_additive ? 0 : (int32_t)ds.key_bits;
     if (c->profiling && c->prof_frames > 0) {
         // mean per frame over the frames recorded since profiling was enabled (at most the last kProfRing)
         const unsigned long long nf = c->prof_frames < kProfRing ? c->prof_frames : kProfRing;
