@@ -31,7 +31,7 @@ namespace splotch {
 constexpr int kMaxSpecies   = 8;
 constexpr int kMaxLut       = 1024;
 constexpr int kChunkMax     = 32768;  // records per work item of k_splat (upper bound; the frame picks its own)
-constexpr int kChunkMin     = 512;
+constexpr int kChunkMin     = 128;
 constexpr int kBinThreads   = 1024;   // k_count / k_scatter block size: one CTA per SM (fewer histogram rows and write streams than 2 x 512)
 constexpr int kSuperShift   = 3;      // super-tile = 8 x 8 tiles (LARGE particles are binned to super-tiles)
 constexpr int kLutSmemMax   = 1024;   // colour-table entries (all species together) staged in shared memory by k_scatter
@@ -392,9 +392,9 @@ k_scan(unsigned int *__restrict__ counts, int nrows, int nbins, int n_tiles, uns
     const unsigned long long off_all = block_excl_scan_256(sum_all, s_warp, &s_tot_all);
     (void)block_excl_scan_256(sum_tiles, s_warp, &s_tot_pairs);
     // chunk size of this frame: about 128 chunks per SM (work items are taken from an atomic counter; many small ones
-    // keep the tail short when their costs differ), between kChunkMin and kChunkMax, a multiple of 256
+    // keep the tail short when their costs differ), between kChunkMin and kChunkMax
     unsigned long long cs = (s_tot_pairs + (unsigned long long)n_sm * 128 - 1) / ((unsigned long long)n_sm * 128);
-    cs = (cs + 255) / 256 * 256;
+    cs = cs >= 512 ? (cs + 255) / 256 * 256 : (cs + 63) / 64 * 64;      // small frames: short chunks, they are latency bound
     cs = min((unsigned long long)kChunkMax, max((unsigned long long)kChunkMin, cs));
     const unsigned int K = (unsigned int)cs;
     const bool overflow = s_tot_all > capacity;
