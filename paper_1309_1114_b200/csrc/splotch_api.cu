@@ -165,9 +165,13 @@ void make_layout_ordered(const splotch_ctx *c, unsigned long long n, int T, unsi
     }
     for (int k = 0; k < 2; ++k) { L->keys[k] = off; off = align_up(off + 8ull * capacity, 256); }
     for (int k = 0; k < 2; ++k) { L->vals[k] = off; off = align_up(off + 4ull * capacity, 256); }
-    // one (t, c_R, c_G, c_B) per pixel and segment; segment slot = chunk + tile, chunks <= ceil(capacity / kOChunkMin)
+    // one (t, c_R, c_G, c_B) per pixel and segment; segment slot = chunk + tile; k_oscan cuts the pairs into at most
+    // 128 chunks per SM, or capacity / kChunkMax when that is more
     L->seg = off;
-    off = align_up(off + sizeof(float4) * (size_t)T * T * ((capacity + kOChunkMin - 1) / kOChunkMin + n_tiles + 1), 256);
+    {
+        const size_t by_sm = (size_t)c->n_sm * 128, by_cap = (size_t)(capacity / kChunkMax);
+        off = align_up(off + sizeof(float4) * (size_t)T * T * ((by_sm > by_cap ? by_sm : by_cap) + n_tiles + 2), 256);
+    }
     L->total = off;
 }
 
@@ -336,7 +340,7 @@ void launch_ordered_tail(splotch_ctx *c, const Layout &L, char *ws, const FrameP
     k_orender<T><<<c->n_sm * c->orender_blocks_per_sm[ti], SplatCfg<T>::kThreads, 0, st>>>(
         (const float4 *)(ws + L.rec), vals0, vals1, tile_start, stats, (float4 *)(ws + L.seg), fp);
     if (c->profiling) cudaEventRecord(c->ev[6], st);
-    k_ocombine<T><<<fp.n_tiles, 256, 0, st>>>((const float4 *)(ws + L.seg), tile_start, stats, fp, image);
+    k_ocombine<T><<<fp.n_tiles * (T * T / kCombinePix), kCombinePix * kCombineSlices, 0, st>>>((const float4 *)(ws + L.seg), tile_start, stats, fp, image);
     if (c->profiling) cudaEventRecord(c->ev[7], st);
 }
 

@@ -29,7 +29,7 @@ constexpr int kRsThreads = 512;                // radix sort: 8 elements per thr
 constexpr int kRsItems = 8;
 constexpr int kRsTile = kRsThreads * kRsItems; // 4096 elements per block and pass
 constexpr int kRsWarps = kRsThreads / 32;
-constexpr int kOChunkMin = 4096;               // records per work item of k_orender (lower bound)
+constexpr int kOChunkMin = 256;                // records per work item of k_orender (lower bound)
 
 __device__ __forceinline__ int tile_pairs(const Geo &g, const FrameParams &fp)
 {
@@ -114,7 +114,7 @@ k_oscan(unsigned int *__restrict__ blk_pairs, int nblk, unsigned long long n, un
     for (int b = b0; b < b1; ++b) { const unsigned int c = blk_pairs[b]; blk_pairs[b] = (unsigned int)run; run += c; }
     if (threadIdx.x == 0) {
         unsigned long long cs = (total + (unsigned long long)n_sm * 128 - 1) / ((unsigned long long)n_sm * 128);
-        cs = (cs + 255) / 256 * 256;
+        cs = (cs + 255) / 256 * 256;             // so that chunks <= 128 n_sm (or capacity / kChunkMax): bounds the segment slots
         cs = min((unsigned long long)kChunkMax, max((unsigned long long)kOChunkMin, cs));
         stats->pairs = total;
         stats->large_pairs = 0ull;
@@ -643,25 +643,54 @@ k_orender(const float4 *__restrict__ rec, const unsigned int *__restrict__ vals0
 }
 
 // ---- A7 + A8: fold the segments of a tile in order, write the image -------------------------------------------------
+// A CTA folds the segments of 64 pixels of one tile: four slices of the segment range are composed in parallel by 64
+// threads each (composition of the maps (t, c) is associative), the four partial maps are then applied in order.  A
+// halo-core tile has more than a thousand segments: one thread per pixel walking them alone was latency bound.
+constexpr int kCombinePix = 64, kCombineSlices = 4;
+
 template <int T>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(kCombinePix * kCombineSlices)
 k_ocombine(const float4 *__restrict__ seg, const unsigned int *__restrict__ tile_start, const DeviceStats *__restrict__ stats,
            const __grid_constant__ FrameParams fp, float *__restrict__ image)
 {
-    constexpr int kPix = T * T;
-    const int tile = blockIdx.x;
+    constexpr int kPix = T * T, kGroups = kPix / kCombinePix;
+    __shared__ double s_map[kCombineSlices][4][kCombinePix];
+    const int tile = blockIdx.x / kGroups;
+    const int p = (blockIdx.x % kGroups) * kCombinePix + (threadIdx.x % kCombinePix);
+    const int slice = threadIdx.x / kCombinePix;
     const int tx0 = (tile % fp.ntx) * T, ty0 = (tile / fp.ntx) * T;
     const unsigned int tb = tile_start[tile], te = tile_start[tile + 1];
     const unsigned int K = stats->chunk_size;
     const bool any = te > tb && stats->overflow == 0u;
     const unsigned int c0 = any ? tb / K : 1u, c1 = any ? (te - 1u) / K : 0u;
-    for (int p = threadIdx.x; p < kPix; p += 256) {
-        double I[3] = {0.0, 0.0, 0.0};
-        for (unsigned int c = c0; c <= c1 && any; ++c) {
-            const float4 m = __ldg(seg + ((size_t)c + (size_t)tile) * kPix + p);
-            I[0] = fma(I[0], (double)m.x, (double)m.y);
-            I[1] = fma(I[1], (double)m.x, (double)m.z);
-            I[2] = fma(I[2], (double)m.x, (double)m.w);
+    const unsigned int nseg = any ? c1 - c0 + 1u : 0u, per = (nseg + kCombineSlices - 1) / kCombineSlices;
+    const unsigned int s0 = c0 + slice * per, s1 = min(s0 + per, c1 + 1u);       // this slice's segments [s0, s1)
+    double t = 1.0, cr = 0.0, cg = 0.0, cb = 0.0;
+    for (unsigned int c = s0; c < s1 && any; c += 8) {          // eight maps in flight, composed in order
+        float4 m[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k)
+            m[k] = c + k < s1 ? __ldg(seg + ((size_t)(c + k) + (size_t)tile) * kPix + p) : make_float4(1.0f, 0.0f, 0.0f, 0.0f);
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const double mt = (double)m[k].x;
+            t *= mt;
+            cr = fma(cr, mt, (double)m[k].y);
+            cg = fma(cg, mt, (double)m[k].z);
+            cb = fma(cb, mt, (double)m[k].w);
+        }
+    }
+    const int q = threadIdx.x % kCombinePix;
+    s_map[slice][0][q] = t; s_map[slice][1][q] = cr; s_map[slice][2][q] = cg; s_map[slice][3][q] = cb;
+    __syncthreads();
+    if (slice == 0) {
+        double I[3] = {0.0, 0.0, 0.0};                          // background (reading R16)
+#pragma unroll
+        for (int s = 0; s < kCombineSlices; ++s) {
+            const double mt = s_map[s][0][q];
+            I[0] = fma(I[0], mt, s_map[s][1][q]);
+            I[1] = fma(I[1], mt, s_map[s][2][q]);
+            I[2] = fma(I[2], mt, s_map[s][3][q]);
         }
         const int ix = tx0 + p % T, iy = ty0 + p / T;
         if (ix < fp.W && iy < fp.H) {
