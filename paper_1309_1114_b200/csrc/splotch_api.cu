@@ -170,7 +170,10 @@ void make_layout_ordered(const splotch_ctx *c, unsigned long long n, int T, unsi
     L->seg = off;
     {
         const size_t by_sm = (size_t)c->n_sm * 128, by_cap = (size_t)(capacity / kChunkMax);
-        off = align_up(off + sizeof(float4) * (size_t)T * T * ((by_sm > by_cap ? by_sm : by_cap) + n_tiles + 2), 256);
+        const size_t by_min = (size_t)(capacity / kOChunkMin) + 1;             // no chunk is shorter than kOChunkMin
+        size_t chunks = by_sm > by_cap ? by_sm : by_cap;
+        if (chunks > by_min) chunks = by_min;
+        off = align_up(off + sizeof(float4) * (size_t)T * T * (chunks + n_tiles + 2), 256);
     }
     L->total = off;
 }
