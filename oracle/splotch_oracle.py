@@ -15,6 +15,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "splotch_oracle.c")
+_SRC_MT = os.path.join(_HERE, "splotch_oracle_mt.c")          # OpenMP drivers around the same functions
 _LIB = os.path.join(_HERE, "libsplotch_oracle.so")
 _lib = None
 
@@ -23,9 +24,9 @@ CULLED, SMALL, MEDIUM, LARGE = 0, 1, 2, 3
 
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (no fast-math, no contraction) if the .so is missing or stale."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fno-fast-math", "-std=c99", "-shared", "-fPIC",
-               "-o", _LIB + ".tmp", _SRC, "-lm"]
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_MT)):
+        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fno-fast-math", "-std=c99", "-fopenmp", "-shared", "-fPIC",
+               "-o", _LIB + ".tmp", _SRC, _SRC_MT, "-lm"]
         subprocess.run(cmd, check=True)
         os.replace(_LIB + ".tmp", _LIB)
     return _LIB
@@ -41,7 +42,21 @@ def lib():
         _lib = C.CDLL(build())
         _lib.orc_camera.restype = C.c_int
         _lib.orc_depth_order.restype = C.c_int64
+        _lib.orc_mt_threads.restype = C.c_int
     return _lib
+
+
+def host_cores() -> int:
+    """Cores this process may run on (the all-cores drivers use that many threads)."""
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
+def _threads(threads: int) -> int:
+    """threads <= 0 means all cores of the host; 1 means the single-threaded definition."""
+    return host_cores() if threads <= 0 else threads
 
 
 def _f32(a) -> np.ndarray:
@@ -59,7 +74,7 @@ def camera_constants(eye, lookat, up, fov_deg: float, W: int, H: int) -> np.ndar
 
 
 def geometry(x, y, z, h, cam: np.ndarray, chi: float, r_small: float, r_large: float,
-             z_near: float, W: int, H: int, T: int) -> Dict[str, np.ndarray]:
+             z_near: float, W: int, H: int, T: int, threads: int = 1) -> Dict[str, np.ndarray]:
     x, y, z, h = _f32(x), _f32(y), _f32(z), _f32(h)
     n = x.shape[0]
     g = {
@@ -69,12 +84,13 @@ def geometry(x, y, z, h, cam: np.ndarray, chi: float, r_small: float, r_large: f
         "ilabel": np.zeros(n, np.int32),
     }
     cam = _f32(cam)
-    lib().orc_geometry(C.c_int64(n), _p(x, C.c_float), _p(y, C.c_float), _p(z, C.c_float),
-                       _p(h, C.c_float), _p(cam, C.c_float), C.c_float(chi), C.c_float(r_small),
-                       C.c_float(r_large), C.c_float(z_near), C.c_int(W), C.c_int(H), C.c_int(T),
-                       _p(g["cls"], C.c_int8), _p(g["px"], C.c_float), _p(g["py"], C.c_float),
-                       _p(g["sp"], C.c_float), _p(g["rp"], C.c_float), _p(g["zc"], C.c_float),
-                       _p(g["pbox"], C.c_int32), _p(g["tbox"], C.c_int32), _p(g["ilabel"], C.c_int32))
+    fn, lead = (lib().orc_geometry, []) if threads == 1 else (lib().orc_geometry_mt, [C.c_int(_threads(threads))])
+    fn(*lead, C.c_int64(n), _p(x, C.c_float), _p(y, C.c_float), _p(z, C.c_float),
+       _p(h, C.c_float), _p(cam, C.c_float), C.c_float(chi), C.c_float(r_small),
+       C.c_float(r_large), C.c_float(z_near), C.c_int(W), C.c_int(H), C.c_int(T),
+       _p(g["cls"], C.c_int8), _p(g["px"], C.c_float), _p(g["py"], C.c_float),
+       _p(g["sp"], C.c_float), _p(g["rp"], C.c_float), _p(g["zc"], C.c_float),
+       _p(g["pbox"], C.c_int32), _p(g["tbox"], C.c_int32), _p(g["ilabel"], C.c_int32))
     return g
 
 
@@ -120,7 +136,7 @@ def _species_arrays(n: int, species: Sequence, luts: Sequence[Optional[np.ndarra
     return species_of, bright, kappa, use_cm, np.ascontiguousarray(fixed), smin, smax, use_log, lut, lut_off, lut_n
 
 
-def amplitude(I, scalar, h, species: Sequence, luts: Sequence) -> Tuple[np.ndarray, np.ndarray, np.ndarray]:
+def amplitude(I, scalar, h, species: Sequence, luts: Sequence, threads: int = 1) -> Tuple[np.ndarray, np.ndarray, np.ndarray]:
     """E[n,3] = brightness * colour, col[n] = sqrt(pi) h I, kappa[n] (species' absorption)."""
     I, scalar, h = _f32(I), _f32(scalar), _f32(h)
     n = I.shape[0]
@@ -128,26 +144,33 @@ def amplitude(I, scalar, h, species: Sequence, luts: Sequence) -> Tuple[np.ndarr
         _species_arrays(n, species, luts)
     E = np.zeros((n, 3))
     col = np.zeros(n)
-    lib().orc_amplitude(C.c_int64(n), _p(I, C.c_float), _p(scalar, C.c_float), _p(h, C.c_float),
-                        _p(species_of, C.c_int32), C.c_int(len(species)), _p(bright, C.c_double),
-                        _p(use_cm, C.c_int32), _p(fixed, C.c_double), _p(smin, C.c_double),
-                        _p(smax, C.c_double), _p(use_log, C.c_int32), _p(lut, C.c_double),
-                        _p(lut_off, C.c_int32), _p(lut_n, C.c_int32), _p(E, C.c_double), _p(col, C.c_double))
+    fn, lead = (lib().orc_amplitude, []) if threads == 1 else (lib().orc_amplitude_mt, [C.c_int(_threads(threads))])
+    fn(*lead, C.c_int64(n), _p(I, C.c_float), _p(scalar, C.c_float), _p(h, C.c_float),
+       _p(species_of, C.c_int32), C.c_int(len(species)), _p(bright, C.c_double),
+       _p(use_cm, C.c_int32), _p(fixed, C.c_double), _p(smin, C.c_double),
+       _p(smax, C.c_double), _p(use_log, C.c_int32), _p(lut, C.c_double),
+       _p(lut_off, C.c_int32), _p(lut_n, C.c_int32), _p(E, C.c_double), _p(col, C.c_double))
     return E, col, kappa[species_of]
 
 
+def _bands(threads: int) -> int:
+    return 4 * _threads(threads)          # several bands per thread: rows through a halo core cost more
+
+
 def render_additive(g, E, col, chi: float, W: int, H: int, window=None, apply_transfer=False,
-                    p_range=None, image: Optional[np.ndarray] = None) -> np.ndarray:
+                    p_range=None, image: Optional[np.ndarray] = None, threads: int = 1) -> np.ndarray:
     n = g["cls"].shape[0]
     if image is None:
         image = np.zeros((H, W, 3))
     wx0, wx1, wy0, wy1 = window if window is not None else (0, W - 1, 0, H - 1)
     pb, pe = p_range if p_range is not None else (0, n)
-    lib().orc_render_additive(C.c_int64(pb), C.c_int64(pe), _p(g["cls"], C.c_int8), _p(g["px"], C.c_float),
-                              _p(g["py"], C.c_float), _p(g["sp"], C.c_float), _p(g["rp"], C.c_float),
-                              _p(g["pbox"], C.c_int32), _p(E, C.c_double), _p(col, C.c_double),
-                              C.c_float(chi), C.c_int(W), C.c_int(H), C.c_int(wx0), C.c_int(wx1),
-                              C.c_int(wy0), C.c_int(wy1), C.c_int(int(apply_transfer)), _p(image, C.c_double))
+    fn, lead = ((lib().orc_render_additive, []) if threads == 1 else
+                (lib().orc_render_additive_mt, [C.c_int(_threads(threads)), C.c_int(_bands(threads))]))
+    fn(*lead, C.c_int64(pb), C.c_int64(pe), _p(g["cls"], C.c_int8), _p(g["px"], C.c_float),
+       _p(g["py"], C.c_float), _p(g["sp"], C.c_float), _p(g["rp"], C.c_float),
+       _p(g["pbox"], C.c_int32), _p(E, C.c_double), _p(col, C.c_double),
+       C.c_float(chi), C.c_int(W), C.c_int(H), C.c_int(wx0), C.c_int(wx1),
+       C.c_int(wy0), C.c_int(wy1), C.c_int(int(apply_transfer)), _p(image, C.c_double))
     return image
 
 
@@ -160,32 +183,38 @@ def depth_order(g) -> np.ndarray:
     return order[:m].copy()
 
 
-def render_ordered(g, E, col, kappa, chi: float, W: int, H: int, window=None, order=None) -> np.ndarray:
+def render_ordered(g, E, col, kappa, chi: float, W: int, H: int, window=None, order=None, threads: int = 1) -> np.ndarray:
     image = np.zeros((H, W, 3))
     if order is None:
         order = depth_order(g)
     order = np.ascontiguousarray(order, np.int64)
     kappa = np.ascontiguousarray(kappa, np.float64)
     wx0, wx1, wy0, wy1 = window if window is not None else (0, W - 1, 0, H - 1)
-    lib().orc_render_ordered(C.c_int64(order.shape[0]), _p(order, C.c_int64), _p(g["cls"], C.c_int8),
-                             _p(g["px"], C.c_float), _p(g["py"], C.c_float), _p(g["sp"], C.c_float),
-                             _p(g["rp"], C.c_float), _p(g["pbox"], C.c_int32), _p(E, C.c_double),
-                             _p(col, C.c_double), _p(kappa, C.c_double), C.c_float(chi), C.c_int(W),
-                             C.c_int(H), C.c_int(wx0), C.c_int(wx1), C.c_int(wy0), C.c_int(wy1),
-                             _p(image, C.c_double))
+    fn, lead = ((lib().orc_render_ordered, []) if threads == 1 else
+                (lib().orc_render_ordered_mt, [C.c_int(_threads(threads)), C.c_int(_threads(threads))]))
+    fn(*lead, C.c_int64(order.shape[0]), _p(order, C.c_int64), _p(g["cls"], C.c_int8),
+       _p(g["px"], C.c_float), _p(g["py"], C.c_float), _p(g["sp"], C.c_float),
+       _p(g["rp"], C.c_float), _p(g["pbox"], C.c_int32), _p(E, C.c_double),
+       _p(col, C.c_double), _p(kappa, C.c_double), C.c_float(chi), C.c_int(W),
+       C.c_int(H), C.c_int(wx0), C.c_int(wx1), C.c_int(wy0), C.c_int(wy1),
+       _p(image, C.c_double))
     return image
 
 
 def render(fields: Dict[str, np.ndarray], species: Sequence, luts: Sequence, camera, W: int, H: int,
            chi: float = 3.0, r_small: float = 0.5, r_large: float = 64.0, z_near: float = 1e-6,
            tile: int = 16, additive: bool = True, apply_transfer: bool = False, window=None,
-           return_geometry: bool = False):
-    """Whole path on numpy float32 fields {x,y,z,h,I,scalar}: camera -> C1 -> C2 -> image (float64 HxWx3)."""
+           return_geometry: bool = False, threads: int = 1):
+    """Whole path on numpy float32 fields {x,y,z,h,I,scalar}: camera -> C1 -> C2 -> image (float64 HxWx3).
+
+    threads = 1 is the definition (single thread, index order); threads = 0 (all cores) or > 1 runs the same
+    functions through the row-band drivers of splotch_oracle_mt.c, bit-identical by construction."""
     cam = camera_constants(camera.eye, camera.lookat, camera.up, camera.fov_deg, W, H)
-    g = geometry(fields["x"], fields["y"], fields["z"], fields["h"], cam, chi, r_small, r_large, z_near, W, H, tile)
-    E, col, kappa = amplitude(fields["I"], fields["scalar"], fields["h"], species, luts)
+    g = geometry(fields["x"], fields["y"], fields["z"], fields["h"], cam, chi, r_small, r_large, z_near, W, H, tile,
+                 threads=threads)
+    E, col, kappa = amplitude(fields["I"], fields["scalar"], fields["h"], species, luts, threads=threads)
     if additive:
-        img = render_additive(g, E, col, chi, W, H, window=window, apply_transfer=apply_transfer)
+        img = render_additive(g, E, col, chi, W, H, window=window, apply_transfer=apply_transfer, threads=threads)
     else:
-        img = render_ordered(g, E, col, kappa, chi, W, H, window=window)
+        img = render_ordered(g, E, col, kappa, chi, W, H, window=window, threads=threads)
     return (img, g, cam) if return_geometry else img

@@ -147,8 +147,6 @@ def test_large_particles_with_8px_tiles_and_a_disc_covering_the_image():
 def test_apply_transfer():
     w = wl.make_config(0, n=30_000)
     w.apply_transfer = True
-    for k in w.fields:
-        pass
     w.fields["I"] = w.fields["I"] * 40.0                        # make 1 - exp(-S) differ visibly from S
     full_check(w, 16)
 

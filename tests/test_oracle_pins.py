@@ -403,3 +403,69 @@ def test_two_species_use_their_own_parameters():
     np.testing.assert_allclose(E[4:], np.tile([0.25, 0.125, 0.0625], (2, 1)))
     np.testing.assert_allclose(col, math.sqrt(math.pi))
     assert kappa.tolist() == [0.5] * 4 + [3.0] * 2
+
+
+# ------------------------------------------------------------------------------------------------
+# closed-form single-Gaussian image: every pixel, to double rounding
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("X,Y,h,chi", [(0.0, 0.0, 2.0, 3.0), (3.25, -2.5, 2.5, 3.0), (-7.75, 5.125, 1.5, 2.0),
+                                       (29.5, -30.0, 3.0, 3.0)])
+def test_single_gaussian_image_closed_form_every_pixel(X, Y, h, chi):
+    """One particle, E = A: S(i, j) = b colour I sqrt(pi) h exp(-d^2 / sp^2) inside the clip disc d <= chi sp, 0 outside.
+
+    fov 90 degrees, W = 64, eye 32 units from the particle's plane: s = 32 and k = s / z_c = 1 exactly, so the screen
+    centre (32 + X, 32 - Y) and sp = h are exact in float32 and the expected image below is exact up to double rounding.
+    The last case sits in the image corner (clipped box, off-axis in both directions)."""
+    W = H = 64
+    cam = camera((0.0, 0.0, 32.0), fov=90.0)
+    I0, b = 1.75, 0.6
+    rgb = (0.9, 0.5, 0.125)
+    f = fields([X], [Y], [0.0], [h], I=[I0])
+    sp = [species(1, fixed_rgb=rgb, brightness=b)]
+    img, g, cam16 = so.render(f, sp, [None], cam, W, H, chi=chi, r_large=1e9, return_geometry=True)
+    assert float(cam16[12]) == 32.0 and float(g["px"][0]) == 32.0 + X and float(g["py"][0]) == 32.0 - Y
+    assert float(g["sp"][0]) == h
+    jj, ii = np.mgrid[0:H, 0:W]
+    d2 = (ii + 0.5 - (32.0 + X)) ** 2 + (jj + 0.5 - (32.0 - Y)) ** 2
+    peak = float(np.float32(b)) * float(np.float32(I0)) * math.sqrt(math.pi) * h
+    expect = np.where(d2 <= (chi * h) ** 2, peak * np.exp(-d2 / h ** 2), 0.0)
+    assert (expect > 0).sum() > 20
+    for c in range(3):
+        np.testing.assert_allclose(img[:, :, c], float(np.float32(rgb[c])) * expect, rtol=1e-14, atol=0.0)
+    # exact transfer of the E = A solution (PAPER.md:85)
+    img_t = so.render(f, sp, [None], cam, W, H, chi=chi, r_large=1e9, apply_transfer=True)
+    np.testing.assert_allclose(img_t[:, :, 0], -np.expm1(-float(np.float32(rgb[0])) * expect), rtol=1e-14, atol=0.0)
+
+
+def test_pixel_box_is_the_tight_bounding_box_of_the_clip_disc():
+    """C1: x0 = ceil((p_x - r) - 0.5), x1 = floor((p_x + r) - 0.5) clamped to the screen -- brute force over every
+    column and row: column i belongs to the box iff |i + 0.5 - p_x| <= r (the disc reaches that column's centre line),
+    rows likewise.  A box one pixel too wide or too narrow on any side fails.  Particles whose disc edge lies within
+    1e-4 px of a column / row centre line are the documented float32 edge case and are skipped (they must be rare)."""
+    W, H = 150, 100
+    f = _random_scene(4000, 77, hmin=0.001, hmax=0.08)
+    cam = so.camera_constants((0, 0, 2.0), (0, 0, 0), (0, 1, 0), 50.0, W, H)
+    g = so.geometry(f["x"], f["y"], f["z"], f["h"], cam, 3.0, 0.5, 20.0, 1e-6, W, H, 16)
+    big = np.flatnonzero(g["cls"] >= so.MEDIUM)
+    assert big.size > 1500
+    cols, rows = np.arange(W) + 0.5, np.arange(H) + 0.5
+    skipped = 0
+    for p in big:
+        px, py, r = float(g["px"][p]), float(g["py"][p]), float(g["rp"][p])
+        ex, ey = np.abs(cols - px) - r, np.abs(rows - py) - r
+        if np.abs(ex).min() < 1e-4 or np.abs(ey).min() < 1e-4:
+            skipped += 1
+            continue
+        ci, rj = np.flatnonzero(ex <= 0), np.flatnonzero(ey <= 0)
+        assert ci.size and rj.size                       # active: the box is not empty
+        assert g["pbox"][p].tolist() == [ci[0], ci[-1], rj[0], rj[-1]], p
+    assert skipped < 0.01 * big.size
+    # inactive although r > r_small: no column or no row centre line is reached on screen
+    off = np.flatnonzero((g["cls"] == so.CULLED) & (g["rp"] > 0.5) & (g["zc"] > 1e-6))
+    assert off.size > 10
+    for p in off:
+        px, py, r = float(g["px"][p]), float(g["py"][p]), float(g["rp"][p])
+        ex, ey = np.abs(cols - px) - r, np.abs(rows - py) - r
+        if np.abs(ex).min() < 1e-4 or np.abs(ey).min() < 1e-4:
+            continue
+        assert not ((ex <= 0).any() and (ey <= 0).any()), p
