@@ -1,19 +1,24 @@
 #!/usr/bin/env python
 """bench.py -- particles/s of the Splotch per-frame rendering path on B200 (BASELINE.json metric).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0..4] [--mode additive|ordered] [--impl ours|reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0..4] [--mode additive|ordered]
+                  [--impl ours|reference] [--no-per-config]
 
-A step is one whole frame (count -> scan -> scatter -> splat -> large -> compose) of BASELINE configs[1]
-(10M particles, 50 Plummer halos + 20 % background, 800 x 800, additive mode) with the particles
-already resident in HBM.  One JSON line is printed by rank 0.  `e2e` is the same frame through
-splotch_render_host: pinned HOST particle arrays in, HOST image out, copies inside the timed region.
-N > 1 runs N independent replicas (the path does not shard: north_star fixes one GPU, DESIGN.md
-"Multi-GPU"), so scaling is weak and no collective is on the data path.
+A step is one whole frame (count -> scan -> scatter -> splat -> large -> compose) with the particles already
+resident in HBM.  BASELINE.json's metric names no config, so the default line is on the largest single-GPU
+configuration, configs[3] (400M particles, camera inside the densest halo, 4096 x 4096, additive mode); the same
+JSON line carries, under `per_config`, frame time, particles/s, per-stage roofline fractions and the fraction of the
+frame roofline for all five configs and for the ordered mode on the 120-frame orbit (cfg4).
+`e2e` is the same frame through splotch_render_host: pinned HOST particle arrays in, HOST image out, copies inside
+the timed region (chunked, copy / compute overlapped on two streams).
+N > 1 runs N independent replicas (the path does not shard: north_star fixes one GPU), so
+scaling is weak and no collective is on the data path.
 `--impl reference` times the CPU oracle (oracle/, test infrastructure) on the host cores instead.
 """
 from __future__ import annotations
 
 import argparse
+import gc
 import json
 import os
 import statistics
@@ -31,10 +36,11 @@ from paper_1309_1114_b200 import workloads as wl  # noqa: E402
 
 KERNELS_ADDITIVE = 6         # k_count, k_scan, k_scatter, k_splat, k_large, k_compose (+ one memset node)
 L2_FLUSH_BYTES = 256 << 20   # written between frames when a config's inputs fit in the 126 MB L2
+DEFAULT_CONFIG = 3           # the largest single-GPU configuration of BASELINE.json
 
 
 def tile_for(cfg: int) -> int:
-    return 32 if cfg == 3 else 16       # 4096^2 at 16 px would need a 65,536-bin per-block histogram
+    return 32 if cfg == 3 else 16       # 4096^2: 16,384 tiles of 32 px (65,536 of 16 px work too, on the slower global-histogram path)
 
 
 def ordered_kernels_per_frame(n_tiles: int) -> int:
@@ -57,7 +63,8 @@ def measured_peaks():
 
 
 class ClockSampler(threading.Thread):
-    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+    """Samples SM clock and throttle reasons through NVML while the timed region runs (as fast as NVML answers, so
+    that even a region of a few milliseconds holds several samples)."""
 
     def __init__(self, index: int):
         super().__init__(daemon=True)
@@ -89,7 +96,7 @@ class ClockSampler(threading.Thread):
     def run(self):
         while not self.stop_flag:
             self.sample()
-            time.sleep(0.01)
+            time.sleep(0.0005 if len(self.sm) < 64 else 0.01)
 
     def result(self):
         if not self.sm:
@@ -102,12 +109,13 @@ def ncu_traffic(kernel: str, workload: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed ncu --set full capture
     (profiles/dram_traffic.csv: kernel,workload,bytes), or None."""
     path = os.path.join(ROOT, "profiles", "dram_traffic.csv")
+    best = None
     if os.path.exists(path):
         for line in open(path).read().splitlines()[1:]:
-            k, wk, b = line.split(",")[:3]
-            if k == kernel and wk == workload:
-                return float(b)
-    return None
+            parts = line.split(",")
+            if len(parts) >= 3 and parts[0] == kernel and parts[1] == workload:
+                best = float(parts[2])                # the last row for a (kernel, workload) is the newest capture
+    return best
 
 
 def max_over_ranks(ms: float, dist, device) -> float:
@@ -123,6 +131,13 @@ def whole_job_value(world: int, n: int, ms_step: float) -> float:
     return world * n / (ms_step * 1e-3)
 
 
+def check_world(gpus: int, world: int) -> None:
+    """--gpus N must agree with the launch (torchrun sets WORLD_SIZE); a silent 1-GPU run under --gpus 8 is refused."""
+    if gpus != world:
+        raise SystemExit(f"bench.py: --gpus {gpus} but WORLD_SIZE is {world}: launch with "
+                         f"`python -m torch.distributed.run --nproc-per-node {gpus} bench.py --gpus {gpus} ...`")
+
+
 def visible_index(local_rank: int) -> int:
     vis = os.environ.get("CUDA_VISIBLE_DEVICES")
     if vis:
@@ -133,14 +148,145 @@ def visible_index(local_rank: int) -> int:
     return local_rank
 
 
-def fragments_estimate(r, fields, species, kw) -> float:
+def fragments_estimate(r, fields, species, kw, chunk=1 << 26):
     """Algorithmic fragments of a frame: 1 per SMALL particle, pixel centres inside the clip disc otherwise
-    (pi r^2, at most the on-screen pixel box).  Computed once, outside the timed region."""
-    d = r.debug_geometry(fields, species, **kw)
-    cls, rp, box = d["cls"], d["rp"].double(), d["pbox"].double()
-    area = (box[:, 1] - box[:, 0] + 1) * (box[:, 3] - box[:, 2] + 1)
-    disc = torch.minimum(torch.pi * rp * rp, area)
-    return float((cls == 1).sum() + disc[cls >= 2].sum()), float(disc[cls == 3].sum())
+    (pi r^2, at most the on-screen pixel box).  Computed once, outside the timed region, in chunks."""
+    n = fields["x"].numel()
+    total = large = 0.0
+    for a in range(0, n, chunk):
+        b = min(n, a + chunk)
+        sub = {k: v[a:b] for k, v in fields.items()}
+        d = r.debug_geometry(sub, [wl.Species(0, b - a)], **dict(kw, additive=True))
+        cls, rp, box = d["cls"], d["rp"].double(), d["pbox"].double()
+        area = (box[:, 1] - box[:, 0] + 1) * (box[:, 3] - box[:, 2] + 1)
+        disc = torch.minimum(torch.pi * rp * rp, area)
+        total += float((cls == 1).sum() + disc[cls >= 2].sum())
+        large += float(disc[cls == 3].sum())
+        del d, cls, rp, box, area, disc
+    return total, large
+
+
+def stage_bytes(additive: bool, w, st, passes: int):
+    """Algorithmic HBM bytes per stage and frame."""
+    pairs = st["pairs"] + st["large_pairs"]
+    active = st["n"] - st["count"][0]
+    if additive:
+        rec_bytes = st.get("record_bytes", 32.0 * pairs)          # 16-byte SMALL records + 32-byte others
+        tile_rec_bytes = st.get("tile_record_bytes", 32.0 * st["pairs"])
+        return {
+            "count": 16.0 * w.n,                                   # x y z h read once
+            "scatter": 24.0 * w.n + rec_bytes,                     # six fields read, one record written per pair
+            "splat": tile_rec_bytes,                               # records read once
+            "large": rec_bytes - tile_rec_bytes,                   # super-tile records read once (the blocks of a super-tile share them in L2)
+            "compose": (24.0 + 12.0) * w.width * w.height,         # fixed-point sums read, image written once
+        }, ("count", "scatter"), ("splat", "large", "compose")
+    return {
+        "count": 16.0 * w.n,
+        "pairs": 24.0 * w.n + 32.0 * active + 12.0 * pairs,        # fields read, one record per particle, key + value per pair
+        "sort": passes * (8.0 + 12.0 + 12.0) * pairs,              # per pass: keys read (histogram), key + value read and written
+        "bounds": 8.0 * pairs,
+        "render": (4.0 + 32.0) * pairs,                            # value + gathered record per pair
+        "combine": 12.0 * w.width * w.height,
+    }, ("count", "pairs", "sort"), ("render", "combine")
+
+
+class Run:
+    """One configuration resident on the device: renderer, fields, parameters."""
+
+    def __init__(self, cfg: int, mode: str, local: int, fields=None, workload=None):
+        from paper_1309_1114_b200 import binding
+        self.cfg, self.mode, self.local = cfg, mode, local
+        self.additive = mode == "additive"
+        self.w = workload if workload is not None else wl.make_config(cfg, device=f"cuda:{local}")
+        w = self.w
+        self.tile = tile_for(cfg)
+        self.lut = wl.palette()
+        self.fields = fields if fields is not None else {k: v.contiguous() for k, v in w.fields.items()}
+        w.fields = self.fields
+        self.r = binding.Renderer(w.width, w.height, w.n, device=local)
+        self.r.set_camera(w.camera)
+        for s, sp in enumerate(w.species):
+            if sp.use_colormap:
+                self.r.set_colormap(s, self.lut)
+        self.kw = dict(chi=w.chi, r_small=w.r_small, r_large=w.r_large, z_near=w.z_near, tile=self.tile,
+                       additive=self.additive, apply_transfer=False)
+        self.image = torch.empty((w.height, w.width, 3), dtype=torch.float32, device=f"cuda:{local}")
+        self.orbit = cfg == 4                    # fly-through: the camera moves 3 degrees per frame
+        self.flush = 24 * w.n < (126 << 20)      # inputs fit in L2: flush it between frames
+        self.fbuf = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=f"cuda:{local}") if self.flush else None
+
+    def frame(self, i: int):
+        if self.orbit:
+            self.r.set_camera(wl.orbit_camera(i % 120))
+        self.r.render(self.fields, self.w.species, image=self.image, **self.kw)
+
+    def timed(self, steps: int, warmup: int, barrier, sampler=None):
+        """(ms per step on this rank, sorted per-frame times, stats with per-stage means)."""
+        stream = torch.cuda.current_stream()
+        for i in range(max(warmup, 3)):
+            self.frame(i)
+        torch.cuda.synchronize()
+        assert self.r.stats()["overflow"] == 0, "pair capacity overflow"
+        self.r.set_profiling(True)
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        barrier()
+        if sampler is not None:
+            sampler.start()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for i in range(steps):
+            if self.flush:
+                self.fbuf.fill_(i & 255)
+            ev[i][0].record(stream)
+            self.frame(i)
+            ev[i][1].record(stream)
+        e1.record(stream)
+        barrier()
+        if sampler is not None:
+            sampler.stop_flag = True
+        per_frame = sorted(a.elapsed_time(b) for a, b in ev)
+        # with an L2 flush between frames the step time is the sum of the frames' own event pairs
+        ms_total = sum(per_frame) if self.flush else e0.elapsed_time(e1)
+        st = self.r.stats()
+        self.r.set_profiling(False)
+        return ms_total / steps, per_frame, st
+
+    def summary(self, ms_step: float, per_frame, st, hbm_gbs: float, fma_peak: float, frags=None):
+        """Per-stage roofline fractions and the frame lower bound (sum over stages)."""
+        w = self.w
+        if self.orbit:
+            self.r.set_camera(wl.orbit_camera((len(per_frame) - 1) % 120))   # the camera of the frame the statistics belong to
+        if frags is None:
+            frags = fragments_estimate(self.r, self.fields, w.species, self.kw)
+        passes = -(-st["sort_key_bits"] // 8) if not self.additive else 0      # radix passes that really ran
+        bytes_by_stage, hbm_stages, alu_stages = stage_bytes(self.additive, w, st, passes)
+        stage = st["stage_ms"]
+        flop = FLOP_PER_FRAGMENT if self.additive else FLOP_PER_FRAGMENT_ORDERED
+        stage_roof = {}
+        for k in stage:
+            stage_roof[k] = {"ms": stage[k]}
+            if k in hbm_stages and stage[k] > 0:
+                gbs = bytes_by_stage[k] / (stage[k] * 1e-3) / 1e9
+                stage_roof[k].update({"GB/s": gbs, "frac_hbm": gbs / hbm_gbs})
+        frag_stage = {"splat": frags[0] - frags[1], "large": frags[1]} if self.additive else {"render": frags[0]}
+        for k, f in frag_stage.items():
+            if k in stage and stage[k] > 0 and f > 0:
+                stage_roof[k]["Gfragments/s"] = f / (stage[k] * 1e-3) / 1e9
+                stage_roof[k]["frac_fma"] = f * flop / (stage[k] * 1e-3) / fma_peak
+        t_min_ms = sum(bytes_by_stage.values()) / (hbm_gbs * 1e9) * 1e3 + frags[0] * flop / fma_peak * 1e3
+        dist_ms = {"min": per_frame[0], "median": per_frame[len(per_frame) // 2],
+                   "p95": per_frame[min(len(per_frame) - 1, int(0.95 * len(per_frame)))], "max": per_frame[-1]}
+        return {"workload": w.name, "mode": self.mode, "tile": self.tile, "ms_per_frame": ms_step,
+                "particles_per_s": w.n / (ms_step * 1e-3), "frame_ms": dist_ms, "stages": stage_roof,
+                "frame_lower_bound_ms": t_min_ms, "frac_of_frame_roofline": t_min_ms / ms_step,
+                "classes": dict(zip(("culled", "small", "medium", "large"), st["count"])),
+                "pairs": st["pairs"] + st["large_pairs"], "fragments_estimate": frags[0], "fragments_large": frags[1],
+                "l2": "256 MB written between frames" if self.flush else "inputs exceed L2, no flush"}, bytes_by_stage, frags
+
+    def close(self):
+        self.r.close()
+        self.fields = self.image = self.fbuf = None
+        self.w.fields = None
 
 
 def run_ours(args):
@@ -148,28 +294,12 @@ def run_ours(args):
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    check_world(args.gpus, world)
     torch.cuda.set_device(local)
     dist = None
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    w = wl.make_config(args.config, device=f"cuda:{local}")
-    TILE = tile_for(args.config)
-    additive = args.mode == "additive"
-    lut = wl.palette()
-    fields = {k: v.contiguous() for k, v in w.fields.items()}
-    r = binding.Renderer(w.width, w.height, w.n, device=local)
-    r.set_camera(w.camera)
-    for s, sp in enumerate(w.species):
-        if sp.use_colormap:
-            r.set_colormap(s, lut)
-    kw = dict(chi=w.chi, r_small=w.r_small, r_large=w.r_large, z_near=w.z_near, tile=TILE, additive=additive,
-              apply_transfer=False)
-    image = torch.empty((w.height, w.width, 3), dtype=torch.float32, device=f"cuda:{local}")
-    stream = torch.cuda.current_stream()
-    orbit = args.config == 4                 # fly-through: the camera moves 3 degrees per frame
-    flush = 24 * w.n < (126 << 20)           # inputs fit in L2: flush it between frames
-    fbuf = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=f"cuda:{local}") if flush else None
 
     def barrier():
         torch.cuda.synchronize()
@@ -177,125 +307,66 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    def frame(i):
-        if orbit:
-            r.set_camera(wl.orbit_camera(i % 120))
-        r.render(fields, w.species, image=image, **kw)
-
+    run = Run(args.config, args.mode, local)
+    w, additive = run.w, run.additive
     # ---- device-resident timing -------------------------------------------------------------------------------
-    for i in range(max(args.warmup, 3)):
-        frame(i)
-    torch.cuda.synchronize()
-    st0 = r.stats()
-    assert st0["overflow"] == 0, "pair capacity overflow"
-    r.set_profiling(True)
     sampler = ClockSampler(visible_index(local))
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    barrier()
-    sampler.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
-    for i in range(args.steps):
-        if flush:
-            fbuf.fill_(i & 255)
-        ev[i][0].record(stream)
-        frame(i)
-        ev[i][1].record(stream)
-    e1.record(stream)
-    barrier()
-    sampler.stop_flag = True
-    per_frame = sorted(a.elapsed_time(b) for a, b in ev)
-    # with an L2 flush between frames the step time is the sum of the frames' own event pairs
-    ms_total = sum(per_frame) if flush else e0.elapsed_time(e1)
-    st = r.stats()
-    r.set_profiling(False)
+    ms_local, per_frame, st = run.timed(args.steps, args.warmup, barrier, sampler)
     sampler.join(timeout=1.0)
-    ms_step = max_over_ranks(ms_total, dist, f"cuda:{local}") / args.steps
-    dist_ms = {"min": per_frame[0], "median": per_frame[len(per_frame) // 2],
-               "p95": per_frame[min(len(per_frame) - 1, int(0.95 * len(per_frame)))], "max": per_frame[-1]}
+    ms_step = max_over_ranks(ms_local, dist, f"cuda:{local}")
 
     # ---- end to end through the C ABI with HOST buffers ---------------------------------------------------------
-    host = {k: v.cpu().pin_memory() for k, v in fields.items()}
+    host = {k: v.cpu().pin_memory() for k, v in run.fields.items()}
     himg = torch.empty((w.height, w.width, 3), dtype=torch.float32).pin_memory()
     e2e_steps = max(3, min(args.steps, 20 if w.n <= 20_000_000 else 3))
-    if orbit:
-        r.set_camera(wl.orbit_camera(0))
-    r.render_host(host, w.species, himg, **kw)
+    if run.orbit:
+        run.r.set_camera(wl.orbit_camera(0))
+    run.r.render_host(host, w.species, himg, **run.kw)
     barrier()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
-        r.render_host(host, w.species, himg, **kw)          # synchronises the stream before returning
+        run.r.render_host(host, w.species, himg, **run.kw)          # synchronises the stream before returning
     t1 = time.perf_counter()
     e2e_ms = max_over_ranks((t1 - t0) * 1e3 / e2e_steps, dist, f"cuda:{local}")
+    del host, himg
 
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
         return
-    # ---- roofline of the dominant kernel ------------------------------------------------------------------------
+    # ---- peaks: measured HBM copy rate (driver) and FP32 FMA / MUFU.EX2 rates measured here by the library ----------
     hbm_gbs, sm_max_mhz, peak_src = measured_peaks()
+    pk = run.r.measure_peaks()
+    fma_peak = pk["fma_lane_ops_per_s"]
+    # ---- roofline of the dominant kernel ------------------------------------------------------------------------
+    summ, bytes_by_stage, frags = run.summary(ms_step, per_frame, st, hbm_gbs, fma_peak)
     stage = st["stage_ms"]
     dom = max(stage, key=stage.get)
-    pairs = st["pairs"] + st["large_pairs"]
-    active = st["n"] - st["count"][0]
-    if orbit:
-        r.set_camera(wl.orbit_camera((args.steps - 1) % 120))     # the camera of the frame the statistics belong to
-    frags, frags_large = fragments_estimate(r, fields, w.species, kw)
-    n_tiles = (-(-w.width // TILE)) * (-(-w.height // TILE))
-    passes = -(-st["sort_key_bits"] // 8) if not additive else 0      # radix passes that really ran
-    # algorithmic bytes per stage and frame
-    if additive:
-        bytes_by_stage = {
-            "count": 16.0 * w.n,                                   # x y z h read once
-            "scatter": 24.0 * w.n + 32.0 * pairs,                  # six fields read, one 32-B record written per pair
-            "splat": 32.0 * st["pairs"],                           # records read once
-            "large": 32.0 * st["large_pairs"],                     # super-tile records read once (64 tiles share them in L2)
-            "compose": (24.0 + 12.0) * w.width * w.height,         # fixed-point sums read, image written once
-        }
-        hbm_stages, alu_stages = ("count", "scatter"), ("splat", "large", "compose")
-    else:
-        bytes_by_stage = {
-            "count": 16.0 * w.n,
-            "pairs": 24.0 * w.n + 32.0 * active + 12.0 * pairs,    # fields read, one record per particle, key + value per pair
-            "sort": passes * (8.0 + 12.0 + 12.0) * pairs,          # per pass: keys read (histogram), key + value read and written
-            "bounds": 8.0 * pairs,
-            "render": (4.0 + 32.0) * pairs,                        # value + gathered record per pair
-            "combine": 12.0 * w.width * w.height,
-        }
-        hbm_stages, alu_stages = ("count", "pairs", "sort"), ("render", "combine")
-    traffic = ncu_traffic("k_" + dom, w.name)
     flop = FLOP_PER_FRAGMENT if additive else FLOP_PER_FRAGMENT_ORDERED
-    peak_tf = 148 * 128 * sm_max_mhz * 1e6 / 1e12              # FP32 lanes x clock, one op per lane per cycle
+    n_tiles = (-(-w.width // run.tile)) * (-(-w.height // run.tile))
+    traffic = ncu_traffic("k_" + dom, w.name)
     bytes_by_stage.setdefault(dom, 0.0)
     t_hbm = bytes_by_stage[dom] / (hbm_gbs * 1e9)
-    dom_frags = {"splat": frags - frags_large, "large": frags_large, "render": frags}.get(dom, 0.0) if additive or dom == "render" else 0.0
-    t_alu = dom_frags * flop / (peak_tf * 1e12)
+    dom_frags = ({"splat": frags[0] - frags[1], "large": frags[1]} if additive else {"render": frags[0]}).get(dom, 0.0)
+    t_alu = dom_frags * flop / fma_peak
     # the roofline that bounds the stage is the larger of its two lower bounds ("report both, take the larger")
     if t_hbm >= t_alu:
         ach = bytes_by_stage[dom] / (stage[dom] * 1e-3) / 1e9
         roof = {"kernel": "k_" + dom, "bound": "hbm", "achieved": ach, "peak": hbm_gbs, "unit": "GB/s",
-                "frac": ach / hbm_gbs, "traffic": traffic, "peak_source": peak_src + " copy bandwidth",
+                "frac": ach / hbm_gbs, "traffic": traffic, "peak_source": peak_src + " copy bandwidth (MEASURED_PEAKS.json)",
                 "other_bound": {"bound": "alu", "lower_bound_ms": t_alu * 1e3}}
     else:
         ach = dom_frags * flop / (stage[dom] * 1e-3) / 1e12
-        roof = {"kernel": "k_" + dom, "bound": "alu", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s",
-                "frac": ach / peak_tf, "traffic": traffic,
-                "peak_source": "148 SM x 128 FP32 lanes x %.0f MHz, FMA = 1 op (DESIGN.md)" % sm_max_mhz,
+        roof = {"kernel": "k_" + dom, "bound": "alu", "achieved": ach, "peak": fma_peak / 1e12, "unit": "TFLOP/s",
+                "frac": ach * 1e12 / fma_peak, "traffic": traffic,
+                "peak_source": "FP32 FMA lane-ops/s measured by splotch_measure_peaks on this GPU (FMA = 1 op; nominal "
+                               "148 SM x 128 lanes x %.0f MHz = %.1f T)" % (sm_max_mhz, 148 * 128 * sm_max_mhz * 1e-6),
+                "algorithmic": "%d lane-ops x %.4g fragments per launch (DESIGN.md section 7)" % (flop, dom_frags),
                 "other_bound": {"bound": "hbm", "lower_bound_ms": t_hbm * 1e3}}
-    stage_roof = {}
-    for k in stage:
-        stage_roof[k] = {"ms": stage[k]}
-        if k in hbm_stages:
-            gbs = bytes_by_stage[k] / (stage[k] * 1e-3) / 1e9
-            stage_roof[k].update({"GB/s": gbs, "frac_hbm": gbs / hbm_gbs})
-    rk = "splat" if additive else "render"
-    stage_roof[rk]["Gfragments/s"] = frags / (stage[rk] * 1e-3) / 1e9
-    # sum of per-stage lower bounds: HBM terms + ALU term
-    flop = FLOP_PER_FRAGMENT if additive else FLOP_PER_FRAGMENT_ORDERED
-    t_min_ms = sum(bytes_by_stage.values()) / (hbm_gbs * 1e9) * 1e3 + frags * flop / (148 * 128 * sm_max_mhz * 1e6) * 1e3
 
-    # ---- CPU baseline: the oracle as it stands, one thread ---------------------------------------------------------
-    cpu = cpu_baseline_frame(w, lut, min(w.n, args.cpu_sample), TILE, additive)
+    # ---- CPU baseline: the oracle as it stands, one thread, and the same code through the all-cores row-band driver ----
+    cpu1 = cpu_baseline_frame(args.config, args.cpu_sample, run.tile, additive, threads=1)
+    cpu_all = cpu_baseline_frame(args.config, args.cpu_sample, run.tile, additive, threads=0)
 
     out = {
         "metric": "particles/s rendered end-to-end per frame",
@@ -303,71 +374,115 @@ def run_ours(args):
         "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": w.name, "particles": w.n, "image": [w.width, w.height], "mode": args.mode,
-                   "tile": TILE, "chi": w.chi, "r_large": w.r_large, "parallelism": "replicas only" if world > 1 else "1 gpu",
-                   "l2": ("256 MB written between frames (inputs fit in L2); step time = sum of per-frame event pairs" if flush else
-                          "inputs (%.0f MB) and records (%.0f MB) exceed the 126 MB L2, no flush" % (24e-6 * w.n, 32e-6 * pairs)),
-                   "camera": "orbit, 3 deg/frame" if orbit else "fixed",
-                   "classes": dict(zip(("culled", "small", "medium", "large"), st["count"])), "pairs": pairs,
-                   "active": active, "fragments_estimate": frags, "fragments_large": frags_large},
+                   "tile": run.tile, "chi": w.chi, "r_large": w.r_large, "parallelism": "replicas only" if world > 1 else "1 gpu",
+                   "l2": ("256 MB written between frames (inputs fit in L2); step time = sum of per-frame event pairs" if run.flush else
+                          "inputs (%.0f MB) and records (%.0f MB) exceed the 126 MB L2, no flush" % (24e-6 * w.n, 32e-6 * summ["pairs"])),
+                   "camera": "orbit, 3 deg/frame" if run.orbit else "fixed",
+                   "classes": summ["classes"], "pairs": summ["pairs"],
+                   "active": st["n"] - st["count"][0], "fragments_estimate": frags[0], "fragments_large": frags[1]},
         "clocks": sampler.result(),
         "e2e": {"value": whole_job_value(world, w.n, e2e_ms), "unit": "particles/s", "ms_per_step": e2e_ms,
                 "h2d_bytes_per_step": 24 * w.n, "d2h_bytes_per_step": 12 * w.width * w.height, "steps": e2e_steps,
-                "api": "splotch_render_host (pinned host arrays in, host image out)"},
+                "api": "splotch_render_host (pinned host arrays in, host image out; chunked, copies overlap the kernels)"},
         "gpu_launches": (KERNELS_ADDITIVE if additive else ordered_kernels_per_frame(n_tiles)) * args.steps,
-        "frame_ms": dist_ms,
+        "frame_ms": summ["frame_ms"],
         "roofline": roof,
-        "stages": stage_roof,
-        "frame_lower_bound_ms": t_min_ms, "frac_of_frame_roofline": t_min_ms / ms_step,
-        "cpu_baseline": cpu,
+        "stages": summ["stages"],
+        "frame_lower_bound_ms": summ["frame_lower_bound_ms"], "frac_of_frame_roofline": summ["frac_of_frame_roofline"],
+        "peaks": {"hbm_GBps": hbm_gbs, "hbm_source": peak_src, "fma_lane_Tops": fma_peak / 1e12,
+                  "mufu_ex2_Tops": pk["mufu_ex2_per_s"] / 1e12, "source": "splotch_measure_peaks (this run, this GPU)"},
+        "cpu_baseline": cpu1,
+        "cpu_baseline_all_cores": cpu_all,
+        "host_cores": cpu_all["host_cores"],
     }
+    # ---- all five configs and the ordered orbit, same run -----------------------------------------------------------
+    if world == 1 and not args.no_per_config:
+        per = {f"cfg{args.config}_{args.mode}": summ}
+        run.close()
+        del run
+        gc.collect()
+        torch.cuda.empty_cache()
+        shared = None
+        for cfg, mode, steps in ((0, "additive", 20), (1, "additive", 20), (2, "additive", 10), (3, "additive", 5),
+                                 (4, "additive", 120), (4, "ordered", 120)):
+            key = f"cfg{cfg}_{mode}"
+            if key in per:
+                continue
+            if cfg == 4 and shared is not None:
+                r2 = Run(cfg, mode, local, fields=shared[0], workload=shared[1])
+                r2.w.camera = wl.orbit_camera(0)
+            else:
+                r2 = Run(cfg, mode, local)
+            ms2, pf2, st2 = r2.timed(steps, 3, barrier)
+            per[key] = r2.summary(ms2, pf2, st2, hbm_gbs, fma_peak)[0]
+            keep = cfg == 4 and mode == "additive"
+            if keep:
+                shared = (r2.fields, r2.w)
+                r2.r.close()
+            else:
+                if cfg == 4:
+                    shared = None
+                r2.close()
+            del r2
+            gc.collect()
+            torch.cuda.empty_cache()
+        out["per_config"] = per
     print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()
 
 
-def cpu_baseline_frame(w, lut, sample_n: int, tile: int = 16, additive: bool = True):
-    """Time the oracle (single thread, as it stands) on the first sample_n particles of the workload."""
+def cpu_baseline_frame(cfg: int, sample_n: int, tile: int = 16, additive: bool = True, threads: int = 1):
+    """Time the oracle on a bounded sample of the workload: the first sample_n particles of the full-size recipe
+    (same densities, smoothing lengths and camera; the generator is counter based), one full frame.
+    threads = 1: the single-threaded definition; threads = 0: the row-band driver on all host cores."""
     from oracle import splotch_oracle as so
-    f = {k: v[:sample_n].cpu().numpy() for k, v in w.fields.items()}
-    import copy
-    species = []
-    for sp in w.species:
-        s2 = copy.copy(sp)
-        s2.begin, s2.end = min(sp.begin, sample_n), min(sp.end, sample_n)
-        species.append(s2)
-    luts = [lut.numpy() if s.use_colormap else None for s in species]
+    w = wl.make_config(cfg, device="cpu", count=sample_n)
+    lut = wl.palette()
+    f = {k: v.numpy() for k, v in w.fields.items()}
+    luts = [lut.numpy() if s.use_colormap else None for s in w.species]
     so.lib()
+    nthreads = so.host_cores() if threads <= 0 else threads
     t0 = time.perf_counter()
-    so.render(f, species, luts, w.camera, w.width, w.height, chi=w.chi, r_small=w.r_small, r_large=w.r_large,
-              z_near=w.z_near, tile=tile, additive=additive)
+    so.render(f, w.species, luts, w.camera, w.width, w.height, chi=w.chi, r_small=w.r_small, r_large=w.r_large,
+              z_near=w.z_near, tile=tile, additive=additive, threads=nthreads)
     dt = time.perf_counter() - t0
-    return {"value": sample_n / dt, "unit": "particles/s", "cores": 1, "kind": "oracle", "seconds": dt,
-            "sample": "first %d of %d particles of %s, one full frame, single thread" % (sample_n, w.n, w.name)}
+    full_n = w.meta.get("full_n", w.n)
+    return {"value": w.n / dt, "unit": "particles/s", "cores": nthreads, "host_cores": so.host_cores(), "kind": "oracle",
+            "seconds": dt,
+            "sample": "first %d of %d particles of %s, one full frame, %s" %
+                      (w.n, full_n, w.name, "single thread" if nthreads == 1 else "row-band driver, %d threads" % nthreads)}
+
+
+def default_cpu_sample(cfg: int) -> int:
+    """About 10-30 s of single-thread oracle time (cfg3 costs ~35 us per particle: ~2400 fragments each)."""
+    return {0: 100_000, 1: 10_000_000, 2: 10_000_000, 3: 500_000, 4: 10_000_000}[cfg]
 
 
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    w = wl.make_config(args.config, device="cpu")
-    lut = wl.palette()
-    # bounded sample: about 0.75 us of oracle time per particle, whole run kept near two minutes
-    sample_n = min(w.n, args.ref_sample, max(100_000, int(1.6e8 / (args.steps + args.warmup))))
+    tile, additive = tile_for(args.config), args.mode == "additive"
+    # bounded sample: the whole --steps / --warmup run stays near two minutes
+    sample_n = max(20_000, min(args.ref_sample, int(6 * default_cpu_sample(args.config) / (args.steps + args.warmup))))
     times = []
-    for _ in range(args.warmup):
-        cpu_baseline_frame(w, lut, sample_n, tile_for(args.config), args.mode == "additive")
-    for _ in range(args.steps):
-        times.append(cpu_baseline_frame(w, lut, sample_n, tile_for(args.config), args.mode == "additive")["seconds"])
+    base = None
+    for i in range(args.warmup + args.steps):
+        base = cpu_baseline_frame(args.config, sample_n, tile, additive, threads=1)
+        if i >= args.warmup:
+            times.append(base["seconds"])
+    w = wl.make_config(args.config, device="cpu", count=1)
     ms = 1e3 * sum(times) / len(times)
     val = sample_n / (ms * 1e-3)
     out = {"impl": "reference", "metric": "particles/s rendered end-to-end per frame", "value": val,
            "unit": "particles/s", "n_gpus": int(os.environ.get("WORLD_SIZE", "1")), "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "f64", "data": "synthetic",
-           "config": {"workload": w.name, "particles": w.n, "image": [w.width, w.height], "mode": args.mode,
-                      "tile": tile_for(args.config), "chi": w.chi, "r_large": w.r_large},
-           "cpu_baseline": {"value": val, "unit": "particles/s", "cores": 1, "kind": "oracle",
-                            "sample": "each step: one frame of the first %d of %d particles, single thread" % (sample_n, w.n)},
+           "config": {"workload": w.name, "particles": w.meta.get("full_n", w.n), "image": [w.width, w.height], "mode": args.mode,
+                      "tile": tile, "chi": w.chi, "r_large": w.r_large},
+           "cpu_baseline": {"value": val, "unit": "particles/s", "cores": 1, "host_cores": base["host_cores"], "kind": "oracle",
+                            "sample": "each step: " + base["sample"]},
            "e2e": {"value": val, "unit": "particles/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(out))
 
@@ -377,17 +492,20 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=None)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=1)
+    ap.add_argument("--config", type=int, default=DEFAULT_CONFIG)
     ap.add_argument("--mode", default="additive", choices=["additive", "ordered"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--cpu-sample", type=int, default=10_000_000)
+    ap.add_argument("--cpu-sample", type=int, default=None)
     ap.add_argument("--ref-sample", type=int, default=10_000_000)
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config sweep over the other configs")
     args = ap.parse_args()
+    if args.cpu_sample is None:
+        args.cpu_sample = default_cpu_sample(args.config)
     if args.impl == "reference":
         args.steps = 3 if args.steps is None else args.steps
         run_reference(args)
     else:
-        args.steps = 100 if args.steps is None else args.steps
+        args.steps = 20 if args.steps is None else args.steps
         run_ours(args)
 
 

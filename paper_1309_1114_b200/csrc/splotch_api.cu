@@ -24,7 +24,7 @@ const char *kStageNamesAdditive[kStagesAdditive] = {"count", "scan", "scatter", 
 const char *kStageNamesOrdered[kStagesOrdered] = {"count", "scan", "pairs", "sort", "bounds", "render", "combine"};
 
 struct Layout {
-    size_t counts, cls_counts, bin_count, bin_start, stats, accum, accum_bytes, records, staging, total;
+    size_t counts, cls_counts, bin_count, bin_start, large_off, stats, accum, accum_bytes, records, staging, total;
     unsigned long long capacity;
     int nrows;
     // ordered mode
@@ -58,7 +58,7 @@ struct splotch_ctx {
     cudaStream_t last_stream = nullptr;
     int splat_blocks_per_sm[3] = {0, 0, 0};  // T = 8, 16, 32
     int orender_blocks_per_sm[3] = {0, 0, 0};
-    int large_blocks_per_sm[3] = {0, 0, 0};
+    int large_blocks_per_sm = 0;
     char err[512] = {0};
 };
 
@@ -86,10 +86,13 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 int tile_shift(int T) { return T == 8 ? 3 : T == 16 ? 4 : T == 32 ? 5 : -1; }
 
+// LARGE particles are binned to super-tiles of 8 x 8 tiles, at most 256 px a side (record boxes are 8 bits per bound)
+int super_shift(int T) { const int s = tile_shift(T) + kSuperShift; return s < kSuperMaxShift ? s : kSuperMaxShift; }
+
 size_t hist_bytes(int W, int H, int T)
 {
     const int ntx = (W + T - 1) / T, nty = (H + T - 1) / T;
-    const int S = T << kSuperShift;
+    const int S = 1 << super_shift(T);
     const int nsx = (W + S - 1) / S, nsy = (H + S - 1) / S;
     return sizeof(unsigned int) * ((size_t)ntx * nty + (size_t)nsx * nsy);
 }
@@ -116,6 +119,7 @@ bool make_layout(const splotch_ctx *c, unsigned long long n, int T, unsigned lon
     L->cls_counts = off;  off = align_up(off + sizeof(unsigned int) * 4 * L->nrows, 256);
     L->bin_count = off;   off = align_up(off + sizeof(unsigned int) * nbins, 256);
     L->bin_start = off;   off = align_up(off + sizeof(unsigned int) * (nbins + 1), 256);
+    L->large_off = off;   off = align_up(off + sizeof(unsigned int) * (nbins - n_tiles + 1), 256);
     // DeviceStats and the tiles' 64-bit sums sit together: one memset clears both before every frame
     L->stats = off;       off = align_up(off + sizeof(DeviceStats), 256);
     L->accum = off;
@@ -232,12 +236,11 @@ int check_params(splotch_ctx *c, const splotch_particles *p, unsigned long long 
     fp->T = q->tile; fp->tshift = ts;
     fp->ntx = (c->width + q->tile - 1) / q->tile; fp->nty = (c->height + q->tile - 1) / q->tile;
     fp->n_tiles = fp->ntx * fp->nty;
-    fp->sshift = ts + kSuperShift;
+    fp->sshift = super_shift(q->tile);
     const int S = 1 << fp->sshift;
     fp->nsx = (c->width + S - 1) / S; fp->nsy = (c->height + S - 1) / S;
     fp->n_super = fp->nsx * fp->nsy;
     fp->nbins = fp->n_tiles + fp->n_super;
-    if (fp->n_super > kMaxSuper) return fail(c, SPLOTCH_EINVAL, "tile %d gives %d super-tiles (at most %d); use a larger tile", q->tile, fp->n_super, kMaxSuper);
     fp->additive = q->additive ? 1 : 0;
     fp->apply_transfer = q->apply_transfer ? 1 : 0;
     fp->n_species = ns;
@@ -285,8 +288,9 @@ int launch_render_tail(splotch_ctx *c, const Layout &L, char *ws, const FramePar
     k_splat<T><<<grid, SplatCfg<T>::kThreads, Splat2Cfg<T>::kSmemBytes, st>>>(
         (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.bin_start), (DeviceStats *)(ws + L.stats), (unsigned long long *)(ws + L.accum), fp);
     if (c->profiling) cudaEventRecord(c->ev[4], st);
-    k_large<T><<<c->n_sm * c->large_blocks_per_sm[ti], kLargeThreads, 0, st>>>(
-        (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.bin_start), (DeviceStats *)(ws + L.stats), (unsigned long long *)(ws + L.accum), fp);
+    k_large<<<c->n_sm * c->large_blocks_per_sm, kLargeThreads, 0, st>>>(
+        (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.bin_start), (const unsigned int *)(ws + L.large_off),
+        (DeviceStats *)(ws + L.stats), (unsigned long long *)(ws + L.accum), fp);
     if (c->profiling) cudaEventRecord(c->ev[5], st);
     k_compose<T><<<fp.n_tiles, 256, 0, st>>>((const unsigned long long *)(ws + L.accum), (const DeviceStats *)(ws + L.stats), fp, image);
     if (c->profiling) cudaEventRecord(c->ev[6], st);
@@ -314,8 +318,10 @@ int render_device(splotch_ctx *c, const splotch_particles *p, unsigned long long
     if (al) k_count<true><<<L.nrows, kBinThreads, hbytes, st>>>(p->x, p->y, p->z, p->h, n, per, fp, counts, cls_counts);
     else    k_count<false><<<L.nrows, kBinThreads, hbytes, st>>>(p->x, p->y, p->z, p->h, n, per, fp, counts, cls_counts);
     if (c->profiling) cudaEventRecord(c->ev[1], st);
+    const int bps = 1 << (fp.sshift - 5);               // 32-px blocks per super-tile side (k_large's work items)
     k_scan<<<(fp.nbins + 31) / 32, kScanThreads, 0, st>>>(counts, L.nrows, fp.nbins, fp.n_tiles, bin_count, bin_start, cls_counts, L.capacity,
-                                                          c->n_sm, stats);
+                                                          c->n_sm, (unsigned int *)(ws + L.large_off), (unsigned int)kLargeChunk,
+                                                          (unsigned int)(bps * bps), stats);
     if (c->profiling) cudaEventRecord(c->ev[2], st);
     if (al) k_scatter<true><<<L.nrows, kBinThreads, hbytes, st>>>(p->x, p->y, p->z, p->h, p->I, p->scalar, n, per, fp, counts,
                                                                   bin_start, stats, (float4 *)(ws + L.records));
@@ -466,10 +472,8 @@ int splotch_create(splotch_ctx **out, int device, int width, int height, uint64_
         CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->orender_blocks_per_sm[1], k_orender<16>, SplatCfg<16>::kThreads, 0));
         CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->orender_blocks_per_sm[2], k_orender<32>, SplatCfg<32>::kThreads, 0));
         for (int k = 0; k < 3; ++k) if (c->orender_blocks_per_sm[k] < 1) c->orender_blocks_per_sm[k] = 1;
-        CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->large_blocks_per_sm[0], k_large<8>, kLargeThreads, 0));
-        CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->large_blocks_per_sm[1], k_large<16>, kLargeThreads, 0));
-        CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->large_blocks_per_sm[2], k_large<32>, kLargeThreads, 0));
-        for (int k = 0; k < 3; ++k) if (c->large_blocks_per_sm[k] < 1) c->large_blocks_per_sm[k] = 1;
+        CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->large_blocks_per_sm, k_large, kLargeThreads, 0));
+        if (c->large_blocks_per_sm < 1) c->large_blocks_per_sm = 1;
         return r;
     }();
     if (rc != SPLOTCH_OK) {

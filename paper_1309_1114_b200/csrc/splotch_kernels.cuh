@@ -33,7 +33,8 @@ constexpr int kMaxLut       = 1024;
 constexpr int kChunkMax     = 32768;  // records per work item of k_splat (upper bound; the frame picks its own)
 constexpr int kChunkMin     = 128;
 constexpr int kBinThreads   = 1024;   // k_count / k_scatter block size: one CTA per SM (fewer histogram rows and write streams than 2 x 512)
-constexpr int kSuperShift   = 3;      // super-tile = 8 x 8 tiles (LARGE particles are binned to super-tiles)
+constexpr int kSuperShift   = 3;      // super-tile = 8 x 8 tiles, at most 256 px (LARGE particles are binned to super-tiles)
+constexpr int kSuperMaxShift = 8;
 constexpr int kLutSmemMax   = 1024;   // colour-table entries (all species together) staged in shared memory by k_scatter
 constexpr int kFixedBits    = 30;     // the largest record amplitude maps to [2^29, 2^30) fixed-point units
 
@@ -315,11 +316,11 @@ __device__ __forceinline__ unsigned long long block_excl_scan_256(unsigned long 
 __global__ void __launch_bounds__(kScanThreads)
 k_scan(unsigned int *__restrict__ counts, int nrows, int nbins, int n_tiles, unsigned int *__restrict__ bin_count,
        unsigned int *__restrict__ bin_start, const unsigned int *__restrict__ cls_counts, unsigned long long capacity, int n_sm,
-       DeviceStats *__restrict__ stats)
+       unsigned int *__restrict__ large_off, unsigned int large_chunk, unsigned int large_blocks, DeviceStats *__restrict__ stats)
 {
     __shared__ unsigned int s_part[8][32];
     __shared__ unsigned long long s_warp[kScanThreads / 32];
-    __shared__ unsigned long long s_tot_pairs, s_tot_all;
+    __shared__ unsigned long long s_tot_pairs, s_tot_all, s_tot_items;
     __shared__ unsigned int s_ticket, s_cls[4];
     {
         const int bin = blockIdx.x * 32 + (threadIdx.x & 31), g = threadIdx.x >> 5;
@@ -410,6 +411,19 @@ k_scan(unsigned int *__restrict__ counts, int nrows, int nbins, int n_tiles, uns
         }
     }
     if (threadIdx.x == kScanThreads - 1) bin_start[nbins] = (unsigned int)s_tot_all;
+    {   // work items of k_large: (chunk of a super-tile's records) x (block of the super-tile), exclusive prefix over the super-tiles
+        const int n_super = nbins - n_tiles;
+        const int sper = (n_super + kScanThreads - 1) / kScanThreads;
+        const int s0 = min(n_super, (int)threadIdx.x * sper), s1 = min(n_super, s0 + sper);
+        unsigned long long items = 0;
+        for (int sb = s0; sb < s1; ++sb) items += (unsigned long long)((__ldcg(bin_count + n_tiles + sb) + large_chunk - 1) / large_chunk) * large_blocks;
+        unsigned long long irun = block_excl_scan_256(items, s_warp, &s_tot_items);
+        for (int sb = s0; sb < s1; ++sb) {
+            large_off[sb] = overflow ? 0u : (unsigned int)irun;
+            irun += (unsigned long long)((__ldcg(bin_count + n_tiles + sb) + large_chunk - 1) / large_chunk) * large_blocks;
+        }
+        if (threadIdx.x == kScanThreads - 1) large_off[n_super] = overflow ? 0u : (unsigned int)irun;
+    }
     if (threadIdx.x < 4) stats->count[threadIdx.x] = s_cls[threadIdx.x];      // block scans above synchronised
     if (threadIdx.x == 0) {
         stats->pairs = s_tot_pairs;

@@ -1,85 +1,61 @@
-// splotch_large.cuh -- A6, the cooperative path for LARGE particles (r(p) > r_0), and A8, the epilogue (sm_100a).
+// splotch_large.cuh -- A6, the cooperative path for LARGE particles (r(p) > r_0) (sm_100a).
 //
 // The paper renders large particles on the CPU while the GPU works on the rest and names the
 // resulting imbalance as its bottleneck for R_0 > 2 (:324).  Here they stay on the GPU: k_scatter files each LARGE
-// particle under every 8 x 8-tile super-tile its box touches, and k_large splits the work into (chunk of a super-tile's
-// records) x (tile of that super-tile) items that CTAs take from an atomic counter, so a tile covered by hundreds of
-// thousands of large discs (camera inside a halo, cfg3) is shared by many CTAs instead of serialising one
-// (the first version gave every tile to one CTA: 494 ms for cfg3, 58 % of the issue slots, profiles/r1_step4_*).
+// particle under every super-tile (up to 256 x 256 px) its box touches, and k_large splits the work into items of
+// (chunk of a super-tile's records) x (32 x 32-pixel block of that super-tile) that CTAs take from an atomic counter,
+// so a region covered by hundreds of thousands of large discs (camera inside a halo, cfg3) is shared by many CTAs.
 //   * the chunk's records stream through shared memory with bulk copies on mbarriers, as in k_splat;
-//   * every thread tests one record's box against the tile; survivors are compacted in order (deterministic sums);
-//   * pixel owners: a thread owns kPpt horizontally adjacent pixels, every pixel of a large disc is a useful lane;
-//   * an item ends with 64-bit fixed-point reductions into the tile's sums in L2 (exact, commutative), the same sums
+//   * every thread tests two records per window against the block (box, then disc against the block's rectangle of
+//     pixel centres) and sorts the survivors into two lists: discs that contain the whole block, and the others;
+//   * pixel owners: a thread owns 8 horizontally adjacent pixels and keeps their sums in registers as packed pairs;
+//       - block inside the disc: no clip test is needed, and the Gaussian along the row follows the recurrence
+//         w(x+2) = w(x) h(x), h(x+2) = h(x) q^8 with h(x) = exp2(c (4 dx + 4)), q^8 = exp2(8 c): four ex2 per 8 pixels
+//         instead of eight (round 1 was bound by MUFU.EX2, one per evaluated pixel, profiles/r1_step5_*);
+//       - otherwise: the C1 inside test of every pixel (bit-exact d2, packed), one ex2 per pixel;
+//   * an item ends with 64-bit fixed-point reductions into the tiles' sums in L2 (exact, commutative), the same sums
 //     k_splat feeds; k_compose turns them into the float32 image.
+// Blocks are 32 x 32 px whatever the tile side T is (a thread's 8-pixel run never straddles a tile).
 #pragma once
 #include "splotch_kernels.cuh"
 #include "splotch_splat.cuh"
 
 namespace splotch {
 
-constexpr int kLargeThreads = 256;
-constexpr int kLargeWin = 256;            // records per bulk copy
+constexpr int kLargeThreads = 128;
+constexpr int kLargeWin = 256;            // records per bulk copy; every thread tests two of them
 constexpr int kLargeStages = 2;
 constexpr int kLargeChunk = 4096;         // records per work item
-constexpr int kMaxSuper = 1024;           // super-tiles an image can have (the per-CTA histograms of k_count bound it)
+constexpr int kLargeBlock = 32;           // block side in px
+constexpr int kLargePpt = 8;              // pixels per thread (one row segment)
 
-template <int T>
 __global__ void __launch_bounds__(kLargeThreads)
-k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin_start, DeviceStats *__restrict__ stats,
+k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin_start,
+        const unsigned int *__restrict__ large_off, DeviceStats *__restrict__ stats,
         unsigned long long *__restrict__ accum, const __grid_constant__ FrameParams fp)
 {
-    constexpr int kPix = T * T;
-    constexpr int kPpt = (kPix + kLargeThreads - 1) / kLargeThreads;
-    constexpr int kTilesPerSuper = 1 << (2 * kSuperShift);
     __shared__ __align__(128) float4 stage[kLargeStages][kLargeWin][2];
     __shared__ float4 sA[kLargeWin], sB[kLargeWin];
-    __shared__ unsigned int s_off[kMaxSuper + 1];                 // first item of every super-tile
-    __shared__ unsigned int s_part[kLargeThreads / 32];
     __shared__ unsigned long long mbar[kLargeStages];
-    __shared__ int s_woff[kLargeThreads / 32];
+    __shared__ int s_cnt[kLargeThreads / 32][2];
     __shared__ unsigned int s_item;
+    __shared__ int s_sup;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     if (stats->overflow || stats->large_pairs == 0ull) return;          // no LARGE particle in this frame
-    // ---- item table: items of super-tile s = ceil(records / kLargeChunk) * 64, exclusive prefix over s
     const int n_super = fp.n_super;
-    {
-        const int per = (n_super + kLargeThreads - 1) / kLargeThreads;
-        const int b0 = min(n_super, (int)threadIdx.x * per), b1 = min(n_super, b0 + per);
-        unsigned int sum = 0u;
-        for (int s = b0; s < b1; ++s) {
-            const unsigned int c = bin_start[fp.n_tiles + s + 1] - bin_start[fp.n_tiles + s];
-            sum += (c + kLargeChunk - 1) / kLargeChunk * kTilesPerSuper;
-        }
-        unsigned int inc = sum;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const unsigned int t = __shfl_up_sync(0xffffffffu, inc, o);
-            if (lane >= o) inc += t;
-        }
-        if (lane == 31) s_part[warp] = inc;
-        __syncthreads();
-        unsigned int run = inc - sum;
-        for (int w = 0; w < warp; ++w) run += s_part[w];
-        for (int s = b0; s < b1; ++s) {
-            const unsigned int c = bin_start[fp.n_tiles + s + 1] - bin_start[fp.n_tiles + s];
-            s_off[s] = run;
-            run += (c + kLargeChunk - 1) / kLargeChunk * kTilesPerSuper;
-        }
-        if (threadIdx.x == kLargeThreads - 1) s_off[n_super] = run;
-        if (threadIdx.x == 0) {
-            for (int s = 0; s < kLargeStages; ++s) mbar_init(smem_u32(mbar + s), 1u);
-            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        }
-        __syncthreads();
-    }
-    const unsigned int total = s_off[n_super];
+    const unsigned int total = large_off[n_super];
     if (total == 0u) return;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < kLargeStages; ++s) mbar_init(smem_u32(mbar + s), 1u);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
     const int e = fixed_exponent(stats->amax_bits);
     const float sc1 = pow2i(e / 2), sc2 = pow2i(e - e / 2);
-    // this thread's pixels inside the tile: kPpt adjacent ones in one row
-    const int p0 = threadIdx.x * kPpt;
-    const bool owner = p0 < kPix;
-    const int row = owner ? p0 / T : 0, col0 = owner ? p0 % T : 0;
+    const int bps = 1 << (fp.sshift - 5);                               // blocks per super-tile side
+    const int nblk = bps * bps;
+    const int T = fp.T, tmask = T - 1, kPix = T * T;
+    // this thread's pixels inside the block: 8 adjacent ones of one row
+    const int row = threadIdx.x >> 2, col0 = (threadIdx.x & 3) * kLargePpt;
     unsigned int wcount = 0u;
     auto issue = [&](unsigned int wbase, unsigned int j, unsigned int r0, unsigned int r1) {
         const unsigned int s = (wbase + j) % kLargeStages;
@@ -90,108 +66,171 @@ k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
     };
     for (;;) {
         __syncthreads();
-        if (threadIdx.x == 0) s_item = atomicAdd(&stats->large_counter, 1u);
+        if (warp == 0) {
+            // next item, and its super-tile: the last s with large_off[s] <= item, by a 32-way search
+            unsigned int it = 0u;
+            if (lane == 0) it = atomicAdd(&stats->large_counter, 1u);
+            it = __shfl_sync(0xffffffffu, it, 0);
+            if (it < total) {
+                int lo = 0, n = n_super;
+                while (n > 1) {
+                    const int step = (n + 31) / 32;
+                    const int t = lo + lane * step;
+                    const bool le = t < lo + n && __ldg(large_off + t) <= it;
+                    const int k = __popc(__ballot_sync(0xffffffffu, le)) - 1;
+                    lo += k * step;
+                    n = min(step, n - k * step);
+                }
+                if (lane == 0) s_sup = lo;
+            }
+            if (lane == 0) s_item = it;
+        }
         __syncthreads();
         const unsigned int item = s_item;
         if (item >= total) break;
-        // super-tile of the item: the last s with s_off[s] <= item (items of one chunk, 64 tiles, are neighbours:
-        // the CTAs that work on them read the same records at about the same time, from L2)
-        int lo = 0, hi = n_super;
-        while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (s_off[mid] <= item) lo = mid; else hi = mid; }
-        const int sup = lo;
-        const unsigned int local = item - s_off[sup];
-        const unsigned int chunk = local >> (2 * kSuperShift);
-        const int tin = (int)(local & (kTilesPerSuper - 1));
-        const int tx = ((sup % fp.nsx) << kSuperShift) + (tin & ((1 << kSuperShift) - 1));
-        const int ty = ((sup / fp.nsx) << kSuperShift) + (tin >> kSuperShift);
-        if (tx >= fp.ntx || ty >= fp.nty) continue;              // the super-tile hangs over the image edge
-        const int tile = ty * fp.ntx + tx;
-        const int tx0 = tx * T, ty0 = ty * T;
+        const int sup = s_sup;
+        const unsigned int local = item - large_off[sup];
+        const unsigned int chunk = local / (unsigned int)nblk;
+        const int blk = (int)(local % (unsigned int)nblk);
+        // block origin inside the super-tile and on the screen (record boxes are relative to the super-tile)
+        const int qx0 = (blk % bps) * kLargeBlock, qy0 = (blk / bps) * kLargeBlock;
+        const int X0 = ((sup % fp.nsx) << fp.sshift) + qx0, Y0 = ((sup / fp.nsx) << fp.sshift) + qy0;
+        if (X0 >= fp.W || Y0 >= fp.H) continue;                  // the super-tile hangs over the image edge
+        const int qx1 = qx0 + kLargeBlock - 1, qy1 = qy0 + kLargeBlock - 1;
         const unsigned int lb = bin_start[fp.n_tiles + sup], le = bin_start[fp.n_tiles + sup + 1];
         const unsigned int r0 = lb + chunk * kLargeChunk, r1 = min(r0 + kLargeChunk, le);
         const unsigned int nwin = (r1 - r0 + kLargeWin - 1) / kLargeWin;
         const unsigned int wbase = wcount;
         if (threadIdx.x == 0)
             for (unsigned int j = 0; j < min(nwin, (unsigned int)kLargeStages); ++j) issue(wbase, j, r0, r1);
-        // the tile inside its super-tile, in pixels (record boxes are relative to the super-tile)
-        const int qx0 = (tin & ((1 << kSuperShift) - 1)) * T, qy0 = (tin >> kSuperShift) * T;
-        const int qx1 = qx0 + T - 1, qy1 = qy0 + T - 1;
-        // centres of the tile's corner pixels
-        const float cxl = __fadd_rn((float)tx0, 0.5f), cxh = __fadd_rn((float)(tx0 + T - 1), 0.5f);
-        const float cyl = __fadd_rn((float)ty0, 0.5f), cyh = __fadd_rn((float)(ty0 + T - 1), 0.5f);
-        float acc[kPpt][3], sub[kPpt][3], fxc[kPpt];
-        const float fyc = __fadd_rn((float)(ty0 + row), 0.5f);
+        // centres of the block's corner pixels
+        const float cxl = __fadd_rn((float)X0, 0.5f), cxh = __fadd_rn((float)(X0 + kLargeBlock - 1), 0.5f);
+        const float cyl = __fadd_rn((float)Y0, 0.5f), cyh = __fadd_rn((float)(Y0 + kLargeBlock - 1), 0.5f);
+        const float fyc = __fadd_rn((float)(Y0 + row), 0.5f);
+        const float fx0 = __fadd_rn((float)(X0 + col0), 0.5f);
+        f32x2 fxp[kLargePpt / 2], acc[kLargePpt / 2][3], sub[kLargePpt / 2][3];
 #pragma unroll
-        for (int k = 0; k < kPpt; ++k) {
-            acc[k][0] = acc[k][1] = acc[k][2] = 0.0f;
-            sub[k][0] = sub[k][1] = sub[k][2] = 0.0f;
-            fxc[k] = __fadd_rn((float)(tx0 + col0 + k), 0.5f);
+        for (int j = 0; j < kLargePpt / 2; ++j) {
+            fxp[j] = pk2(__fadd_rn((float)(X0 + col0 + 2 * j), 0.5f), __fadd_rn((float)(X0 + col0 + 2 * j + 1), 0.5f));
+#pragma unroll
+            for (int c = 0; c < 3; ++c) acc[j][c] = sub[j][c] = 0ull;
         }
         for (unsigned int k = 0; k < nwin; ++k, ++wcount) {
             const unsigned int st = wcount % kLargeStages;
             mbar_wait(smem_u32(mbar + st), (wcount / kLargeStages) & 1u);
             const unsigned int wb = r0 + k * kLargeWin, cntw = min(wb + kLargeWin, r1) - wb;
-            bool hit = false;
-            float4 ra = make_float4(0.f, 0.f, 0.f, 0.f), rb = ra;
-            if (threadIdx.x < cntw) {
-                ra = stage[st][threadIdx.x][0]; rb = stage[st][threadIdx.x][1];
-                const unsigned int box = __float_as_uint(rb.w);
-                const int bx0 = (int)(box & 255u), by0 = (int)((box >> 8) & 255u);
-                const int bx1 = (int)((box >> 16) & 255u), by1 = (int)(box >> 24);
-                hit = bx0 <= qx1 && bx1 >= qx0 && by0 <= qy1 && by1 >= qy0;
-                if (hit) {
-                    // the disc against the tile: skip it when even the nearest point of the tile's pixel-centre
-                    // rectangle is outside (with a margin that covers the float32 rounding of the C1 test)
-                    const float nx = fmaxf(fmaxf(cxl - ra.x, ra.x - cxh), 0.0f), ny = fmaxf(fmaxf(cyl - ra.y, ra.y - cyh), 0.0f);
-                    hit = fmaf(nx, nx, ny * ny) <= ra.w * 1.0001f;
+            // ---- test two records per thread: 0 = miss, 1 = the disc contains the block, 2 = the disc cuts the block
+            float4 ra[2], rb[2];
+            int kind[2];
+#pragma unroll
+            for (int t = 0; t < 2; ++t) {
+                const unsigned int idx = threadIdx.x + t * kLargeThreads;
+                kind[t] = 0;
+                ra[t] = rb[t] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (idx < cntw) {
+                    ra[t] = stage[st][idx][0]; rb[t] = stage[st][idx][1];
+                    const unsigned int box = __float_as_uint(rb[t].w);
+                    const int bx0 = (int)(box & 255u), by0 = (int)((box >> 8) & 255u);
+                    const int bx1 = (int)((box >> 16) & 255u), by1 = (int)(box >> 24);
+                    if (bx0 <= qx1 && bx1 >= qx0 && by0 <= qy1 && by1 >= qy0) {
+                        // nearest and farthest point of the block's rectangle of pixel centres (margins cover the
+                        // float32 rounding of the C1 test: a skipped block has no pixel inside, a "contained" block none outside)
+                        const float ax = cxl - ra[t].x, bx = ra[t].x - cxh, ay = cyl - ra[t].y, by = ra[t].y - cyh;
+                        const float nx = fmaxf(fmaxf(ax, bx), 0.0f), ny = fmaxf(fmaxf(ay, by), 0.0f);
+                        const float gx = fmaxf(-ax, -bx), gy = fmaxf(-ay, -by);         // farthest: max(|cxl - px|, |cxh - px|)
+                        if (fmaf(nx, nx, ny * ny) <= ra[t].w * 1.0001f)
+                            kind[t] = (fmaf(gx, gx, gy * gy) <= ra[t].w * 0.9999f && bx0 <= qx0 && bx1 >= qx1 && by0 <= qy0 && by1 >= qy1) ? 1 : 2;
+                    }
                 }
             }
-            const unsigned int bal = __ballot_sync(0xffffffffu, hit);
-            if (lane == 0) s_woff[warp] = __popc(bal);
-            __syncthreads();                 // counts visible; every warp is done with the previous window's hits
+            const unsigned int mi0 = __ballot_sync(0xffffffffu, kind[0] == 1), mi1 = __ballot_sync(0xffffffffu, kind[1] == 1);
+            const unsigned int mb0 = __ballot_sync(0xffffffffu, kind[0] == 2), mb1 = __ballot_sync(0xffffffffu, kind[1] == 2);
+            if (lane == 0) { s_cnt[warp][0] = __popc(mi0) + __popc(mi1); s_cnt[warp][1] = __popc(mb0) + __popc(mb1); }
+            __syncthreads();                 // counts visible; every warp is done with the previous window's lists
             // the stage of the previous window is free now: refill it
             if (k >= 1u && threadIdx.x == 0 && k - 1u + kLargeStages < nwin) issue(wbase, k - 1u + kLargeStages, r0, r1);
-            int woff = 0, cnt = 0;
+            int ioff = 0, boff = 0, n_in = 0, n_cut = 0;
 #pragma unroll
-            for (int w = 0; w < kLargeThreads / 32; ++w) { const int c = s_woff[w]; woff += w < warp ? c : 0; cnt += c; }
-            if (hit) {
-                const int pos = woff + __popc(bal & ((1u << lane) - 1u));
-                sA[pos] = ra; sB[pos] = rb;
+            for (int w = 0; w < kLargeThreads / 32; ++w) {
+                const int ci = s_cnt[w][0], cb = s_cnt[w][1];
+                ioff += w < warp ? ci : 0; boff += w < warp ? cb : 0;
+                n_in += ci; n_cut += cb;
+            }
+            const unsigned int lt = (1u << lane) - 1u;
+#pragma unroll
+            for (int t = 0; t < 2; ++t) {
+                if (kind[t] == 1) {           // the list of containing discs grows from the front
+                    const int pos = ioff + (t ? __popc(mi0) : 0) + __popc((t ? mi1 : mi0) & lt);
+                    sA[pos] = ra[t];
+                    sB[pos] = make_float4(rb[t].x, rb[t].y, rb[t].z, ex2_approx(8.0f * ra[t].z));      // q^8
+                } else if (kind[t] == 2) {    // the list of cutting discs grows from the back
+                    const int pos = kLargeWin - 1 - (boff + (t ? __popc(mb0) : 0) + __popc((t ? mb1 : mb0) & lt));
+                    sA[pos] = ra[t];
+                    sB[pos] = rb[t];
+                }
             }
             __syncthreads();
-            if (owner) {
-                for (int m = 0; m < cnt; ++m) {
-                    const float4 a = sA[m], b = sB[m];
-                    const float dyf = __fsub_rn(fyc, a.y);
-                    const float t2 = __fmul_rn(dyf, dyf);
+            // ---- discs that contain the block: recurrence along the row, no clip test
+            for (int m = 0; m < n_in; ++m) {
+                const float4 a = sA[m], b = sB[m];
+                const float dy = fyc - a.y, dx0 = fx0 - a.x;
+                const float d20 = fmaf(dx0, dx0, dy * dy);
+                const float d21 = d20 + fmaf(2.0f, dx0, 1.0f);
+                const float u0 = fmaf(4.0f, dx0, 4.0f);
+                f32x2 P = pk2(ex2_approx(a.z * d20), ex2_approx(a.z * d21));
+                f32x2 H = pk2(ex2_approx(a.z * u0), ex2_approx(a.z * (u0 + 4.0f)));
+                const f32x2 Q = pk2(b.w, b.w), BR = pk2(b.x, b.x), BG = pk2(b.y, b.y), BB = pk2(b.z, b.z);
 #pragma unroll
-                    for (int q = 0; q < kPpt; ++q) {
-                        const float dxf = __fsub_rn(fxc[q], a.x);
-                        const float d2 = __fmaf_rn(dxf, dxf, t2);
-                        const float wgt = d2 <= a.w ? ex2_approx(d2 * a.z) : 0.0f;
-                        sub[q][0] = fmaf(b.x, wgt, sub[q][0]);
-                        sub[q][1] = fmaf(b.y, wgt, sub[q][1]);
-                        sub[q][2] = fmaf(b.z, wgt, sub[q][2]);
-                    }
+                for (int j = 0; j < kLargePpt / 2; ++j) {
+                    sub[j][0] = ffma2(BR, P, sub[j][0]); sub[j][1] = ffma2(BG, P, sub[j][1]); sub[j][2] = ffma2(BB, P, sub[j][2]);
+                    if (j + 1 < kLargePpt / 2) P = fmul2(P, H);
+                    if (j + 2 < kLargePpt / 2) H = fmul2(H, Q);
+                }
+            }
+            // ---- discs that cut the block: the C1 inside test per pixel
+            for (int m = 0; m < n_cut; ++m) {
+                const float4 a = sA[kLargeWin - 1 - m], b = sB[kLargeWin - 1 - m];
+                const float dyf = __fsub_rn(fyc, a.y);
+                const float t2 = __fmul_rn(dyf, dyf);
+                const f32x2 T2 = pk2(t2, t2), NX = pk2(-a.x, -a.x), C = pk2(a.z, a.z);
+                const f32x2 BR = pk2(b.x, b.x), BG = pk2(b.y, b.y), BB = pk2(b.z, b.z);
+#pragma unroll
+                for (int j = 0; j < kLargePpt / 2; ++j) {
+                    const f32x2 dx = fadd2(fxp[j], NX);
+                    const f32x2 d2 = ffma2(dx, dx, T2);
+                    const f32x2 arg = fmul2(d2, C);
+                    float d2a, d2b, aa, ab;
+                    upk2(d2, d2a, d2b); upk2(arg, aa, ab);
+                    const float wa = d2a <= a.w ? ex2_approx(aa) : 0.0f;
+                    const float wb2 = d2b <= a.w ? ex2_approx(ab) : 0.0f;
+                    const f32x2 Wp = pk2(wa, wb2);
+                    sub[j][0] = ffma2(BR, Wp, sub[j][0]); sub[j][1] = ffma2(BG, Wp, sub[j][1]); sub[j][2] = ffma2(BB, Wp, sub[j][2]);
                 }
             }
             if ((k & 3u) == 3u || k + 1u == nwin) {              // two-level sums: fold the sub-sums every 4 windows
 #pragma unroll
-                for (int q = 0; q < kPpt; ++q)
+                for (int j = 0; j < kLargePpt / 2; ++j)
 #pragma unroll
-                    for (int c = 0; c < 3; ++c) { acc[q][c] += sub[q][c]; sub[q][c] = 0.0f; }
+                    for (int c = 0; c < 3; ++c) { acc[j][c] = fadd2(acc[j][c], sub[j][c]); sub[j][c] = 0ull; }
             }
         }
-        // ---- the item's sums -> the tile's 64-bit fixed-point sums
-        if (owner) {
-            unsigned long long *out = accum + (size_t)tile * (3 * kPix) + p0;
+        // ---- the item's sums -> the tiles' 64-bit fixed-point sums
+        {
+            const int X = X0 + col0, Y = Y0 + row;
+            const int tx = X >> fp.tshift, ty = Y >> fp.tshift;
+            if (tx < fp.ntx && ty < fp.nty) {
+                unsigned long long *out = accum + (size_t)(ty * fp.ntx + tx) * (3 * kPix) + (Y & tmask) * T + (X & tmask);
 #pragma unroll
-            for (int q = 0; q < kPpt; ++q)
+                for (int j = 0; j < kLargePpt / 2; ++j)
 #pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    const long long f = __float2ll_rn(acc[q][c] * sc1 * sc2);
-                    if (f != 0ll) atomicAdd(out + c * kPix + q, (unsigned long long)f);
-                }
+                    for (int c = 0; c < 3; ++c) {
+                        float v0, v1;
+                        upk2(acc[j][c], v0, v1);
+                        const long long f0 = __float2ll_rn(v0 * sc1 * sc2), f1 = __float2ll_rn(v1 * sc1 * sc2);
+                        if (f0 != 0ll) atomicAdd(out + c * kPix + 2 * j, (unsigned long long)f0);
+                        if (f1 != 0ll) atomicAdd(out + c * kPix + 2 * j + 1, (unsigned long long)f1);
+                    }
+            }
         }
     }
 }

@@ -158,9 +158,10 @@ def halo_table(seed: int, n_halos: int = 50):
     return mass, scale, centre
 
 
-def _single_plummer(seed: int, n: int, device) -> Dict[str, torch.Tensor]:
-    out = {f: torch.empty(n, dtype=torch.float32, device=device) for f in FIELD_NAMES}
-    for s, e in _chunks(n, 1 << 22):
+def _single_plummer(seed: int, n: int, device, count: Optional[int] = None) -> Dict[str, torch.Tensor]:
+    count = n if count is None else min(count, n)
+    out = {f: torch.empty(count, dtype=torch.float32, device=device) for f in FIELD_NAMES}
+    for s, e in _chunks(count, 1 << 22):
         idx = torch.arange(s, e, dtype=torch.int64, device=device)
         dx, dy, dz, _ = _plummer_offset(seed, idx, 0, 0.1)
         out["x"][s:e] = (0.5 + dx).to(torch.float32)
@@ -172,17 +173,23 @@ def _single_plummer(seed: int, n: int, device) -> Dict[str, torch.Tensor]:
     return out
 
 
-def _halo_set(seed: int, n: int, eta: float, device, star_begin: Optional[int] = None):
-    """50 Plummer halos + 20 % uniform background; h from the analytic local number density."""
+def _halo_set(seed: int, n: int, eta: float, device, star_begin: Optional[int] = None, count: Optional[int] = None):
+    """50 Plummer halos + 20 % uniform background; h from the analytic local number density.
+
+    `count` draws only particles [0, count) of the n-particle set (the generator is counter based, so these are the
+    same particles the full set starts with; densities and smoothing lengths are those of the full set).  The
+    scalar range is then the analytic one of the full set: [log10(0.2 n), log10 of the densest halo centre]."""
     mass, scale, centre = halo_table(seed)
     msum = float(mass.sum())
     cum = (torch.cumsum(mass, 0) / msum).to(device)
     cum[-1] = 1.0
     mass_d, scale_d, centre_d = mass.to(device), scale.to(device), centre.to(device)
     n_bg = 0.2 * n
-    out = {f: torch.empty(n, dtype=torch.float32, device=device) for f in FIELD_NAMES}
+    partial = count is not None and count < n
+    count = n if count is None else min(count, n)
+    out = {f: torch.empty(count, dtype=torch.float32, device=device) for f in FIELD_NAMES}
     dmin, dmax = math.inf, -math.inf
-    for s, e in _chunks(n, 1 << 22):
+    for s, e in _chunks(count, 1 << 22):
         idx = torch.arange(s, e, dtype=torch.int64, device=device)
         is_bg = uniform(seed, idx, 0) < 0.2
         hk = torch.clamp(torch.searchsorted(cum, uniform(seed, idx, 1)), max=mass.numel() - 1)
@@ -208,6 +215,9 @@ def _halo_set(seed: int, n: int, eta: float, device, star_begin: Optional[int] =
         out["I"][s:e] = inten.to(torch.float32)
         dmin = min(dmin, float(sc.min()))
         dmax = max(dmax, float(sc.max()))
+    if partial:      # the prefix does not see the extremes of the full set: use the analytic bounds of the recipe
+        dmin = math.log10(n_bg)
+        dmax = math.log10(n_bg + float((3.0 * (0.8 * n * mass / msum) / (4.0 * math.pi * scale ** 3)).max()))
     info = {"scalar_min": dmin, "scalar_max": dmax, "halo_mass": mass, "halo_scale": scale,
             "halo_centre": centre}
     return out, info
@@ -221,21 +231,33 @@ def orbit_camera(frame: int, fov_deg: float = 45.0) -> Camera:
 
 
 def make_config(cfg: int, n: Optional[int] = None, device="cpu", size: Optional[Tuple[int, int]] = None,
-                eta: Optional[float] = None) -> Workload:
-    """Workload for BASELINE.json configs[cfg] (0-based). `n` / `size` shrink it for oracle-sized tests."""
+                eta: Optional[float] = None, count: Optional[int] = None) -> Workload:
+    """Workload for BASELINE.json configs[cfg] (0-based). `n` / `size` shrink it for oracle-sized tests.
+    `count` keeps the n-particle recipe (densities, smoothing lengths, camera) but draws only its first `count`
+    particles: a bounded sample of the same workload for the timed CPU baseline."""
+    w = _make_config(cfg, n, device, size, eta, count)
+    if count is not None and count < w.n:
+        w.meta["full_n"] = w.n
+        w.n = count
+        for sp in w.species:
+            sp.begin, sp.end = min(sp.begin, count), min(sp.end, count)
+    return w
+
+
+def _make_config(cfg, n, device, size, eta, count) -> Workload:
     seed = 1000 + cfg
     centre = (0.5, 0.5, 0.5)
     front = Camera((0.5, 0.5, 2.5), centre, (0.0, 1.0, 0.0), 45.0)
     if cfg == 0:
         n = 100_000 if n is None else n
         w, h = size or (256, 256)
-        f = _single_plummer(seed, n, device)
+        f = _single_plummer(seed, n, device, count)
         sp = [Species(0, n, brightness=1.0, scalar_min=-2.0, scalar_max=2.0, scalar_log10=True)]
         return Workload("cfg0_plummer_100k", n, w, h, f, sp, front)
     if cfg == 1:
         n = 10_000_000 if n is None else n
         w, h = size or (800, 800)
-        f, info = _halo_set(seed, n, 0.25 if eta is None else eta, device)
+        f, info = _halo_set(seed, n, 0.25 if eta is None else eta, device, count=count)
         sp = [Species(0, n, brightness=1.0, scalar_min=info["scalar_min"], scalar_max=info["scalar_max"])]
         return Workload("cfg1_halos_10M", n, w, h, f, sp, front, meta=info)
     if cfg in (2, 4):
@@ -243,7 +265,7 @@ def make_config(cfg: int, n: Optional[int] = None, device="cpu", size: Optional[
         w, h = size or (1920, 1080)
         n_gas = (6 * n) // 10
         f, info = _halo_set(seed if cfg == 2 else 1002, n, 0.25 if eta is None else eta, device,
-                            star_begin=n_gas)
+                            star_begin=n_gas, count=count)
         sp = [Species(0, n_gas, brightness=1.0, absorb=0.5, scalar_min=info["scalar_min"],
                       scalar_max=info["scalar_max"]),
               Species(n_gas, n, brightness=0.3, absorb=2.0, use_colormap=False,
@@ -257,7 +279,7 @@ def make_config(cfg: int, n: Optional[int] = None, device="cpu", size: Optional[
     if cfg == 3:
         n = 400_000_000 if n is None else n
         w, h = size or (4096, 4096)
-        f, info = _halo_set(seed, n, 1.5 if eta is None else eta, device)
+        f, info = _halo_set(seed, n, 1.5 if eta is None else eta, device, count=count)
         k = int(torch.argmax(info["halo_mass"]))
         c = info["halo_centre"][k]
         a = float(info["halo_scale"][k])
