@@ -69,6 +69,8 @@ class ClockSampler(threading.Thread):
     def __init__(self, index: int):
         super().__init__(daemon=True)
         self.index, self.stop_flag, self.sm, self.reasons, self.max_mhz = index, False, [], set(), None
+        self.t_begin = self.t_end = None          # the timed region (perf_counter); samples outside it are dropped
+        self.stamps, self.flags = [], []
         try:
             import pynvml
             pynvml.nvmlInit()
@@ -82,27 +84,42 @@ class ClockSampler(threading.Thread):
         if self.nv is None:
             return
         nv = self.nv
-        self.sm.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+        t = time.perf_counter()
+        mhz = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
         try:
             r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
         except Exception:
             r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
-        names = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
-                 0x80: "hw_power_brake", 0x2: "applications_clocks_setting"}
-        for bit, name in names.items():
-            if r & bit:
-                self.reasons.add(name)
+        self.stamps.append(0.5 * (t + time.perf_counter()))
+        self.sm.append(mhz)
+        self.flags.append(r)
 
     def run(self):
+        # started BEFORE the timed region so that the first NVML call (slow) is not inside it; begin() / end() mark it
         while not self.stop_flag:
             self.sample()
-            time.sleep(0.0005 if len(self.sm) < 64 else 0.01)
+            time.sleep(0.0002 if len(self.sm) < 256 else 0.01)
+
+    def begin(self):
+        self.t_begin = time.perf_counter()
+
+    def end(self):
+        self.t_end = time.perf_counter()
+        self.stop_flag = True
 
     def result(self):
-        if not self.sm:
-            self.sample()
-        return {"sm_mhz": statistics.median(self.sm) if self.sm else None, "sm_max_mhz": self.max_mhz,
-                "reasons": sorted(self.reasons), "samples": len(self.sm)}
+        names = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+                 0x80: "hw_power_brake", 0x2: "applications_clocks_setting"}
+        inside = [i for i, t in enumerate(self.stamps)
+                  if self.t_begin is not None and self.t_end is not None and self.t_begin <= t <= self.t_end]
+        sm = [self.sm[i] for i in inside]
+        reasons = set()
+        for i in inside:
+            for bit, name in names.items():
+                if self.flags[i] & bit:
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(reasons), "samples": len(sm)}
 
 
 def ncu_traffic(kernel: str, workload: str):
@@ -229,9 +246,12 @@ class Run:
         assert self.r.stats()["overflow"] == 0, "pair capacity overflow"
         self.r.set_profiling(True)
         ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
-        barrier()
         if sampler is not None:
             sampler.start()
+            time.sleep(0.05)
+        barrier()
+        if sampler is not None:
+            sampler.begin()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
         for i in range(steps):
@@ -243,7 +263,7 @@ class Run:
         e1.record(stream)
         barrier()
         if sampler is not None:
-            sampler.stop_flag = True
+            sampler.end()
         per_frame = sorted(a.elapsed_time(b) for a, b in ev)
         # with an L2 flush between frames the step time is the sum of the frames' own event pairs
         ms_total = sum(per_frame) if self.flush else e0.elapsed_time(e1)

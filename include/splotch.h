@@ -119,7 +119,8 @@ int splotch_get_camera_constants(const splotch_ctx *ctx, float out[16]);
 int splotch_set_colormap(splotch_ctx *ctx, int species, const float *rgb, int n_entries);
 
 /* Record per-stage CUDA-event timings on the render stream during splotch_render.  splotch_get_stats then
- * returns, per stage, the mean over the frames rendered since this call (at most the last 256). */
+ * returns, per stage, the mean over the frames rendered since this call (at most the last 256).  A profiling
+ * session covers one mode and one stream: a frame of the other mode, or on another stream, starts it afresh. */
 int splotch_set_profiling(splotch_ctx *ctx, int enabled);
 
 /* Bytes of DEVICE scratch splotch_render needs for n particles, a tile side `tile` and room for
@@ -150,6 +151,11 @@ int splotch_render_host(splotch_ctx *ctx, const splotch_particles *host_particle
 /* Statistics of the last frame.  Synchronises the stream of that frame.  HOST out. */
 int splotch_get_stats(splotch_ctx *ctx, splotch_stats *out);
 const char *splotch_stage_name(int additive, int stage);   /* stage names of an additive / ordered frame */
+
+/* The two ALU rates the splat stages' roofline fractions are quoted against, measured on this context's device by
+ * a register-only microbenchmark: out[0] = FP32 FMA lane-operations per second (one FMA = one
+ * operation), out[1] = ex2.approx results per second, whole GPU.  HOST out; synchronises `cuda_stream`. */
+int splotch_measure_peaks(splotch_ctx *ctx, double out[2], void *cuda_stream);
 
 /* Test hooks: the per-particle results of the classification stage, written to DEVICE arrays of length n
  * (any may be NULL): cls int8; px, py (screen centre), sp (sigma in px), rp (r(p)), zc (camera depth)

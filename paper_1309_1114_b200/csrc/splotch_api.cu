@@ -5,6 +5,7 @@
 #include "splotch_splat.cuh"
 #include "splotch_large.cuh"
 #include "splotch_ordered.cuh"
+#include "splotch_peaks.cuh"
 #include "../../include/splotch.h"
 
 #include <math.h>
@@ -311,6 +312,7 @@ int render_device(splotch_ctx *c, const splotch_particles *p, unsigned long long
     unsigned int *bin_start = (unsigned int *)(ws + L.bin_start);
     DeviceStats *stats = (DeviceStats *)(ws + L.stats);
     if (c->profiling) {
+        if (c->prof_stages != kStagesAdditive || c->last_stream != st) c->prof_frames = 0;   // a session covers one mode and one stream
         c->ev = c->ev_ring[c->prof_frames % kProfRing];
         cudaEventRecord(c->ev[0], st);
     }
@@ -364,6 +366,7 @@ int render_ordered(splotch_ctx *c, const splotch_particles *p, unsigned long lon
     unsigned long long *keys[2] = {(unsigned long long *)(ws + L.keys[0]), (unsigned long long *)(ws + L.keys[1])};
     unsigned int *vals[2] = {(unsigned int *)(ws + L.vals[0]), (unsigned int *)(ws + L.vals[1])};
     if (c->profiling) {
+        if (c->prof_stages != kStagesOrdered || c->last_stream != st) c->prof_frames = 0;    // a session covers one mode and one stream
         c->ev = c->ev_ring[c->prof_frames % kProfRing];
         cudaEventRecord(c->ev[0], st);
     }
@@ -580,7 +583,8 @@ size_t splotch_workspace_bytes(const splotch_ctx *c, uint64_t n, int tile, uint6
     Layout L, Lo;
     make_layout(c, n, tile, pair_capacity, 0, with_host_staging != 0, &L);
     make_layout_ordered(c, n, tile, pair_capacity, with_host_staging != 0, &Lo);       // either mode must fit
-    return (L.total > Lo.total + 8192 ? L.total : Lo.total + 8192) + 4096;
+    // the same 8192-byte reserve on both sides: splotch_render derives its capacity as (bytes - fixed - 8192) / 32
+    return (L.total > Lo.total ? L.total : Lo.total) + 8192 + 4096;
 }
 
 int splotch_render(splotch_ctx *c, const splotch_particles *p, uint64_t n, const splotch_params *q, float *image_out,
@@ -661,6 +665,41 @@ int splotch_get_stats(splotch_ctx *c, splotch_stats *out)
         }
     }
     return SPLOTCH_OK;
+}
+
+int splotch_measure_peaks(splotch_ctx *c, double out[2], void *cuda_stream)
+{
+    if (!c || !out) return SPLOTCH_EINVAL;
+    CU_TRY(c, cudaSetDevice(c->device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int grid = 2 * c->n_sm;
+    float *buf = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    CU_TRY(c, cudaMalloc(&buf, sizeof(float) * (size_t)grid * kPeakThreads));
+    int rc = [&]() -> int {
+        CU_TRY(c, cudaEventCreate(&e0));
+        CU_TRY(c, cudaEventCreate(&e1));
+        const double ops = (double)grid * kPeakThreads * kPeakIters * kPeakChains;
+        for (int op = 0; op < 2; ++op) {
+            float best = 0.0f;
+            for (int rep = 0; rep < 4; ++rep) {           // the first launch warms up; keep the best of the rest
+                CU_TRY(c, cudaEventRecord(e0, st));
+                if (op == 0) k_peak<0><<<grid, kPeakThreads, 0, st>>>(buf, 0.3f);
+                else         k_peak<1><<<grid, kPeakThreads, 0, st>>>(buf, 0.3f);
+                CU_TRY(c, cudaEventRecord(e1, st));
+                CU_TRY(c, cudaEventSynchronize(e1));
+                float ms = 0.0f;
+                CU_TRY(c, cudaEventElapsedTime(&ms, e0, e1));
+                if (rep > 0 && (best == 0.0f || ms < best)) best = ms;
+            }
+            out[op] = ops / ((double)best * 1e-3);
+        }
+        return SPLOTCH_OK;
+    }();
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaFree(buf);
+    return rc;
 }
 
 int splotch_debug_geometry(splotch_ctx *c, const splotch_particles *p, uint64_t n, const splotch_params *q, int8_t *cls,

@@ -138,8 +138,12 @@ k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
                         const float ax = cxl - ra[t].x, bx = ra[t].x - cxh, ay = cyl - ra[t].y, by = ra[t].y - cyh;
                         const float nx = fmaxf(fmaxf(ax, bx), 0.0f), ny = fmaxf(fmaxf(ay, by), 0.0f);
                         const float gx = fmaxf(-ax, -bx), gy = fmaxf(-ay, -by);         // farthest: max(|cxl - px|, |cxh - px|)
-                        if (fmaf(nx, nx, ny * ny) <= ra[t].w * 1.0001f)
+                        if (fmaf(nx, nx, ny * ny) <= ra[t].w * 1.0001f) {
                             kind[t] = (fmaf(gx, gx, gy * gy) <= ra[t].w * 0.9999f && bx0 <= qx0 && bx1 >= qx1 && by0 <= qy0 && by1 >= qy1) ? 1 : 2;
+                            // the recurrence is used only where its factors cannot overflow: the largest |log2 h| inside the disc
+                            // is -c (4 r + 8); the weights themselves are at least exp2(c r^2) there
+                            if (kind[t] == 1 && !(-ra[t].z * (4.0f * sqrtf(ra[t].w) + 8.0f) < 120.0f && -ra[t].z * ra[t].w < 100.0f)) kind[t] = 2;
+                        }
                     }
                 }
             }
@@ -187,7 +191,8 @@ k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
                     if (j + 2 < kLargePpt / 2) H = fmul2(H, Q);
                 }
             }
-            // ---- discs that cut the block: the C1 inside test per pixel
+            // ---- discs that cut the block: the C1 inside test per pixel (bit-exact d2, packed), one ex2 per pixel (the
+            //      recurrence was measured here too: its extra multiplications cost more FMA-pipe time than the ex2 they save)
             for (int m = 0; m < n_cut; ++m) {
                 const float4 a = sA[kLargeWin - 1 - m], b = sB[kLargeWin - 1 - m];
                 const float dyf = __fsub_rn(fyc, a.y);
