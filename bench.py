@@ -188,8 +188,8 @@ def stage_bytes(additive: bool, w, st, passes: int):
     pairs = st["pairs"] + st["large_pairs"]
     active = st["n"] - st["count"][0]
     if additive:
-        rec_bytes = st.get("record_bytes", 32.0 * pairs)          # 16-byte SMALL records + 32-byte others
-        tile_rec_bytes = st.get("tile_record_bytes", 32.0 * st["pairs"])
+        rec_bytes = 32.0 * pairs - 16.0 * st["count"][1]          # a SMALL particle has one pair, a 16-byte record; the others 32 bytes
+        tile_rec_bytes = 32.0 * st["pairs"] - 16.0 * st["count"][1]
         return {
             "count": 16.0 * w.n,                                   # x y z h read once
             "scatter": 24.0 * w.n + rec_bytes,                     # six fields read, one record written per pair

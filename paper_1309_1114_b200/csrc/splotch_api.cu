@@ -25,7 +25,8 @@ const char *kStageNamesAdditive[kStagesAdditive] = {"count", "scan", "scatter", 
 const char *kStageNamesOrdered[kStagesOrdered] = {"count", "scan", "pairs", "sort", "bounds", "render", "combine"};
 
 struct Layout {
-    size_t counts, cls_counts, bin_count, bin_start, large_off, stats, accum, accum_bytes, records, staging, total;
+    size_t counts, counts_bytes, cls_counts, bin_count, vstart, large_off, run, stats, accum, accum_bytes, records, staging, total;
+    bool ghist;
     unsigned long long capacity;
     int nrows;
     // ordered mode
@@ -57,7 +58,7 @@ struct splotch_ctx {
     bool last_additive = true;
     int prof_stages = kStagesAdditive;              // stages of the frames recorded since profiling was enabled
     cudaStream_t last_stream = nullptr;
-    int splat_blocks_per_sm[3] = {0, 0, 0};  // T = 8, 16, 32
+    int splat_blocks_per_sm[4] = {0, 0, 0, 0};  // T = 8, 16, 32, 64
     int orender_blocks_per_sm[3] = {0, 0, 0};
     int large_blocks_per_sm = 0;
     char err[512] = {0};
@@ -85,7 +86,7 @@ int fail(splotch_ctx *c, int code, const char *fmt, ...)
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
-int tile_shift(int T) { return T == 8 ? 3 : T == 16 ? 4 : T == 32 ? 5 : -1; }
+int tile_shift(int T) { return T == 8 ? 3 : T == 16 ? 4 : T == 32 ? 5 : T == 64 ? 6 : -1; }
 
 // LARGE particles are binned to super-tiles of 8 x 8 tiles, at most 256 px a side (record boxes are 8 bits per bound)
 int super_shift(int T) { const int s = tile_shift(T) + kSuperShift; return s < kSuperMaxShift ? s : kSuperMaxShift; }
@@ -95,11 +96,17 @@ size_t hist_bytes(int W, int H, int T)
     const int ntx = (W + T - 1) / T, nty = (H + T - 1) / T;
     const int S = 1 << super_shift(T);
     const int nsx = (W + S - 1) / S, nsy = (H + S - 1) / S;
-    return sizeof(unsigned int) * ((size_t)ntx * nty + (size_t)nsx * nsy);
+    return sizeof(unsigned int) * (2 * (size_t)ntx * nty + (size_t)nsx * nsy);      // two bins per tile (MEDIUM, SMALL) + one per super-tile
 }
 
 // dynamic shared memory of k_count / k_scatter: the block's histogram / cursors plus room for the colour tables
 size_t bin_smem_bytes(int W, int H, int T) { return hist_bytes(W, H, T) + 16 + sizeof(float4) * kLutSmemMax; }
+
+// images with more bins than fit in shared memory (4096^2 at 16 px: 131,072 + 1,024 bins) keep the histogram / cursors
+// in the block's row of the count matrix instead (global atomics, L2 resident)
+bool use_global_hist(const splotch_ctx *c, int T);
+
+bool use_global_hist(const splotch_ctx *c, int T) { return bin_smem_bytes(c->width, c->height, T) + 1024 > (size_t)c->smem_optin; }
 
 int bin_rows(const splotch_ctx *c, int T)
 {
@@ -115,12 +122,14 @@ bool make_layout(const splotch_ctx *c, unsigned long long n, int T, unsigned lon
     const size_t n_tiles = (size_t)ntx * nty;
     const size_t nbins = hist_bytes(c->width, c->height, T) / sizeof(unsigned int);
     L->nrows = bin_rows(c, T);
+    L->ghist = use_global_hist(c, T);
     size_t off = 0;
-    L->counts = off;      off = align_up(off + sizeof(unsigned int) * nbins * L->nrows, 256);
+    L->counts = off;      L->counts_bytes = sizeof(unsigned int) * nbins * L->nrows; off = align_up(off + L->counts_bytes, 256);
     L->cls_counts = off;  off = align_up(off + sizeof(unsigned int) * 4 * L->nrows, 256);
     L->bin_count = off;   off = align_up(off + sizeof(unsigned int) * nbins, 256);
-    L->bin_start = off;   off = align_up(off + sizeof(unsigned int) * (nbins + 1), 256);
-    L->large_off = off;   off = align_up(off + sizeof(unsigned int) * (nbins - n_tiles + 1), 256);
+    L->vstart = off;      off = align_up(off + sizeof(unsigned int) * (nbins + 1), 256);
+    L->large_off = off;   off = align_up(off + sizeof(unsigned int) * (nbins - 2 * n_tiles + 1), 256);
+    L->run = off;         off = align_up(off + sizeof(uint2) * kMaxSlabs * nbins, 256);
     // DeviceStats and the tiles' 64-bit sums sit together: one memset clears both before every frame
     L->stats = off;       off = align_up(off + sizeof(DeviceStats), 256);
     L->accum = off;
@@ -131,16 +140,18 @@ bool make_layout(const splotch_ctx *c, unsigned long long n, int T, unsigned lon
         off = align_up(off + 6 * align_up(sizeof(float) * n, 256), 256);
         off = align_up(off + sizeof(float) * 3 * (size_t)c->width * c->height, 256);
     }
-    const size_t fixed = off;
+    // every run of SMALL records may be padded by one 16-byte unit (k_layout): an allowance beside the capacity
+    const size_t pad = align_up(16 * (size_t)kMaxSlabs * n_tiles + 16 * nbins, 256);
+    const size_t fixed = off + pad;
     if (capacity == 0) {
-        // derive from bytes: capacity * 32 <= bytes - fixed
+        // derive from bytes: capacity * 32 <= bytes - fixed - reserve
         const size_t need0 = fixed + 8192;
         if (bytes < need0) return false;
         capacity = (unsigned long long)((bytes - need0) / 32);
-        if (capacity > 0xfffffff0ull) capacity = 0xfffffff0ull;
+        if (capacity > 0x7ff00000ull) capacity = 0x7ff00000ull;            // 16-byte unit offsets are 32 bits
     }
     L->capacity = capacity;
-    L->records = off;  off = align_up(off + 32ull * capacity, 256);
+    L->records = off;  off = align_up(off + 32ull * capacity + pad, 256);
     L->total = off;
     return bytes == 0 || off <= bytes;
 }
@@ -202,7 +213,7 @@ template <int T>
 int query_splat_occupancy(splotch_ctx *c, int *out)
 {
     CU_TRY(c, cudaFuncSetAttribute(k_splat<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Splat2Cfg<T>::kSmemBytes));
-    CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, k_splat<T>, SplatCfg<T>::kThreads, Splat2Cfg<T>::kSmemBytes));
+    CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, k_splat<T>, Splat2Cfg<T>::kThreads, Splat2Cfg<T>::kSmemBytes));
     if (*out < 1) *out = 1;
     return SPLOTCH_OK;
 }
@@ -216,12 +227,10 @@ int check_params(splotch_ctx *c, const splotch_particles *p, unsigned long long 
         return fail(c, SPLOTCH_EINVAL, "null particle field");
     if (!c->camera_set) return fail(c, SPLOTCH_ESTATE, "camera not set");
     const int ts = tile_shift(q->tile);
-    if (ts < 0) return fail(c, SPLOTCH_EINVAL, "tile must be 8, 16 or 32 (got %d)", q->tile);
+    if (ts < 0) return fail(c, SPLOTCH_EINVAL, "tile must be 8, 16, 32 or 64 (got %d)", q->tile);
+    if (!q->additive && q->tile == 64) return fail(c, SPLOTCH_EINVAL, "the ordered mode takes tiles of 8, 16 or 32 px");
     if (!(q->chi > 0.0f) || !(q->r_small >= 0.0f) || !(q->r_small < q->r_large))
         return fail(c, SPLOTCH_EINVAL, "need chi > 0 and 0 <= r_small < r_large");
-    if (bin_smem_bytes(c->width, c->height, q->tile) + 1024 > (size_t)c->smem_optin)
-        return fail(c, SPLOTCH_EINVAL, "tile %d gives too many tiles for a %dx%d image (per-block histogram exceeds shared memory); use a larger tile",
-                    q->tile, c->width, c->height);
     if (!q->additive)
         for (int s = 0; s < (p->species_offsets ? p->n_species : 1) && s < kMaxSpecies && q->species; ++s)
             if (!(q->species[s].absorb >= 0.0f)) return fail(c, SPLOTCH_EINVAL, "species %d: absorb must be >= 0", s);
@@ -241,7 +250,7 @@ int check_params(splotch_ctx *c, const splotch_particles *p, unsigned long long 
     const int S = 1 << fp->sshift;
     fp->nsx = (c->width + S - 1) / S; fp->nsy = (c->height + S - 1) / S;
     fp->n_super = fp->nsx * fp->nsy;
-    fp->nbins = fp->n_tiles + fp->n_super;
+    fp->nbins = 2 * fp->n_tiles + fp->n_super;
     fp->additive = q->additive ? 1 : 0;
     fp->apply_transfer = q->apply_transfer ? 1 : 0;
     fp->n_species = ns;
@@ -284,18 +293,34 @@ bool aligned16(const splotch_particles *p)
 template <int T>
 int launch_render_tail(splotch_ctx *c, const Layout &L, char *ws, const FrameParams &fp, float *image, cudaStream_t st)
 {
-    const int ti = T == 8 ? 0 : T == 16 ? 1 : 2;
+    const int ti = T == 8 ? 0 : T == 16 ? 1 : T == 32 ? 2 : 3;
     const int grid = c->n_sm * c->splat_blocks_per_sm[ti];
-    k_splat<T><<<grid, SplatCfg<T>::kThreads, Splat2Cfg<T>::kSmemBytes, st>>>(
-        (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.bin_start), (DeviceStats *)(ws + L.stats), (unsigned long long *)(ws + L.accum), fp);
+    k_splat<T><<<grid, Splat2Cfg<T>::kThreads, Splat2Cfg<T>::kSmemBytes, st>>>(
+        (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.vstart), (const uint2 *)(ws + L.run), (DeviceStats *)(ws + L.stats),
+        (unsigned long long *)(ws + L.accum), fp);
     if (c->profiling) cudaEventRecord(c->ev[4], st);
     k_large<<<c->n_sm * c->large_blocks_per_sm, kLargeThreads, 0, st>>>(
-        (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.bin_start), (const unsigned int *)(ws + L.large_off),
+        (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.bin_count), (const uint2 *)(ws + L.run), (const unsigned int *)(ws + L.large_off),
         (DeviceStats *)(ws + L.stats), (unsigned long long *)(ws + L.accum), fp);
     if (c->profiling) cudaEventRecord(c->ev[5], st);
     k_compose<T><<<fp.n_tiles, 256, 0, st>>>((const unsigned long long *)(ws + L.accum), (const DeviceStats *)(ws + L.stats), fp, image);
     if (c->profiling) cudaEventRecord(c->ev[6], st);
     return SPLOTCH_OK;
+}
+
+template <bool AL, bool GH>
+void launch_count(const Layout &L, size_t hbytes, const splotch_particles *p, unsigned long long n, unsigned long long per,
+                  const FrameParams &fp, unsigned int *counts, unsigned int *cls_counts, cudaStream_t st)
+{
+    k_count<AL, GH><<<L.nrows, kBinThreads, GH ? 0 : hbytes, st>>>(p->x, p->y, p->z, p->h, n, per, fp, counts, cls_counts);
+}
+
+template <bool AL, bool GH>
+void launch_scatter(const Layout &L, size_t hbytes, const splotch_particles *p, unsigned long long n, unsigned long long per,
+                    const FrameParams &fp, unsigned int *counts, const uint2 *run, DeviceStats *stats, float4 *records, cudaStream_t st)
+{
+    k_scatter<AL, GH><<<L.nrows, kBinThreads, GH ? sizeof(float4) * kLutSmemMax : hbytes, st>>>(p->x, p->y, p->z, p->h, p->I, p->scalar, n, per, fp,
+                                                                                           counts, run, stats, records);
 }
 
 int render_device(splotch_ctx *c, const splotch_particles *p, unsigned long long n, const FrameParams &fp,
@@ -309,7 +334,8 @@ int render_device(splotch_ctx *c, const splotch_particles *p, unsigned long long
     unsigned int *counts = (unsigned int *)(ws + L.counts);
     unsigned int *cls_counts = (unsigned int *)(ws + L.cls_counts);
     unsigned int *bin_count = (unsigned int *)(ws + L.bin_count);
-    unsigned int *bin_start = (unsigned int *)(ws + L.bin_start);
+    unsigned int *vstart = (unsigned int *)(ws + L.vstart);
+    uint2 *run = (uint2 *)(ws + L.run);
     DeviceStats *stats = (DeviceStats *)(ws + L.stats);
     if (c->profiling) {
         if (c->prof_stages != kStagesAdditive || c->last_stream != st) c->prof_frames = 0;   // a session covers one mode and one stream
@@ -317,23 +343,25 @@ int render_device(splotch_ctx *c, const splotch_particles *p, unsigned long long
         cudaEventRecord(c->ev[0], st);
     }
     cudaMemsetAsync(ws + L.stats, 0, (L.accum - L.stats) + L.accum_bytes, st);      // DeviceStats + the tiles' sums
-    if (al) k_count<true><<<L.nrows, kBinThreads, hbytes, st>>>(p->x, p->y, p->z, p->h, n, per, fp, counts, cls_counts);
-    else    k_count<false><<<L.nrows, kBinThreads, hbytes, st>>>(p->x, p->y, p->z, p->h, n, per, fp, counts, cls_counts);
+    if (L.ghist) cudaMemsetAsync(counts, 0, L.counts_bytes, st);                    // the blocks count straight into their rows
+    if (L.ghist) { if (al) launch_count<true, true>(L, hbytes, p, n, per, fp, counts, cls_counts, st); else launch_count<false, true>(L, hbytes, p, n, per, fp, counts, cls_counts, st); }
+    else         { if (al) launch_count<true, false>(L, hbytes, p, n, per, fp, counts, cls_counts, st); else launch_count<false, false>(L, hbytes, p, n, per, fp, counts, cls_counts, st); }
     if (c->profiling) cudaEventRecord(c->ev[1], st);
     const int bps = 1 << (fp.sshift - 5);               // 32-px blocks per super-tile side (k_large's work items)
-    k_scan<<<(fp.nbins + 31) / 32, kScanThreads, 0, st>>>(counts, L.nrows, fp.nbins, fp.n_tiles, bin_count, bin_start, cls_counts, L.capacity,
+    k_scan<<<(fp.nbins + 31) / 32, kScanThreads, 0, st>>>(counts, L.nrows, fp.nbins, fp.n_tiles, bin_count, vstart, cls_counts, 2ull * L.capacity,
                                                           c->n_sm, (unsigned int *)(ws + L.large_off), (unsigned int)kLargeChunk,
                                                           (unsigned int)(bps * bps), stats);
+    k_layout<<<kMaxSlabs, kLayoutThreads, 0, st>>>(counts, bin_count, L.nrows, fp.nbins, fp.n_tiles, run, stats);
     if (c->profiling) cudaEventRecord(c->ev[2], st);
-    if (al) k_scatter<true><<<L.nrows, kBinThreads, hbytes, st>>>(p->x, p->y, p->z, p->h, p->I, p->scalar, n, per, fp, counts,
-                                                                  bin_start, stats, (float4 *)(ws + L.records));
-    else    k_scatter<false><<<L.nrows, kBinThreads, hbytes, st>>>(p->x, p->y, p->z, p->h, p->I, p->scalar, n, per, fp, counts,
-                                                                   bin_start, stats, (float4 *)(ws + L.records));
+    float4 *records = (float4 *)(ws + L.records);
+    if (L.ghist) { if (al) launch_scatter<true, true>(L, hbytes, p, n, per, fp, counts, run, stats, records, st); else launch_scatter<false, true>(L, hbytes, p, n, per, fp, counts, run, stats, records, st); }
+    else         { if (al) launch_scatter<true, false>(L, hbytes, p, n, per, fp, counts, run, stats, records, st); else launch_scatter<false, false>(L, hbytes, p, n, per, fp, counts, run, stats, records, st); }
     if (c->profiling) cudaEventRecord(c->ev[3], st);
     int rc;
     if (fp.T == 8) rc = launch_render_tail<8>(c, L, ws, fp, image, st);
     else if (fp.T == 16) rc = launch_render_tail<16>(c, L, ws, fp, image, st);
-    else rc = launch_render_tail<32>(c, L, ws, fp, image, st);
+    else if (fp.T == 32) rc = launch_render_tail<32>(c, L, ws, fp, image, st);
+    else rc = launch_render_tail<64>(c, L, ws, fp, image, st);
     if (rc != SPLOTCH_OK) return rc;
     CU_TRY(c, cudaGetLastError());
     c->have_frame = true; c->ws = ws; c->lay = L; c->fp = fp; c->last_n = n; c->last_stream = st; c->last_additive = true;
@@ -462,13 +490,14 @@ int splotch_create(splotch_ctx **out, int device, int width, int height, uint64_
     int rc = [&]() -> int {
         CU_TRY(c, cudaMalloc(&c->lut, sizeof(float4) * kMaxSpecies * kMaxLut));
         CU_TRY(c, cudaMemset(c->lut, 0, sizeof(float4) * kMaxSpecies * kMaxLut));
-        CU_TRY(c, cudaFuncSetAttribute(k_count<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb));
-        CU_TRY(c, cudaFuncSetAttribute(k_count<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb));
-        CU_TRY(c, cudaFuncSetAttribute(k_scatter<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb));
-        CU_TRY(c, cudaFuncSetAttribute(k_scatter<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb));
+        CU_TRY(c, (cudaFuncSetAttribute(k_count<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb)));
+        CU_TRY(c, (cudaFuncSetAttribute(k_count<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb)));
+        CU_TRY(c, (cudaFuncSetAttribute(k_scatter<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb)));
+        CU_TRY(c, (cudaFuncSetAttribute(k_scatter<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb)));
         int r = query_splat_occupancy<8>(c, &c->splat_blocks_per_sm[0]);
         if (r == SPLOTCH_OK) r = query_splat_occupancy<16>(c, &c->splat_blocks_per_sm[1]);
         if (r == SPLOTCH_OK) r = query_splat_occupancy<32>(c, &c->splat_blocks_per_sm[2]);
+        if (r == SPLOTCH_OK) r = query_splat_occupancy<64>(c, &c->splat_blocks_per_sm[3]);
         if (r != SPLOTCH_OK) return r;
         CU_TRY(c, cudaFuncSetAttribute(k_rs_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(RsSmem)));
         CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->orender_blocks_per_sm[0], k_orender<8>, SplatCfg<8>::kThreads, 0));
@@ -577,9 +606,8 @@ int splotch_set_profiling(splotch_ctx *c, int enabled)
 size_t splotch_workspace_bytes(const splotch_ctx *c, uint64_t n, int tile, uint64_t pair_capacity, int with_host_staging)
 {
     if (!c || tile_shift(tile) < 0 || n > c->max_particles) return 0;
-    if (bin_smem_bytes(c->width, c->height, tile) + 1024 > (size_t)c->smem_optin) return 0;
     if (pair_capacity == 0) pair_capacity = 2ull * n + (1ull << 20);
-    if (pair_capacity > 0xfffffff0ull) return 0;
+    if (pair_capacity > 0x7ff00000ull) return 0;
     Layout L, Lo;
     make_layout(c, n, tile, pair_capacity, 0, with_host_staging != 0, &L);
     make_layout_ordered(c, n, tile, pair_capacity, with_host_staging != 0, &Lo);       // either mode must fit
@@ -724,8 +752,9 @@ int splotch_debug_tile_counts(splotch_ctx *c, uint32_t *out, void *cuda_stream)
     if (!c->have_frame) return fail(c, SPLOTCH_ESTATE, "no frame rendered yet");
     CU_TRY(c, cudaSetDevice(c->device));
     if (c->last_additive) {
-        CU_TRY(c, cudaMemcpyAsync(out, c->ws + c->lay.bin_count, sizeof(uint32_t) * (size_t)c->fp.n_tiles,
-                                  cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
+        k_tile_counts<<<(c->fp.n_tiles + 255) / 256, 256, 0, (cudaStream_t)cuda_stream>>>((const unsigned int *)(c->ws + c->lay.bin_count),
+                                                                                            c->fp.n_tiles, out);
+        CU_TRY(c, cudaGetLastError());
     } else {
         k_odiff<<<(c->fp.n_tiles + 255) / 256, 256, 0, (cudaStream_t)cuda_stream>>>((const unsigned int *)(c->ws + c->lay.tile_start),
                                                                                      c->fp.n_tiles, out);

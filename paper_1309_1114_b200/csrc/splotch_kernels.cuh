@@ -30,8 +30,8 @@ namespace splotch {
 
 constexpr int kMaxSpecies   = 8;
 constexpr int kMaxLut       = 1024;
-constexpr int kChunkMax     = 32768;  // records per work item of k_splat (upper bound; the frame picks its own)
-constexpr int kChunkMin     = 128;
+constexpr int kChunkMax     = 32768;  // 16-byte units per work item of k_splat (upper bound; the frame picks its own)
+constexpr int kChunkMin     = 256;
 constexpr int kBinThreads   = 1024;   // k_count / k_scatter block size: one CTA per SM (fewer histogram rows and write streams than 2 x 512)
 constexpr int kSuperShift   = 3;      // super-tile = 8 x 8 tiles, at most 256 px (LARGE particles are binned to super-tiles)
 constexpr int kSuperMaxShift = 8;
@@ -70,6 +70,9 @@ struct DeviceStats {             // cleared before every frame; written by k_sca
     // ordered mode, sort key = tile << zbits | (~bits(z_c) - zkey_min): only the bits that differ in this frame are sorted
     unsigned int zkey_max, nzkey_max, zkey_min, zbits, key_bits, pad2;     // nzkey_max = max of ~zkey (its complement is the min)
     unsigned int overflow, work_counter, chunk_size, amax_bits, scan_done, large_counter;   // large_counter: work items of k_large
+    // additive layout (k_scan, k_layout): all offsets in 16-byte units
+    unsigned int slabs, rows_per_slab, tile_units, total_units, layout_done, small_pairs;
+    unsigned int slab_base[32];
 };
 
 struct Geo {
@@ -86,6 +89,12 @@ __device__ __forceinline__ float dot3(const float *a, float dx, float dy, float 
 constexpr float kMagic     = 12582912.0f;     // 1.5 * 2^23: v + kMagic has ulp 1 for |v| < 2^22
 constexpr int   kMagicBits = 0x4B400000;
 
+// floor / ceil of v in [-1, 2^22] as an int: v + 1.5 * 2^23 is rounded toward -inf / +inf to a multiple of one ulp = 1
+// (FADD.RM / FADD.RP on the FMA pipe; the integer is the mantissa).  One add and one integer subtract per bound,
+// instead of the quarter-rate conversion pipe (FRND, F2I) or a round-to-nearest add with a compare-and-fix-up.
+__device__ __forceinline__ int floor_magic(float v) { return __float_as_int(__fadd_rd(v, kMagic)) - kMagicBits; }
+__device__ __forceinline__ int ceil_magic(float v)  { return __float_as_int(__fadd_ru(v, kMagic)) - kMagicBits; }
+
 // round-to-nearest-even integer of v in [-1, 32768] and the float it came from: r = rint(v), i = (int)r
 __device__ __forceinline__ int rint_small(float v, float &r)
 {
@@ -93,8 +102,6 @@ __device__ __forceinline__ int rint_small(float v, float &r)
     r = __fsub_rn(t, kMagic);
     return __float_as_int(t) - kMagicBits;
 }
-__device__ __forceinline__ int floor_small(float v) { float r; const int i = rint_small(v, r); return i - (r > v ? 1 : 0); }
-__device__ __forceinline__ int ceil_small(float v)  { float r; const int i = rint_small(v, r); return i + (r < v ? 1 : 0); }
 
 // C1 of DESIGN.md: the canonical float32 sequence (PAPER.md:76 projection, Eq. 7 :138 radius, :156-160 classes).
 // Written without branches (every lane evaluates both the SMALL and the box formulas and selects): the warps of
@@ -119,26 +126,21 @@ __device__ __forceinline__ Geo geometry(float x, float y, float z, float h, cons
     ok = ok && g.rp >= 0.0f && g.rp <= 3.0e38f;
     const bool small = g.rp <= fp.r_small;
     const bool s_ok = g.px >= 0.0f && g.px < fp.fW && g.py >= 0.0f && g.py < fp.fH;
-    // lower bounds: SMALL floor(p), else ceil((p - rp) - 0.5); one rounding serves both
-    const float ax = small ? g.px : __fsub_rn(__fsub_rn(g.px, g.rp), 0.5f);
-    const float ay = small ? g.py : __fsub_rn(__fsub_rn(g.py, g.rp), 0.5f);
-    const float axc = fminf(fmaxf(ax, 0.0f), fp.fW), ayc = fminf(fmaxf(ay, 0.0f), fp.fH);
-    float rx, ry;
-    const int ix = rint_small(axc, rx), iy = rint_small(ayc, ry);
-    const int x0 = ix + (small ? -(int)(rx > axc) : (int)(rx < axc));
-    const int y0 = iy + (small ? -(int)(ry > ayc) : (int)(ry < ayc));
-    // upper bounds: floor((p + rp) - 0.5) clamped to [-1, W - 1]
-    const float bxc = fmaxf(fminf(__fsub_rn(__fadd_rn(g.px, g.rp), 0.5f), fp.fWm1), -1.0f);
-    const float byc = fmaxf(fminf(__fsub_rn(__fadd_rn(g.py, g.rp), 0.5f), fp.fHm1), -1.0f);
-    const int x1 = floor_small(bxc), y1 = floor_small(byc);
-    const bool b_ok = x0 <= x1 && y0 <= y1;
+    // MEDIUM / LARGE: x0 = ceil((p - rp) - 0.5) clamped to [0, W], x1 = floor((p + rp) - 0.5) clamped to [-1, W - 1]
+    const int x0m = ceil_magic(fminf(fmaxf(__fsub_rn(__fsub_rn(g.px, g.rp), 0.5f), 0.0f), fp.fW));
+    const int y0m = ceil_magic(fminf(fmaxf(__fsub_rn(__fsub_rn(g.py, g.rp), 0.5f), 0.0f), fp.fH));
+    const int x1m = floor_magic(fmaxf(fminf(__fsub_rn(__fadd_rn(g.px, g.rp), 0.5f), fp.fWm1), -1.0f));
+    const int y1m = floor_magic(fmaxf(fminf(__fsub_rn(__fadd_rn(g.py, g.rp), 0.5f), fp.fHm1), -1.0f));
+    // SMALL: the pixel that holds the centre (used only when s_ok: 0 <= p < W <= 32768)
+    const int x0s = floor_magic(g.px), y0s = floor_magic(g.py);
+    const bool b_ok = x0m <= x1m && y0m <= y1m;
     const int big = (g.rp <= fp.r_large) ? MEDIUM : LARGE;
     g.cls = ok ? (small ? (s_ok ? SMALL : CULLED) : (b_ok ? big : CULLED)) : CULLED;
     const bool act = g.cls != CULLED;
-    g.x0 = act ? x0 : 0;
-    g.x1 = act ? (small ? x0 : x1) : -1;
-    g.y0 = act ? y0 : 0;
-    g.y1 = act ? (small ? y0 : y1) : -1;
+    g.x0 = act ? (small ? x0s : x0m) : 0;
+    g.x1 = act ? (small ? x0s : x1m) : -1;
+    g.y0 = act ? (small ? y0s : y0m) : 0;
+    g.y1 = act ? (small ? y0s : y1m) : -1;
     return g;
 }
 
@@ -153,21 +155,12 @@ __device__ __forceinline__ int paper_label(const Geo &g, const FrameParams &fp)
     return ((int)cy >> fp.tshift) * fp.ntx + ((int)cx >> fp.tshift);
 }
 
-// Bin box of an active particle: tiles of its pixel box (SMALL, MEDIUM) or super-tiles (LARGE, bins n_tiles ...).
-// k_count and k_scatter share this traversal: bins are base + by * pitch + bx for bx in [bx0, bx1], by in [by0, by1].
-struct BinBox { int bx0, bx1, by0, by1, pitch, base, n; };      // n = number of bins (0 for CULLED)
-
-__device__ __forceinline__ BinBox bin_box(const Geo &g, const FrameParams &fp)
-{
-    BinBox b;
-    const int sh = (g.cls == LARGE) ? fp.sshift : fp.tshift;
-    b.bx0 = g.x0 >> sh; b.bx1 = g.x1 >> sh;
-    b.by0 = g.y0 >> sh; b.by1 = g.y1 >> sh;
-    b.pitch = (g.cls == LARGE) ? fp.nsx : fp.ntx;
-    b.base = (g.cls == LARGE) ? fp.n_tiles : 0;
-    b.n = (g.cls == CULLED) ? 0 : (b.bx1 - b.bx0 + 1) * (b.by1 - b.by0 + 1);
-    return b;
-}
+// ---- bins ----------------------------------------------------------------------------------------------------------
+// Bin b < 2 n_tiles: tile b >> 1; even bins hold the tile's MEDIUM records (32 bytes = 2 units of 16 bytes), odd bins
+// its SMALL records (16 bytes = 1 unit: "only their location ... has to be calculated").  Bins
+// 2 n_tiles + s hold the LARGE records of super-tile s (2 units).  A tile's two bins are neighbours, so the tile
+// renderer meets them back to back.
+__device__ __forceinline__ unsigned int bin_unit_size(int b, int n_tiles) { return (b < 2 * n_tiles && (b & 1)) ? 1u : 2u; }
 
 // ---- streaming loads / stores ----------------------------------------------------------------------------------
 __device__ __forceinline__ float4 ldg_stream4(const float *p)
@@ -178,11 +171,11 @@ __device__ __forceinline__ float4 ldg_stream4(const float *p)
     return v;
 }
 
-// one 32-byte render record, one request (256-bit global access, sm_100)
-__device__ __forceinline__ void st_record(float4 *rec, unsigned int slot, const float4 &a, const float4 &b)
+// one 32-byte render record at 16-byte unit `unit` (even), one request (256-bit global access, sm_100)
+__device__ __forceinline__ void st_record(float4 *rec, unsigned int unit, const float4 &a, const float4 &b)
 {
     asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
-                 :: "l"(rec + 2ull * slot), "f"(a.x), "f"(a.y), "f"(a.z), "f"(a.w), "f"(b.x), "f"(b.y), "f"(b.z), "f"(b.w)
+                 :: "l"(rec + unit), "f"(a.x), "f"(a.y), "f"(a.z), "f"(a.w), "f"(b.x), "f"(b.y), "f"(b.z), "f"(b.w)
                  : "memory");
 }
 
@@ -205,10 +198,13 @@ __device__ __forceinline__ void load4(const float *__restrict__ a, unsigned int 
     }
 }
 
-// shared-memory reduction without a return value and with a register operand: one instruction, no branch around it
-__device__ __forceinline__ void red_add_shared(unsigned int *p, unsigned int v)
+// histogram / cursor update without a return value: shared memory (the common case) or, when the bins of a large
+// image do not fit in shared memory, the block's own row of the count matrix in global memory (L2 resident)
+template <bool GHIST>
+__device__ __forceinline__ void hist_inc(unsigned int *p)
 {
-    asm volatile("red.shared.add.u32 [%0], %1;" :: "r"((unsigned int)__cvta_generic_to_shared(p)), "r"(v) : "memory");
+    if (GHIST) asm volatile("red.global.add.u32 [%0], 1;" :: "l"(p) : "memory");
+    else asm volatile("red.shared.add.u32 [%0], 1;" :: "r"((unsigned int)__cvta_generic_to_shared(p)) : "memory");
 }
 
 __device__ __forceinline__ unsigned int warp_sum(unsigned int v)
@@ -217,23 +213,26 @@ __device__ __forceinline__ unsigned int warp_sum(unsigned int v)
 }
 
 // ---- A1 + A3 + A4a: classify and count ------------------------------------------------------------------------
-// Block b owns the particle range [b*per, (b+1)*per) and a private histogram over all bins in shared memory;
-// row b of `counts` receives it, so the count stage needs no global atomics and is deterministic.
-template <bool ALIGNED>
+// Block b owns the particle range [b*per, (b+1)*per) and a private histogram over all bins; row b of `counts`
+// receives it, so the count stage needs no atomics between blocks and is deterministic.
+template <bool ALIGNED, bool GHIST>
 __global__ void __launch_bounds__(kBinThreads, 1)
 k_count(const float *__restrict__ x, const float *__restrict__ y, const float *__restrict__ z,
         const float *__restrict__ h, unsigned long long n, unsigned long long per, const __grid_constant__ FrameParams fp,
         unsigned int *__restrict__ counts, unsigned int *__restrict__ cls_counts)
 {
-    extern __shared__ unsigned int hist[];
+    extern __shared__ unsigned int hist_s[];
     __shared__ unsigned int s_cls[4];
-    for (int i = threadIdx.x; i < fp.nbins; i += kBinThreads) hist[i] = 0u;
+    unsigned int *row = counts + (size_t)blockIdx.x * fp.nbins;
+    unsigned int *hist = GHIST ? row : hist_s;          // GHIST: the row was cleared with the frame's memset
+    if (!GHIST) for (int i = threadIdx.x; i < fp.nbins; i += kBinThreads) hist_s[i] = 0u;
     if (threadIdx.x < 4) s_cls[threadIdx.x] = 0u;
     __syncthreads();
     const unsigned long long lo = (unsigned long long)blockIdx.x * per;
     const unsigned int len = lo < n ? (unsigned int)min(n - lo, per) : 0u;
     x += lo; y += lo; z += lo; h += lo;
-    unsigned int c1 = 0, c2 = 0, c3 = 0;          // per-warp class counts (every lane holds the same value)
+    unsigned int c2 = 0, c3 = 0;                  // MEDIUM / LARGE particles of this thread (SMALL ones are the sum of the odd bins)
+    const int ts = fp.tshift, ntx2 = 2 * fp.ntx;
     // the loop bound is the same for the 32 lanes of a warp (lanes past the end idle), so warps stay converged
     const unsigned int lane4 = 4u * (threadIdx.x & 31u);
     for (unsigned int iw = 4u * (threadIdx.x & ~31u); iw < len; iw += 4u * kBinThreads) {
@@ -245,44 +244,46 @@ k_count(const float *__restrict__ x, const float *__restrict__ y, const float *_
         load4<ALIGNED>(h, i, len, hs);
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            Geo g = geometry(xs[j], ys[j], zs[j], hs[j], fp);
-            if (!(i + j < len)) { g.cls = CULLED; g.x1 = -1; g.y1 = -1; g.x0 = 0; g.y0 = 0; }
-            c1 += g.cls == SMALL; c2 += g.cls == MEDIUM; c3 += g.cls == LARGE;        // per thread, summed at the end
-            const BinBox b = bin_box(g, fp);
-            // a box covers at most 2 x 2 bins unless it is wider than a tile: four unconditional reductions with a 0 / 1
-            // operand (no branches; a CULLED particle adds 0 to bin 0, the +1 / +pitch neighbours of the last bin fall into
-            // the unused colour-table area behind the histogram)
-            const bool any = b.n > 0, w2 = b.bx1 > b.bx0, h2 = b.by1 > b.by0;
-            unsigned int *h00 = hist + (b.base + b.by0 * b.pitch + b.bx0);
-            red_add_shared(h00, any ? 1u : 0u);
-            red_add_shared(h00 + 1, (any && w2) ? 1u : 0u);
-            red_add_shared(h00 + b.pitch, (any && h2) ? 1u : 0u);
-            red_add_shared(h00 + b.pitch + 1, (any && w2 && h2) ? 1u : 0u);
-            const bool big = any && (b.bx1 - b.bx0 > 1 || b.by1 - b.by0 > 1);
-            if (__any_sync(0xffffffffu, big)) {          // the bins beyond the first 2 x 2
-                const int nmax = __reduce_max_sync(0xffffffffu, big ? b.n : 0);
-                int bx = b.bx0, by = b.by0;
-                for (int t = 0; t < nmax; ++t) {
-                    if (big && t < b.n && (bx - b.bx0 > 1 || by - b.by0 > 1)) atomicAdd(&hist[b.base + by * b.pitch + bx], 1u);
-                    const bool wrap = bx == b.bx1;
-                    bx = wrap ? b.bx0 : bx + 1;
-                    by += wrap;
+            const Geo g = geometry(xs[j], ys[j], zs[j], hs[j], fp);
+            const int cls = (i + j < len) ? g.cls : CULLED;
+            c2 += cls == MEDIUM; c3 += cls == LARGE;
+            // SMALL and MEDIUM: the tiles of the pixel box.  A box covers at most 2 x 2 tiles unless it is wider than a
+            // tile: four predicated reductions, no loop
+            const int tx0 = g.x0 >> ts, ty0 = g.y0 >> ts, tx1 = g.x1 >> ts, ty1 = g.y1 >> ts;
+            const bool tile = cls == SMALL || cls == MEDIUM, w2 = tx1 > tx0, h2 = ty1 > ty0;
+            unsigned int *h00 = hist + (2 * (ty0 * fp.ntx + tx0) + (cls == SMALL ? 1 : 0));
+            if (tile) hist_inc<GHIST>(h00);
+            if (tile && w2) hist_inc<GHIST>(h00 + 2);
+            if (tile && h2) hist_inc<GHIST>(h00 + ntx2);
+            if (tile && w2 && h2) hist_inc<GHIST>(h00 + ntx2 + 2);
+            // rare: MEDIUM boxes over more than 2 x 2 tiles, and LARGE particles (super-tile bins)
+            const bool big = tile && (tx1 - tx0 > 1 || ty1 - ty0 > 1);
+            if (__any_sync(0xffffffffu, big || cls == LARGE)) {
+                if (big) {
+                    for (int ty = ty0; ty <= ty1; ++ty)
+                        for (int tx = tx0; tx <= tx1; ++tx)
+                            if (tx - tx0 > 1 || ty - ty0 > 1) hist_inc<GHIST>(hist + 2 * (ty * fp.ntx + tx));
+                } else if (cls == LARGE) {
+                    const int ss = fp.sshift;
+                    for (int sy = g.y0 >> ss; sy <= (g.y1 >> ss); ++sy)
+                        for (int sx = g.x0 >> ss; sx <= (g.x1 >> ss); ++sx) hist_inc<GHIST>(hist + 2 * fp.n_tiles + sy * fp.nsx + sx);
                 }
             }
         }
     }
-    c1 = warp_sum(c1); c2 = warp_sum(c2); c3 = warp_sum(c3);
-    if ((threadIdx.x & 31) == 0) { atomicAdd(&s_cls[1], c1); atomicAdd(&s_cls[2], c2); atomicAdd(&s_cls[3], c3); }
+    c2 = warp_sum(c2); c3 = warp_sum(c3);
+    if ((threadIdx.x & 31) == 0) { atomicAdd(&s_cls[2], c2); atomicAdd(&s_cls[3], c3); }
     __syncthreads();
-    unsigned int *row = counts + (size_t)blockIdx.x * fp.nbins;
-    for (int i = threadIdx.x; i < fp.nbins; i += kBinThreads) row[i] = hist[i];
-    if (threadIdx.x == 0) s_cls[0] = len - s_cls[1] - s_cls[2] - s_cls[3];
+    if (!GHIST) for (int i = threadIdx.x; i < fp.nbins; i += kBinThreads) row[i] = hist_s[i];
+    if (threadIdx.x == 0) s_cls[0] = len;           // particles of this block: k_scan turns it into the CULLED count
     __syncthreads();
     if (threadIdx.x < 4) cls_counts[blockIdx.x * 4 + threadIdx.x] = s_cls[threadIdx.x];
 }
 
 // ---- A4b + A4c: scans ----------------------------------------------------------------------------------------------
 constexpr int kScanThreads = 256;
+constexpr int kMaxSlabs = 32;                 // the record array is cut into at most 32 slabs (one lane of a warp each)
+constexpr unsigned int kSlabBytes = 96u << 20;   // target size of a slab (see k_scan)
 
 __device__ __forceinline__ unsigned long long block_excl_scan_256(unsigned long long v, unsigned long long *s_warp,
                                                                   unsigned long long *total)
@@ -309,18 +310,27 @@ __device__ __forceinline__ unsigned long long block_excl_scan_256(unsigned long 
 
 // Phase 1, every block: 32 bins x 8 row groups.  Thread (bin, g) sums its rows of the count matrix (independent
 // loads, bins of neighbouring lanes are neighbours in memory), the groups are combined through shared memory, and
-// the rows are rewritten as exclusive prefixes: counts[b][bin] becomes the offset of block b inside the bin.
-// Phase 2, the last block to finish (a counter in DeviceStats, cleared with it before every frame): exclusive scan
-// over the bins -> bin_start, frame statistics, and the chunk size: the tile part of the record array, [0, pairs),
-// is cut into chunks of chunk_size consecutive records, the work items of k_splat.
+// the rows are rewritten as exclusive prefixes: counts[b][bin] becomes the number of the bin's records that blocks
+// before b produce.
+// Phase 2, the last block to finish (a counter in DeviceStats, cleared with it before every frame): the frame's
+// statistics and its layout parameters:
+//   * vstart[bin], the bin's first 16-byte unit in the VIRTUAL order the renderers consume (bin after bin; a bin's
+//     units are padded to an even number so that 32-byte records never straddle a chunk boundary); the tile part,
+//     [0, tile_units), is cut into chunks of chunk_size units, the work items of k_splat;
+//   * the number of slabs: in MEMORY the records are slab-major.  The count / scatter blocks are divided into groups of
+//     rows_per_slab consecutive blocks; a group writes its records, bin after bin, into its own contiguous slab of about
+//     96 MB.  A block's stores then stay inside a window the TLB covers (256 MB) instead of wandering over the whole
+//     array (measured: 32-byte stores spread over 4 GB reach 1.2 TB/s, inside 128 MB windows 2.3 - 5.8 TB/s depending on
+//     the number of bins); the renderers read a bin as `slabs` runs (k_layout builds the run table);
+//   * the item table of k_large.
 __global__ void __launch_bounds__(kScanThreads)
 k_scan(unsigned int *__restrict__ counts, int nrows, int nbins, int n_tiles, unsigned int *__restrict__ bin_count,
-       unsigned int *__restrict__ bin_start, const unsigned int *__restrict__ cls_counts, unsigned long long capacity, int n_sm,
+       unsigned int *__restrict__ vstart, const unsigned int *__restrict__ cls_counts, unsigned long long capacity_units, int n_sm,
        unsigned int *__restrict__ large_off, unsigned int large_chunk, unsigned int large_blocks, DeviceStats *__restrict__ stats)
 {
     __shared__ unsigned int s_part[8][32];
     __shared__ unsigned long long s_warp[kScanThreads / 32];
-    __shared__ unsigned long long s_tot_pairs, s_tot_all, s_tot_items;
+    __shared__ unsigned long long s_tot_tiles, s_tot_all, s_tot_items, s_tot_small;
     __shared__ unsigned int s_ticket, s_cls[4];
     {
         const int bin = blockIdx.x * 32 + (threadIdx.x & 31), g = threadIdx.x >> 5;
@@ -365,16 +375,22 @@ k_scan(unsigned int *__restrict__ counts, int nrows, int nbins, int n_tiles, uns
     __syncthreads();
     if (s_ticket != gridDim.x - 1) return;
     __threadfence();
-    // ---- phase 2: one block
+    // ---- phase 2: one block.  Units of a bin: records x unit size, padded to even
     const int per = (nbins + kScanThreads - 1) / kScanThreads;
     const int b0 = min(nbins, (int)threadIdx.x * per), b1 = min(nbins, b0 + per);
-    unsigned long long sum_all = 0, sum_tiles = 0;
+    unsigned long long u_all = 0, u_tiles = 0, n_small = 0, n_tilerec = 0, n_largerec = 0;
     for (int bb = b0; bb < b1; bb += 8) {
         unsigned int c8[8];
 #pragma unroll
         for (int k = 0; k < 8; ++k) c8[k] = (bb + k < b1) ? __ldcg(bin_count + bb + k) : 0u;
 #pragma unroll
-        for (int k = 0; k < 8; ++k) { sum_all += c8[k]; if (bb + k < n_tiles) sum_tiles += c8[k]; }
+        for (int k = 0; k < 8; ++k) {
+            const int b = bb + k;
+            const unsigned int u = (c8[k] * bin_unit_size(b, n_tiles) + 1u) & ~1u;
+            u_all += u;
+            if (b < 2 * n_tiles) { u_tiles += u; n_tilerec += c8[k]; if (b & 1) n_small += c8[k]; }
+            else n_largerec += c8[k];
+        }
     }
     if (threadIdx.x < 4) s_cls[threadIdx.x] = 0u;
     __syncthreads();
@@ -390,15 +406,19 @@ k_scan(unsigned int *__restrict__ counts, int nrows, int nbins, int n_tiles, uns
             if ((threadIdx.x & 31) == 0 && t) atomicAdd(&s_cls[k], t);
         }
     }
-    const unsigned long long off_all = block_excl_scan_256(sum_all, s_warp, &s_tot_all);
-    (void)block_excl_scan_256(sum_tiles, s_warp, &s_tot_pairs);
-    // chunk size of this frame: about 128 chunks per SM (work items are taken from an atomic counter; many small ones
-    // keep the tail short when their costs differ), between kChunkMin and kChunkMax
-    unsigned long long cs = (s_tot_pairs + (unsigned long long)n_sm * 128 - 1) / ((unsigned long long)n_sm * 128);
-    cs = cs >= 512 ? (cs + 255) / 256 * 256 : (cs + 63) / 64 * 64;      // small frames: short chunks, they are latency bound
+    const unsigned long long off_all = block_excl_scan_256(u_all, s_warp, &s_tot_all);
+    (void)block_excl_scan_256(u_tiles, s_warp, &s_tot_tiles);
+    (void)block_excl_scan_256(n_small, s_warp, &s_tot_small);
+    const unsigned long long tile_records = block_excl_scan_256(n_tilerec, s_warp, &s_tot_items) * 0ull + s_tot_items;
+    const unsigned long long large_records = block_excl_scan_256(n_largerec, s_warp, &s_tot_items) * 0ull + s_tot_items;
+    // chunk size of this frame, in units: about 128 chunks per SM (work items are taken from an atomic counter; many
+    // small ones keep the tail short when their costs differ), between kChunkMin and kChunkMax
+    unsigned long long cs = (s_tot_tiles + (unsigned long long)n_sm * 128 - 1) / ((unsigned long long)n_sm * 128);
+    cs = cs >= 1024 ? (cs + 511) / 512 * 512 : (cs + 127) / 128 * 128;      // small frames: short chunks, they are latency bound
     cs = min((unsigned long long)kChunkMax, max((unsigned long long)kChunkMin, cs));
     const unsigned int K = (unsigned int)cs;
-    const bool overflow = s_tot_all > capacity;
+    // capacity counts true record units; the padding of bins and runs has its own allowance in the workspace
+    const bool overflow = 2ull * (tile_records - s_tot_small) + s_tot_small + 2ull * large_records > capacity_units || s_tot_all > 0xffff0000ull;
     unsigned long long run = off_all;
     for (int bb = b0; bb < b1; bb += 8) {            // eight independent loads per round (this block is latency bound)
         unsigned int c8[8];
@@ -406,35 +426,117 @@ k_scan(unsigned int *__restrict__ counts, int nrows, int nbins, int n_tiles, uns
         for (int k = 0; k < 8; ++k) c8[k] = (bb + k < b1) ? __ldcg(bin_count + bb + k) : 0u;
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
-            if (bb + k < b1) bin_start[bb + k] = (unsigned int)run;
-            run += c8[k];
+            if (bb + k < b1) vstart[bb + k] = (unsigned int)run;
+            run += (c8[k] * bin_unit_size(bb + k, n_tiles) + 1u) & ~1u;
         }
     }
-    if (threadIdx.x == kScanThreads - 1) bin_start[nbins] = (unsigned int)s_tot_all;
+    if (threadIdx.x == kScanThreads - 1) vstart[nbins] = (unsigned int)s_tot_all;
     {   // work items of k_large: (chunk of a super-tile's records) x (block of the super-tile), exclusive prefix over the super-tiles
-        const int n_super = nbins - n_tiles;
+        const int n_super = nbins - 2 * n_tiles;
         const int sper = (n_super + kScanThreads - 1) / kScanThreads;
         const int s0 = min(n_super, (int)threadIdx.x * sper), s1 = min(n_super, s0 + sper);
         unsigned long long items = 0;
-        for (int sb = s0; sb < s1; ++sb) items += (unsigned long long)((__ldcg(bin_count + n_tiles + sb) + large_chunk - 1) / large_chunk) * large_blocks;
+        for (int sb = s0; sb < s1; ++sb) items += (unsigned long long)((__ldcg(bin_count + 2 * n_tiles + sb) + large_chunk - 1) / large_chunk) * large_blocks;
         unsigned long long irun = block_excl_scan_256(items, s_warp, &s_tot_items);
         for (int sb = s0; sb < s1; ++sb) {
             large_off[sb] = overflow ? 0u : (unsigned int)irun;
-            irun += (unsigned long long)((__ldcg(bin_count + n_tiles + sb) + large_chunk - 1) / large_chunk) * large_blocks;
+            irun += (unsigned long long)((__ldcg(bin_count + 2 * n_tiles + sb) + large_chunk - 1) / large_chunk) * large_blocks;
         }
         if (threadIdx.x == kScanThreads - 1) large_off[n_super] = overflow ? 0u : (unsigned int)irun;
     }
-    if (threadIdx.x < 4) stats->count[threadIdx.x] = s_cls[threadIdx.x];      // block scans above synchronised
     if (threadIdx.x == 0) {
-        stats->pairs = s_tot_pairs;
-        stats->large_pairs = s_tot_all - s_tot_pairs;
-        stats->chunks = overflow ? 0ull : (s_tot_pairs + K - 1) / K;
-        stats->capacity = capacity;
+        // slabs of about 96 MB, at most 32 and at most one per row
+        unsigned int G = (unsigned int)((s_tot_all * 16ull + kSlabBytes - 1) / kSlabBytes);
+        G = max(1u, min(min(G, (unsigned int)kMaxSlabs), (unsigned int)nrows));
+        const unsigned int cps = ((unsigned int)nrows + G - 1) / G;
+        stats->slabs = ((unsigned int)nrows + cps - 1) / cps;
+        stats->rows_per_slab = cps;
+        stats->tile_units = overflow ? 0u : (unsigned int)s_tot_tiles;
+        stats->total_units = overflow ? 0u : (unsigned int)s_tot_all;
+        stats->count[0] = (unsigned long long)s_cls[0] - s_tot_small - s_cls[2] - s_cls[3];
+        stats->count[1] = s_tot_small;
+        stats->count[2] = s_cls[2];
+        stats->count[3] = s_cls[3];
+        stats->pairs = tile_records;
+        stats->small_pairs = s_tot_small;
+        stats->large_pairs = large_records;
+        stats->chunks = overflow ? 0ull : (s_tot_tiles + K - 1) / K;
+        stats->capacity = capacity_units / 2;
         stats->overflow = overflow ? 1u : 0u;
         stats->work_counter = 0u;
         stats->chunk_size = K;
-        stats->amax_bits = 0u;
         stats->scan_done = 0u;
+    }
+}
+
+// One block per slab s (blocks beyond the frame's slab count leave at once): the slab's runs.  Run (s, bin) holds the
+// bin's records that the rows of slab s produce: cnt = P[(s + 1) rows_per_slab][bin] - P[s rows_per_slab][bin] with P the
+// exclusive row prefixes k_scan left in `counts`; the runs of a slab follow each other in bin order, each padded to an
+// even number of units.  run[bin * 32 + s] = {first unit inside the slab, records}; the last block to finish turns the slab
+// sizes into slab_base[] (DeviceStats).
+constexpr int kLayoutThreads = 1024;
+
+__global__ void __launch_bounds__(kLayoutThreads)
+k_layout(const unsigned int *__restrict__ counts, const unsigned int *__restrict__ bin_count, int nrows, int nbins, int n_tiles,
+         uint2 *__restrict__ run, DeviceStats *__restrict__ stats)
+{
+    __shared__ unsigned int s_warp[32], s_total;
+    __shared__ unsigned int s_ticket;
+    const unsigned int G = stats->slabs, cps = stats->rows_per_slab;
+    const unsigned int s = blockIdx.x;
+    if (s < G) {
+        const unsigned int rlo = s * cps, rhi = (s + 1) * cps;
+        const unsigned int *plo = counts + (size_t)rlo * nbins;
+        const unsigned int *phi = rhi < (unsigned int)nrows ? counts + (size_t)rhi * nbins : bin_count;
+        const int per = (nbins + kLayoutThreads - 1) / kLayoutThreads;
+        const int b0 = min(nbins, (int)threadIdx.x * per), b1 = min(nbins, b0 + per);
+        unsigned int sum = 0u;
+        for (int b = b0; b < b1; ++b) sum += ((__ldcg(phi + b) - __ldcg(plo + b)) * bin_unit_size(b, n_tiles) + 1u) & ~1u;
+        const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+        unsigned int inc = sum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const unsigned int t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += t;
+        }
+        if (lane == 31) s_warp[w] = inc;
+        __syncthreads();
+        if (w == 0) {
+            const unsigned int c = s_warp[lane];
+            unsigned int ci = c;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const unsigned int t = __shfl_up_sync(0xffffffffu, ci, o);
+                if (lane >= o) ci += t;
+            }
+            s_warp[lane] = ci - c;
+            if (lane == 31) s_total = ci;
+        }
+        __syncthreads();
+        unsigned int off = s_warp[w] + inc - sum;
+        for (int b = b0; b < b1; ++b) {
+            const unsigned int cnt = __ldcg(phi + b) - __ldcg(plo + b);
+            run[(size_t)b * kMaxSlabs + s] = make_uint2(off, cnt);
+            off += (cnt * bin_unit_size(b, n_tiles) + 1u) & ~1u;
+        }
+        if (threadIdx.x == 0) stats->slab_base[s] = s_total;        // the slab's size for now
+    } else {
+        for (int b = threadIdx.x; b < nbins; b += kLayoutThreads) run[(size_t)b * kMaxSlabs + s] = make_uint2(0u, 0u);   // no such run
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_ticket = atomicAdd(&stats->layout_done, 1u);
+    __syncthreads();
+    if (s_ticket != gridDim.x - 1) return;
+    __threadfence();
+    if (threadIdx.x == 0) {
+        unsigned int base = 0u;
+        for (unsigned int k = 0; k < (unsigned int)kMaxSlabs; ++k) {
+            const unsigned int sz = k < G ? *(volatile unsigned int *)&stats->slab_base[k] : 0u;
+            stats->slab_base[k] = base;
+            base += sz;
+        }
+        stats->layout_done = 0u;
     }
 }
 
@@ -482,40 +584,61 @@ __device__ __forceinline__ float3 amplitude(float I, float scalar, float h, cons
     return make_float3(c.x * col, c.y * col, c.z * col);
 }
 
-// Render record, 32 bytes: {px, py, c, r2} {aR, aG, aB, box}
-//   MEDIUM / LARGE: c = -log2(e) / sp^2, r2 = rp^2 (float32, the C1 inside test compares d2 with it), a = E * col.
-//   SMALL: c = 0 and r2 = +inf, so the one pixel of its box passes the inside test with weight exp2(0) = 1;
-//          a = E * col * pi sp^2 (1 - exp(-chi^2)) (the whole clipped flux).
-//   box: the particle's pixel box clipped to the bin it is filed under, relative to the bin's origin.  Tile bins
-//        (SMALL, MEDIUM): x0 | y0 << 5 | (x1 - x0) << 10 | (y1 - y0) << 15.  Super-tile bins (LARGE):
-//        x0 | y0 << 8 | x1 << 16 | y1 << 24.  The renderers never round a float again.
+// Render records.
+//   MEDIUM / LARGE, 32 bytes: {px, py, c, r2} {aR, aG, aB, box}
+//     c = -log2(e) / sp^2, r2 = rp^2 (float32, the C1 inside test compares d2 with it), a = E * col.
+//     box: the particle's pixel box clipped to the bin it is filed under, relative to the bin's origin.  Tile bins
+//     (MEDIUM): x0 | y0 << 6 | (x1 - x0) << 12 | (y1 - y0) << 18.  Super-tile bins (LARGE): x0 | y0 << 8 | x1 << 16 |
+//     y1 << 24.  The renderers never round a float again.
+//   SMALL, 16 bytes: {pixel, aR, aG, aB}: pixel = y * T + x inside the tile, a = E * col * pi sp^2 (1 - exp(-chi^2)),
+//     the whole clipped flux (R6): a SMALL particle needs "only its location".
 // A record whose amplitude is not finite (I or scalar = Inf / NaN) carries amplitude 0.
-__device__ __forceinline__ unsigned int pack_box(const Geo &g, int cls, int bx, int by, const FrameParams &fp)
+__device__ __forceinline__ unsigned int pack_box_tile(const Geo &g, int tx, int ty, const FrameParams &fp)
 {
-    if (cls == LARGE) {
-        const int ox = bx << fp.sshift, oy = by << fp.sshift, m = (1 << fp.sshift) - 1;
-        const int cx0 = max(g.x0 - ox, 0), cx1 = min(g.x1 - ox, m), cy0 = max(g.y0 - oy, 0), cy1 = min(g.y1 - oy, m);
-        return (unsigned int)cx0 | ((unsigned int)cy0 << 8) | ((unsigned int)cx1 << 16) | ((unsigned int)cy1 << 24);
-    }
-    const int ox = bx << fp.tshift, oy = by << fp.tshift, m = fp.T - 1;
+    const int ox = tx << fp.tshift, oy = ty << fp.tshift, m = fp.T - 1;
     const int cx0 = max(g.x0 - ox, 0), cx1 = min(g.x1 - ox, m), cy0 = max(g.y0 - oy, 0), cy1 = min(g.y1 - oy, m);
-    return (unsigned int)cx0 | ((unsigned int)cy0 << 5) | ((unsigned int)(cx1 - cx0) << 10) | ((unsigned int)(cy1 - cy0) << 15);
+    return (unsigned int)cx0 | ((unsigned int)cy0 << 6) | ((unsigned int)(cx1 - cx0) << 12) | ((unsigned int)(cy1 - cy0) << 18);
 }
 
-template <bool ALIGNED>
+__device__ __forceinline__ unsigned int pack_box_super(const Geo &g, int sx, int sy, const FrameParams &fp)
+{
+    const int ox = sx << fp.sshift, oy = sy << fp.sshift, m = (1 << fp.sshift) - 1;
+    const int cx0 = max(g.x0 - ox, 0), cx1 = min(g.x1 - ox, m), cy0 = max(g.y0 - oy, 0), cy1 = min(g.y1 - oy, m);
+    return (unsigned int)cx0 | ((unsigned int)cy0 << 8) | ((unsigned int)cx1 << 16) | ((unsigned int)cy1 << 24);
+}
+
+// next free unit of a bin's run: shared-memory cursor, or the block's row of the count matrix (see hist_inc)
+template <bool GHIST>
+__device__ __forceinline__ unsigned int cursor_take(unsigned int *p, unsigned int units)
+{
+    return atomicAdd(p, units);
+}
+
+template <bool ALIGNED, bool GHIST>
 __global__ void __launch_bounds__(kBinThreads, 1)
 k_scatter(const float *__restrict__ x, const float *__restrict__ y, const float *__restrict__ z,
           const float *__restrict__ h, const float *__restrict__ I, const float *__restrict__ scalar,
           unsigned long long n, unsigned long long per, const __grid_constant__ FrameParams fp,
-          const unsigned int *__restrict__ counts, const unsigned int *__restrict__ bin_start,
+          unsigned int *__restrict__ counts, const uint2 *__restrict__ run,
           DeviceStats *__restrict__ stats, float4 *__restrict__ records)
 {
-    extern __shared__ unsigned int cursor[];                 // nbins cursors, then the packed colour tables
+    extern __shared__ unsigned int cursor_s[];               // nbins cursors, then the packed colour tables
     __shared__ float s_amax[kBinThreads / 32];
     if (stats->overflow) return;
-    float4 *s_lut = reinterpret_cast<float4 *>(cursor + ((fp.nbins + 3) & ~3));
-    const unsigned int *row = counts + (size_t)blockIdx.x * fp.nbins;
-    for (int i = threadIdx.x; i < fp.nbins; i += kBinThreads) cursor[i] = bin_start[i] + row[i];
+    float4 *s_lut = reinterpret_cast<float4 *>(cursor_s + (GHIST ? 0 : ((fp.nbins + 3) & ~3)));
+    // this block's cursors: slab base + the run's first unit + the units of the slab's rows before this one
+    unsigned int *row = counts + (size_t)blockIdx.x * fp.nbins;
+    unsigned int *cursor = GHIST ? row : cursor_s;
+    {
+        const unsigned int cps = stats->rows_per_slab, s = blockIdx.x / cps;
+        const unsigned int base = stats->slab_base[s];
+        const unsigned int *row0 = counts + (size_t)(s * cps) * fp.nbins;
+        const bool first = blockIdx.x == s * cps;
+        for (int i = threadIdx.x; i < fp.nbins; i += kBinThreads) {
+            const unsigned int before = first ? 0u : row[i] - row0[i];
+            cursor[i] = base + run[(size_t)i * kMaxSlabs + s].x + before * bin_unit_size(i, fp.n_tiles);
+        }
+    }
     if (fp.lut_total > 0) {
         for (int s = 0; s < fp.n_species; ++s)
             if (fp.sp[s].use_colormap)
@@ -531,6 +654,7 @@ k_scatter(const float *__restrict__ x, const float *__restrict__ y, const float 
     const int s_first = species_of(lo32, fp), s_last = species_of(lo32 + (len ? len - 1 : 0), fp);
     float amax = 0.0f;
     const bool one_species = s_first == s_last;
+    const int ts = fp.tshift, tmask = fp.T - 1, ntx2 = 2 * fp.ntx;
     const unsigned int lane4 = 4u * (threadIdx.x & 31u);
     for (unsigned int iw = 4u * (threadIdx.x & ~31u); iw < len; iw += 4u * kBinThreads) {
         const unsigned int i = iw + lane4;
@@ -543,41 +667,46 @@ k_scatter(const float *__restrict__ x, const float *__restrict__ y, const float 
         load4<ALIGNED>(scalar, i, len, ss);
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            Geo g = geometry(xs[j], ys[j], zs[j], hs[j], fp);
-            if (!(i + j < len)) { g.cls = CULLED; g.x1 = -1; g.y1 = -1; g.x0 = 0; g.y0 = 0; }
+            const Geo g = geometry(xs[j], ys[j], zs[j], hs[j], fp);
+            const int cls = (i + j < len) ? g.cls : CULLED;
             const int s = one_species ? s_first : species_of(min(lo32 + i + j, lo32 + len - 1), fp);
             const SpeciesDev &S = fp.sp[s];
             const float4 *lut = fp.lut_total > 0 ? s_lut + S.lut_off : fp.lut + s * kMaxLut;
             float3 a = amplitude(Is[j], ss[j], hs[j], S, lut);
-            const bool small = g.cls == SMALL;
+            const bool small = cls == SMALL;
             const float sp2 = __fmul_rn(g.sp, g.sp);
             const float w = small ? fp.csmall * sp2 : 1.0f;
             a.x *= w; a.y *= w; a.z *= w;
-            float4 ra, rb;
-            ra.x = g.px; ra.y = g.py;
-            ra.z = small ? 0.0f : __fdividef(-1.4426950408889634f, sp2);
-            ra.w = small ? __int_as_float(0x7f800000) : __fmul_rn(g.rp, g.rp);
             const float am = fmaxf(fabsf(a.x), fmaxf(fabsf(a.y), fabsf(a.z)));
             if (!(am <= 3.0e38f)) a = make_float3(0.0f, 0.0f, 0.0f);             // Inf / NaN amplitude
-            else if (g.cls != CULLED) amax = fmaxf(amax, am);
-            rb = make_float4(a.x, a.y, a.z, 0.0f);
-            const BinBox b = bin_box(g, fp);
-            if (b.n > 0) {
-                rb.w = __uint_as_float(pack_box(g, g.cls, b.bx0, b.by0, fp));
-                st_record(records, atomicAdd(&cursor[b.base + b.by0 * b.pitch + b.bx0], 1u), ra, rb);
+            else if (cls != CULLED) amax = fmaxf(amax, am);
+            const int tx0 = g.x0 >> ts, ty0 = g.y0 >> ts, tx1 = g.x1 >> ts, ty1 = g.y1 >> ts;
+            unsigned int *c00 = cursor + 2 * (ty0 * fp.ntx + tx0);
+            if (small) {
+                const unsigned int pix = (unsigned int)(((g.y0 & tmask) << ts) | (g.x0 & tmask));
+                const unsigned int u = cursor_take<GHIST>(c00 + 1, 1u);
+                asm volatile("st.global.v4.f32 [%0], {%1,%2,%3,%4};" :: "l"(records + u), "f"(__uint_as_float(pix)), "f"(a.x), "f"(a.y), "f"(a.z) : "memory");
             }
-            if (__any_sync(0xffffffffu, b.n > 1)) {
-                const int nmax = __reduce_max_sync(0xffffffffu, b.n);
-                int bx = b.bx0, by = b.by0;
-                for (int t = 1; t < nmax; ++t) {
-                    const bool wrap = bx == b.bx1;
-                    bx = wrap ? b.bx0 : bx + 1;
-                    by += wrap;
-                    if (t < b.n) {
-                        rb.w = __uint_as_float(pack_box(g, g.cls, bx, by, fp));
-                        st_record(records, atomicAdd(&cursor[b.base + by * b.pitch + bx], 1u), ra, rb);
-                    }
+            const float4 ra = make_float4(g.px, g.py, __fdividef(-1.4426950408889634f, sp2), __fmul_rn(g.rp, g.rp));
+            if (cls == MEDIUM) {
+                const bool w2 = tx1 > tx0, h2 = ty1 > ty0;
+                st_record(records, cursor_take<GHIST>(c00, 2u), ra, make_float4(a.x, a.y, a.z, __uint_as_float(pack_box_tile(g, tx0, ty0, fp))));
+                if (w2) st_record(records, cursor_take<GHIST>(c00 + 2, 2u), ra, make_float4(a.x, a.y, a.z, __uint_as_float(pack_box_tile(g, tx0 + 1, ty0, fp))));
+                if (h2) st_record(records, cursor_take<GHIST>(c00 + ntx2, 2u), ra, make_float4(a.x, a.y, a.z, __uint_as_float(pack_box_tile(g, tx0, ty0 + 1, fp))));
+                if (w2 && h2) st_record(records, cursor_take<GHIST>(c00 + ntx2 + 2, 2u), ra, make_float4(a.x, a.y, a.z, __uint_as_float(pack_box_tile(g, tx0 + 1, ty0 + 1, fp))));
+                if (tx1 - tx0 > 1 || ty1 - ty0 > 1) {
+                    for (int ty = ty0; ty <= ty1; ++ty)
+                        for (int tx = tx0; tx <= tx1; ++tx)
+                            if (tx - tx0 > 1 || ty - ty0 > 1)
+                                st_record(records, cursor_take<GHIST>(cursor + 2 * (ty * fp.ntx + tx), 2u), ra,
+                                          make_float4(a.x, a.y, a.z, __uint_as_float(pack_box_tile(g, tx, ty, fp))));
                 }
+            } else if (cls == LARGE) {
+                const int ss2 = fp.sshift;
+                for (int sy = g.y0 >> ss2; sy <= (g.y1 >> ss2); ++sy)
+                    for (int sx = g.x0 >> ss2; sx <= (g.x1 >> ss2); ++sx)
+                        st_record(records, cursor_take<GHIST>(cursor + 2 * fp.n_tiles + sy * fp.nsx + sx, 2u), ra,
+                                  make_float4(a.x, a.y, a.z, __uint_as_float(pack_box_super(g, sx, sy, fp))));
             }
         }
     }
@@ -632,17 +761,17 @@ __device__ __forceinline__ void fixed_add(unsigned int *lo, unsigned int *hi, fl
                  :: "r"(alo), "r"(ahi), "r"((unsigned int)v & 0xffffu), "r"(up) : "memory");
 }
 
-// Geometry of the tile renderer: a warp owns a strip of 64 pixels (16 x 4, or 8 x 8 for T = 8), a lane owns two
-// horizontally adjacent pixels of it and keeps their RGB sums in registers as packed pairs.
+// Geometry of the tile renderer: a warp owns a strip of the tile (16 x 4 pixels; 8 x 8 for T = 8; 64 x 4 for T = 64), a
+// lane owns kNP pairs of horizontally adjacent pixels of it and keeps their RGB sums in registers as packed pairs.
 template <int T> struct SplatCfg {
     static constexpr int kPix = T * T;
-    static constexpr int kSW = T >= 16 ? 16 : 8;         // strip width
-    static constexpr int kSH = 64 / kSW;                 // strip height
+    static constexpr int kNP = T == 64 ? 4 : 1;          // pixel pairs per lane
+    static constexpr int kSW = T == 64 ? 64 : (T >= 16 ? 16 : 8);   // strip width
+    static constexpr int kSH = 64 * kNP / kSW;           // strip height
     static constexpr int kStripsX = T / kSW, kStripsY = T / kSH;
-    static constexpr int kWarps = kStripsX * kStripsY;   // 1, 4, 16 for T = 8, 16, 32
+    static constexpr int kWarps = kStripsX * kStripsY;   // 1, 4, 16, 16 for T = 8, 16, 32, 64
     static constexpr int kThreads = 32 * kWarps;         // one record per thread and batch
     static constexpr int kFoldBatches = 1024 / kThreads > 0 ? 1024 / kThreads : 1;   // fold the sub-sums every ~1024 records
-    static constexpr size_t kSmemBytes = sizeof(unsigned int) * 6 * kPix + (sizeof(float4) * 2 + sizeof(unsigned int)) * kThreads;
 };
 
 // k_splat itself lives in splotch_splat.cuh.
@@ -672,6 +801,14 @@ k_compose(const unsigned long long *__restrict__ accum, const DeviceStats *__res
             }
         }
     }
+}
+
+// ---- test hook: per-tile pair counts (SMALL + MEDIUM bins of every tile) ---------------------------------------------
+__global__ void __launch_bounds__(256)
+k_tile_counts(const unsigned int *__restrict__ bin_count, int n_tiles, unsigned int *__restrict__ out)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < n_tiles) out[t] = bin_count[2 * t] + bin_count[2 * t + 1];
 }
 
 // ---- test hook: per-particle classification results -----------------------------------------------------------

@@ -30,7 +30,7 @@ constexpr int kLargeBlock = 32;           // block side in px
 constexpr int kLargePpt = 8;              // pixels per thread (one row segment)
 
 __global__ void __launch_bounds__(kLargeThreads)
-k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin_start,
+k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin_count, const uint2 *__restrict__ run,
         const unsigned int *__restrict__ large_off, DeviceStats *__restrict__ stats,
         unsigned long long *__restrict__ accum, const __grid_constant__ FrameParams fp)
 {
@@ -57,12 +57,17 @@ k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
     // this thread's pixels inside the block: 8 adjacent ones of one row
     const int row = threadIdx.x >> 2, col0 = (threadIdx.x & 3) * kLargePpt;
     unsigned int wcount = 0u;
+    const unsigned int slab_base_l = stats->slab_base[lane];
+    uint2 myrun = make_uint2(0u, 0u);            // warp 0: lane s holds run s of the item's super-tile bin
+    // window j of the current item (records [r0, r1) of the bin, counted over its runs) -> stage (wbase + j) % kLargeStages;
+    // called by all lanes of warp 0: every lane copies the part of its run inside the window
     auto issue = [&](unsigned int wbase, unsigned int j, unsigned int r0, unsigned int r1) {
         const unsigned int s = (wbase + j) % kLargeStages;
-        const unsigned int wb = r0 + j * kLargeWin, bytes = 32u * (min(wb + kLargeWin, r1) - wb);
+        const unsigned int wb = r0 + j * kLargeWin, cnt = min(wb + kLargeWin, r1) - wb;
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        mbar_expect_tx(smem_u32(mbar + s), bytes);
-        bulk_copy_g2s(smem_u32(&stage[s][0][0]), records + 2ull * wb, bytes, smem_u32(mbar + s));
+        (void)gather_bin(records, myrun, slab_base_l, 2u, 2u * wb, 2u * cnt, smem_u32(&stage[s][0][0]), smem_u32(mbar + s), lane);
+        if (lane == 0) mbar_expect_tx(smem_u32(mbar + s), 32u * cnt);
+        __syncwarp();
     };
     for (;;) {
         __syncthreads();
@@ -97,12 +102,14 @@ k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
         const int X0 = ((sup % fp.nsx) << fp.sshift) + qx0, Y0 = ((sup / fp.nsx) << fp.sshift) + qy0;
         if (X0 >= fp.W || Y0 >= fp.H) continue;                  // the super-tile hangs over the image edge
         const int qx1 = qx0 + kLargeBlock - 1, qy1 = qy0 + kLargeBlock - 1;
-        const unsigned int lb = bin_start[fp.n_tiles + sup], le = bin_start[fp.n_tiles + sup + 1];
-        const unsigned int r0 = lb + chunk * kLargeChunk, r1 = min(r0 + kLargeChunk, le);
+        const unsigned int le = bin_count[2 * fp.n_tiles + sup];              // records of the super-tile's bin
+        const unsigned int r0 = chunk * kLargeChunk, r1 = min(r0 + kLargeChunk, le);
         const unsigned int nwin = (r1 - r0 + kLargeWin - 1) / kLargeWin;
         const unsigned int wbase = wcount;
-        if (threadIdx.x == 0)
+        if (warp == 0) {
+            myrun = __ldg(run + (size_t)(2 * fp.n_tiles + sup) * kMaxSlabs + lane);
             for (unsigned int j = 0; j < min(nwin, (unsigned int)kLargeStages); ++j) issue(wbase, j, r0, r1);
+        }
         // centres of the block's corner pixels
         const float cxl = __fadd_rn((float)X0, 0.5f), cxh = __fadd_rn((float)(X0 + kLargeBlock - 1), 0.5f);
         const float cyl = __fadd_rn((float)Y0, 0.5f), cyh = __fadd_rn((float)(Y0 + kLargeBlock - 1), 0.5f);
@@ -152,7 +159,7 @@ k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
             if (lane == 0) { s_cnt[warp][0] = __popc(mi0) + __popc(mi1); s_cnt[warp][1] = __popc(mb0) + __popc(mb1); }
             __syncthreads();                 // counts visible; every warp is done with the previous window's lists
             // the stage of the previous window is free now: refill it
-            if (k >= 1u && threadIdx.x == 0 && k - 1u + kLargeStages < nwin) issue(wbase, k - 1u + kLargeStages, r0, r1);
+            if (k >= 1u && warp == 0 && k - 1u + kLargeStages < nwin) issue(wbase, k - 1u + kLargeStages, r0, r1);
             int ioff = 0, boff = 0, n_in = 0, n_cut = 0;
 #pragma unroll
             for (int w = 0; w < kLargeThreads / 32; ++w) {

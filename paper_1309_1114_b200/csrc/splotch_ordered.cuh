@@ -222,7 +222,7 @@ k_opairs(const float *__restrict__ x, const float *__restrict__ y, const float *
         }
         const float am = fmaxf(fmaxf(fabsf(rb.x), fabsf(rb.y)), fmaxf(fabsf(rb.z), fabsf(rb.w)));
         if (!(am <= 3.0e38f)) rb = make_float4(0.0f, 0.0f, 0.0f, 0.0f);   // Inf / NaN: a record without effect
-        st_record(rec, idx, ra, rb);
+        st_record(rec + (size_t)idx, idx, ra, rb);      // 32-byte record idx = units 2 idx
         const unsigned long long zkey = (unsigned long long)(~__float_as_uint(g[j].zc) - zkey_min);
         const int tx0 = g[j].x0 >> fp.tshift, tx1 = g[j].x1 >> fp.tshift;
         const int ty0 = g[j].y0 >> fp.tshift, ty1 = g[j].y1 >> fp.tshift;
