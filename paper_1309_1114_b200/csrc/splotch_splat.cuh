@@ -91,6 +91,19 @@ __device__ __forceinline__ unsigned int gather_bin(const float4 *__restrict__ re
     return total;
 }
 
+// the producer's wait for a free window: it is usually far ahead of the consumers, so it sleeps between polls instead of
+// taking issue slots from them (a spinning producer warp was 13 % of k_splat's instructions, profiles/r2_step2_*)
+__device__ __forceinline__ void mbar_wait_relaxed(unsigned int bar, unsigned int parity)
+{
+    unsigned int ok;
+    for (;;) {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+        if (ok) break;
+        __nanosleep(256);
+    }
+}
+
 template <int T>
 __global__ void __launch_bounds__(Splat2Cfg<T>::kThreads)
 k_splat(const float4 *__restrict__ records, const unsigned int *__restrict__ vstart, const uint2 *__restrict__ run,
@@ -101,7 +114,7 @@ k_splat(const float4 *__restrict__ records, const unsigned int *__restrict__ vst
     constexpr int kPix = Cfg::kPix, kConsumers = Cfg::kConsumers, kMaxRec = Cfg::kMaxRec, kNP = Geo::kNP;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float4 *stage = reinterpret_cast<float4 *>(smem_raw);                                        // [kSplatStages][kSplatWinUnits]
-    unsigned int *fb = reinterpret_cast<unsigned int *>(smem_raw + Cfg::kStageBytes * kSplatStages);   // lo R G B, hi R G B
+    unsigned int *fb = reinterpret_cast<unsigned int *>(stage + kSplatStages * kSplatWinUnits);  // lo R G B, hi R G B
     unsigned int *stM = fb + 6 * kPix;                                                           // [2][kMaxRec] strip masks
     unsigned short *hits = reinterpret_cast<unsigned short *>(stM + 2 * kMaxRec);                // [warps][kMaxRec] per-warp hit lists
     SplatWin *wins = reinterpret_cast<SplatWin *>(hits + kMaxRec * Geo::kWarps);
@@ -145,7 +158,7 @@ k_splat(const float4 *__restrict__ records, const unsigned int *__restrict__ vst
             uint2 myrun = __ldg(run + (size_t)bin * kMaxSlabs + lane);
             while (pos < v1) {
                 const unsigned int st = it % kSplatStages;
-                mbar_wait(smem_u32(empty + st), ((it / kSplatStages) & 1u) ^ 1u);
+                mbar_wait_relaxed(smem_u32(empty + st), ((it / kSplatStages) & 1u) ^ 1u);
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                 SplatWin *wd = wins + st;
                 unsigned int fill = 0u;
@@ -185,7 +198,7 @@ k_splat(const float4 *__restrict__ records, const unsigned int *__restrict__ vst
         }
         // no chunk is left: tell the consumers
         const unsigned int st = it % kSplatStages;
-        mbar_wait(smem_u32(empty + st), ((it / kSplatStages) & 1u) ^ 1u);
+        mbar_wait_relaxed(smem_u32(empty + st), ((it / kSplatStages) & 1u) ^ 1u);
         if (lane == 0) { wins[st].n_sub = 0; wins[st].flags = kSplatExit; mbar_arrive(smem_u32(full + st)); }
         return;
     }
@@ -316,7 +329,8 @@ k_splat(const float4 *__restrict__ records, const unsigned int *__restrict__ vst
                 nh += __popc(m);
             }
             __syncwarp();
-            auto eval = [&](const float4 &A, const float4 &B) {
+            auto eval = [&](unsigned int r) {
+                const float4 A = recs[2 * r], B = recs[2 * r + 1];
                 const float dyf = __fsub_rn(fy, A.y);
                 const float t2 = __fmul_rn(dyf, dyf);
                 const f32x2 NX = pk2(-A.x, -A.x), T2 = pk2(t2, t2), C = pk2(A.z, A.z);
@@ -336,17 +350,11 @@ k_splat(const float4 *__restrict__ records, const unsigned int *__restrict__ vst
             };
             unsigned int j = 0u;
 #pragma unroll 1
-            for (; j + 1u < nh; j += 2u) {
-                const unsigned int pr = *reinterpret_cast<const unsigned int *>(hl + j);
-                const float4 A0 = recs[2 * (pr & 0xffffu)], B0 = recs[2 * (pr & 0xffffu) + 1];
-                const float4 A1 = recs[2 * (pr >> 16)], B1 = recs[2 * (pr >> 16) + 1];
-                eval(A0, B0);
-                eval(A1, B1);
+            for (; j + 3u < nh; j += 4u) {           // four hits per round: one 64-bit read of the list, four independent chains
+                const uint2 pr = *reinterpret_cast<const uint2 *>(hl + j);
+                eval(pr.x & 0xffffu); eval(pr.x >> 16); eval(pr.y & 0xffffu); eval(pr.y >> 16);
             }
-            if (j < nh) {
-                const unsigned int r = hl[j];
-                eval(recs[2 * r], recs[2 * r + 1]);
-            }
+            for (; j < nh; ++j) eval(hl[j]);
             __syncwarp();                            // the list is rewritten in the next sub-range
             since += cnt;
             if (since >= 1024u) {                    // two-level sums: float32 stays accurate to ~1e-6
