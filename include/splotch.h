@@ -141,12 +141,24 @@ int splotch_render(splotch_ctx *ctx, const splotch_particles *particles, uint64_
                    const splotch_params *params, float *image_out,
                    void *workspace, size_t workspace_bytes, void *cuda_stream);
 
-/* Same frame from HOST particle arrays into a HOST image: copies the six fields to the staging area of the
- * workspace, renders, copies the image back and synchronises the stream before returning.
- * workspace must have been sized with with_host_staging = 1. */
+/* Same frame from HOST particle arrays into a HOST image, synchronising the stream before returning.
+ * workspace must have been sized with with_host_staging = 1.
+ * Additive mode: the paper's per-chunk offload loop (Fig. 3; Eq. 3-4 :111-120) with copy / compute
+ * overlap (:354): the set streams through two staging buffers in chunks (splotch_set_host_chunk), the copy of chunk
+ * k + 1 runs on a second stream while chunk k is binned and splatted, the chunks' partial images add up exactly in the
+ * tiles' fixed-point sums.  Only one chunk's records live in the workspace at a time, so a set whose pairs exceed the
+ * workspace's record capacity still renders as long as every chunk's pairs fit (out-of-core rendering).
+ * splotch_get_stats then reports the totals of the frame; splotch_debug_tile_counts the last chunk only; per-stage
+ * timings are not recorded for chunked frames.
+ * Ordered mode: the depth order needs the whole set: one copy in, one frame, one copy out, nothing overlaps. */
 int splotch_render_host(splotch_ctx *ctx, const splotch_particles *host_particles, uint64_t n,
                         const splotch_params *params, float *host_image_out,
                         void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* Particles per chunk of splotch_render_host (additive mode).  0 (the default) picks about eight chunks of 2^20 ..
+ * 2^25 particles.  The staging buffers of the workspace are sized for this value: set it before asking
+ * splotch_workspace_bytes. */
+int splotch_set_host_chunk(splotch_ctx *ctx, uint64_t particles_per_chunk);
 
 /* Statistics of the last frame.  Synchronises the stream of that frame.  HOST out. */
 int splotch_get_stats(splotch_ctx *ctx, splotch_stats *out);

@@ -25,7 +25,7 @@ EXPORTS = (
     "splotch_create", "splotch_destroy", "splotch_set_camera", "splotch_get_camera_constants",
     "splotch_set_colormap", "splotch_set_profiling", "splotch_workspace_bytes", "splotch_render",
     "splotch_render_host", "splotch_get_stats", "splotch_stage_name", "splotch_debug_geometry",
-    "splotch_debug_tile_counts", "splotch_last_error", "splotch_version", "splotch_measure_peaks",
+    "splotch_debug_tile_counts", "splotch_last_error", "splotch_version", "splotch_measure_peaks", "splotch_set_host_chunk",
 )
 
 
@@ -88,6 +88,7 @@ def load() -> C.CDLL:
     lib.splotch_debug_geometry.argtypes = [vp, C.POINTER(SplotchParticles), u64, C.POINTER(SplotchParams)] + [vp] * 10
     lib.splotch_debug_tile_counts.argtypes = [vp, vp, vp]
     lib.splotch_measure_peaks.argtypes = [vp, C.POINTER(C.c_double), vp]
+    lib.splotch_set_host_chunk.argtypes = [vp, u64]
     lib.splotch_last_error.argtypes = [vp]
     lib.splotch_last_error.restype = C.c_char_p
     lib.splotch_version.restype = C.c_char_p
@@ -199,6 +200,10 @@ class Renderer:
 
     def set_profiling(self, on: bool) -> None:
         _check(self.ctx, self.lib.splotch_set_profiling(self.ctx, int(on)))
+
+    def set_host_chunk(self, particles_per_chunk: int) -> None:
+        _check(self.ctx, self.lib.splotch_set_host_chunk(self.ctx, particles_per_chunk))
+        self._ws = None
 
     def measure_peaks(self) -> Dict[str, float]:
         out = (C.c_double * 2)()

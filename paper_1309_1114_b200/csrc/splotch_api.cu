@@ -25,7 +25,7 @@ const char *kStageNamesAdditive[kStagesAdditive] = {"count", "scan", "scatter", 
 const char *kStageNamesOrdered[kStagesOrdered] = {"count", "scan", "pairs", "sort", "bounds", "render", "combine"};
 
 struct Layout {
-    size_t counts, counts_bytes, cls_counts, bin_count, vstart, large_off, run, stats, accum, accum_bytes, records, staging, total;
+    size_t counts, counts_bytes, cursors, cls_counts, bin_count, vstart, large_off, run, stats, accum, accum_bytes, records, staging, total;
     bool ghist;
     unsigned long long capacity;
     int nrows;
@@ -58,6 +58,9 @@ struct splotch_ctx {
     bool last_additive = true;
     int prof_stages = kStagesAdditive;              // stages of the frames recorded since profiling was enabled
     cudaStream_t last_stream = nullptr;
+    unsigned long long host_chunk = 0;       // particles per chunk of splotch_render_host (0: automatic)
+    cudaStream_t copy_stream = nullptr;      // host-to-device copies of splotch_render_host run here, beside the kernels
+    cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_consumed[2] = {nullptr, nullptr}, ev_start = nullptr;
     int splat_blocks_per_sm[4] = {0, 0, 0, 0};  // T = 8, 16, 32, 64
     int orender_blocks_per_sm[3] = {0, 0, 0};
     int large_blocks_per_sm = 0;
@@ -114,6 +117,28 @@ int bin_rows(const splotch_ctx *c, int T)
     return c->n_sm;                         // one 1024-thread CTA per SM, each with a private histogram over all bins
 }
 
+// Particles per chunk of a chunked host frame: about eight chunks, between 2^20 and 2^25 particles, a multiple of 4
+unsigned long long host_chunk_particles(const splotch_ctx *c, unsigned long long n)
+{
+    unsigned long long ch = c->host_chunk;
+    if (ch == 0) {
+        ch = (n + 7) / 8;
+        if (ch < (1ull << 20)) ch = 1ull << 20;
+        if (ch > (1ull << 25)) ch = 1ull << 25;
+    }
+    ch = (ch + 3) / 4 * 4;
+    return ch < n ? ch : (n + 3) / 4 * 4;
+}
+
+// staging of splotch_render_host: two buffers of six fields for one chunk each (additive) or one buffer for the whole
+// set (ordered), then the device image
+size_t staging_bytes(const splotch_ctx *c, unsigned long long n, bool additive)
+{
+    const unsigned long long per = additive ? host_chunk_particles(c, n) : n;
+    const size_t fields = 6 * align_up(sizeof(float) * per, 256) * (additive ? 2 : 1);
+    return align_up(fields, 256) + align_up(sizeof(float) * 3 * (size_t)c->width * c->height, 256);
+}
+
 // Workspace layout.  Either `capacity` is given (sizing query) or derived from `bytes` (render).
 bool make_layout(const splotch_ctx *c, unsigned long long n, int T, unsigned long long capacity, size_t bytes,
                  bool staging, Layout *L)
@@ -125,6 +150,7 @@ bool make_layout(const splotch_ctx *c, unsigned long long n, int T, unsigned lon
     L->ghist = use_global_hist(c, T);
     size_t off = 0;
     L->counts = off;      L->counts_bytes = sizeof(unsigned int) * nbins * L->nrows; off = align_up(off + L->counts_bytes, 256);
+    L->cursors = off;     if (L->ghist) off = align_up(off + L->counts_bytes, 256);      // k_scatter's cursors when they do not fit in shared memory
     L->cls_counts = off;  off = align_up(off + sizeof(unsigned int) * 4 * L->nrows, 256);
     L->bin_count = off;   off = align_up(off + sizeof(unsigned int) * nbins, 256);
     L->vstart = off;      off = align_up(off + sizeof(unsigned int) * (nbins + 1), 256);
@@ -136,10 +162,7 @@ bool make_layout(const splotch_ctx *c, unsigned long long n, int T, unsigned lon
     L->accum_bytes = sizeof(unsigned long long) * 3 * (size_t)T * T * n_tiles;
     off = align_up(off + L->accum_bytes, 256);
     L->staging = off;
-    if (staging) {
-        off = align_up(off + 6 * align_up(sizeof(float) * n, 256), 256);
-        off = align_up(off + sizeof(float) * 3 * (size_t)c->width * c->height, 256);
-    }
+    if (staging) off = align_up(off + staging_bytes(c, n, true), 256);
     // every run of SMALL records may be padded by one 16-byte unit (k_layout): an allowance beside the capacity
     const size_t pad = align_up(16 * (size_t)kMaxSlabs * n_tiles + 16 * nbins, 256);
     const size_t fixed = off + pad;
@@ -175,10 +198,7 @@ void make_layout_ordered(const splotch_ctx *c, unsigned long long n, int T, unsi
     L->sums = off;        off = align_up(off + sizeof(unsigned int) * (size_t)L->n_sums, 256);
     L->rec = off;         off = align_up(off + 32ull * n, 256);
     L->staging = off;
-    if (staging) {
-        off = align_up(off + 6 * align_up(sizeof(float) * n, 256), 256);
-        off = align_up(off + sizeof(float) * 3 * (size_t)c->width * c->height, 256);
-    }
+    if (staging) off = align_up(off + staging_bytes(c, n, false), 256);
     for (int k = 0; k < 2; ++k) { L->keys[k] = off; off = align_up(off + 8ull * capacity, 256); }
     for (int k = 0; k < 2; ++k) { L->vals[k] = off; off = align_up(off + 4ull * capacity, 256); }
     // one (t, c_R, c_G, c_B) per pixel and segment; segment slot = chunk + tile; k_oscan cuts the pairs into at most
@@ -291,20 +311,20 @@ bool aligned16(const splotch_particles *p)
 }
 
 template <int T>
-int launch_render_tail(splotch_ctx *c, const Layout &L, char *ws, const FrameParams &fp, float *image, cudaStream_t st)
+int launch_render_tail(splotch_ctx *c, const Layout &L, char *ws, const FrameParams &fp, float *image, cudaStream_t st, bool prof, bool compose)
 {
     const int ti = T == 8 ? 0 : T == 16 ? 1 : T == 32 ? 2 : 3;
     const int grid = c->n_sm * c->splat_blocks_per_sm[ti];
     k_splat<T><<<grid, Splat2Cfg<T>::kThreads, Splat2Cfg<T>::kSmemBytes, st>>>(
         (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.vstart), (const uint2 *)(ws + L.run), (DeviceStats *)(ws + L.stats),
         (unsigned long long *)(ws + L.accum), fp);
-    if (c->profiling) cudaEventRecord(c->ev[4], st);
+    if (prof) cudaEventRecord(c->ev[4], st);
     k_large<<<c->n_sm * c->large_blocks_per_sm, kLargeThreads, 0, st>>>(
         (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.bin_count), (const uint2 *)(ws + L.run), (const unsigned int *)(ws + L.large_off),
         (DeviceStats *)(ws + L.stats), (unsigned long long *)(ws + L.accum), fp);
-    if (c->profiling) cudaEventRecord(c->ev[5], st);
-    k_compose<T><<<fp.n_tiles, 256, 0, st>>>((const unsigned long long *)(ws + L.accum), (const DeviceStats *)(ws + L.stats), fp, image);
-    if (c->profiling) cudaEventRecord(c->ev[6], st);
+    if (prof) cudaEventRecord(c->ev[5], st);
+    if (compose) k_compose<T><<<fp.n_tiles, 256, 0, st>>>((const unsigned long long *)(ws + L.accum), (const DeviceStats *)(ws + L.stats), fp, image);
+    if (prof) cudaEventRecord(c->ev[6], st);
     return SPLOTCH_OK;
 }
 
@@ -317,16 +337,20 @@ void launch_count(const Layout &L, size_t hbytes, const splotch_particles *p, un
 
 template <bool AL, bool GH>
 void launch_scatter(const Layout &L, size_t hbytes, const splotch_particles *p, unsigned long long n, unsigned long long per,
-                    const FrameParams &fp, unsigned int *counts, const uint2 *run, DeviceStats *stats, float4 *records, cudaStream_t st)
+                    const FrameParams &fp, unsigned int *counts, unsigned int *cursors, const uint2 *run, DeviceStats *stats, float4 *records,
+                    cudaStream_t st)
 {
     k_scatter<AL, GH><<<L.nrows, kBinThreads, GH ? sizeof(float4) * kLutSmemMax : hbytes, st>>>(p->x, p->y, p->z, p->h, p->I, p->scalar, n, per, fp,
-                                                                                           counts, run, stats, records);
+                                                                                           counts, cursors, run, stats, records);
 }
 
+struct ChunkCtl { bool first, last, chunked; };     // one-shot frame: {true, true, false}
+
 int render_device(splotch_ctx *c, const splotch_particles *p, unsigned long long n, const FrameParams &fp,
-                  const Layout &L, float *image, char *ws, cudaStream_t st)
+                  const Layout &L, float *image, char *ws, cudaStream_t st, ChunkCtl ctl = {true, true, false})
 {
     const bool al = aligned16(p);
+    const bool prof = c->profiling && !ctl.chunked;          // per-stage events describe one-shot frames
     const size_t hbytes = bin_smem_bytes(fp.W, fp.H, fp.T);
     unsigned long long per = (n + L.nrows - 1) / L.nrows;
     per = (per + 3) / 4 * 4;
@@ -337,35 +361,41 @@ int render_device(splotch_ctx *c, const splotch_particles *p, unsigned long long
     unsigned int *vstart = (unsigned int *)(ws + L.vstart);
     uint2 *run = (uint2 *)(ws + L.run);
     DeviceStats *stats = (DeviceStats *)(ws + L.stats);
-    if (c->profiling) {
+    if (prof) {
         if (c->prof_stages != kStagesAdditive || c->last_stream != st) c->prof_frames = 0;   // a session covers one mode and one stream
         c->ev = c->ev_ring[c->prof_frames % kProfRing];
         cudaEventRecord(c->ev[0], st);
     }
-    cudaMemsetAsync(ws + L.stats, 0, (L.accum - L.stats) + L.accum_bytes, st);      // DeviceStats + the tiles' sums
+    if (ctl.first) cudaMemsetAsync(ws + L.stats, 0, (L.accum - L.stats) + L.accum_bytes, st);      // DeviceStats + the tiles' sums
+    else cudaMemsetAsync(ws + L.stats, 0, offsetof(DeviceStats, f_count), st);                     // the chunk part of DeviceStats
     if (L.ghist) cudaMemsetAsync(counts, 0, L.counts_bytes, st);                    // the blocks count straight into their rows
     if (L.ghist) { if (al) launch_count<true, true>(L, hbytes, p, n, per, fp, counts, cls_counts, st); else launch_count<false, true>(L, hbytes, p, n, per, fp, counts, cls_counts, st); }
     else         { if (al) launch_count<true, false>(L, hbytes, p, n, per, fp, counts, cls_counts, st); else launch_count<false, false>(L, hbytes, p, n, per, fp, counts, cls_counts, st); }
-    if (c->profiling) cudaEventRecord(c->ev[1], st);
+    if (prof) cudaEventRecord(c->ev[1], st);
     const int bps = 1 << (fp.sshift - 5);               // 32-px blocks per super-tile side (k_large's work items)
     k_scan<<<(fp.nbins + 31) / 32, kScanThreads, 0, st>>>(counts, L.nrows, fp.nbins, fp.n_tiles, bin_count, vstart, cls_counts, 2ull * L.capacity,
                                                           c->n_sm, (unsigned int *)(ws + L.large_off), (unsigned int)kLargeChunk,
                                                           (unsigned int)(bps * bps), stats);
     k_layout<<<kMaxSlabs, kLayoutThreads, 0, st>>>(counts, bin_count, L.nrows, fp.nbins, fp.n_tiles, run, stats);
-    if (c->profiling) cudaEventRecord(c->ev[2], st);
+    if (prof) cudaEventRecord(c->ev[2], st);
     float4 *records = (float4 *)(ws + L.records);
-    if (L.ghist) { if (al) launch_scatter<true, true>(L, hbytes, p, n, per, fp, counts, run, stats, records, st); else launch_scatter<false, true>(L, hbytes, p, n, per, fp, counts, run, stats, records, st); }
-    else         { if (al) launch_scatter<true, false>(L, hbytes, p, n, per, fp, counts, run, stats, records, st); else launch_scatter<false, false>(L, hbytes, p, n, per, fp, counts, run, stats, records, st); }
-    if (c->profiling) cudaEventRecord(c->ev[3], st);
+    unsigned int *cursors = (unsigned int *)(ws + L.cursors);
+    if (L.ghist) { if (al) launch_scatter<true, true>(L, hbytes, p, n, per, fp, counts, cursors, run, stats, records, st); else launch_scatter<false, true>(L, hbytes, p, n, per, fp, counts, cursors, run, stats, records, st); }
+    else         { if (al) launch_scatter<true, false>(L, hbytes, p, n, per, fp, counts, cursors, run, stats, records, st); else launch_scatter<false, false>(L, hbytes, p, n, per, fp, counts, cursors, run, stats, records, st); }
+    if (prof) cudaEventRecord(c->ev[3], st);
+    if (ctl.chunked) {        // the tiles' sums follow the fixed-point unit of the largest amplitude so far
+        k_rescale<<<4 * c->n_sm, 256, 0, st>>>((long long *)(ws + L.accum), L.accum_bytes / sizeof(long long), stats);
+        k_rescale_done<<<1, 1, 0, st>>>(stats);
+    }
     int rc;
-    if (fp.T == 8) rc = launch_render_tail<8>(c, L, ws, fp, image, st);
-    else if (fp.T == 16) rc = launch_render_tail<16>(c, L, ws, fp, image, st);
-    else if (fp.T == 32) rc = launch_render_tail<32>(c, L, ws, fp, image, st);
-    else rc = launch_render_tail<64>(c, L, ws, fp, image, st);
+    if (fp.T == 8) rc = launch_render_tail<8>(c, L, ws, fp, image, st, prof, ctl.last);
+    else if (fp.T == 16) rc = launch_render_tail<16>(c, L, ws, fp, image, st, prof, ctl.last);
+    else if (fp.T == 32) rc = launch_render_tail<32>(c, L, ws, fp, image, st, prof, ctl.last);
+    else rc = launch_render_tail<64>(c, L, ws, fp, image, st, prof, ctl.last);
     if (rc != SPLOTCH_OK) return rc;
     CU_TRY(c, cudaGetLastError());
     c->have_frame = true; c->ws = ws; c->lay = L; c->fp = fp; c->last_n = n; c->last_stream = st; c->last_additive = true;
-    if (c->profiling) { ++c->prof_frames; c->prof_stages = kStagesAdditive; }
+    if (prof) { ++c->prof_frames; c->prof_stages = kStagesAdditive; }
     return SPLOTCH_OK;
 }
 
@@ -522,6 +552,9 @@ int splotch_destroy(splotch_ctx *c)
     if (!c) return SPLOTCH_EINVAL;
     cudaSetDevice(c->device);
     if (c->lut) cudaFree(c->lut);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    for (int k = 0; k < 2; ++k) { if (c->ev_copied[k]) cudaEventDestroy(c->ev_copied[k]); if (c->ev_consumed[k]) cudaEventDestroy(c->ev_consumed[k]); }
+    if (c->ev_start) cudaEventDestroy(c->ev_start);
     if (c->ev_ring) {
         for (int f = 0; f < kProfRing; ++f)
             for (int i = 0; i <= kStages; ++i)
@@ -632,6 +665,18 @@ int splotch_render(splotch_ctx *c, const splotch_particles *p, uint64_t n, const
     return render_device(c, p, n, fp, L, image_out, (char *)workspace, (cudaStream_t)cuda_stream);
 }
 
+int splotch_set_host_chunk(splotch_ctx *c, uint64_t particles_per_chunk)
+{
+    if (!c) return SPLOTCH_EINVAL;
+    c->host_chunk = particles_per_chunk;
+    return SPLOTCH_OK;
+}
+
+// The paper's per-chunk offload loop (Fig. 3; Eq. 3-4 :111-120) with the copy / compute overlap it names
+// as future work (:354): the particle set streams through two staging buffers, the host-to-device copy of chunk k + 1 runs
+// on the context's copy stream while chunk k is counted, binned and splatted on the caller's stream; the chunks' partial
+// images accumulate in the tiles' fixed-point sums (exact, order independent), one k_compose and one copy back at the end.
+// The ordered mode needs the whole set for its depth sort: one copy in, one frame, one copy out.
 int splotch_render_host(splotch_ctx *c, const splotch_particles *hp, uint64_t n, const splotch_params *q,
                         float *host_image_out, void *workspace, size_t workspace_bytes, void *cuda_stream)
 {
@@ -647,19 +692,66 @@ int splotch_render_host(splotch_ctx *c, const splotch_particles *hp, uint64_t n,
     CU_TRY(c, cudaSetDevice(c->device));
     cudaStream_t st = (cudaStream_t)cuda_stream;
     char *ws = (char *)workspace;
-    const size_t fstride = align_up(sizeof(float) * n, 256);
     const float *src[6] = {hp->x, hp->y, hp->z, hp->h, hp->I, hp->scalar};
-    float *dst[6];
-    for (int k = 0; k < 6; ++k) {
-        dst[k] = (float *)(ws + L.staging + k * fstride);
-        if (n) CU_TRY(c, cudaMemcpyAsync(dst[k], src[k], sizeof(float) * n, cudaMemcpyHostToDevice, st));
+    const size_t image_bytes = sizeof(float) * 3 * (size_t)c->width * c->height;
+    if (!q->additive) {
+        const size_t fstride = align_up(sizeof(float) * n, 256);
+        float *dst[6];
+        for (int k = 0; k < 6; ++k) {
+            dst[k] = (float *)(ws + L.staging + k * fstride);
+            if (n) CU_TRY(c, cudaMemcpyAsync(dst[k], src[k], sizeof(float) * n, cudaMemcpyHostToDevice, st));
+        }
+        float *dimg = (float *)(ws + L.staging + align_up(6 * fstride, 256));
+        splotch_particles dp = *hp;
+        dp.x = dst[0]; dp.y = dst[1]; dp.z = dst[2]; dp.h = dst[3]; dp.I = dst[4]; dp.scalar = dst[5];
+        rc = render_ordered(c, &dp, n, fp, L, dimg, ws, st);
+        if (rc != SPLOTCH_OK) return rc;
+        CU_TRY(c, cudaMemcpyAsync(host_image_out, dimg, image_bytes, cudaMemcpyDeviceToHost, st));
+        CU_TRY(c, cudaStreamSynchronize(st));
+        return SPLOTCH_OK;
     }
-    float *dimg = (float *)(ws + L.staging + align_up(6 * fstride, 256));
-    splotch_particles dp = *hp;
-    dp.x = dst[0]; dp.y = dst[1]; dp.z = dst[2]; dp.h = dst[3]; dp.I = dst[4]; dp.scalar = dst[5];
-    rc = q->additive ? render_device(c, &dp, n, fp, L, dimg, ws, st) : render_ordered(c, &dp, n, fp, L, dimg, ws, st);
-    if (rc != SPLOTCH_OK) return rc;
-    CU_TRY(c, cudaMemcpyAsync(host_image_out, dimg, sizeof(float) * 3 * (size_t)c->width * c->height, cudaMemcpyDeviceToHost, st));
+    // ---- additive: chunks on two streams
+    if (!c->copy_stream) {
+        CU_TRY(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+        for (int k = 0; k < 2; ++k) {
+            CU_TRY(c, cudaEventCreateWithFlags(&c->ev_copied[k], cudaEventDisableTiming));
+            CU_TRY(c, cudaEventCreateWithFlags(&c->ev_consumed[k], cudaEventDisableTiming));
+        }
+        CU_TRY(c, cudaEventCreateWithFlags(&c->ev_start, cudaEventDisableTiming));
+    }
+    const unsigned long long ch = host_chunk_particles(c, n);
+    const size_t fstride = align_up(sizeof(float) * ch, 256);
+    float *dimg = (float *)(ws + L.staging + align_up(2 * 6 * fstride, 256));
+    const unsigned long long nchunks = n ? (n + ch - 1) / ch : 1;
+    const int ns = fp.n_species;
+    unsigned long long sp_begin[kMaxSpecies + 1];
+    for (int s = 0; s <= ns; ++s) sp_begin[s] = hp->species_offsets ? hp->species_offsets[s] : (s == 0 ? 0ull : n);
+    CU_TRY(c, cudaEventRecord(c->ev_start, st));                 // the staging buffers are free once earlier work on `st` is done
+    CU_TRY(c, cudaStreamWaitEvent(c->copy_stream, c->ev_start, 0));
+    for (unsigned long long k = 0; k < nchunks; ++k) {
+        const unsigned long long lo = k * ch, len = n ? (lo + ch < n ? ch : n - lo) : 0;
+        const int b = (int)(k & 1);
+        float *dst[6];
+        if (k >= 2) CU_TRY(c, cudaStreamWaitEvent(c->copy_stream, c->ev_consumed[b], 0));
+        for (int f = 0; f < 6; ++f) {
+            dst[f] = (float *)(ws + L.staging + (size_t)(6 * b + f) * fstride);
+            if (len) CU_TRY(c, cudaMemcpyAsync(dst[f], src[f] + lo, sizeof(float) * len, cudaMemcpyHostToDevice, c->copy_stream));
+        }
+        CU_TRY(c, cudaEventRecord(c->ev_copied[b], c->copy_stream));
+        CU_TRY(c, cudaStreamWaitEvent(st, c->ev_copied[b], 0));
+        splotch_particles dp = *hp;
+        dp.x = dst[0]; dp.y = dst[1]; dp.z = dst[2]; dp.h = dst[3]; dp.I = dst[4]; dp.scalar = dst[5];
+        FrameParams fc = fp;                                      // the chunk's own species ranges
+        for (int s = 0; s <= ns; ++s) {
+            const unsigned long long o = sp_begin[s] < lo ? 0ull : (sp_begin[s] - lo < len ? sp_begin[s] - lo : len);
+            fc.sp_begin[s] = (unsigned int)o;
+        }
+        rc = render_device(c, &dp, len, fc, L, dimg, ws, st, ChunkCtl{k == 0, k + 1 == nchunks, nchunks > 1});
+        if (rc != SPLOTCH_OK) return rc;
+        CU_TRY(c, cudaEventRecord(c->ev_consumed[b], st));
+    }
+    c->last_n = n;
+    CU_TRY(c, cudaMemcpyAsync(host_image_out, dimg, image_bytes, cudaMemcpyDeviceToHost, st));
     CU_TRY(c, cudaStreamSynchronize(st));
     return SPLOTCH_OK;
 }
@@ -674,9 +766,16 @@ int splotch_get_stats(splotch_ctx *c, splotch_stats *out)
     CU_TRY(c, cudaMemcpy(&ds, c->ws + c->lay.stats, sizeof ds, cudaMemcpyDeviceToHost));
     memset(out, 0, sizeof *out);
     out->n = c->last_n;
-    for (int k = 0; k < 4; ++k) out->count[k] = ds.count[k];
-    out->pairs = ds.pairs; out->large_pairs = ds.large_pairs; out->chunks = ds.chunks;
-    out->pair_capacity = ds.capacity; out->overflow = (int32_t)ds.overflow;
+    if (c->last_additive) {       // totals of the frame (a chunked host frame sums its chunks)
+        for (int k = 0; k < 4; ++k) out->count[k] = ds.f_count[k];
+        out->pairs = ds.f_pairs; out->large_pairs = ds.f_large_pairs; out->chunks = ds.f_chunks;
+        out->overflow = (int32_t)ds.f_overflow;
+    } else {
+        for (int k = 0; k < 4; ++k) out->count[k] = ds.count[k];
+        out->pairs = ds.pairs; out->large_pairs = ds.large_pairs; out->chunks = ds.chunks;
+        out->overflow = (int32_t)ds.overflow;
+    }
+    out->pair_capacity = ds.capacity;
     out->sort_key_bits = c->last_additive ? 0 : (int32_t)ds.key_bits;
     if (c->profiling && c->prof_frames > 0) {
         // mean per frame over the frames recorded since profiling was enabled (at most the last kProfRing)

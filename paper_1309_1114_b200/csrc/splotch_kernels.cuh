@@ -69,10 +69,17 @@ struct DeviceStats {             // cleared before every frame; written by k_sca
     unsigned long long sort_n;   // ordered mode: pairs the sort and the renderer work on (0 on overflow)
     // ordered mode, sort key = tile << zbits | (~bits(z_c) - zkey_min): only the bits that differ in this frame are sorted
     unsigned int zkey_max, nzkey_max, zkey_min, zbits, key_bits, pad2;     // nzkey_max = max of ~zkey (its complement is the min)
-    unsigned int overflow, work_counter, chunk_size, amax_bits, scan_done, large_counter;   // large_counter: work items of k_large
+    unsigned int overflow, work_counter, chunk_size, pad3, scan_done, large_counter;   // large_counter: work items of k_large
     // additive layout (k_scan, k_layout): all offsets in 16-byte units
     unsigned int slabs, rows_per_slab, tile_units, total_units, layout_done, small_pairs;
     unsigned int slab_base[32];
+    // ---- frame part: cleared once per frame.  A frame rendered in chunks (splotch_render_host streams the particle set
+    //      through the device) clears only what is above between chunks and sums its totals here
+    unsigned long long f_count[4], f_pairs, f_large_pairs, f_chunks;
+    unsigned int f_overflow;
+    unsigned int amax_bits;      // largest record amplitude so far (float bits): fixes the fixed-point unit of the tiles' sums
+    int accum_exp;               // exponent the tiles' sums are held in (chunked frames: k_rescale follows amax_bits)
+    unsigned int accum_exp_set;
 };
 
 struct Geo {
@@ -466,8 +473,19 @@ k_scan(unsigned int *__restrict__ counts, int nrows, int nbins, int n_tiles, uns
         stats->work_counter = 0u;
         stats->chunk_size = K;
         stats->scan_done = 0u;
+        // totals of the frame (the only chunk of a one-shot frame, or this chunk added to the earlier ones)
+        stats->f_count[0] += stats->count[0]; stats->f_count[1] += s_tot_small; stats->f_count[2] += s_cls[2]; stats->f_count[3] += s_cls[3];
+        stats->f_pairs += tile_records; stats->f_large_pairs += large_records;
+        stats->f_chunks += stats->chunks;
+        stats->f_overflow |= overflow ? 1u : 0u;
     }
 }
+
+// Chunked frames: the fixed-point unit of the tiles' sums follows the largest record amplitude seen so far.  When a chunk
+// raises it, the sums of the earlier chunks are shifted to the new unit (rounded to nearest) before the chunk is added.
+__global__ void __launch_bounds__(256)
+k_rescale(long long *__restrict__ accum, size_t n, const DeviceStats *__restrict__ stats);
+__global__ void k_rescale_done(DeviceStats *stats);
 
 // One block per slab s (blocks beyond the frame's slab count leave at once): the slab's runs.  Run (s, bin) holds the
 // bin's records that the rows of slab s produce: cnt = P[(s + 1) rows_per_slab][bin] - P[s rows_per_slab][bin] with P the
@@ -619,7 +637,7 @@ __global__ void __launch_bounds__(kBinThreads, 1)
 k_scatter(const float *__restrict__ x, const float *__restrict__ y, const float *__restrict__ z,
           const float *__restrict__ h, const float *__restrict__ I, const float *__restrict__ scalar,
           unsigned long long n, unsigned long long per, const __grid_constant__ FrameParams fp,
-          unsigned int *__restrict__ counts, const uint2 *__restrict__ run,
+          const unsigned int *__restrict__ counts, unsigned int *__restrict__ cursor_rows, const uint2 *__restrict__ run,
           DeviceStats *__restrict__ stats, float4 *__restrict__ records)
 {
     extern __shared__ unsigned int cursor_s[];               // nbins cursors, then the packed colour tables
@@ -627,8 +645,8 @@ k_scatter(const float *__restrict__ x, const float *__restrict__ y, const float 
     if (stats->overflow) return;
     float4 *s_lut = reinterpret_cast<float4 *>(cursor_s + (GHIST ? 0 : ((fp.nbins + 3) & ~3)));
     // this block's cursors: slab base + the run's first unit + the units of the slab's rows before this one
-    unsigned int *row = counts + (size_t)blockIdx.x * fp.nbins;
-    unsigned int *cursor = GHIST ? row : cursor_s;
+    const unsigned int *row = counts + (size_t)blockIdx.x * fp.nbins;
+    unsigned int *cursor = GHIST ? cursor_rows + (size_t)blockIdx.x * fp.nbins : cursor_s;     // GHIST: a row of its own in global memory
     {
         const unsigned int cps = stats->rows_per_slab, s = blockIdx.x / cps;
         const unsigned int base = stats->slab_base[s];
@@ -739,6 +757,24 @@ __device__ __forceinline__ int fixed_exponent(unsigned int amax_bits)
     return kFixedBits - ex;
 }
 
+__global__ void __launch_bounds__(256)
+k_rescale(long long *__restrict__ accum, size_t n, const DeviceStats *__restrict__ stats)
+{
+    const int e_new = fixed_exponent(stats->amax_bits);
+    const int sh = stats->accum_exp_set ? stats->accum_exp - e_new : 0;     // > 0: the unit grew by 2^sh
+    if (sh <= 0) return;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const long long v = accum[i];
+        accum[i] = sh >= 63 ? 0ll : (v + (1ll << (sh - 1))) >> sh;
+    }
+}
+
+__global__ void k_rescale_done(DeviceStats *stats)
+{
+    stats->accum_exp = fixed_exponent(stats->amax_bits);
+    stats->accum_exp_set = 1u;
+}
+
 // ---- packed float32 pairs (Blackwell FADD2 / FMUL2 / FFMA2: two IEEE round-to-nearest results per issue slot) ----
 typedef unsigned long long f32x2;
 __device__ __forceinline__ f32x2 pk2(float a, float b) { f32x2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
@@ -787,7 +823,7 @@ k_compose(const unsigned long long *__restrict__ accum, const DeviceStats *__res
     constexpr int kPix = T * T;
     const int tile = blockIdx.x;
     const int tx0 = (tile % fp.ntx) * T, ty0 = (tile / fp.ntx) * T;
-    const bool ok = stats->overflow == 0u;
+    const bool ok = stats->f_overflow == 0u;
     const double unit = ldexp(1.0, -fixed_exponent(stats->amax_bits));       // one fixed-point unit
     for (int p = threadIdx.x; p < kPix; p += 256) {
         const int ix = tx0 + p % T, iy = ty0 + p / T;

@@ -92,10 +92,10 @@ def assert_counts_exact(r, w, tile, g):
     return st
 
 
-def full_check(w, tile, lut=None):
+def full_check(w, tile, lut=None, pair_capacity=0):
     lut = wl.palette() if lut is None else lut
     ref, g, cam = oracle_frame(w, lut, tile)
-    r, f, kw, img = gpu_frame(w, lut, tile)
+    r, f, kw, img = gpu_frame(w, lut, tile, pair_capacity=pair_capacity)
     assert_geometry_exact(r, f, w, kw, g, cam)
     st = assert_counts_exact(r, w, tile, g)
     assert_image_close(img, ref, w.name)
@@ -263,6 +263,93 @@ def test_permutation_invariance_on_gpu():
     torch.cuda.synchronize()
     a, b_ = img.double().cpu().numpy(), img2.double().cpu().numpy()
     assert np.linalg.norm(a - b_) <= 2e-6 * np.linalg.norm(a)
+
+
+def test_two_renders_of_one_frame_agree():
+    """The integer work is bit-reproducible (classes, per-tile counts; SMALL and small-box contributions are exact
+    fixed-point sums).  The pixel owners add float32 contributions in the order the records sit in their bins, which
+    depends on the scheduling of the scatter stage: two renders agree to float32 rounding, not bit for bit."""
+    w = wl.make_config(1, n=500_000, size=(400, 300))
+    lut = wl.palette()
+    r, f, kw, img = gpu_frame(w, lut, 16)
+    a = img.clone()
+    c0 = r.debug_tile_counts(16).clone()
+    st0 = r.stats()
+    b_ = r.render(f, w.species, **kw)
+    torch.cuda.synchronize()
+    assert torch.equal(c0, r.debug_tile_counts(16)) and st0["count"] == r.stats()["count"] and st0["pairs"] == r.stats()["pairs"]
+    d = (a.double() - b_.double())
+    assert float(d.norm()) <= 1e-6 * float(a.double().norm())
+    assert float(d.abs().max()) <= 1e-6 * float(a.max())
+
+
+def test_all_small_frame_is_bit_reproducible():
+    """Only SMALL particles: every contribution is an integer addition, the image does not depend on the order."""
+    w = wl.make_config(1, n=300_000, size=(200, 150))
+    w.fields["h"] = torch.full_like(w.fields["h"], 1e-5)
+    lut = wl.palette()
+    r, f, kw, img = gpu_frame(w, lut, 16)
+    a = img.clone()
+    assert r.stats()["count"][2] == 0 and r.stats()["count"][1] > 100_000
+    perm = torch.randperm(w.n, generator=torch.Generator().manual_seed(9)).cuda()
+    b_ = r.render({k: v[perm].contiguous() for k, v in f.items()}, w.species, **kw)
+    torch.cuda.synchronize()
+    assert torch.equal(a, b_)
+
+
+def test_amplitudes_spanning_ten_decades_document_the_fixed_point_limit():
+    """The tiles' sums are fixed point in units of 2^-30 of the frame's largest record amplitude:
+    the image meets the north_star tolerance (which is relative to the image's maximum), while contributions more than
+    about nine decades below the brightest record fall under one unit and vanish; the double-precision oracle keeps them."""
+    n = 40_000
+    w = wl.make_config(0, n=n, size=(128, 128))
+    w.fields["h"] = torch.full_like(w.fields["h"], 1e-5)                     # all SMALL: one contribution per particle
+    I = torch.full((n,), 1e-10)
+    I[: n // 2] = 1.0                                                         # bright half, faint half ten decades below
+    w.fields["I"] = I.to(torch.float32)
+    xs = w.fields["x"].clone()
+    w.fields["x"] = torch.where(torch.arange(n) < n // 2, 0.35 + 0.2 * (xs - 0.5), 0.65 + 0.2 * (xs - 0.5))   # left / right
+    lut = wl.palette()
+    ref, g, cam = oracle_frame(w, lut, 16)
+    r, f, kw, img = gpu_frame(w, lut, 16)
+    assert_image_close(img, ref, "ten decades")
+    gi = img.double().cpu().numpy()
+    faint = (ref > 0) & (ref < 1e-8 * ref.max())
+    assert faint.sum() > 100
+    assert (gi[faint] == 0).all()                                             # below one fixed-point unit: lost
+    # seven decades are still resolved to a few per cent
+    I2 = I.clone(); I2[n // 2:] = 1e-7
+    w.fields["I"] = I2.to(torch.float32)
+    ref2, g2, cam2 = oracle_frame(w, lut, 16)
+    r2, f2, kw2, img2 = gpu_frame(w, lut, 16)
+    gi2 = img2.double().cpu().numpy()
+    faint2 = (ref2 > 0) & (ref2 < 1e-5 * ref2.max())
+    assert faint2.sum() > 100
+    assert np.abs(gi2[faint2] - ref2[faint2]).max() <= 0.05 * ref2[faint2].max()
+
+
+def test_tile_64_and_global_histogram_paths():
+    """tile = 64 (pixel owners hold 8 pixels per lane) and an image with more bins than fit in shared memory
+    (2048 x 1536 at 8 px: 98,304 + 768 bins -> the blocks count into their rows of the count matrix in L2)."""
+    w = wl.make_config(1, n=200_000, size=(400, 300))
+    full_check(w, 64)
+    w3 = wl.make_config(3, n=120_000, size=(512, 384))
+    w3.r_large = 24.0
+    full_check(w3, 64)
+    wg = wl.make_config(1, n=300_000, size=(2048, 1536))
+    st, g = full_check(wg, 8, pair_capacity=40_000_000)          # a 60-px disc covers 15 x 15 tiles of 8 px
+    assert st["count"][wl_MEDIUM] > 50_000
+
+
+def test_requested_pair_capacity_is_honoured():
+    b = _binding()
+    for additive in (True, False):
+        w = wl.make_config(0, n=20_000, size=(1024, 1024))
+        w.additive = additive
+        lut = wl.palette()
+        r, f, kw, img = gpu_frame(w, lut, 16, pair_capacity=30_000)
+        assert r.stats()["pair_capacity"] >= 30_000
+        r.close()
 
 
 def test_cfg1_full_size_bench_configuration():
