@@ -21,7 +21,7 @@
  * Fig. 2's five-particle scenario, resolution scaling, brute-force tile recount.
  * "Parity unpinned" by the paper itself (pinned only by DESIGN.md readings): the value of chi,
  * the SMALL-particle deposit rule (R6), the E/A/rho0 input mapping (R12), the depth-order rule
- * for E != A (R15).
+ * for E != A (R15), the normalisation of the vector colour mode (R24).
  *
  * Build: gcc -O2 -ffp-contract=off -fno-fast-math -shared -fPIC splotch_oracle.c -lm
  */
@@ -349,5 +349,60 @@ void orc_render_ordered(int64_t m, const int64_t *order, const int8_t *cls,
                     else I[c] += E[3 * p + c] * tau;
                 }
             }
+    }
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * Pre-processing.
+ *
+ * Normalisation range of a species' colour quantity when the user gives none: "normalization together
+ * with other necessary calculations (e.g. for logarithms of processed quantities)";
+ * the extrema are "user-specified ... otherwise they are precomputed" (:166 fn. 1).  Plain loop over
+ * ALL particles of the species (active or not): v = scalar, or log10(scalar) when use_log10; values
+ * that are not finite (NaN, +-Inf, log10 of a non-positive number) are skipped.  The extrema are the
+ * float32 values themselves (log10 is taken in double and rounded once to float32, the precision the
+ * range is handed on in).  A species without a finite value gets min = 0, max = 1.
+ * ------------------------------------------------------------------------------------------- */
+void orc_scalar_range(int64_t n, const float *scalar, const int32_t *species_of, int n_species,
+                      const int32_t *use_log10, float *vmin /* n_species */, float *vmax /* n_species */)
+{
+    int64_t p;
+    int s;
+    for (s = 0; s < n_species; ++s) { vmin[s] = INFINITY; vmax[s] = -INFINITY; }
+    for (p = 0; p < n; ++p) {
+        float v = scalar[p];
+        s = species_of[p];
+        if (use_log10[s]) v = (float)log10((double)v);
+        if (!(v >= -3.0e38f && v <= 3.0e38f)) continue;      /* NaN and +-Inf are skipped */
+        if (v < vmin[s]) vmin[s] = v;
+        if (v > vmax[s]) vmax[s] = v;
+    }
+    for (s = 0; s < n_species; ++s)
+        if (!(vmin[s] <= vmax[s])) { vmin[s] = 0.0f; vmax[s] = 1.0f; }
+}
+
+/* Vector colour mode: "for velocity v = (v_x, v_y, v_z) we assign rho^R = v_x, rho^G = v_y and
+ * rho^B = v_z".  Reading R24 of DESIGN.md: each component is normalised with the
+ * species' range like the scalar of the look-up-table mode (:76), t_c = clamp((v_c - min) /
+ * (max - min), 0, 1), NaN -> 0, and E[c] = brightness * t_c; the column constant is the one of
+ * orc_amplitude.  Overwrites E for the particles of species with vector_mode != 0 only. */
+void orc_amplitude_vector(int64_t n, const float *vr, const float *vg, const float *vb,
+                          const int32_t *species_of, const int32_t *vector_mode,
+                          const double *brightness, const double *smin, const double *smax,
+                          double *E /* 3n */)
+{
+    int64_t p;
+    int c;
+    for (p = 0; p < n; ++p) {
+        int s = species_of[p];
+        double v[3];
+        if (!vector_mode[s]) continue;
+        v[0] = (double)vr[p]; v[1] = (double)vg[p]; v[2] = (double)vb[p];
+        for (c = 0; c < 3; ++c) {
+            double t = (v[c] - smin[s]) / (smax[s] - smin[s]);
+            if (!(t > 0.0)) t = 0.0;
+            if (t > 1.0) t = 1.0;
+            E[3 * p + c] = brightness[s] * t;
+        }
     }
 }

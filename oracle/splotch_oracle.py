@@ -9,7 +9,7 @@ from __future__ import annotations
 import ctypes as C
 import os
 import subprocess
-from typing import Dict, Optional, Sequence, Tuple
+from typing import Dict, List, Optional, Sequence, Tuple
 
 import numpy as np
 
@@ -122,12 +122,12 @@ def _species_arrays(n: int, species: Sequence, luts: Sequence[Optional[np.ndarra
         # parameters are float32 at the C ABI; the oracle sees those same float32 values
         bright[s] = np.float32(sp.brightness)
         kappa[s] = np.float32(sp.absorb)
-        use_cm[s] = int(sp.use_colormap)
+        use_cm[s] = int(sp.use_colormap) if not getattr(sp, "vector_colour", False) else 0
         fixed[s] = np.asarray(sp.fixed_rgb, np.float32)
         smin[s] = np.float32(sp.scalar_min)
         smax[s] = np.float32(sp.scalar_max)
         use_log[s] = int(sp.scalar_log10)
-        if sp.use_colormap:
+        if use_cm[s]:
             t = np.asarray(luts[s], np.float32).astype(np.float64).reshape(-1, 3)
             lut_off[s], lut_n[s] = off, t.shape[0]
             tables.append(t)
@@ -136,8 +136,59 @@ def _species_arrays(n: int, species: Sequence, luts: Sequence[Optional[np.ndarra
     return species_of, bright, kappa, use_cm, np.ascontiguousarray(fixed), smin, smax, use_log, lut, lut_off, lut_n
 
 
-def amplitude(I, scalar, h, species: Sequence, luts: Sequence, threads: int = 1) -> Tuple[np.ndarray, np.ndarray, np.ndarray]:
-    """E[n,3] = brightness * colour, col[n] = sqrt(pi) h I, kappa[n] (species' absorption)."""
+def scalar_range(scalar, species: Sequence, vec=None) -> List[Tuple[float, float]]:
+    """Per species (min, max) of the colour quantity over all its finite values: the scalar (after log10 if the species
+    asks for it), or the three vector components together for a vector-colour species."""
+    scalar = _f32(scalar)
+    n = scalar.shape[0]
+    ns = len(species)
+    species_of = np.zeros(n, np.int32)
+    use_log = np.zeros(ns, np.int32)
+    for s, sp in enumerate(species):
+        species_of[sp.begin:sp.end] = s
+        use_log[s] = int(sp.scalar_log10) if not getattr(sp, "vector_colour", False) else 0
+    out = []
+    vmin, vmax = np.zeros(ns, np.float32), np.zeros(ns, np.float32)
+    lib().orc_scalar_range(C.c_int64(n), _p(scalar, C.c_float), _p(species_of, C.c_int32), C.c_int(ns),
+                           _p(use_log, C.c_int32), _p(vmin, C.c_float), _p(vmax, C.c_float))
+    comp = []
+    if vec is not None:
+        for v in vec:
+            a, b = np.zeros(ns, np.float32), np.zeros(ns, np.float32)
+            v = _f32(v)
+            lib().orc_scalar_range(C.c_int64(n), _p(v, C.c_float), _p(species_of, C.c_int32), C.c_int(ns),
+                                   _p(np.zeros(ns, np.int32), C.c_int32), _p(a, C.c_float), _p(b, C.c_float))
+            comp.append((a, b))
+    for s, sp in enumerate(species):
+        if getattr(sp, "vector_colour", False) and comp:
+            # a component without a finite value reports (0, 1): leave it out unless all three are empty
+            have = [(a[s], b[s]) for a, b in comp
+                    if np.isfinite(_f32(vec[comp.index((a, b))])[sp.begin:sp.end]).any()]
+            out.append((float(min(a for a, _ in have)), float(max(b for _, b in have))) if have else (0.0, 1.0))
+        else:
+            out.append((float(vmin[s]), float(vmax[s])))
+    return out
+
+
+def resolve_ranges(fields: Dict[str, np.ndarray], species: Sequence):
+    """Species parameters with the automatic ranges filled in (copies; the callers' objects stay untouched)."""
+    import copy
+    if not any(getattr(sp, "auto_range", False) for sp in species):
+        return list(species)
+    vec = [fields[k] for k in ("cr", "cg", "cb")] if "cr" in fields else None
+    rng = scalar_range(fields["scalar"], species, vec)
+    out = []
+    for sp, (a, b) in zip(species, rng):
+        sp2 = copy.copy(sp)
+        if getattr(sp, "auto_range", False):
+            sp2.scalar_min, sp2.scalar_max = a, b
+        out.append(sp2)
+    return out
+
+
+def amplitude(I, scalar, h, species: Sequence, luts: Sequence, threads: int = 1, vec=None) -> Tuple[np.ndarray, np.ndarray, np.ndarray]:
+    """E[n,3] = brightness * colour, col[n] = sqrt(pi) h I, kappa[n] (species' absorption).  vec = (cr, cg, cb) feeds
+    the species in vector-colour mode."""
     I, scalar, h = _f32(I), _f32(scalar), _f32(h)
     n = I.shape[0]
     (species_of, bright, kappa, use_cm, fixed, smin, smax, use_log, lut, lut_off, lut_n) = \
@@ -150,6 +201,14 @@ def amplitude(I, scalar, h, species: Sequence, luts: Sequence, threads: int = 1)
        _p(use_cm, C.c_int32), _p(fixed, C.c_double), _p(smin, C.c_double),
        _p(smax, C.c_double), _p(use_log, C.c_int32), _p(lut, C.c_double),
        _p(lut_off, C.c_int32), _p(lut_n, C.c_int32), _p(E, C.c_double), _p(col, C.c_double))
+    vmode = np.array([int(getattr(sp, "vector_colour", False)) for sp in species], np.int32)
+    if vmode.any():
+        if vec is None:
+            raise ValueError("a species is in vector-colour mode but no vector fields were given")
+        vr, vg, vb = (_f32(v) for v in vec)
+        lib().orc_amplitude_vector(C.c_int64(n), _p(vr, C.c_float), _p(vg, C.c_float), _p(vb, C.c_float),
+                                   _p(species_of, C.c_int32), _p(vmode, C.c_int32), _p(bright, C.c_double),
+                                   _p(smin, C.c_double), _p(smax, C.c_double), _p(E, C.c_double))
     return E, col, kappa[species_of]
 
 
@@ -212,7 +271,9 @@ def render(fields: Dict[str, np.ndarray], species: Sequence, luts: Sequence, cam
     cam = camera_constants(camera.eye, camera.lookat, camera.up, camera.fov_deg, W, H)
     g = geometry(fields["x"], fields["y"], fields["z"], fields["h"], cam, chi, r_small, r_large, z_near, W, H, tile,
                  threads=threads)
-    E, col, kappa = amplitude(fields["I"], fields["scalar"], fields["h"], species, luts, threads=threads)
+    species = resolve_ranges(fields, species)
+    vec = [fields[k] for k in ("cr", "cg", "cb")] if "cr" in fields else None
+    E, col, kappa = amplitude(fields["I"], fields["scalar"], fields["h"], species, luts, threads=threads, vec=vec)
     if additive:
         img = render_additive(g, E, col, chi, W, H, window=window, apply_transfer=apply_transfer, threads=threads)
     else:

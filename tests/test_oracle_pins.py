@@ -469,3 +469,71 @@ def test_pixel_box_is_the_tight_bounding_box_of_the_clip_disc():
         if np.abs(ex).min() < 1e-4 or np.abs(ey).min() < 1e-4:
             continue
         assert not ((ex <= 0).any() and (ey <= 0).any()), p
+
+
+# ------------------------------------------------------------------------------------------------
+# pre-processing: normalisation range found from the data (PAPER.md:76, :166 fn. 1), vector colours (:85)
+# ------------------------------------------------------------------------------------------------
+def test_scalar_range_is_the_min_max_of_the_finite_values_per_species():
+    rng = np.random.default_rng(12)
+    n = 5000
+    sc = rng.lognormal(0.0, 2.0, n).astype(np.float32)
+    sc[::97] = np.nan
+    sc[5::301] = np.inf
+    sc[7::211] = -1.0                                            # log10 of a negative number: skipped in the log species
+    sc[11::503] = 0.0                                            # log10(0) = -inf: skipped
+    sps = [species(3000, use_colormap=True, scalar_log10=True), species(0, use_colormap=True)]
+    sps[1].begin, sps[1].end = 3000, n
+    got = so.scalar_range(sc, sps)
+    a = np.log10(sc[:3000].astype(np.float64), where=sc[:3000] > 0, out=np.full(3000, np.nan)).astype(np.float32)
+    a = a[np.isfinite(a)]
+    b = sc[3000:][np.isfinite(sc[3000:])]
+    assert got[0] == (float(a.min()), float(a.max()))
+    assert got[1] == (float(b.min()), float(b.max())) and got[1][0] == -1.0
+    # a species without a finite value: (0, 1)
+    assert so.scalar_range(np.full(4, np.nan, np.float32), [species(4, use_colormap=True)]) == [(0.0, 1.0)]
+
+
+def test_automatic_range_equals_the_same_frame_with_the_range_given():
+    n, W, H = 1500, 64, 48
+    f = _random_scene(n, 31)
+    lut = np.asarray(np.random.default_rng(2).uniform(0, 1, (9, 3)), np.float32)
+    auto = [species(n, use_colormap=True, auto_range=True, scalar_min=123.0, scalar_max=124.0)]     # given values are ignored
+    lo, hi = float(f["scalar"].min()), float(f["scalar"].max())
+    given = [species(n, use_colormap=True, scalar_min=lo, scalar_max=hi)]
+    cam = camera((0.0, 0.2, 2.1))
+    a = so.render(f, auto, [lut], cam, W, H)
+    b = so.render(f, given, [lut], cam, W, H)
+    assert a.max() > 0 and np.array_equal(a, b)
+    # the extreme particles get the first and the last table entry exactly
+    E, _, _ = so.amplitude(f["I"], f["scalar"], f["h"], so.resolve_ranges(f, auto), [lut])
+    np.testing.assert_allclose(E[f["scalar"].argmin()], lut[0].astype(float), rtol=0, atol=0)
+    np.testing.assert_allclose(E[f["scalar"].argmax()], lut[-1].astype(float), rtol=1e-15)
+
+
+def test_vector_colour_mode_maps_components_to_channels():
+    """rho^R = v_x, rho^G = v_y, rho^B = v_z, each normalised over the species' range and clamped."""
+    vr = np.array([-2.0, 2.0, 0.0, 5.0, np.nan], np.float32)
+    vg = np.array([2.0, -2.0, 1.0, -9.0, 0.0], np.float32)
+    vb = np.array([0.0, 0.0, -1.0, 2.0, 0.0], np.float32)
+    n = 5
+    sp = [species(n, vector_colour=True, scalar_min=-2.0, scalar_max=2.0, brightness=0.5)]
+    E, col, _ = so.amplitude(np.ones(n), np.zeros(n), np.ones(n), sp, [None], vec=(vr, vg, vb))
+    np.testing.assert_allclose(E, 0.5 * np.array([[0, 1, 0.5], [1, 0, 0.5], [0.5, 0.75, 0.25], [1, 0, 1], [0, 0.5, 0.5]]), atol=1e-15)
+    # the image of a vector-coloured set is the stack of three single-channel images: channel c sees only component c
+    rng = np.random.default_rng(8)
+    m, W, H = 800, 48, 40
+    f = _random_scene(m, 41)
+    f["cr"], f["cg"], f["cb"] = (rng.uniform(-1, 1, m).astype(np.float32) for _ in range(3))
+    spv = [species(m, vector_colour=True, scalar_min=-1.0, scalar_max=1.0)]
+    cam = camera((0.1, 0.0, 2.0))
+    img = so.render(f, spv, [None], cam, W, H)
+    for c, key in enumerate(("cr", "cg", "cb")):
+        ramp = np.array([[0, 0, 0], [1, 1, 1]], np.float32)               # K = 2 table: colour = t, all channels
+        f1 = dict(f, scalar=f[key])
+        one = so.render(f1, [species(m, use_colormap=True, scalar_min=-1.0, scalar_max=1.0)], [ramp], cam, W, H)
+        np.testing.assert_allclose(img[:, :, c], one[:, :, c], rtol=1e-13, atol=1e-300)
+    # automatic range of a vector species: over the three components together
+    spa = so.resolve_ranges(f, [species(m, vector_colour=True, auto_range=True)])
+    allv = np.concatenate([f["cr"], f["cg"], f["cb"]])
+    assert (spa[0].scalar_min, spa[0].scalar_max) == (float(allv.min()), float(allv.max()))
