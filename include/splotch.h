@@ -61,6 +61,9 @@ typedef struct {
                                         species s owns the index range [off[s], off[s+1]) (Gadget-style
                                         type blocks).  NULL means one species.                */
     int n_species;                   /* 1 .. SPLOTCH_MAX_SPECIES (ignored when species_offsets is NULL)     */
+    const float *cr, *cg, *cb;       /* vector quantity (e.g. velocity) for species in vector colour mode:
+                                        rho^R = v_x, rho^G = v_y, rho^B = v_z.  Same placement and
+                                        length as the other fields; may be NULL when no species uses them.   */
 } splotch_particles;
 
 typedef struct {
@@ -70,6 +73,12 @@ typedef struct {
     float fixed_rgb[3];
     float scalar_min, scalar_max;    /* user-specified normalisation range (PAPER.md:166 fn. 1)             */
     int   scalar_log10;              /* take log10(scalar) before normalising                 */
+    int   auto_range;                /* 1: ignore scalar_min / scalar_max and take the extrema of the species' finite
+                                        values, found on the device (PAPER.md:166 fn. 1 "otherwise they are
+                                        precomputed"): of the scalar (after log10 if set), or of the three vector
+                                        components together in vector colour mode                             */
+    int   vector_colour;             /* 1: colour[c] = clamp((v_c - min) / (max - min), 0, 1) from cr, cg, cb
+                                        (reading R24); use_colormap is then ignored    */
 } splotch_species_params;
 
 typedef struct {

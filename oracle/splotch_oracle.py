@@ -162,8 +162,7 @@ def scalar_range(scalar, species: Sequence, vec=None) -> List[Tuple[float, float
     for s, sp in enumerate(species):
         if getattr(sp, "vector_colour", False) and comp:
             # a component without a finite value reports (0, 1): leave it out unless all three are empty
-            have = [(a[s], b[s]) for a, b in comp
-                    if np.isfinite(_f32(vec[comp.index((a, b))])[sp.begin:sp.end]).any()]
+            have = [(a[s], b[s]) for k, (a, b) in enumerate(comp) if np.isfinite(_f32(vec[k])[sp.begin:sp.end]).any()]
             out.append((float(min(a for a, _ in have)), float(max(b for _, b in have))) if have else (0.0, 1.0))
         else:
             out.append((float(vmin[s]), float(vmax[s])))

@@ -31,13 +31,14 @@ EXPORTS = (
 
 class SplotchParticles(C.Structure):
     _fields_ = [("x", C.c_void_p), ("y", C.c_void_p), ("z", C.c_void_p), ("h", C.c_void_p), ("I", C.c_void_p),
-                ("scalar", C.c_void_p), ("species_offsets", C.POINTER(C.c_uint64)), ("n_species", C.c_int)]
+                ("scalar", C.c_void_p), ("species_offsets", C.POINTER(C.c_uint64)), ("n_species", C.c_int),
+                ("cr", C.c_void_p), ("cg", C.c_void_p), ("cb", C.c_void_p)]
 
 
 class SplotchSpeciesParams(C.Structure):
     _fields_ = [("brightness", C.c_float), ("absorb", C.c_float), ("use_colormap", C.c_int),
                 ("fixed_rgb", C.c_float * 3), ("scalar_min", C.c_float), ("scalar_max", C.c_float),
-                ("scalar_log10", C.c_int)]
+                ("scalar_log10", C.c_int), ("auto_range", C.c_int), ("vector_colour", C.c_int)]
 
 
 class SplotchParams(C.Structure):
@@ -152,6 +153,8 @@ def make_params(species: Sequence, chi=3.0, r_small=0.5, r_large=64.0, z_near=1e
         arr[k].scalar_min = s.scalar_min
         arr[k].scalar_max = s.scalar_max
         arr[k].scalar_log10 = int(s.scalar_log10)
+        arr[k].auto_range = int(getattr(s, "auto_range", False))
+        arr[k].vector_colour = int(getattr(s, "vector_colour", False))
     p = SplotchParams(chi, r_small, r_large, z_near, tile, int(additive), int(apply_transfer),
                       C.cast(arr, C.POINTER(SplotchSpeciesParams)))
     return p, arr
@@ -167,8 +170,14 @@ def make_particles(fields: Dict[str, torch.Tensor], species: Sequence):
             raise ValueError(f"field {k} must be a contiguous float32 tensor of length {n}")
         ptrs[k] = t.data_ptr()
     offs = (C.c_uint64 * (len(species) + 1))(*([s.begin for s in species] + [species[-1].end]))
+    vec = []
+    for k in ("cr", "cg", "cb"):
+        t = fields.get(k)
+        if t is not None and (t.dtype != torch.float32 or not t.is_contiguous() or t.numel() != n):
+            raise ValueError(f"field {k} must be a contiguous float32 tensor of length {n}")
+        vec.append(t.data_ptr() if t is not None else None)
     p = SplotchParticles(ptrs["x"], ptrs["y"], ptrs["z"], ptrs["h"], ptrs["I"], ptrs["scalar"],
-                         C.cast(offs, C.POINTER(C.c_uint64)), len(species))
+                         C.cast(offs, C.POINTER(C.c_uint64)), len(species), *vec)
     return p, offs
 
 

@@ -25,7 +25,7 @@ const char *kStageNamesAdditive[kStagesAdditive] = {"count", "scan", "scatter", 
 const char *kStageNamesOrdered[kStagesOrdered] = {"count", "scan", "pairs", "sort", "bounds", "render", "combine"};
 
 struct Layout {
-    size_t counts, counts_bytes, cursors, cls_counts, bin_count, vstart, large_off, run, stats, accum, accum_bytes, records, staging, total;
+    size_t ranges, counts, counts_bytes, cursors, cls_counts, bin_count, vstart, large_off, run, stats, accum, accum_bytes, records, staging, total;
     bool ghist;
     unsigned long long capacity;
     int nrows;
@@ -117,6 +117,8 @@ int bin_rows(const splotch_ctx *c, int T)
     return c->n_sm;                         // one 1024-thread CTA per SM, each with a private histogram over all bins
 }
 
+constexpr int kHostFields = 9;
+
 // Particles per chunk of a chunked host frame: about eight chunks, between 2^20 and 2^25 particles, a multiple of 4
 unsigned long long host_chunk_particles(const splotch_ctx *c, unsigned long long n)
 {
@@ -135,7 +137,7 @@ unsigned long long host_chunk_particles(const splotch_ctx *c, unsigned long long
 size_t staging_bytes(const splotch_ctx *c, unsigned long long n, bool additive)
 {
     const unsigned long long per = additive ? host_chunk_particles(c, n) : n;
-    const size_t fields = 6 * align_up(sizeof(float) * per, 256) * (additive ? 2 : 1);
+    const size_t fields = kHostFields * align_up(sizeof(float) * per, 256) * (additive ? 2 : 1);     // six fields + the vector components
     return align_up(fields, 256) + align_up(sizeof(float) * 3 * (size_t)c->width * c->height, 256);
 }
 
@@ -149,6 +151,7 @@ bool make_layout(const splotch_ctx *c, unsigned long long n, int T, unsigned lon
     L->nrows = bin_rows(c, T);
     L->ghist = use_global_hist(c, T);
     size_t off = 0;
+    L->ranges = off;      off = align_up(off + (sizeof(RangeRaw) + sizeof(float2)) * kMaxSpecies, 256);
     L->counts = off;      L->counts_bytes = sizeof(unsigned int) * nbins * L->nrows; off = align_up(off + L->counts_bytes, 256);
     L->cursors = off;     if (L->ghist) off = align_up(off + L->counts_bytes, 256);      // k_scatter's cursors when they do not fit in shared memory
     L->cls_counts = off;  off = align_up(off + sizeof(unsigned int) * 4 * L->nrows, 256);
@@ -191,6 +194,7 @@ void make_layout_ordered(const splotch_ctx *c, unsigned long long n, int T, unsi
     L->m_hist = 256u * (unsigned int)L->nblk_rs;
     L->n_sums = (int)((L->m_hist + kScTile - 1) / kScTile);
     size_t off = 0;
+    L->ranges = off;      off = align_up(off + (sizeof(RangeRaw) + sizeof(float2)) * kMaxSpecies, 256);
     L->stats = off;       off = align_up(off + sizeof(DeviceStats), 256);
     L->blk_pairs = off;   off = align_up(off + sizeof(unsigned int) * (size_t)(L->nblk_o + 1), 256);
     L->tile_start = off;  off = align_up(off + sizeof(unsigned int) * (n_tiles + 1), 256);
@@ -287,7 +291,10 @@ int check_params(splotch_ctx *c, const splotch_particles *p, unsigned long long 
         SpeciesDev &d = fp->sp[s];
         d.brightness = sp.brightness; d.absorb = sp.absorb;
         d.fixed_r = sp.fixed_rgb[0]; d.fixed_g = sp.fixed_rgb[1]; d.fixed_b = sp.fixed_rgb[2];
-        d.use_colormap = sp.use_colormap ? 1 : 0; d.use_log10 = sp.scalar_log10 ? 1 : 0;
+        d.vector = sp.vector_colour ? 1 : 0; d.auto_range = sp.auto_range ? 1 : 0;
+        d.use_colormap = (sp.use_colormap && !d.vector) ? 1 : 0; d.use_log10 = sp.scalar_log10 ? 1 : 0;
+        if (d.vector) { fp->any_vector = 1; d.use_log10 = 0; }
+        if (d.auto_range) fp->any_auto = 1;
         d.smin = sp.scalar_min;
         d.inv_range = (float)(1.0 / ((double)sp.scalar_max - (double)sp.scalar_min));
         d.lut_n = c->lut_n[s];
@@ -296,10 +303,13 @@ int check_params(splotch_ctx *c, const splotch_particles *p, unsigned long long 
         if (d.use_colormap) lut_total += d.lut_n;
         if (d.use_colormap) {
             if (d.lut_n < 2) return fail(c, SPLOTCH_ESTATE, "species %d uses a colour map but none was set", s);
-            if (!(sp.scalar_max != sp.scalar_min)) return fail(c, SPLOTCH_EINVAL, "species %d: scalar_min == scalar_max", s);
+            if (!d.auto_range && !(sp.scalar_max != sp.scalar_min)) return fail(c, SPLOTCH_EINVAL, "species %d: scalar_min == scalar_max", s);
         }
+        if (d.vector && !d.auto_range && !(sp.scalar_max != sp.scalar_min)) return fail(c, SPLOTCH_EINVAL, "species %d: scalar_min == scalar_max", s);
     }
     fp->lut_total = lut_total <= kLutSmemMax ? lut_total : 0;      // larger tables are read from global memory
+    if (fp->any_vector && n > 0 && (!p->cr || !p->cg || !p->cb)) return fail(c, SPLOTCH_EINVAL, "a species is in vector colour mode but cr / cg / cb are null");
+    fp->vec[0] = p->cr; fp->vec[1] = p->cg; fp->vec[2] = p->cb;
     return SPLOTCH_OK;
 }
 
@@ -342,6 +352,30 @@ void launch_scatter(const Layout &L, size_t hbytes, const splotch_particles *p, 
 {
     k_scatter<AL, GH><<<L.nrows, kBinThreads, GH ? sizeof(float4) * kLutSmemMax : hbytes, st>>>(p->x, p->y, p->z, p->h, p->I, p->scalar, n, per, fp,
                                                                                            counts, cursors, run, stats, records);
+}
+
+// Normalisation ranges found on the device (PAPER.md:166 fn. 1) for the species with auto_range: particles [lo, lo + len) of
+// the set the pointers of `p` address; species ranges sp_begin are relative to that set.  init / finish bracket the passes.
+void range_pass(splotch_ctx *c, const splotch_particles *p, unsigned long long len, const FrameParams &fp, char *ws, const Layout &L,
+                cudaStream_t st, bool init, bool finish)
+{
+    RangeRaw *raw = (RangeRaw *)(ws + L.ranges);
+    float2 *rng = (float2 *)(raw + kMaxSpecies);
+    if (init) k_range_init<<<1, 32, 0, st>>>(raw);
+    for (int s = 0; s < fp.n_species && len > 0; ++s) {
+        if (!fp.sp[s].auto_range) continue;
+        const unsigned long long b = fp.sp_begin[s], e = fp.sp_begin[s + 1] < len ? fp.sp_begin[s + 1] : len;
+        if (b >= e) continue;
+        const unsigned long long cnt = e - b;
+        const int grid = (int)((cnt + 511) / 512 < (unsigned long long)(8 * c->n_sm) ? (cnt + 511) / 512 : 8 * c->n_sm);
+        if (fp.sp[s].vector) {
+            const float *v[3] = {p->cr, p->cg, p->cb};
+            for (int k = 0; k < 3; ++k) k_minmax<<<grid, 512, 0, st>>>(v[k] + b, cnt, 0, raw, s);
+        } else {
+            k_minmax<<<grid, 512, 0, st>>>(p->scalar + b, cnt, fp.sp[s].use_log10, raw, s);
+        }
+    }
+    if (finish) k_range_finish<<<1, 32, 0, st>>>(raw, rng);
 }
 
 struct ChunkCtl { bool first, last, chunked; };     // one-shot frame: {true, true, false}
@@ -661,6 +695,8 @@ int splotch_render(splotch_ctx *c, const splotch_particles *p, uint64_t n, const
     rc = frame_layout(c, n, q, workspace_bytes, false, &L);
     if (rc != SPLOTCH_OK) return rc;
     CU_TRY(c, cudaSetDevice(c->device));
+    fp.dev_range = (const float2 *)((RangeRaw *)((char *)workspace + L.ranges) + kMaxSpecies);
+    if (fp.any_auto) range_pass(c, p, n, fp, (char *)workspace, L, (cudaStream_t)cuda_stream, true, true);
     if (!q->additive) return render_ordered(c, p, n, fp, L, image_out, (char *)workspace, (cudaStream_t)cuda_stream);
     return render_device(c, p, n, fp, L, image_out, (char *)workspace, (cudaStream_t)cuda_stream);
 }
@@ -692,18 +728,27 @@ int splotch_render_host(splotch_ctx *c, const splotch_particles *hp, uint64_t n,
     CU_TRY(c, cudaSetDevice(c->device));
     cudaStream_t st = (cudaStream_t)cuda_stream;
     char *ws = (char *)workspace;
-    const float *src[6] = {hp->x, hp->y, hp->z, hp->h, hp->I, hp->scalar};
+    const int nf = fp.any_vector ? kHostFields : 6;
+    const float *src[kHostFields] = {hp->x, hp->y, hp->z, hp->h, hp->I, hp->scalar, hp->cr, hp->cg, hp->cb};
     const size_t image_bytes = sizeof(float) * 3 * (size_t)c->width * c->height;
-    if (!q->additive) {
-        const size_t fstride = align_up(sizeof(float) * n, 256);
-        float *dst[6];
-        for (int k = 0; k < 6; ++k) {
-            dst[k] = (float *)(ws + L.staging + k * fstride);
-            if (n) CU_TRY(c, cudaMemcpyAsync(dst[k], src[k], sizeof(float) * n, cudaMemcpyHostToDevice, st));
-        }
-        float *dimg = (float *)(ws + L.staging + align_up(6 * fstride, 256));
+    fp.dev_range = (const float2 *)((RangeRaw *)(ws + L.ranges) + kMaxSpecies);
+    auto device_view = [&](float *const *dst) {
         splotch_particles dp = *hp;
         dp.x = dst[0]; dp.y = dst[1]; dp.z = dst[2]; dp.h = dst[3]; dp.I = dst[4]; dp.scalar = dst[5];
+        dp.cr = dst[6]; dp.cg = dst[7]; dp.cb = dst[8];
+        return dp;
+    };
+    if (!q->additive) {
+        const size_t fstride = align_up(sizeof(float) * n, 256);
+        float *dst[kHostFields];
+        for (int k = 0; k < kHostFields; ++k) {
+            dst[k] = (float *)(ws + L.staging + k * fstride);
+            if (n && k < nf) CU_TRY(c, cudaMemcpyAsync(dst[k], src[k], sizeof(float) * n, cudaMemcpyHostToDevice, st));
+        }
+        float *dimg = (float *)(ws + L.staging + align_up(kHostFields * fstride, 256));
+        const splotch_particles dp = device_view(dst);
+        fp.vec[0] = dp.cr; fp.vec[1] = dp.cg; fp.vec[2] = dp.cb;
+        if (fp.any_auto) range_pass(c, &dp, n, fp, ws, L, st, true, true);
         rc = render_ordered(c, &dp, n, fp, L, dimg, ws, st);
         if (rc != SPLOTCH_OK) return rc;
         CU_TRY(c, cudaMemcpyAsync(host_image_out, dimg, image_bytes, cudaMemcpyDeviceToHost, st));
@@ -721,31 +766,50 @@ int splotch_render_host(splotch_ctx *c, const splotch_particles *hp, uint64_t n,
     }
     const unsigned long long ch = host_chunk_particles(c, n);
     const size_t fstride = align_up(sizeof(float) * ch, 256);
-    float *dimg = (float *)(ws + L.staging + align_up(2 * 6 * fstride, 256));
+    float *dimg = (float *)(ws + L.staging + align_up(2 * kHostFields * fstride, 256));
     const unsigned long long nchunks = n ? (n + ch - 1) / ch : 1;
     const int ns = fp.n_species;
     unsigned long long sp_begin[kMaxSpecies + 1];
     for (int s = 0; s <= ns; ++s) sp_begin[s] = hp->species_offsets ? hp->species_offsets[s] : (s == 0 ? 0ull : n);
+    auto chunk_params = [&](unsigned long long lo, unsigned long long len, float *const *dst) {
+        FrameParams fc = fp;                                      // the chunk's own species ranges and field pointers
+        for (int s = 0; s <= ns; ++s) {
+            const unsigned long long o = sp_begin[s] < lo ? 0ull : (sp_begin[s] - lo < len ? sp_begin[s] - lo : len);
+            fc.sp_begin[s] = (unsigned int)o;
+        }
+        fc.vec[0] = dst[6]; fc.vec[1] = dst[7]; fc.vec[2] = dst[8];
+        return fc;
+    };
+    if (fp.any_auto) {
+        // the ranges need the whole set before the first chunk is coloured: one more pass over the colour quantities
+        // (scalar, or the vector components), through staging buffer 0 on the caller's stream
+        for (unsigned long long k = 0; k < nchunks; ++k) {
+            const unsigned long long lo = k * ch, len = n ? (lo + ch < n ? ch : n - lo) : 0;
+            float *dst[kHostFields];
+            for (int f = 0; f < kHostFields; ++f) {
+                dst[f] = (float *)(ws + L.staging + (size_t)f * fstride);
+                if (len && f >= 5 && f < nf) CU_TRY(c, cudaMemcpyAsync(dst[f], src[f] + lo, sizeof(float) * len, cudaMemcpyHostToDevice, st));
+            }
+            const splotch_particles dp = device_view(dst);
+            const FrameParams fc = chunk_params(lo, len, dst);
+            range_pass(c, &dp, len, fc, ws, L, st, k == 0, k + 1 == nchunks);
+        }
+    }
     CU_TRY(c, cudaEventRecord(c->ev_start, st));                 // the staging buffers are free once earlier work on `st` is done
     CU_TRY(c, cudaStreamWaitEvent(c->copy_stream, c->ev_start, 0));
     for (unsigned long long k = 0; k < nchunks; ++k) {
         const unsigned long long lo = k * ch, len = n ? (lo + ch < n ? ch : n - lo) : 0;
         const int b = (int)(k & 1);
-        float *dst[6];
+        float *dst[kHostFields];
         if (k >= 2) CU_TRY(c, cudaStreamWaitEvent(c->copy_stream, c->ev_consumed[b], 0));
-        for (int f = 0; f < 6; ++f) {
-            dst[f] = (float *)(ws + L.staging + (size_t)(6 * b + f) * fstride);
-            if (len) CU_TRY(c, cudaMemcpyAsync(dst[f], src[f] + lo, sizeof(float) * len, cudaMemcpyHostToDevice, c->copy_stream));
+        for (int f = 0; f < kHostFields; ++f) {
+            dst[f] = (float *)(ws + L.staging + (size_t)(kHostFields * b + f) * fstride);
+            if (len && f < nf) CU_TRY(c, cudaMemcpyAsync(dst[f], src[f] + lo, sizeof(float) * len, cudaMemcpyHostToDevice, c->copy_stream));
         }
         CU_TRY(c, cudaEventRecord(c->ev_copied[b], c->copy_stream));
         CU_TRY(c, cudaStreamWaitEvent(st, c->ev_copied[b], 0));
-        splotch_particles dp = *hp;
-        dp.x = dst[0]; dp.y = dst[1]; dp.z = dst[2]; dp.h = dst[3]; dp.I = dst[4]; dp.scalar = dst[5];
-        FrameParams fc = fp;                                      // the chunk's own species ranges
-        for (int s = 0; s <= ns; ++s) {
-            const unsigned long long o = sp_begin[s] < lo ? 0ull : (sp_begin[s] - lo < len ? sp_begin[s] - lo : len);
-            fc.sp_begin[s] = (unsigned int)o;
-        }
+        const splotch_particles dp = device_view(dst);
+        const FrameParams fc = chunk_params(lo, len, dst);
         rc = render_device(c, &dp, len, fc, L, dimg, ws, st, ChunkCtl{k == 0, k + 1 == nchunks, nchunks > 1});
         if (rc != SPLOTCH_OK) return rc;
         CU_TRY(c, cudaEventRecord(c->ev_consumed[b], st));

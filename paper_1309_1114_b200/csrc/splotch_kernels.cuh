@@ -46,6 +46,7 @@ struct SpeciesDev {
     float smin, inv_range;                           // t = (v - smin) * inv_range
     float lut_nm1, lut_nm2;                          // (float)(lut_n - 1), (float)(lut_n - 2)
     int   use_colormap, use_log10, lut_n, lut_off;   // lut_off: first entry in the packed shared-memory table
+    int   vector, auto_range;                        // colour from the vector fields; range found on the device (:166 fn. 1)
 };
 
 struct FrameParams {
@@ -58,6 +59,9 @@ struct FrameParams {
     int   sshift, nsx, nsy, n_super, nbins;
     int   additive, apply_transfer;
     int   n_species, lut_total;  // lut_total: packed entries of all colour-mapped species, 0 = read tables from global
+    int   any_vector, any_auto;
+    const float *vec[3];         // cr, cg, cb: per-particle vector components for species in vector colour mode
+    const float2 *dev_range;     // [kMaxSpecies] {min, 1 / (max - min)} of the species with auto_range (k_range_finish)
     unsigned int sp_begin[kMaxSpecies + 1];
     SpeciesDev sp[kMaxSpecies];
     const float4 *lut;           // [kMaxSpecies][kMaxLut] rgb0
@@ -558,6 +562,39 @@ k_layout(const unsigned int *__restrict__ counts, const unsigned int *__restrict
     }
 }
 
+// ---- pre-processing: normalisation range found from the data (PAPER.md:76, :166 fn. 1) ----------------------------
+// Floats as unsigned keys whose order is the order of the values, so that atomicMin / atomicMax reduce them.
+__device__ __forceinline__ unsigned int float_key(float v) { const unsigned int b = __float_as_uint(v); return (b & 0x80000000u) ? ~b : b | 0x80000000u; }
+__device__ __forceinline__ float key_float(unsigned int k) { return __uint_as_float((k & 0x80000000u) ? k & 0x7fffffffu : ~k); }
+
+struct RangeRaw { unsigned int kmin, kmax; };            // per species; k_range_init sets {0xffffffff, 0}
+
+__global__ void k_range_init(RangeRaw *raw) { if (threadIdx.x < kMaxSpecies) raw[threadIdx.x] = RangeRaw{0xffffffffu, 0u}; }
+
+// min / max of the finite values of v[0, n) (log10 first when asked), reduced into raw[s]
+__global__ void __launch_bounds__(512)
+k_minmax(const float *__restrict__ v, unsigned long long n, int use_log10, RangeRaw *__restrict__ raw, int s)
+{
+    unsigned int kmin = 0xffffffffu, kmax = 0u;
+    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (unsigned long long)gridDim.x * blockDim.x) {
+        float x = __ldg(v + i);
+        if (use_log10) x = log10f(x);
+        if (x >= -3.0e38f && x <= 3.0e38f) { const unsigned int k = float_key(x); kmin = min(kmin, k); kmax = max(kmax, k); }
+    }
+    kmin = __reduce_min_sync(0xffffffffu, kmin); kmax = __reduce_max_sync(0xffffffffu, kmax);
+    if ((threadIdx.x & 31) == 0 && kmin <= kmax) { atomicMin(&raw[s].kmin, kmin); atomicMax(&raw[s].kmax, kmax); }
+}
+
+// {min, 1 / (max - min)} per species; a species without a finite value gets the range (0, 1)
+__global__ void k_range_finish(const RangeRaw *__restrict__ raw, float2 *__restrict__ out)
+{
+    if (threadIdx.x < kMaxSpecies) {
+        const RangeRaw r = raw[threadIdx.x];
+        const float lo = r.kmin <= r.kmax ? key_float(r.kmin) : 0.0f, hi = r.kmin <= r.kmax ? key_float(r.kmax) : 1.0f;
+        out[threadIdx.x] = make_float2(lo, __fdiv_rn(1.0f, __fsub_rn(hi, lo)));
+    }
+}
+
 // ---- A2: colour + amplitude (PAPER.md:76 normalisation/log, :85 look-up table) -------------------------------
 __device__ __forceinline__ int species_of(unsigned int i, const FrameParams &fp)
 {
@@ -569,13 +606,18 @@ __device__ __forceinline__ int species_of(unsigned int i, const FrameParams &fp)
 
 // lut: the species' table (shared or global memory), lut_n entries.  Colour and amplitude are continuous in the
 // inputs (no integer is decided here beyond the table cell), so plain float32 with a reciprocal range is enough.
-__device__ __forceinline__ float3 colour_of(float scalar, const SpeciesDev &S, const float4 *lut)
+__device__ __forceinline__ float3 colour_of(float scalar, const SpeciesDev &S, const float4 *lut, float2 rng, float3 vec)
 {
     float r = S.fixed_r, g = S.fixed_g, b = S.fixed_b;
-    if (S.use_colormap) {
+    if (S.vector) {                                // rho^R = v_x, rho^G = v_y, rho^B = v_z, normalised like the scalar
+        const float tr = (vec.x - rng.x) * rng.y, tg = (vec.y - rng.x) * rng.y, tb = (vec.z - rng.x) * rng.y;
+        r = fminf(tr > 0.0f ? tr : 0.0f, 1.0f);
+        g = fminf(tg > 0.0f ? tg : 0.0f, 1.0f);
+        b = fminf(tb > 0.0f ? tb : 0.0f, 1.0f);
+    } else if (S.use_colormap) {
         float v = scalar;
         if (S.use_log10) v = log10f(v);
-        float t = (v - S.smin) * S.inv_range;
+        float t = (v - rng.x) * rng.y;
         t = (t > 0.0f) ? t : 0.0f;                 // NaN clamps to 0
         t = fminf(t, 1.0f);
         const float u = t * S.lut_nm1;             // 0 <= u <= lut_n - 1 <= 1023
@@ -594,10 +636,16 @@ __device__ __forceinline__ float3 colour_of(float scalar, const SpeciesDev &S, c
     return make_float3(r, g, b);
 }
 
-// E_p * (column constant) = b_s * colour * sqrt(pi) h I (PAPER.md:85, DESIGN.md R12, R13)
-__device__ __forceinline__ float3 amplitude(float I, float scalar, float h, const SpeciesDev &S, const float4 *lut)
+// normalisation range of a species: the caller's, or the one found on the device (k_minmax / k_range_finish)
+__device__ __forceinline__ float2 species_range(const FrameParams &fp, int s)
 {
-    const float3 c = colour_of(scalar, S, lut);
+    return fp.sp[s].auto_range ? fp.dev_range[s] : make_float2(fp.sp[s].smin, fp.sp[s].inv_range);
+}
+
+// E_p * (column constant) = b_s * colour * sqrt(pi) h I (PAPER.md:85, DESIGN.md R12, R13)
+__device__ __forceinline__ float3 amplitude(float I, float scalar, float h, const SpeciesDev &S, const float4 *lut, float2 rng, float3 vec)
+{
+    const float3 c = colour_of(scalar, S, lut, rng, vec);
     const float col = S.brightness * (1.7724538509055160273f * h * I);   // b_s * sqrt(pi) h I
     return make_float3(c.x * col, c.y * col, c.z * col);
 }
@@ -642,7 +690,9 @@ k_scatter(const float *__restrict__ x, const float *__restrict__ y, const float 
 {
     extern __shared__ unsigned int cursor_s[];               // nbins cursors, then the packed colour tables
     __shared__ float s_amax[kBinThreads / 32];
+    __shared__ float2 s_rng[kMaxSpecies];
     if (stats->overflow) return;
+    if (threadIdx.x < kMaxSpecies) s_rng[threadIdx.x] = threadIdx.x < fp.n_species ? species_range(fp, threadIdx.x) : make_float2(0.0f, 0.0f);
     float4 *s_lut = reinterpret_cast<float4 *>(cursor_s + (GHIST ? 0 : ((fp.nbins + 3) & ~3)));
     // this block's cursors: slab base + the run's first unit + the units of the slab's rows before this one
     const unsigned int *row = counts + (size_t)blockIdx.x * fp.nbins;
@@ -683,6 +733,12 @@ k_scatter(const float *__restrict__ x, const float *__restrict__ y, const float 
         load4<ALIGNED>(h, i, len, hs);
         load4<ALIGNED>(I, i, len, Is);
         load4<ALIGNED>(scalar, i, len, ss);
+        float vr[4] = {0.f, 0.f, 0.f, 0.f}, vg[4] = {0.f, 0.f, 0.f, 0.f}, vb[4] = {0.f, 0.f, 0.f, 0.f};
+        if (fp.any_vector) {
+            load4<false>(fp.vec[0] + lo, i, len, vr);
+            load4<false>(fp.vec[1] + lo, i, len, vg);
+            load4<false>(fp.vec[2] + lo, i, len, vb);
+        }
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const Geo g = geometry(xs[j], ys[j], zs[j], hs[j], fp);
@@ -690,7 +746,7 @@ k_scatter(const float *__restrict__ x, const float *__restrict__ y, const float 
             const int s = one_species ? s_first : species_of(min(lo32 + i + j, lo32 + len - 1), fp);
             const SpeciesDev &S = fp.sp[s];
             const float4 *lut = fp.lut_total > 0 ? s_lut + S.lut_off : fp.lut + s * kMaxLut;
-            float3 a = amplitude(Is[j], ss[j], hs[j], S, lut);
+            float3 a = amplitude(Is[j], ss[j], hs[j], S, lut, s_rng[s], make_float3(vr[j], vg[j], vb[j]));
             const bool small = cls == SMALL;
             const float sp2 = __fmul_rn(g.sp, g.sp);
             const float w = small ? fp.csmall * sp2 : 1.0f;

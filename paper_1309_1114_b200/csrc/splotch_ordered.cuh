@@ -198,7 +198,9 @@ k_opairs(const float *__restrict__ x, const float *__restrict__ y, const float *
         const int s = species_of(idx, fp);
         const SpeciesDev &S = fp.sp[s];
         const float4 *lut = fp.lut_total > 0 ? s_lut + S.lut_off : fp.lut + s * kMaxLut;
-        const float3 rgb = colour_of(ss[j], S, lut);
+        float3 vv = make_float3(0.0f, 0.0f, 0.0f);
+        if (fp.any_vector && idx < n) vv = make_float3(__ldg(fp.vec[0] + idx), __ldg(fp.vec[1] + idx), __ldg(fp.vec[2] + idx));
+        const float3 rgb = colour_of(ss[j], S, lut, species_range(fp, s), vv);
         const float3 E = make_float3(S.brightness * rgb.x, S.brightness * rgb.y, S.brightness * rgb.z);
         const bool small = g[j].cls == SMALL;
         const float sp2 = __fmul_rn(g[j].sp, g[j].sp);

@@ -93,6 +93,8 @@ class Species:
     scalar_min: float = 0.0
     scalar_max: float = 1.0
     scalar_log10: bool = False
+    auto_range: bool = False            # normalisation range found from the data instead of scalar_min / scalar_max
+    vector_colour: bool = False         # colour from the vector fields cr, cg, cb
 
 
 @dataclass
