@@ -173,6 +173,11 @@ int splotch_set_host_chunk(splotch_ctx *ctx, uint64_t particles_per_chunk);
 int splotch_get_stats(splotch_ctx *ctx, splotch_stats *out);
 const char *splotch_stage_name(int additive, int stage);   /* stage names of an additive / ordered frame */
 
+/* image <- 1 - exp(-image) in place (DEVICE, height x width x 3 float32): the exact E = A transfer for a
+ * frame whose partial images S were rendered with apply_transfer = 0 and summed elsewhere, e.g. by the image all-reduce of
+ * a particle-sharded multi-GPU frame.  Asynchronous on `cuda_stream`. */
+int splotch_apply_transfer(splotch_ctx *ctx, float *image, void *cuda_stream);
+
 /* The two ALU rates the splat stages' roofline fractions are quoted against, measured on this context's device by
  * a register-only microbenchmark: out[0] = FP32 FMA lane-operations per second (one FMA = one
  * operation), out[1] = ex2.approx results per second, whole GPU.  HOST out; synchronises `cuda_stream`. */

@@ -25,7 +25,7 @@ EXPORTS = (
     "splotch_create", "splotch_destroy", "splotch_set_camera", "splotch_get_camera_constants",
     "splotch_set_colormap", "splotch_set_profiling", "splotch_workspace_bytes", "splotch_render",
     "splotch_render_host", "splotch_get_stats", "splotch_stage_name", "splotch_debug_geometry",
-    "splotch_debug_tile_counts", "splotch_last_error", "splotch_version", "splotch_measure_peaks", "splotch_set_host_chunk",
+    "splotch_debug_tile_counts", "splotch_last_error", "splotch_version", "splotch_measure_peaks", "splotch_set_host_chunk", "splotch_apply_transfer",
 )
 
 
@@ -90,6 +90,7 @@ def load() -> C.CDLL:
     lib.splotch_debug_tile_counts.argtypes = [vp, vp, vp]
     lib.splotch_measure_peaks.argtypes = [vp, C.POINTER(C.c_double), vp]
     lib.splotch_set_host_chunk.argtypes = [vp, u64]
+    lib.splotch_apply_transfer.argtypes = [vp, vp, vp]
     lib.splotch_last_error.argtypes = [vp]
     lib.splotch_last_error.restype = C.c_char_p
     lib.splotch_version.restype = C.c_char_p
@@ -213,6 +214,11 @@ class Renderer:
     def set_host_chunk(self, particles_per_chunk: int) -> None:
         _check(self.ctx, self.lib.splotch_set_host_chunk(self.ctx, particles_per_chunk))
         self._ws = None
+
+    def apply_transfer(self, image: torch.Tensor) -> torch.Tensor:
+        stream = torch.cuda.current_stream(self.device).cuda_stream
+        _check(self.ctx, self.lib.splotch_apply_transfer(self.ctx, image.data_ptr(), stream))
+        return image
 
     def measure_peaks(self) -> Dict[str, float]:
         out = (C.c_double * 2)()

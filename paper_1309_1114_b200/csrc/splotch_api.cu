@@ -858,6 +858,15 @@ int splotch_get_stats(splotch_ctx *c, splotch_stats *out)
     return SPLOTCH_OK;
 }
 
+int splotch_apply_transfer(splotch_ctx *c, float *image, void *cuda_stream)
+{
+    if (!c || !image) return SPLOTCH_EINVAL;
+    CU_TRY(c, cudaSetDevice(c->device));
+    k_apply_transfer<<<4 * c->n_sm, 256, 0, (cudaStream_t)cuda_stream>>>(image, 3 * (size_t)c->width * c->height);
+    CU_TRY(c, cudaGetLastError());
+    return SPLOTCH_OK;
+}
+
 int splotch_measure_peaks(splotch_ctx *c, double out[2], void *cuda_stream)
 {
     if (!c || !out) return SPLOTCH_EINVAL;

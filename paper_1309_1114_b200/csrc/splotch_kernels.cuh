@@ -895,6 +895,13 @@ k_compose(const unsigned long long *__restrict__ accum, const DeviceStats *__res
     }
 }
 
+// ---- 1 - exp(-S) on a finished image: the transfer of a frame whose partial images were summed elsewhere (multi-GPU) ----
+__global__ void __launch_bounds__(256)
+k_apply_transfer(float *__restrict__ image, size_t n)
+{
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) image[i] = -expm1f(-image[i]);
+}
+
 // ---- test hook: per-tile pair counts (SMALL + MEDIUM bins of every tile) ---------------------------------------------
 __global__ void __launch_bounds__(256)
 k_tile_counts(const unsigned int *__restrict__ bin_count, int n_tiles, unsigned int *__restrict__ out)
