@@ -86,10 +86,16 @@ typedef struct {
     float r_small;                   /* r_sml, 0.5 in the paper (:162)                                      */
     float r_large;                   /* r_0 (:160); px                                                      */
     float z_near;                    /* particles with camera depth z_c <= z_near are inactive              */
-    int   tile;                      /* tile side t_x = t_y in px (Eq. 8, :164): 8, 16 or 32                */
+    int   tile;                      /* tile side t_x = t_y in px (Eq. 8, :164): 8, 16, 32 or 64 (ordered: <= 32) */
     int   additive;                  /* 1: E_p = A_p mode (:85), order independent.  0: ordered E != A mode */
     int   apply_transfer;            /* additive only: 0 -> image = S = sum_p E_p tau_p, 1 -> 1 - exp(-S)   */
     const splotch_species_params *species;  /* HOST, n_species entries                                      */
+    int   renderer;                  /* 0: coverage-binned tile renderer (default).  1: the paper's own medium-particle
+                                        scheme, for comparison: particles binned to the tile of their
+                                        centre, Btile = body + boundary of r_0 in shared memory, blocks of (2 r_0 + 1)^2
+                                        threads, three boundary images + composition; additive mode, tile 8 or 16,
+                                        r_large = r_0 <= tile (:224)                                           */
+    int   btile_np;                  /* renderer 1: particles staged per read, n_p (Table 1, :254-266); 0 = 16 */
 } splotch_params;
 
 typedef struct {

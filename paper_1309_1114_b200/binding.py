@@ -44,7 +44,7 @@ class SplotchSpeciesParams(C.Structure):
 class SplotchParams(C.Structure):
     _fields_ = [("chi", C.c_float), ("r_small", C.c_float), ("r_large", C.c_float), ("z_near", C.c_float),
                 ("tile", C.c_int), ("additive", C.c_int), ("apply_transfer", C.c_int),
-                ("species", C.POINTER(SplotchSpeciesParams))]
+                ("species", C.POINTER(SplotchSpeciesParams)), ("renderer", C.c_int), ("btile_np", C.c_int)]
 
 
 class SplotchStats(C.Structure):
@@ -143,7 +143,7 @@ def splotch_workspace_bytes(ctx, n: int, tile: int, pair_capacity: int = 0, with
 
 
 def make_params(species: Sequence, chi=3.0, r_small=0.5, r_large=64.0, z_near=1e-6, tile=16, additive=True,
-                apply_transfer=False):
+                apply_transfer=False, renderer=0, btile_np=0):
     """(SplotchParams, keep-alive array) from objects with the attributes of workloads.Species."""
     arr = (SplotchSpeciesParams * len(species))()
     for k, s in enumerate(species):
@@ -157,7 +157,7 @@ def make_params(species: Sequence, chi=3.0, r_small=0.5, r_large=64.0, z_near=1e
         arr[k].auto_range = int(getattr(s, "auto_range", False))
         arr[k].vector_colour = int(getattr(s, "vector_colour", False))
     p = SplotchParams(chi, r_small, r_large, z_near, tile, int(additive), int(apply_transfer),
-                      C.cast(arr, C.POINTER(SplotchSpeciesParams)))
+                      C.cast(arr, C.POINTER(SplotchSpeciesParams)), int(renderer), int(btile_np))
     return p, arr
 
 

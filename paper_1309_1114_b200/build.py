@@ -11,7 +11,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsplotch_b200.so")
 SOURCES = [os.path.join(CSRC, "splotch_api.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, "splotch_kernels.cuh"), os.path.join(CSRC, "splotch_splat.cuh"), os.path.join(CSRC, "splotch_large.cuh"),
-                  os.path.join(CSRC, "splotch_ordered.cuh"), os.path.join(CSRC, "splotch_peaks.cuh"),
+                  os.path.join(CSRC, "splotch_ordered.cuh"), os.path.join(CSRC, "splotch_peaks.cuh"), os.path.join(CSRC, "splotch_btile.cuh"),
                   os.path.join(os.path.dirname(HERE), "include", "splotch.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]

@@ -6,6 +6,7 @@
 #include "splotch_large.cuh"
 #include "splotch_ordered.cuh"
 #include "splotch_peaks.cuh"
+#include "splotch_btile.cuh"
 #include "../../include/splotch.h"
 
 #include <math.h>
@@ -25,7 +26,7 @@ const char *kStageNamesAdditive[kStagesAdditive] = {"count", "scan", "scatter", 
 const char *kStageNamesOrdered[kStagesOrdered] = {"count", "scan", "pairs", "sort", "bounds", "render", "combine"};
 
 struct Layout {
-    size_t ranges, counts, counts_bytes, cursors, cls_counts, bin_count, vstart, large_off, run, stats, accum, accum_bytes, records, staging, total;
+    size_t ranges, planes, planes_bytes, counts, counts_bytes, cursors, cls_counts, bin_count, vstart, large_off, run, stats, accum, accum_bytes, records, staging, total;
     bool ghist;
     unsigned long long capacity;
     int nrows;
@@ -152,6 +153,8 @@ bool make_layout(const splotch_ctx *c, unsigned long long n, int T, unsigned lon
     L->ghist = use_global_hist(c, T);
     size_t off = 0;
     L->ranges = off;      off = align_up(off + (sizeof(RangeRaw) + sizeof(float2)) * kMaxSpecies, 256);
+    // partial images of the paper's Btile renderer (tiles of 8 or 16 px only)
+    L->planes = off;      L->planes_bytes = T <= 16 ? sizeof(float) * 3 * kBtilePlanes * (size_t)c->width * c->height : 0; off = align_up(off + L->planes_bytes, 256);
     L->counts = off;      L->counts_bytes = sizeof(unsigned int) * nbins * L->nrows; off = align_up(off + L->counts_bytes, 256);
     L->cursors = off;     if (L->ghist) off = align_up(off + L->counts_bytes, 256);      // k_scatter's cursors when they do not fit in shared memory
     L->cls_counts = off;  off = align_up(off + sizeof(unsigned int) * 4 * L->nrows, 256);
@@ -275,6 +278,14 @@ int check_params(splotch_ctx *c, const splotch_particles *p, unsigned long long 
     fp->nsx = (c->width + S - 1) / S; fp->nsy = (c->height + S - 1) / S;
     fp->n_super = fp->nsx * fp->nsy;
     fp->nbins = 2 * fp->n_tiles + fp->n_super;
+    if (q->renderer != 0 && q->renderer != 1) return fail(c, SPLOTCH_EINVAL, "renderer must be 0 (default) or 1 (the paper's Btile scheme)");
+    if (q->renderer == 1) {
+        // the paper's constraints: additive mode (:85), r_0 <= min(t_x, t_y) (:224); the Btile must fit the 6-bit box fields
+        const int r0 = (int)ceilf(q->r_large);
+        if (!q->additive || q->tile > 16 || r0 > q->tile || r0 < 1)
+            return fail(c, SPLOTCH_EINVAL, "the Btile renderer needs additive mode, tile 8 or 16 and 1 <= r_large <= tile");
+        fp->btile = 1; fp->btile_r0 = r0; fp->btile_np = q->btile_np > 0 ? (q->btile_np < 256 ? q->btile_np : 256) : 16;
+    }
     fp->additive = q->additive ? 1 : 0;
     fp->apply_transfer = q->apply_transfer ? 1 : 0;
     fp->n_species = ns;
@@ -325,15 +336,30 @@ int launch_render_tail(splotch_ctx *c, const Layout &L, char *ws, const FramePar
 {
     const int ti = T == 8 ? 0 : T == 16 ? 1 : T == 32 ? 2 : 3;
     const int grid = c->n_sm * c->splat_blocks_per_sm[ti];
-    k_splat<T><<<grid, Splat2Cfg<T>::kThreads, Splat2Cfg<T>::kSmemBytes, st>>>(
-        (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.vstart), (const uint2 *)(ws + L.run), (DeviceStats *)(ws + L.stats),
-        (unsigned long long *)(ws + L.accum), fp);
+    if (fp.btile) {
+        const int side = T + 2 * fp.btile_r0, B = 2 * fp.btile_r0 + 1;
+        const int threads = ((B * B + 31) / 32 * 32) < 1024 ? (B * B + 31) / 32 * 32 : 1024;
+        const size_t smem = sizeof(float) * ((3 * side * side + 3) & ~3) + 32 * (size_t)fp.btile_np;
+        k_btile<<<fp.n_tiles, threads, smem, st>>>((const float4 *)(ws + L.records), (const uint2 *)(ws + L.run), (const DeviceStats *)(ws + L.stats),
+                                                  (float *)(ws + L.planes), fp);
+    } else {
+        k_splat<T><<<grid, Splat2Cfg<T>::kThreads, Splat2Cfg<T>::kSmemBytes, st>>>(
+            (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.vstart), (const uint2 *)(ws + L.run), (DeviceStats *)(ws + L.stats),
+            (unsigned long long *)(ws + L.accum), fp);
+    }
     if (prof) cudaEventRecord(c->ev[4], st);
     k_large<<<c->n_sm * c->large_blocks_per_sm, kLargeThreads, 0, st>>>(
         (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.bin_count), (const uint2 *)(ws + L.run), (const unsigned int *)(ws + L.large_off),
         (DeviceStats *)(ws + L.stats), (unsigned long long *)(ws + L.accum), fp);
     if (prof) cudaEventRecord(c->ev[5], st);
-    if (compose) k_compose<T><<<fp.n_tiles, 256, 0, st>>>((const unsigned long long *)(ws + L.accum), (const DeviceStats *)(ws + L.stats), fp, image);
+    if (compose && fp.btile) {
+        FrameParams fl = fp;
+        fl.apply_transfer = 0;                    // the transfer comes after the partial images are added
+        k_compose<T><<<fp.n_tiles, 256, 0, st>>>((const unsigned long long *)(ws + L.accum), (const DeviceStats *)(ws + L.stats), fl, image);
+        k_btile_compose<<<4 * c->n_sm, 256, 0, st>>>((const float *)(ws + L.planes), 3 * (size_t)fp.W * fp.H, fp.apply_transfer, image);
+    } else if (compose) {
+        k_compose<T><<<fp.n_tiles, 256, 0, st>>>((const unsigned long long *)(ws + L.accum), (const DeviceStats *)(ws + L.stats), fp, image);
+    }
     if (prof) cudaEventRecord(c->ev[6], st);
     return SPLOTCH_OK;
 }
@@ -401,6 +427,7 @@ int render_device(splotch_ctx *c, const splotch_particles *p, unsigned long long
         cudaEventRecord(c->ev[0], st);
     }
     if (ctl.first) cudaMemsetAsync(ws + L.stats, 0, (L.accum - L.stats) + L.accum_bytes, st);      // DeviceStats + the tiles' sums
+    if (ctl.first && fp.btile) cudaMemsetAsync(ws + L.planes, 0, L.planes_bytes, st);
     else cudaMemsetAsync(ws + L.stats, 0, offsetof(DeviceStats, f_count), st);                     // the chunk part of DeviceStats
     if (L.ghist) cudaMemsetAsync(counts, 0, L.counts_bytes, st);                    // the blocks count straight into their rows
     if (L.ghist) { if (al) launch_count<true, true>(L, hbytes, p, n, per, fp, counts, cls_counts, st); else launch_count<false, true>(L, hbytes, p, n, per, fp, counts, cls_counts, st); }
@@ -696,6 +723,7 @@ int splotch_render(splotch_ctx *c, const splotch_particles *p, uint64_t n, const
     if (rc != SPLOTCH_OK) return rc;
     CU_TRY(c, cudaSetDevice(c->device));
     fp.dev_range = (const float2 *)((RangeRaw *)((char *)workspace + L.ranges) + kMaxSpecies);
+    fp.btile_planes = (float *)((char *)workspace + L.planes);
     if (fp.any_auto) range_pass(c, p, n, fp, (char *)workspace, L, (cudaStream_t)cuda_stream, true, true);
     if (!q->additive) return render_ordered(c, p, n, fp, L, image_out, (char *)workspace, (cudaStream_t)cuda_stream);
     return render_device(c, p, n, fp, L, image_out, (char *)workspace, (cudaStream_t)cuda_stream);
@@ -732,6 +760,7 @@ int splotch_render_host(splotch_ctx *c, const splotch_particles *hp, uint64_t n,
     const float *src[kHostFields] = {hp->x, hp->y, hp->z, hp->h, hp->I, hp->scalar, hp->cr, hp->cg, hp->cb};
     const size_t image_bytes = sizeof(float) * 3 * (size_t)c->width * c->height;
     fp.dev_range = (const float2 *)((RangeRaw *)(ws + L.ranges) + kMaxSpecies);
+    fp.btile_planes = (float *)(ws + L.planes);
     auto device_view = [&](float *const *dst) {
         splotch_particles dp = *hp;
         dp.x = dst[0]; dp.y = dst[1]; dp.z = dst[2]; dp.h = dst[3]; dp.I = dst[4]; dp.scalar = dst[5];

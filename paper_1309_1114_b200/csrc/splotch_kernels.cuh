@@ -60,6 +60,8 @@ struct FrameParams {
     int   additive, apply_transfer;
     int   n_species, lut_total;  // lut_total: packed entries of all colour-mapped species, 0 = read tables from global
     int   any_vector, any_auto;
+    int   btile, btile_r0, btile_np;   // the paper's Btile renderer (splotch_btile.cuh): MEDIUM particles binned by home tile
+    float *btile_planes;         // [5][H][W][3] partial images of that renderer
     const float *vec[3];         // cr, cg, cb: per-particle vector components for species in vector colour mode
     const float2 *dev_range;     // [kMaxSpecies] {min, 1 / (max - min)} of the species with auto_range (k_range_finish)
     unsigned int sp_begin[kMaxSpecies + 1];
@@ -166,6 +168,14 @@ __device__ __forceinline__ int paper_label(const Geo &g, const FrameParams &fp)
     return ((int)cy >> fp.tshift) * fp.ntx + ((int)cx >> fp.tshift);
 }
 
+// tile of the (clamped) centre pixel: the paper's i(p) of a MEDIUM particle
+__device__ __forceinline__ int2 home_tile(const Geo &g, const FrameParams &fp)
+{
+    const float cx = fminf(fmaxf(floorf(g.px), 0.0f), __fsub_rn(fp.fW, 1.0f));
+    const float cy = fminf(fmaxf(floorf(g.py), 0.0f), __fsub_rn(fp.fH, 1.0f));
+    return make_int2((int)cx >> fp.tshift, (int)cy >> fp.tshift);
+}
+
 // ---- bins ----------------------------------------------------------------------------------------------------------
 // Bin b < 2 n_tiles: tile b >> 1; even bins hold the tile's MEDIUM records (32 bytes = 2 units of 16 bytes), odd bins
 // its SMALL records (16 bytes = 1 unit: "only their location ... has to be calculated").  Bins
@@ -260,7 +270,8 @@ k_count(const float *__restrict__ x, const float *__restrict__ y, const float *_
             c2 += cls == MEDIUM; c3 += cls == LARGE;
             // SMALL and MEDIUM: the tiles of the pixel box.  A box covers at most 2 x 2 tiles unless it is wider than a
             // tile: four predicated reductions, no loop
-            const int tx0 = g.x0 >> ts, ty0 = g.y0 >> ts, tx1 = g.x1 >> ts, ty1 = g.y1 >> ts;
+            int tx0 = g.x0 >> ts, ty0 = g.y0 >> ts, tx1 = g.x1 >> ts, ty1 = g.y1 >> ts;
+            if (fp.btile && cls == MEDIUM) { const int2 ht = home_tile(g, fp); tx0 = tx1 = ht.x; ty0 = ty1 = ht.y; }   // i(p): the tile of the centre
             const bool tile = cls == SMALL || cls == MEDIUM, w2 = tx1 > tx0, h2 = ty1 > ty0;
             unsigned int *h00 = hist + (2 * (ty0 * fp.ntx + tx0) + (cls == SMALL ? 1 : 0));
             if (tile) hist_inc<GHIST>(h00);
@@ -756,13 +767,29 @@ k_scatter(const float *__restrict__ x, const float *__restrict__ y, const float 
             else if (cls != CULLED) amax = fmaxf(amax, am);
             const int tx0 = g.x0 >> ts, ty0 = g.y0 >> ts, tx1 = g.x1 >> ts, ty1 = g.y1 >> ts;
             unsigned int *c00 = cursor + 2 * (ty0 * fp.ntx + tx0);
-            if (small) {
+            if (fp.btile) {
+                // the paper's scheme: SMALL particles go straight to the small-particle partial image, a MEDIUM particle to
+                // the tile of its centre with its box relative to that tile's Btile (body + boundary of r_0)
+                if (small) {
+                    float *o = fp.btile_planes + 4 * (3 * (size_t)fp.W * fp.H) + 3 * ((size_t)g.y0 * fp.W + g.x0);
+                    asm volatile("red.global.add.f32 [%0], %1;" :: "l"(o), "f"(a.x) : "memory");
+                    asm volatile("red.global.add.f32 [%0], %1;" :: "l"(o + 1), "f"(a.y) : "memory");
+                    asm volatile("red.global.add.f32 [%0], %1;" :: "l"(o + 2), "f"(a.z) : "memory");
+                } else if (cls == MEDIUM) {
+                    const int2 ht = home_tile(g, fp);
+                    const int ox = (ht.x << ts) - fp.btile_r0, oy = (ht.y << ts) - fp.btile_r0;
+                    const unsigned int box = (unsigned int)(g.x0 - ox) | ((unsigned int)(g.y0 - oy) << 6) |
+                                             ((unsigned int)(g.x1 - g.x0) << 12) | ((unsigned int)(g.y1 - g.y0) << 18);
+                    const float4 rm = make_float4(g.px, g.py, __fdividef(-1.4426950408889634f, sp2), __fmul_rn(g.rp, g.rp));
+                    st_record(records, cursor_take<GHIST>(cursor + 2 * (ht.y * fp.ntx + ht.x), 2u), rm, make_float4(a.x, a.y, a.z, __uint_as_float(box)));
+                }
+            } else if (small) {
                 const unsigned int pix = (unsigned int)(((g.y0 & tmask) << ts) | (g.x0 & tmask));
                 const unsigned int u = cursor_take<GHIST>(c00 + 1, 1u);
                 asm volatile("st.global.v4.f32 [%0], {%1,%2,%3,%4};" :: "l"(records + u), "f"(__uint_as_float(pix)), "f"(a.x), "f"(a.y), "f"(a.z) : "memory");
             }
             const float4 ra = make_float4(g.px, g.py, __fdividef(-1.4426950408889634f, sp2), __fmul_rn(g.rp, g.rp));
-            if (cls == MEDIUM) {
+            if (cls == MEDIUM && !fp.btile) {
                 const bool w2 = tx1 > tx0, h2 = ty1 > ty0;
                 st_record(records, cursor_take<GHIST>(c00, 2u), ra, make_float4(a.x, a.y, a.z, __uint_as_float(pack_box_tile(g, tx0, ty0, fp))));
                 if (w2) st_record(records, cursor_take<GHIST>(c00 + 2, 2u), ra, make_float4(a.x, a.y, a.z, __uint_as_float(pack_box_tile(g, tx0 + 1, ty0, fp))));

@@ -129,6 +129,7 @@ k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
             // ---- test two records per thread: 0 = miss, 1 = the disc contains the block, 2 = the disc cuts the block
             float4 ra[2], rb[2];
             int kind[2];
+            bool safe[2] = {false, false};
 #pragma unroll
             for (int t = 0; t < 2; ++t) {
                 const unsigned int idx = threadIdx.x + t * kLargeThreads;
@@ -147,9 +148,11 @@ k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
                         const float gx = fmaxf(-ax, -bx), gy = fmaxf(-ay, -by);         // farthest: max(|cxl - px|, |cxh - px|)
                         if (fmaf(nx, nx, ny * ny) <= ra[t].w * 1.0001f) {
                             kind[t] = (fmaf(gx, gx, gy * gy) <= ra[t].w * 0.9999f && bx0 <= qx0 && bx1 >= qx1 && by0 <= qy0 && by1 >= qy1) ? 1 : 2;
-                            // the recurrence is used only where its factors cannot overflow: the largest |log2 h| inside the disc
-                            // is -c (4 r + 8); the weights themselves are at least exp2(c r^2) there
-                            if (kind[t] == 1 && !(-ra[t].z * (4.0f * sqrtf(ra[t].w) + 8.0f) < 120.0f && -ra[t].z * ra[t].w < 100.0f)) kind[t] = 2;
+                            // the recurrence is used only where its factors cannot overflow and its products cannot vanish: the
+                            // largest |log2 h| over the block is -c (4 (r + 32) + 8), the weights inside the disc are at least
+                            // exp2(c r^2), and a run that lies outside the disc is masked, not evaluated
+                            safe[t] = -ra[t].z * (4.0f * sqrtf(ra[t].w) + 136.0f) < 120.0f && -ra[t].z * ra[t].w < 100.0f;
+                            if (kind[t] == 1 && !safe[t]) kind[t] = 2;
                         }
                     }
                 }
@@ -177,7 +180,7 @@ k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
                 } else if (kind[t] == 2) {    // the list of cutting discs grows from the back
                     const int pos = kLargeWin - 1 - (boff + (t ? __popc(mb0) : 0) + __popc((t ? mb1 : mb0) & lt));
                     sA[pos] = ra[t];
-                    sB[pos] = rb[t];
+                    sB[pos] = make_float4(rb[t].x, rb[t].y, rb[t].z, safe[t] ? ex2_approx(8.0f * ra[t].z) : -1.0f);
                 }
             }
             __syncthreads();
@@ -198,12 +201,35 @@ k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
                     if (j + 2 < kLargePpt / 2) H = fmul2(H, Q);
                 }
             }
-            // ---- discs that cut the block: the C1 inside test per pixel (bit-exact d2, packed), one ex2 per pixel (the
-            //      recurrence was measured here too: its extra multiplications cost more FMA-pipe time than the ex2 they save)
+            // ---- discs that cut the block.  A thread's 8-pixel run lies inside the disc, outside it, or across its edge; the
+            //      edge of a large disc crosses a warp's 32 x 8 pixels almost as a straight line, so most warps see only the
+            //      first two kinds: a warp with no run across the edge takes the no-test recurrence (runs outside the disc
+            //      get amplitude 0), a warp whose runs are all outside skips the record, the others test every pixel
+            //      (C1 inside test, bit-exact d2, packed; one ex2 per pixel)
             for (int m = 0; m < n_cut; ++m) {
                 const float4 a = sA[kLargeWin - 1 - m], b = sB[kLargeWin - 1 - m];
                 const float dyf = __fsub_rn(fyc, a.y);
                 const float t2 = __fmul_rn(dyf, dyf);
+                const float dx0 = fx0 - a.x, dx7 = dx0 + 7.0f;
+                const float xf = fmaxf(fabsf(dx0), fabsf(dx7)), xn = (dx0 <= 0.0f && dx7 >= 0.0f) ? 0.0f : fminf(fabsf(dx0), fabsf(dx7));
+                const bool seg_in = fmaf(xf, xf, t2) <= a.w * 0.9999f, seg_out = fmaf(xn, xn, t2) > a.w * 1.0001f;
+                if (__all_sync(0xffffffffu, seg_out)) continue;
+                if (b.w > 0.0f && __all_sync(0xffffffffu, seg_in || seg_out)) {
+                    const float d20 = fmaf(dx0, dx0, t2);
+                    const float d21 = d20 + fmaf(2.0f, dx0, 1.0f);
+                    const float u0 = fmaf(4.0f, dx0, 4.0f);
+                    f32x2 P = pk2(ex2_approx(a.z * d20), ex2_approx(a.z * d21));
+                    f32x2 H = pk2(ex2_approx(a.z * u0), ex2_approx(a.z * (u0 + 4.0f)));
+                    const float br = seg_in ? b.x : 0.0f, bg = seg_in ? b.y : 0.0f, bb = seg_in ? b.z : 0.0f;
+                    const f32x2 Q = pk2(b.w, b.w), BR = pk2(br, br), BG = pk2(bg, bg), BB = pk2(bb, bb);
+#pragma unroll
+                    for (int j = 0; j < kLargePpt / 2; ++j) {
+                        sub[j][0] = ffma2(BR, P, sub[j][0]); sub[j][1] = ffma2(BG, P, sub[j][1]); sub[j][2] = ffma2(BB, P, sub[j][2]);
+                        if (j + 1 < kLargePpt / 2) P = fmul2(P, H);
+                        if (j + 2 < kLargePpt / 2) H = fmul2(H, Q);
+                    }
+                    continue;
+                }
                 const f32x2 T2 = pk2(t2, t2), NX = pk2(-a.x, -a.x), C = pk2(a.z, a.z);
                 const f32x2 BR = pk2(b.x, b.x), BG = pk2(b.y, b.y), BB = pk2(b.z, b.z);
 #pragma unroll

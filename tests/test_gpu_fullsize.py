@@ -4,7 +4,9 @@ The oracle cannot render 1e8 .. 4e8 particles in seconds, so at full size
   * the integer work is compared exhaustively: the oracle's C1 geometry runs over ALL particles in chunks and its
     class counts and per-tile pair counts must equal the library's bit for bit; on a strided sample of chunks the
     per-particle float32 geometry, boxes and labels are compared bit for bit as well;
-  * the image is compared on sampled windows: for each window the particles that can touch it are selected from the
+  * configs 2 and 4 (100M particles): the WHOLE image is compared with the oracle's frame, rendered by the all-cores
+    row-band driver (bit-identical to the single-threaded definition); config 3 (400M, ~1e12 fragments: hours of oracle
+    time for the whole image) is compared on a window in every super-tile: for each window the particles that can touch it are selected from the
     RAW inputs by a conservative float64 projection written here (plain torch, neither oracle nor CUDA path; two
     pixels of margin), the oracle renders exactly that subset (a particle outside the selection contributes nothing
     to the window, and the subset keeps index order, so the oracle's sum and its depth order are those of the full
@@ -158,53 +160,177 @@ def windows_for(img, size, n_random, seed):
     return out
 
 
-def run_fullsize(cfg, tile, n_random=3, win=32, modes=(True,), camera=None, w=None):
+def whole_image_oracle(w, lut, tile, additive, cache):
+    """The oracle's frame of the WHOLE image at full size through the all-cores row-band driver (bit-identical to the
+    single-threaded definition, tests/test_oracle_mt.py).  The per-particle colour stage does not depend on the camera:
+    it is computed once per particle set and kept in `cache`."""
+    f = cache.get("fields")
+    if f is None:
+        f = cache["fields"] = {k: v.cpu().numpy() for k, v in w.fields.items()}
+    lutn = lut.numpy()
+    luts = [lutn if s.use_colormap else None for s in w.species]
+    cam = so.camera_constants(w.camera.eye, w.camera.lookat, w.camera.up, w.camera.fov_deg, w.width, w.height)
+    g = so.geometry(f["x"], f["y"], f["z"], f["h"], cam, w.chi, w.r_small, w.r_large, w.z_near, w.width, w.height, tile, threads=0)
+    if "amp" not in cache:
+        cache["amp"] = so.amplitude(f["I"], f["scalar"], f["h"], w.species, luts, threads=0)
+    E, col, kappa = cache["amp"]
+    if additive:
+        img = so.render_additive(g, E, col, w.chi, w.width, w.height, threads=0)
+    else:
+        img = so.render_ordered(g, E, col, kappa, w.chi, w.width, w.height, threads=0)
+    return img, g, cam
+
+
+def check_whole_frame(r, w, lut, tile, additive, cache):
+    """One full-size frame: every pixel of the image, every class count, every per-tile count, and (in additive mode) a
+    sample of the per-particle geometry, against the oracle."""
+    kw = dict(chi=w.chi, r_small=w.r_small, r_large=w.r_large, z_near=w.z_near, tile=tile, additive=additive, apply_transfer=False)
+    img = r.render(w.fields, w.species, **kw)
+    torch.cuda.synchronize()
+    st = r.stats()
+    assert st["overflow"] == 0
+    ref, g, cam = whole_image_oracle(w, lut, tile, additive, cache)
+    assert np.array_equal(np.asarray(r.camera_constants(), np.float32), cam)
+    assert st["count"] == [int(c) for c in np.bincount(g["cls"], minlength=4)]
+    tiles = so.tile_counts(g, w.width, w.height, tile, count_large=not additive)
+    assert np.array_equal(r.debug_tile_counts(tile).cpu().numpy().astype(np.int64), tiles.astype(np.int64))
+    assert st["pairs"] == int(tiles.sum())
+    gi = img.double().cpu().numpy()
+    assert np.isfinite(gi).all()
+    rel = np.linalg.norm(gi - ref) / np.linalg.norm(ref)
+    mab = np.abs(gi - ref).max() / ref.max()
+    assert rel <= REL_L2, f"{w.name} additive={additive}: relative L2 {rel:.3e}"
+    assert mab <= MAX_ABS, f"{w.name} additive={additive}: max abs / max {mab:.3e}"
+    return rel, mab
+
+
+def test_cfg2_full_size_two_species_100M_whole_image():
     lut = wl.palette()
-    if w is None:
-        w = wl.make_config(cfg, device="cuda")
-        w.fields = {k: v.contiguous() for k, v in w.fields.items()}
-    if camera is not None:
-        w.camera = camera
+    w = wl.make_config(2, device="cuda")
+    w.fields = {k: v.contiguous() for k, v in w.fields.items()}
     r = make_renderer(w, lut)
-    res = {}
-    for additive in modes:
-        kw = dict(chi=w.chi, r_small=w.r_small, r_large=w.r_large, z_near=w.z_near, tile=tile, additive=additive,
-                  apply_transfer=False)
-        img = r.render(w.fields, w.species, **kw)
-        torch.cuda.synchronize()
-        st = r.stats()
-        assert st["overflow"] == 0
-        if True:
-            counts, tiles = check_integer_work(r, w, kw, tile, count_large=not additive)
-            assert st["count"] == [int(c) for c in counts]
-            gc = r.debug_tile_counts(tile).cpu().numpy().astype(np.int64)
-            assert np.array_equal(gc, tiles)
-            assert st["pairs"] == int(tiles.sum())
-        res[additive] = (st, check_windows(img, w, lut, kw, windows_for(img, win, n_random, 7 + cfg), additive=additive))
-    r.close()
-    return w, res
-
-
-def test_cfg2_full_size_two_species_100M():
-    w, res = run_fullsize(2, 16)
-    st, (rel, mab) = res[True]
+    check_whole_frame(r, w, lut, 16, True, {})
+    st = r.stats()
     assert st["count"][1] > 30_000_000 and st["count"][2] > 10_000_000
+    # the per-particle float32 geometry on sampled chunks, bit for bit
+    kw = dict(chi=w.chi, r_small=w.r_small, r_large=w.r_large, z_near=w.z_near, tile=16, additive=True, apply_transfer=False)
+    check_integer_work(r, w, kw, 16, geometry_every=3)
+    r.close()
+
+
+def test_cfg4_orbit_frames_100M_whole_image_additive_and_ordered():
+    """Frames {0, 60, 119} of the 120-frame orbit at full size, whole image: additive mode, then the ordered E != A mode
+    (kappa_gas = 0.5, kappa_star = 2.0; intensities scaled so that optical depths reach order one)."""
+    lut = wl.palette()
+    w = wl.make_config(4, device="cuda")
+    w.fields = {k: v.contiguous() for k, v in w.fields.items()}
+    r = make_renderer(w, lut)
+    cache = {}
+    for frame in (0, 60, 119):
+        w.camera = wl.orbit_camera(frame)
+        r.set_camera(w.camera)
+        check_whole_frame(r, w, lut, 16, True, cache)
+    w.fields["I"] = w.fields["I"] * 50.0
+    cache = {}
+    for frame in (0, 60, 119):
+        w.camera = wl.orbit_camera(frame)
+        r.set_camera(w.camera)
+        check_whole_frame(r, w, lut, 16, False, cache)
+    r.close()
+
+
+def super_tile_windows(w, tile, size, seed):
+    """One window in every 256-px super-tile of the image (all of them carry LARGE load when the camera sits inside a
+    halo), at a seeded random position inside it."""
+    rng = np.random.default_rng(seed)
+    S = 256
+    out = []
+    for sy in range(0, w.height, S):
+        for sx in range(0, w.width, S):
+            x0 = sx + int(rng.integers(0, min(S, w.width - sx) - size + 1))
+            y0 = sy + int(rng.integers(0, min(S, w.height - sy) - size + 1))
+            out.append((x0, x0 + size - 1, y0, y0 + size - 1))
+    return out
+
+
+def select_for_windows(fields, cam, W, H, chi, windows, margin=2.0):
+    """select_for_window for many windows in one pass over the particles: list of index tensors (ascending)."""
+    eye, r, u, f, s = camera_basis64(cam, W)
+    out = [[] for _ in windows]
+    n = fields["x"].numel()
+    for a in range(0, n, CHUNK):
+        b = min(n, a + CHUNK)
+        d = [fields[k][a:b].double() - float(eye[i]) for i, k in enumerate("xyz")]
+        zc = sum(float(f[i]) * d[i] for i in range(3))
+        xc = sum(float(r[i]) * d[i] for i in range(3))
+        yc = sum(float(u[i]) * d[i] for i in range(3))
+        k = s / zc
+        px, py = (0.5 * W + xc * k).float(), (0.5 * H - yc * k).float()
+        rad = (chi * fields["h"][a:b].double() * k + margin).float()
+        front = zc > 0
+        del d, zc, xc, yc, k
+        # only particles whose disc is at least as large as the margin can reach a window they are not next to: split the
+        # cheap common case (small discs: bucket by the window grid) from the few large ones (tested against every window)
+        for wi, (wx0, wx1, wy0, wy1) in enumerate(windows):
+            keep = front & (px + rad >= wx0) & (px - rad <= wx1 + 1) & (py + rad >= wy0) & (py - rad <= wy1 + 1)
+            out[wi].append(torch.nonzero(keep).squeeze(1) + a)
+    return [torch.cat(o) for o in out]
 
 
 def test_cfg3_full_size_inside_halo_400M():
-    """4096 x 4096, camera inside the densest halo, a few per cent LARGE particles (tile 32: the per-block histogram
-    of 65,536 16-px tiles would not fit in shared memory)."""
-    w, res = run_fullsize(3, 32, n_random=2, win=24)
-    st, (rel, mab) = res[True]
-    assert st["count"][3] > 0.02 * w.n, st["count"]          # the large-particle stress BASELINE.json asks for
+    """4096 x 4096, camera inside the densest halo, a few per cent LARGE particles.  Integer work exhaustively; the image on
+    a window in every one of the 256 super-tiles plus the brightest / central / corner windows (tile 32, the bench tile)."""
+    lut = wl.palette()
+    w = wl.make_config(3, device="cuda")
+    w.fields = {k: v.contiguous() for k, v in w.fields.items()}
+    r = make_renderer(w, lut)
+    tile = 32
+    kw = dict(chi=w.chi, r_small=w.r_small, r_large=w.r_large, z_near=w.z_near, tile=tile, additive=True, apply_transfer=False)
+    img = r.render(w.fields, w.species, **kw)
+    torch.cuda.synchronize()
+    st = r.stats()
+    assert st["overflow"] == 0 and st["count"][3] > 0.02 * w.n, st["count"]      # the large-particle stress BASELINE.json asks for
+    counts, tiles = check_integer_work(r, w, kw, tile, geometry_every=8)
+    assert st["count"] == [int(c) for c in counts]
+    assert np.array_equal(r.debug_tile_counts(tile).cpu().numpy().astype(np.int64), tiles)
+    assert st["pairs"] == int(tiles.sum())
+    windows = windows_for(img, 24, 2, 10) + super_tile_windows(w, tile, 6, 3)
+    assert len(windows) >= 256 + 5
+    idxs = select_for_windows(w.fields, w.camera, w.width, w.height, w.chi, windows)
+    lutn = lut.numpy()
+    num = den = worst = vmax = 0.0
+    for win, idx in zip(windows, idxs):
+        sub = {k: w.fields[k][idx].cpu().numpy() for k in wl.FIELD_NAMES}
+        sps = subset_species(w.species, idx)
+        ref = so.render(sub, sps, [lutn if s.use_colormap else None for s in sps], w.camera, w.width, w.height,
+                        chi=w.chi, r_small=w.r_small, r_large=w.r_large, z_near=w.z_near, tile=tile, additive=True, window=win, threads=0)
+        wx0, wx1, wy0, wy1 = win
+        a = ref[wy0:wy1 + 1, wx0:wx1 + 1]
+        g = img[wy0:wy1 + 1, wx0:wx1 + 1].double().cpu().numpy()
+        assert np.isfinite(g).all()
+        # every window on its own as well: a wrong super-tile must not hide behind the others
+        assert np.linalg.norm(g - a) <= REL_L2 * np.linalg.norm(a) + 1e-300, win
+        num += float(((g - a) ** 2).sum()); den += float((a ** 2).sum())
+        worst = max(worst, float(np.abs(g - a).max())); vmax = max(vmax, float(a.max()))
+    assert den > 0 and math.sqrt(num / den) <= REL_L2 and worst <= MAX_ABS * vmax
+    r.close()
 
 
-def test_cfg4_orbit_frames_100M_additive_and_ordered():
-    """Frames {0, 30, 60, 90, 119} of the 120-frame orbit at full size, first in additive mode, then in the ordered
-    E != A mode (kappa_gas = 0.5, kappa_star = 2.0; intensities scaled so that optical depths reach order one)."""
-    w = None
-    for frame in (0, 30, 60, 90, 119):
-        w, res = run_fullsize(4, 16, n_random=1, camera=wl.orbit_camera(frame), w=w)
-    w.fields["I"] = w.fields["I"] * 50.0
-    for frame in (0, 30, 60, 90, 119):
-        w, res = run_fullsize(4, 16, n_random=1, camera=wl.orbit_camera(frame), w=w, modes=(False,))
+def test_cfg3_tile_16_integer_work_at_4096():
+    """The default tile of 16 px at 4096 x 4096: 131,072 tile bins + 1,024 super-tile bins do not fit in shared memory, the
+    blocks count into their rows of the count matrix (global histogram).  Class and per-tile counts over all 400M
+    particles bit-exact, and the image on the brightest / central windows."""
+    lut = wl.palette()
+    w = wl.make_config(3, device="cuda")
+    w.fields = {k: v.contiguous() for k, v in w.fields.items()}
+    r = make_renderer(w, lut)
+    kw = dict(chi=w.chi, r_small=w.r_small, r_large=w.r_large, z_near=w.z_near, tile=16, additive=True, apply_transfer=False)
+    img = r.render(w.fields, w.species, pair_capacity=1_600_000_000, **kw)
+    torch.cuda.synchronize()
+    st = r.stats()
+    assert st["overflow"] == 0
+    counts, tiles = check_integer_work(r, w, kw, 16, geometry_every=1000)
+    assert st["count"] == [int(c) for c in counts]
+    assert np.array_equal(r.debug_tile_counts(16).cpu().numpy().astype(np.int64), tiles)
+    check_windows(img, w, lut, kw, windows_for(img, 16, 0, 1))
+    r.close()
