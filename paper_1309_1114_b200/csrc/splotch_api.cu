@@ -364,21 +364,30 @@ int launch_render_tail(splotch_ctx *c, const Layout &L, char *ws, const FramePar
     return SPLOTCH_OK;
 }
 
-template <bool AL, bool GH>
-void launch_count(const Layout &L, size_t hbytes, const splotch_particles *p, unsigned long long n, unsigned long long per,
-                  const FrameParams &fp, unsigned int *counts, unsigned int *cls_counts, cudaStream_t st)
+template <bool AL, bool GH, bool BT>
+void launch_bin_kernels_count(const Layout &L, size_t hbytes, const splotch_particles *p, unsigned long long n, unsigned long long per,
+                              const FrameParams &fp, unsigned int *counts, unsigned int *cls_counts, cudaStream_t st)
 {
-    k_count<AL, GH><<<L.nrows, kBinThreads, GH ? 0 : hbytes, st>>>(p->x, p->y, p->z, p->h, n, per, fp, counts, cls_counts);
+    k_count<AL, GH, BT><<<L.nrows, kBinThreads, GH ? 0 : hbytes, st>>>(p->x, p->y, p->z, p->h, n, per, fp, counts, cls_counts);
 }
 
-template <bool AL, bool GH>
-void launch_scatter(const Layout &L, size_t hbytes, const splotch_particles *p, unsigned long long n, unsigned long long per,
-                    const FrameParams &fp, unsigned int *counts, unsigned int *cursors, const uint2 *run, DeviceStats *stats, float4 *records,
-                    cudaStream_t st)
+template <bool AL, bool GH, bool BT>
+void launch_bin_kernels_scatter(const Layout &L, size_t hbytes, const splotch_particles *p, unsigned long long n, unsigned long long per,
+                                const FrameParams &fp, unsigned int *counts, unsigned int *cursors, const uint2 *run, DeviceStats *stats,
+                                float4 *records, cudaStream_t st)
 {
-    k_scatter<AL, GH><<<L.nrows, kBinThreads, GH ? sizeof(float4) * kLutSmemMax : hbytes, st>>>(p->x, p->y, p->z, p->h, p->I, p->scalar, n, per, fp,
-                                                                                           counts, cursors, run, stats, records);
+    k_scatter<AL, GH, BT><<<L.nrows, kBinThreads, GH ? sizeof(float4) * kLutSmemMax : hbytes, st>>>(p->x, p->y, p->z, p->h, p->I, p->scalar, n, per, fp,
+                                                                                               counts, cursors, run, stats, records);
 }
+
+// the eight variants: 16-byte aligned fields or not, histogram in shared memory or in the count matrix, default or Btile binning
+#define SPLOTCH_DISPATCH3(fn, al, gh, bt, ...)                                                                          \
+    do {                                                                                                                \
+        if (al) { if (gh) { if (bt) fn<true, true, true>(__VA_ARGS__); else fn<true, true, false>(__VA_ARGS__); }       \
+                  else    { if (bt) fn<true, false, true>(__VA_ARGS__); else fn<true, false, false>(__VA_ARGS__); } }   \
+        else    { if (gh) { if (bt) fn<false, true, true>(__VA_ARGS__); else fn<false, true, false>(__VA_ARGS__); }     \
+                  else    { if (bt) fn<false, false, true>(__VA_ARGS__); else fn<false, false, false>(__VA_ARGS__); } } \
+    } while (0)
 
 // Normalisation ranges found on the device (PAPER.md:166 fn. 1) for the species with auto_range: particles [lo, lo + len) of
 // the set the pointers of `p` address; species ranges sp_begin are relative to that set.  init / finish bracket the passes.
@@ -430,8 +439,7 @@ int render_device(splotch_ctx *c, const splotch_particles *p, unsigned long long
     if (ctl.first && fp.btile) cudaMemsetAsync(ws + L.planes, 0, L.planes_bytes, st);
     else cudaMemsetAsync(ws + L.stats, 0, offsetof(DeviceStats, f_count), st);                     // the chunk part of DeviceStats
     if (L.ghist) cudaMemsetAsync(counts, 0, L.counts_bytes, st);                    // the blocks count straight into their rows
-    if (L.ghist) { if (al) launch_count<true, true>(L, hbytes, p, n, per, fp, counts, cls_counts, st); else launch_count<false, true>(L, hbytes, p, n, per, fp, counts, cls_counts, st); }
-    else         { if (al) launch_count<true, false>(L, hbytes, p, n, per, fp, counts, cls_counts, st); else launch_count<false, false>(L, hbytes, p, n, per, fp, counts, cls_counts, st); }
+    SPLOTCH_DISPATCH3(launch_bin_kernels_count, al, L.ghist, fp.btile != 0, L, hbytes, p, n, per, fp, counts, cls_counts, st);
     if (prof) cudaEventRecord(c->ev[1], st);
     const int bps = 1 << (fp.sshift - 5);               // 32-px blocks per super-tile side (k_large's work items)
     k_scan<<<(fp.nbins + 31) / 32, kScanThreads, 0, st>>>(counts, L.nrows, fp.nbins, fp.n_tiles, bin_count, vstart, cls_counts, 2ull * L.capacity,
@@ -441,8 +449,7 @@ int render_device(splotch_ctx *c, const splotch_particles *p, unsigned long long
     if (prof) cudaEventRecord(c->ev[2], st);
     float4 *records = (float4 *)(ws + L.records);
     unsigned int *cursors = (unsigned int *)(ws + L.cursors);
-    if (L.ghist) { if (al) launch_scatter<true, true>(L, hbytes, p, n, per, fp, counts, cursors, run, stats, records, st); else launch_scatter<false, true>(L, hbytes, p, n, per, fp, counts, cursors, run, stats, records, st); }
-    else         { if (al) launch_scatter<true, false>(L, hbytes, p, n, per, fp, counts, cursors, run, stats, records, st); else launch_scatter<false, false>(L, hbytes, p, n, per, fp, counts, cursors, run, stats, records, st); }
+    SPLOTCH_DISPATCH3(launch_bin_kernels_scatter, al, L.ghist, fp.btile != 0, L, hbytes, p, n, per, fp, counts, cursors, run, stats, records, st);
     if (prof) cudaEventRecord(c->ev[3], st);
     if (ctl.chunked) {        // the tiles' sums follow the fixed-point unit of the largest amplitude so far
         k_rescale<<<4 * c->n_sm, 256, 0, st>>>((long long *)(ws + L.accum), L.accum_bytes / sizeof(long long), stats);
@@ -581,10 +588,14 @@ int splotch_create(splotch_ctx **out, int device, int width, int height, uint64_
     int rc = [&]() -> int {
         CU_TRY(c, cudaMalloc(&c->lut, sizeof(float4) * kMaxSpecies * kMaxLut));
         CU_TRY(c, cudaMemset(c->lut, 0, sizeof(float4) * kMaxSpecies * kMaxLut));
-        CU_TRY(c, (cudaFuncSetAttribute(k_count<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb)));
-        CU_TRY(c, (cudaFuncSetAttribute(k_count<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb)));
-        CU_TRY(c, (cudaFuncSetAttribute(k_scatter<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb)));
-        CU_TRY(c, (cudaFuncSetAttribute(k_scatter<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb)));
+        CU_TRY(c, (cudaFuncSetAttribute(k_count<true, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb)));
+        CU_TRY(c, (cudaFuncSetAttribute(k_count<false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb)));
+        CU_TRY(c, (cudaFuncSetAttribute(k_scatter<true, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb)));
+        CU_TRY(c, (cudaFuncSetAttribute(k_scatter<false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb)));
+        CU_TRY(c, (cudaFuncSetAttribute(k_count<true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb)));
+        CU_TRY(c, (cudaFuncSetAttribute(k_count<false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb)));
+        CU_TRY(c, (cudaFuncSetAttribute(k_scatter<true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb)));
+        CU_TRY(c, (cudaFuncSetAttribute(k_scatter<false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb)));
         int r = query_splat_occupancy<8>(c, &c->splat_blocks_per_sm[0]);
         if (r == SPLOTCH_OK) r = query_splat_occupancy<16>(c, &c->splat_blocks_per_sm[1]);
         if (r == SPLOTCH_OK) r = query_splat_occupancy<32>(c, &c->splat_blocks_per_sm[2]);

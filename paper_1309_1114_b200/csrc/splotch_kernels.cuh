@@ -236,7 +236,31 @@ __device__ __forceinline__ unsigned int warp_sum(unsigned int v)
 // ---- A1 + A3 + A4a: classify and count ------------------------------------------------------------------------
 // Block b owns the particle range [b*per, (b+1)*per) and a private histogram over all bins; row b of `counts`
 // receives it, so the count stage needs no atomics between blocks and is deterministic.
-template <bool ALIGNED, bool GHIST>
+// Bins of an active particle: the tiles of its pixel box (SMALL: its pixel's tile, odd bin; MEDIUM: even bins) or the
+// super-tiles of the box (LARGE).  k_count and k_scatter walk them with ONE warp-uniform loop (lanes whose box is
+// exhausted idle): a single call site keeps the kernels small (divergent per-lane loops with several inlined record
+// writers ran at 5 active lanes per instruction and stalled on instruction fetch on cfg3, profiles/r2_step3_*).
+struct BinWalk {
+    int bx0, bx1, by0, by1, sh, pitch, base, mult, odd, n;      // bin = base + mult * (by * pitch + bx) + odd
+};
+
+template <bool BTILE>
+__device__ __forceinline__ BinWalk bin_walk(const Geo &g, int cls, const FrameParams &fp)
+{
+    BinWalk w;
+    const bool large = cls == LARGE;
+    w.sh = large ? fp.sshift : fp.tshift;
+    w.pitch = large ? fp.nsx : fp.ntx;
+    w.base = large ? 2 * fp.n_tiles : 0;
+    w.mult = large ? 1 : 2;
+    w.odd = cls == SMALL ? 1 : 0;
+    w.bx0 = g.x0 >> w.sh; w.bx1 = g.x1 >> w.sh; w.by0 = g.y0 >> w.sh; w.by1 = g.y1 >> w.sh;
+    if (BTILE && cls == MEDIUM) { const int2 ht = home_tile(g, fp); w.bx0 = w.bx1 = ht.x; w.by0 = w.by1 = ht.y; }   // i(p): the tile of the centre
+    w.n = cls == CULLED ? 0 : (w.bx1 - w.bx0 + 1) * (w.by1 - w.by0 + 1);
+    return w;
+}
+
+template <bool ALIGNED, bool GHIST, bool BTILE>
 __global__ void __launch_bounds__(kBinThreads, 1)
 k_count(const float *__restrict__ x, const float *__restrict__ y, const float *__restrict__ z,
         const float *__restrict__ h, unsigned long long n, unsigned long long per, const __grid_constant__ FrameParams fp,
@@ -253,7 +277,6 @@ k_count(const float *__restrict__ x, const float *__restrict__ y, const float *_
     const unsigned int len = lo < n ? (unsigned int)min(n - lo, per) : 0u;
     x += lo; y += lo; z += lo; h += lo;
     unsigned int c2 = 0, c3 = 0;                  // MEDIUM / LARGE particles of this thread (SMALL ones are the sum of the odd bins)
-    const int ts = fp.tshift, ntx2 = 2 * fp.ntx;
     // the loop bound is the same for the 32 lanes of a warp (lanes past the end idle), so warps stay converged
     const unsigned int lane4 = 4u * (threadIdx.x & 31u);
     for (unsigned int iw = 4u * (threadIdx.x & ~31u); iw < len; iw += 4u * kBinThreads) {
@@ -268,27 +291,25 @@ k_count(const float *__restrict__ x, const float *__restrict__ y, const float *_
             const Geo g = geometry(xs[j], ys[j], zs[j], hs[j], fp);
             const int cls = (i + j < len) ? g.cls : CULLED;
             c2 += cls == MEDIUM; c3 += cls == LARGE;
-            // SMALL and MEDIUM: the tiles of the pixel box.  A box covers at most 2 x 2 tiles unless it is wider than a
-            // tile: four predicated reductions, no loop
-            int tx0 = g.x0 >> ts, ty0 = g.y0 >> ts, tx1 = g.x1 >> ts, ty1 = g.y1 >> ts;
-            if (fp.btile && cls == MEDIUM) { const int2 ht = home_tile(g, fp); tx0 = tx1 = ht.x; ty0 = ty1 = ht.y; }   // i(p): the tile of the centre
-            const bool tile = cls == SMALL || cls == MEDIUM, w2 = tx1 > tx0, h2 = ty1 > ty0;
-            unsigned int *h00 = hist + (2 * (ty0 * fp.ntx + tx0) + (cls == SMALL ? 1 : 0));
-            if (tile) hist_inc<GHIST>(h00);
-            if (tile && w2) hist_inc<GHIST>(h00 + 2);
-            if (tile && h2) hist_inc<GHIST>(h00 + ntx2);
-            if (tile && w2 && h2) hist_inc<GHIST>(h00 + ntx2 + 2);
-            // rare: MEDIUM boxes over more than 2 x 2 tiles, and LARGE particles (super-tile bins)
-            const bool big = tile && (tx1 - tx0 > 1 || ty1 - ty0 > 1);
-            if (__any_sync(0xffffffffu, big || cls == LARGE)) {
-                if (big) {
-                    for (int ty = ty0; ty <= ty1; ++ty)
-                        for (int tx = tx0; tx <= tx1; ++tx)
-                            if (tx - tx0 > 1 || ty - ty0 > 1) hist_inc<GHIST>(hist + 2 * (ty * fp.ntx + tx));
-                } else if (cls == LARGE) {
-                    const int ss = fp.sshift;
-                    for (int sy = g.y0 >> ss; sy <= (g.y1 >> ss); ++sy)
-                        for (int sx = g.x0 >> ss; sx <= (g.x1 >> ss); ++sx) hist_inc<GHIST>(hist + 2 * fp.n_tiles + sy * fp.nsx + sx);
+            const BinWalk w = bin_walk<BTILE>(g, cls, fp);
+            // a box covers at most 2 x 2 bins unless it is wider than a bin: four predicated increments, then (rare) one
+            // warp-uniform walk over the bins beyond the first 2 x 2
+            unsigned int *h00 = hist + (w.base + w.mult * (w.by0 * w.pitch + w.bx0) + w.odd);
+            const bool any = w.n > 0, w2 = w.bx1 > w.bx0, h2 = w.by1 > w.by0;
+            if (any) hist_inc<GHIST>(h00);
+            if (any && w2) hist_inc<GHIST>(h00 + w.mult);
+            if (any && h2) hist_inc<GHIST>(h00 + w.mult * w.pitch);
+            if (any && w2 && h2) hist_inc<GHIST>(h00 + w.mult * w.pitch + w.mult);
+            const bool big = any && (w.bx1 - w.bx0 > 1 || w.by1 - w.by0 > 1);
+            if (__any_sync(0xffffffffu, big)) {
+                const int nmax = __reduce_max_sync(0xffffffffu, big ? w.n : 0);
+                int bx = w.bx0, by = w.by0;
+#pragma unroll 1
+                for (int t = 1; t < nmax; ++t) {
+                    const bool wrap = bx == w.bx1;
+                    bx = wrap ? w.bx0 : bx + 1;
+                    by += wrap;
+                    if (big && t < w.n && (bx - w.bx0 > 1 || by - w.by0 > 1)) hist_inc<GHIST>(hist + (w.base + w.mult * (by * w.pitch + bx)));
                 }
             }
         }
@@ -670,18 +691,13 @@ __device__ __forceinline__ float3 amplitude(float I, float scalar, float h, cons
 //   SMALL, 16 bytes: {pixel, aR, aG, aB}: pixel = y * T + x inside the tile, a = E * col * pi sp^2 (1 - exp(-chi^2)),
 //     the whole clipped flux (R6): a SMALL particle needs "only its location".
 // A record whose amplitude is not finite (I or scalar = Inf / NaN) carries amplitude 0.
-__device__ __forceinline__ unsigned int pack_box_tile(const Geo &g, int tx, int ty, const FrameParams &fp)
+// box of the particle clipped to bin (bx, by), relative to the bin's origin
+__device__ __forceinline__ unsigned int pack_box(const Geo &g, int bx, int by, int sh, bool large)
 {
-    const int ox = tx << fp.tshift, oy = ty << fp.tshift, m = fp.T - 1;
+    const int ox = bx << sh, oy = by << sh, m = (1 << sh) - 1;
     const int cx0 = max(g.x0 - ox, 0), cx1 = min(g.x1 - ox, m), cy0 = max(g.y0 - oy, 0), cy1 = min(g.y1 - oy, m);
-    return (unsigned int)cx0 | ((unsigned int)cy0 << 6) | ((unsigned int)(cx1 - cx0) << 12) | ((unsigned int)(cy1 - cy0) << 18);
-}
-
-__device__ __forceinline__ unsigned int pack_box_super(const Geo &g, int sx, int sy, const FrameParams &fp)
-{
-    const int ox = sx << fp.sshift, oy = sy << fp.sshift, m = (1 << fp.sshift) - 1;
-    const int cx0 = max(g.x0 - ox, 0), cx1 = min(g.x1 - ox, m), cy0 = max(g.y0 - oy, 0), cy1 = min(g.y1 - oy, m);
-    return (unsigned int)cx0 | ((unsigned int)cy0 << 8) | ((unsigned int)cx1 << 16) | ((unsigned int)cy1 << 24);
+    return large ? ((unsigned int)cx0 | ((unsigned int)cy0 << 8) | ((unsigned int)cx1 << 16) | ((unsigned int)cy1 << 24))
+                 : ((unsigned int)cx0 | ((unsigned int)cy0 << 6) | ((unsigned int)(cx1 - cx0) << 12) | ((unsigned int)(cy1 - cy0) << 18));
 }
 
 // next free unit of a bin's run: shared-memory cursor, or the block's row of the count matrix (see hist_inc)
@@ -691,7 +707,7 @@ __device__ __forceinline__ unsigned int cursor_take(unsigned int *p, unsigned in
     return atomicAdd(p, units);
 }
 
-template <bool ALIGNED, bool GHIST>
+template <bool ALIGNED, bool GHIST, bool BTILE>
 __global__ void __launch_bounds__(kBinThreads, 1)
 k_scatter(const float *__restrict__ x, const float *__restrict__ y, const float *__restrict__ z,
           const float *__restrict__ h, const float *__restrict__ I, const float *__restrict__ scalar,
@@ -733,7 +749,7 @@ k_scatter(const float *__restrict__ x, const float *__restrict__ y, const float 
     const int s_first = species_of(lo32, fp), s_last = species_of(lo32 + (len ? len - 1 : 0), fp);
     float amax = 0.0f;
     const bool one_species = s_first == s_last;
-    const int ts = fp.tshift, tmask = fp.T - 1, ntx2 = 2 * fp.ntx;
+    const int ts = fp.tshift, tmask = fp.T - 1;
     const unsigned int lane4 = 4u * (threadIdx.x & 31u);
     for (unsigned int iw = 4u * (threadIdx.x & ~31u); iw < len; iw += 4u * kBinThreads) {
         const unsigned int i = iw + lane4;
@@ -760,54 +776,51 @@ k_scatter(const float *__restrict__ x, const float *__restrict__ y, const float 
             float3 a = amplitude(Is[j], ss[j], hs[j], S, lut, s_rng[s], make_float3(vr[j], vg[j], vb[j]));
             const bool small = cls == SMALL;
             const float sp2 = __fmul_rn(g.sp, g.sp);
-            const float w = small ? fp.csmall * sp2 : 1.0f;
-            a.x *= w; a.y *= w; a.z *= w;
+            const float wsm = small ? fp.csmall * sp2 : 1.0f;
+            a.x *= wsm; a.y *= wsm; a.z *= wsm;
             const float am = fmaxf(fabsf(a.x), fmaxf(fabsf(a.y), fabsf(a.z)));
             if (!(am <= 3.0e38f)) a = make_float3(0.0f, 0.0f, 0.0f);             // Inf / NaN amplitude
             else if (cls != CULLED) amax = fmaxf(amax, am);
-            const int tx0 = g.x0 >> ts, ty0 = g.y0 >> ts, tx1 = g.x1 >> ts, ty1 = g.y1 >> ts;
-            unsigned int *c00 = cursor + 2 * (ty0 * fp.ntx + tx0);
-            if (fp.btile) {
-                // the paper's scheme: SMALL particles go straight to the small-particle partial image, a MEDIUM particle to
-                // the tile of its centre with its box relative to that tile's Btile (body + boundary of r_0)
-                if (small) {
+            const BinWalk w = bin_walk<BTILE>(g, cls, fp);
+            if (small) {
+                if (BTILE) {       // the paper's scheme: SMALL particles go straight to the small-particle partial image
                     float *o = fp.btile_planes + 4 * (3 * (size_t)fp.W * fp.H) + 3 * ((size_t)g.y0 * fp.W + g.x0);
                     asm volatile("red.global.add.f32 [%0], %1;" :: "l"(o), "f"(a.x) : "memory");
                     asm volatile("red.global.add.f32 [%0], %1;" :: "l"(o + 1), "f"(a.y) : "memory");
                     asm volatile("red.global.add.f32 [%0], %1;" :: "l"(o + 2), "f"(a.z) : "memory");
-                } else if (cls == MEDIUM) {
-                    const int2 ht = home_tile(g, fp);
-                    const int ox = (ht.x << ts) - fp.btile_r0, oy = (ht.y << ts) - fp.btile_r0;
-                    const unsigned int box = (unsigned int)(g.x0 - ox) | ((unsigned int)(g.y0 - oy) << 6) |
-                                             ((unsigned int)(g.x1 - g.x0) << 12) | ((unsigned int)(g.y1 - g.y0) << 18);
-                    const float4 rm = make_float4(g.px, g.py, __fdividef(-1.4426950408889634f, sp2), __fmul_rn(g.rp, g.rp));
-                    st_record(records, cursor_take<GHIST>(cursor + 2 * (ht.y * fp.ntx + ht.x), 2u), rm, make_float4(a.x, a.y, a.z, __uint_as_float(box)));
+                } else {
+                    const unsigned int pix = (unsigned int)(((g.y0 & tmask) << ts) | (g.x0 & tmask));
+                    const unsigned int u = cursor_take<GHIST>(cursor + (2 * (w.by0 * fp.ntx + w.bx0) + 1), 1u);
+                    asm volatile("st.global.v4.f32 [%0], {%1,%2,%3,%4};" :: "l"(records + u), "f"(__uint_as_float(pix)), "f"(a.x), "f"(a.y), "f"(a.z) : "memory");
                 }
-            } else if (small) {
-                const unsigned int pix = (unsigned int)(((g.y0 & tmask) << ts) | (g.x0 & tmask));
-                const unsigned int u = cursor_take<GHIST>(c00 + 1, 1u);
-                asm volatile("st.global.v4.f32 [%0], {%1,%2,%3,%4};" :: "l"(records + u), "f"(__uint_as_float(pix)), "f"(a.x), "f"(a.y), "f"(a.z) : "memory");
             }
-            const float4 ra = make_float4(g.px, g.py, __fdividef(-1.4426950408889634f, sp2), __fmul_rn(g.rp, g.rp));
-            if (cls == MEDIUM && !fp.btile) {
-                const bool w2 = tx1 > tx0, h2 = ty1 > ty0;
-                st_record(records, cursor_take<GHIST>(c00, 2u), ra, make_float4(a.x, a.y, a.z, __uint_as_float(pack_box_tile(g, tx0, ty0, fp))));
-                if (w2) st_record(records, cursor_take<GHIST>(c00 + 2, 2u), ra, make_float4(a.x, a.y, a.z, __uint_as_float(pack_box_tile(g, tx0 + 1, ty0, fp))));
-                if (h2) st_record(records, cursor_take<GHIST>(c00 + ntx2, 2u), ra, make_float4(a.x, a.y, a.z, __uint_as_float(pack_box_tile(g, tx0, ty0 + 1, fp))));
-                if (w2 && h2) st_record(records, cursor_take<GHIST>(c00 + ntx2 + 2, 2u), ra, make_float4(a.x, a.y, a.z, __uint_as_float(pack_box_tile(g, tx0 + 1, ty0 + 1, fp))));
-                if (tx1 - tx0 > 1 || ty1 - ty0 > 1) {
-                    for (int ty = ty0; ty <= ty1; ++ty)
-                        for (int tx = tx0; tx <= tx1; ++tx)
-                            if (tx - tx0 > 1 || ty - ty0 > 1)
-                                st_record(records, cursor_take<GHIST>(cursor + 2 * (ty * fp.ntx + tx), 2u), ra,
-                                          make_float4(a.x, a.y, a.z, __uint_as_float(pack_box_tile(g, tx, ty, fp))));
+            // MEDIUM and LARGE: one 32-byte record per bin of the box, one warp-uniform walk, one call site
+            const int nrec = (cls == MEDIUM || cls == LARGE) ? w.n : 0;
+            if (__any_sync(0xffffffffu, nrec > 0)) {
+                const float4 ra = make_float4(g.px, g.py, __fdividef(-1.4426950408889634f, sp2), __fmul_rn(g.rp, g.rp));
+                int bx = w.bx0, by = w.by0;
+                auto emit = [&]() {
+                    unsigned int box;
+                    if (BTILE && cls == MEDIUM) {      // box relative to the home tile's Btile (body + boundary of r_0)
+                        const int ox = (bx << ts) - fp.btile_r0, oy = (by << ts) - fp.btile_r0;
+                        box = (unsigned int)(g.x0 - ox) | ((unsigned int)(g.y0 - oy) << 6) | ((unsigned int)(g.x1 - g.x0) << 12) | ((unsigned int)(g.y1 - g.y0) << 18);
+                    } else {
+                        box = pack_box(g, bx, by, w.sh, cls == LARGE);
+                    }
+                    st_record(records, cursor_take<GHIST>(cursor + (w.base + w.mult * (by * w.pitch + bx)), 2u), ra,
+                              make_float4(a.x, a.y, a.z, __uint_as_float(box)));
+                };
+                if (nrec > 0) emit();                          // most particles have one bin
+                if (__any_sync(0xffffffffu, nrec > 1)) {
+                    const int nmax = __reduce_max_sync(0xffffffffu, nrec);
+#pragma unroll 1
+                    for (int t = 1; t < nmax; ++t) {
+                        const bool wrap = bx == w.bx1;
+                        bx = wrap ? w.bx0 : bx + 1;
+                        by += wrap;
+                        if (t < nrec) emit();
+                    }
                 }
-            } else if (cls == LARGE) {
-                const int ss2 = fp.sshift;
-                for (int sy = g.y0 >> ss2; sy <= (g.y1 >> ss2); ++sy)
-                    for (int sx = g.x0 >> ss2; sx <= (g.x1 >> ss2); ++sx)
-                        st_record(records, cursor_take<GHIST>(cursor + 2 * fp.n_tiles + sy * fp.nsx + sx, 2u), ra,
-                                  make_float4(a.x, a.y, a.z, __uint_as_float(pack_box_super(g, sx, sy, fp))));
             }
         }
     }
