@@ -36,6 +36,7 @@ k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
 {
     __shared__ __align__(128) float4 stage[kLargeStages][kLargeWin][2];
     __shared__ float4 sA[kLargeWin], sB[kLargeWin];
+    __shared__ unsigned int sC[kLargeWin];                       // cutting discs: 2 bits per warp band (0 cut, 1 inside, 2 outside)
     __shared__ unsigned long long mbar[kLargeStages];
     __shared__ int s_cnt[kLargeThreads / 32][2];
     __shared__ unsigned int s_item;
@@ -181,6 +182,21 @@ k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
                     const int pos = kLargeWin - 1 - (boff + (t ? __popc(mb0) : 0) + __popc((t ? mb1 : mb0) & lt));
                     sA[pos] = ra[t];
                     sB[pos] = make_float4(rb[t].x, rb[t].y, rb[t].z, safe[t] ? ex2_approx(8.0f * ra[t].z) : -1.0f);
+                    // the disc against each warp's band of 8 rows: its edge crosses a block almost as a straight line, so most
+                    // bands lie wholly inside (no-test recurrence) or wholly outside (skipped); decided once per record here
+                    unsigned int code = 0u;
+                    const float ax = cxl - ra[t].x, bx = ra[t].x - cxh;
+                    const float nx = fmaxf(fmaxf(ax, bx), 0.0f), gx = fmaxf(-ax, -bx);
+#pragma unroll
+                    for (int w = 0; w < kLargeThreads / 32; ++w) {
+                        const float yl = cyl + (float)(8 * w), yh = yl + 7.0f;
+                        const float ay = yl - ra[t].y, by = ra[t].y - yh;
+                        const float ny = fmaxf(fmaxf(ay, by), 0.0f), gy = fmaxf(-ay, -by);
+                        const bool out = fmaf(nx, nx, ny * ny) > ra[t].w * 1.0001f;
+                        const bool in = safe[t] && fmaf(gx, gx, gy * gy) <= ra[t].w * 0.9999f;
+                        code |= (out ? 2u : (in ? 1u : 0u)) << (2 * w);
+                    }
+                    sC[pos] = code;
                 }
             }
             __syncthreads();
@@ -201,27 +217,21 @@ k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
                     if (j + 2 < kLargePpt / 2) H = fmul2(H, Q);
                 }
             }
-            // ---- discs that cut the block.  A thread's 8-pixel run lies inside the disc, outside it, or across its edge; the
-            //      edge of a large disc crosses a warp's 32 x 8 pixels almost as a straight line, so most warps see only the
-            //      first two kinds: a warp with no run across the edge takes the no-test recurrence (runs outside the disc
-            //      get amplitude 0), a warp whose runs are all outside skips the record, the others test every pixel
-            //      (C1 inside test, bit-exact d2, packed; one ex2 per pixel)
+            // ---- discs that cut the block: per band of 8 rows (one warp) skipped, no-test recurrence, or the C1 inside test per
+            //      pixel (bit-exact d2, packed), one ex2 per pixel.  (The recurrence with a 0 / 1 mask for every pixel was
+            //      measured and dropped: its extra multiplications cost more FMA-pipe time than the ex2 they save.)
             for (int m = 0; m < n_cut; ++m) {
+                const unsigned int code = (sC[kLargeWin - 1 - m] >> (2 * warp)) & 3u;      // the same for all lanes of the warp
+                if (code == 2u) continue;
                 const float4 a = sA[kLargeWin - 1 - m], b = sB[kLargeWin - 1 - m];
-                const float dyf = __fsub_rn(fyc, a.y);
-                const float t2 = __fmul_rn(dyf, dyf);
-                const float dx0 = fx0 - a.x, dx7 = dx0 + 7.0f;
-                const float xf = fmaxf(fabsf(dx0), fabsf(dx7)), xn = (dx0 <= 0.0f && dx7 >= 0.0f) ? 0.0f : fminf(fabsf(dx0), fabsf(dx7));
-                const bool seg_in = fmaf(xf, xf, t2) <= a.w * 0.9999f, seg_out = fmaf(xn, xn, t2) > a.w * 1.0001f;
-                if (__all_sync(0xffffffffu, seg_out)) continue;
-                if (b.w > 0.0f && __all_sync(0xffffffffu, seg_in || seg_out)) {
-                    const float d20 = fmaf(dx0, dx0, t2);
+                if (code == 1u) {
+                    const float dy = fyc - a.y, dx0 = fx0 - a.x;
+                    const float d20 = fmaf(dx0, dx0, dy * dy);
                     const float d21 = d20 + fmaf(2.0f, dx0, 1.0f);
                     const float u0 = fmaf(4.0f, dx0, 4.0f);
                     f32x2 P = pk2(ex2_approx(a.z * d20), ex2_approx(a.z * d21));
                     f32x2 H = pk2(ex2_approx(a.z * u0), ex2_approx(a.z * (u0 + 4.0f)));
-                    const float br = seg_in ? b.x : 0.0f, bg = seg_in ? b.y : 0.0f, bb = seg_in ? b.z : 0.0f;
-                    const f32x2 Q = pk2(b.w, b.w), BR = pk2(br, br), BG = pk2(bg, bg), BB = pk2(bb, bb);
+                    const f32x2 Q = pk2(b.w, b.w), BR = pk2(b.x, b.x), BG = pk2(b.y, b.y), BB = pk2(b.z, b.z);
 #pragma unroll
                     for (int j = 0; j < kLargePpt / 2; ++j) {
                         sub[j][0] = ffma2(BR, P, sub[j][0]); sub[j][1] = ffma2(BG, P, sub[j][1]); sub[j][2] = ffma2(BB, P, sub[j][2]);
@@ -230,6 +240,8 @@ k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
                     }
                     continue;
                 }
+                const float dyf = __fsub_rn(fyc, a.y);
+                const float t2 = __fmul_rn(dyf, dyf);
                 const f32x2 T2 = pk2(t2, t2), NX = pk2(-a.x, -a.x), C = pk2(a.z, a.z);
                 const f32x2 BR = pk2(b.x, b.x), BG = pk2(b.y, b.y), BB = pk2(b.z, b.z);
 #pragma unroll

@@ -23,7 +23,6 @@
 
 namespace splotch {
 
-constexpr int kSplatWinUnits = 512;        // 16-byte units per window (8 KB): 256 MEDIUM or 512 SMALL records
 constexpr int kSplatStages = 3;
 constexpr int kSplatMaxSub = 16;           // sub-ranges (runs of one bin) a window may hold
 constexpr int kSplatEndChunk = 1, kSplatExit = 2;
@@ -37,8 +36,12 @@ struct SplatWin {                          // what the producer tells the consum
 template <int T> struct Splat2Cfg {
     using Base = SplatCfg<T>;
     static constexpr int kPix = Base::kPix, kConsumers = Base::kThreads, kThreads = Base::kThreads + 32;
-    static constexpr int kMaxRec = kSplatWinUnits / 2;               // MEDIUM records per sub-range
-    static constexpr size_t kStageBytes = 16u * kSplatWinUnits;
+    // 16-byte units per window: 256 MEDIUM or 512 SMALL records for the 4-warp tiles, twice that for the 16-warp ones
+    // (one record per consumer thread and decode round, as many records per barrier)
+    static constexpr int kWinUnits = T >= 32 ? 1024 : 512;
+    static constexpr int kMaxRec = kWinUnits / 2;                    // MEDIUM records per sub-range
+    static constexpr size_t kStageBytes = 16u * kWinUnits;
+    static constexpr int kMinBlocks = T == 8 ? 12 : (T == 16 ? 6 : (T == 32 ? 2 : 1));     // T = 32: two 17-warp CTAs per SM need <= 60 registers
     static constexpr size_t kSmemBytes = kStageBytes * kSplatStages + sizeof(unsigned int) * (6 * kPix + 2 * kMaxRec) +
                                          sizeof(unsigned short) * kMaxRec * Base::kWarps + sizeof(SplatWin) * kSplatStages + 16 * kSplatStages;
 };
@@ -105,13 +108,13 @@ __device__ __forceinline__ void mbar_wait_relaxed(unsigned int bar, unsigned int
 }
 
 template <int T>
-__global__ void __launch_bounds__(Splat2Cfg<T>::kThreads)
+__global__ void __launch_bounds__(Splat2Cfg<T>::kThreads, Splat2Cfg<T>::kMinBlocks)
 k_splat(const float4 *__restrict__ records, const unsigned int *__restrict__ vstart, const uint2 *__restrict__ run,
         DeviceStats *__restrict__ stats, unsigned long long *__restrict__ accum, const __grid_constant__ FrameParams fp)
 {
     using Cfg = Splat2Cfg<T>;
     using Geo = SplatCfg<T>;
-    constexpr int kPix = Cfg::kPix, kConsumers = Cfg::kConsumers, kMaxRec = Cfg::kMaxRec, kNP = Geo::kNP;
+    constexpr int kPix = Cfg::kPix, kConsumers = Cfg::kConsumers, kMaxRec = Cfg::kMaxRec, kNP = Geo::kNP, kSplatWinUnits = Cfg::kWinUnits;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float4 *stage = reinterpret_cast<float4 *>(smem_raw);                                        // [kSplatStages][kSplatWinUnits]
     unsigned int *fb = reinterpret_cast<unsigned int *>(stage + kSplatStages * kSplatWinUnits);  // lo R G B, hi R G B
