@@ -39,7 +39,12 @@ L2_FLUSH_BYTES = 256 << 20   # written between frames when a config's inputs fit
 DEFAULT_CONFIG = 3           # the largest single-GPU configuration of BASELINE.json
 
 
+TILE_OVERRIDE = 0
+
+
 def tile_for(cfg: int) -> int:
+    if TILE_OVERRIDE:
+        return TILE_OVERRIDE
     return 32 if cfg == 3 else 16       # 4096^2: 16,384 tiles of 32 px (65,536 of 16 px work too, on the slower global-histogram path)
 
 
@@ -518,9 +523,12 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=None)
     ap.add_argument("--ref-sample", type=int, default=10_000_000)
     ap.add_argument("--no-per-config", action="store_true", help="skip the per_config sweep over the other configs")
+    ap.add_argument("--tile", type=int, default=0, help="tile side in px (default: 32 for config 3, 16 otherwise)")
     args = ap.parse_args()
     if args.cpu_sample is None:
         args.cpu_sample = default_cpu_sample(args.config)
+    global TILE_OVERRIDE
+    TILE_OVERRIDE = args.tile
     if args.impl == "reference":
         args.steps = 3 if args.steps is None else args.steps
         run_reference(args)
