@@ -2,7 +2,7 @@
 """bench.py -- particles/s of the Splotch per-frame rendering path on B200 (BASELINE.json metric).
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0..4] [--mode additive|ordered]
-                  [--impl ours|reference] [--no-per-config]
+                  [--impl ours|reference] [--no-per-config] [--frames-only] [--tile T]
 
 A step is one whole frame (count -> scan -> scatter -> splat -> large -> compose) with the particles already
 resident in HBM.  BASELINE.json's metric names no config, so the default line is on the largest single-GPU
@@ -340,6 +340,13 @@ def run_ours(args):
     sampler.join(timeout=1.0)
     ms_step = max_over_ranks(ms_local, dist, f"cuda:{local}")
 
+    if args.frames_only:          # profiling runs (ncu): the timed frames only, no end-to-end leg, no CPU baseline
+        if rank == 0:
+            print(json.dumps({"frames_only": True, "workload": w.name, "mode": args.mode, "tile": run.tile, "ms_per_step": ms_step,
+                              "stages": st["stage_ms"]}))
+        if dist is not None:
+            dist.destroy_process_group()
+        return
     # ---- end to end through the C ABI with HOST buffers ---------------------------------------------------------
     host = {k: v.cpu().pin_memory() for k, v in run.fields.items()}
     himg = torch.empty((w.height, w.width, 3), dtype=torch.float32).pin_memory()
@@ -523,6 +530,7 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=None)
     ap.add_argument("--ref-sample", type=int, default=10_000_000)
     ap.add_argument("--no-per-config", action="store_true", help="skip the per_config sweep over the other configs")
+    ap.add_argument("--frames-only", action="store_true", help="time the frames and stop (for runs under ncu)")
     ap.add_argument("--tile", type=int, default=0, help="tile side in px (default: 32 for config 3, 16 otherwise)")
     args = ap.parse_args()
     if args.cpu_sample is None:
