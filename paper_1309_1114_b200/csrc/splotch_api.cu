@@ -348,7 +348,7 @@ int launch_render_tail(splotch_ctx *c, const Layout &L, char *ws, const FramePar
             (unsigned long long *)(ws + L.accum), fp);
     }
     if (prof) cudaEventRecord(c->ev[4], st);
-    k_large<<<c->n_sm * c->large_blocks_per_sm, kLargeThreads, 0, st>>>(
+    k_large<<<c->n_sm * c->large_blocks_per_sm, kLargeThreads, sizeof(LargeSmem), st>>>(
         (const float4 *)(ws + L.records), (const unsigned int *)(ws + L.bin_count), (const uint2 *)(ws + L.run), (const unsigned int *)(ws + L.large_off),
         (DeviceStats *)(ws + L.stats), (unsigned long long *)(ws + L.accum), fp);
     if (prof) cudaEventRecord(c->ev[5], st);
@@ -606,8 +606,21 @@ int splotch_create(splotch_ctx **out, int device, int width, int height, uint64_
         CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->orender_blocks_per_sm[1], k_orender<16>, SplatCfg<16>::kThreads, 0));
         CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->orender_blocks_per_sm[2], k_orender<32>, SplatCfg<32>::kThreads, 0));
         for (int k = 0; k < 3; ++k) if (c->orender_blocks_per_sm[k] < 1) c->orender_blocks_per_sm[k] = 1;
-        CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->large_blocks_per_sm, k_large, kLargeThreads, 0));
-        if (c->large_blocks_per_sm < 1) c->large_blocks_per_sm = 1;
+        {   // k_large allocates tensor memory, which the occupancy calculator answers with one block per SM: count registers,
+            // shared memory and tensor-memory columns here
+            cudaFuncAttributes fa;
+            cudaDeviceProp prop;
+            CU_TRY(c, cudaFuncSetAttribute(k_large, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(LargeSmem)));
+            CU_TRY(c, cudaFuncGetAttributes(&fa, k_large));
+            CU_TRY(c, cudaGetDeviceProperties(&prop, c->device));
+            const int regs_per_block = ((fa.numRegs + 7) / 8 * 8) * kLargeThreads;
+            const int by_regs = prop.regsPerMultiprocessor / (regs_per_block > 0 ? regs_per_block : 1);
+            const int by_smem = (int)(prop.sharedMemPerMultiprocessor / (fa.sharedSizeBytes + sizeof(LargeSmem) + 1024));
+            const int by_tmem = 512 / (int)kLargeTmemCols;
+            int b = by_regs < by_smem ? by_regs : by_smem;
+            if (by_tmem < b) b = by_tmem;
+            c->large_blocks_per_sm = b < 1 ? 1 : b;
+        }
         return r;
     }();
     if (rc != SPLOTCH_OK) {

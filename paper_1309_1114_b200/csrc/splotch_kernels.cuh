@@ -878,6 +878,8 @@ __device__ __forceinline__ void upk2(f32x2 v, float &a, float &b) { asm("mov.b64
 __device__ __forceinline__ f32x2 fadd2(f32x2 a, f32x2 b) { f32x2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 __device__ __forceinline__ f32x2 fmul2(f32x2 a, f32x2 b) { f32x2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 __device__ __forceinline__ f32x2 ffma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+// c += a * b with the sum pinned to its register pair (a separate result register made ptxas copy 24 accumulator registers per record)
+__device__ __forceinline__ void ffma2_acc(f32x2 &c, f32x2 a, f32x2 b) { asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(c) : "l"(a), "l"(b)); }
 
 // Framebuffer of a tile in shared memory, fixed point: per channel a low plane (sums of the low 16 bits of each
 // contribution, unsigned) and a high plane (sums of the signed upper bits).  value = hi * 65536 + lo, in units of
