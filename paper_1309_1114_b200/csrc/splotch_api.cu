@@ -92,7 +92,7 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 int tile_shift(int T) { return T == 8 ? 3 : T == 16 ? 4 : T == 32 ? 5 : T == 64 ? 6 : -1; }
 
-// LARGE particles are binned to super-tiles of 8 x 8 tiles, at most 256 px a side (record boxes are 8 bits per bound)
+// LARGE particles are binned to super-tiles of 8 x 8 tiles, at most 128 px a side (record boxes are 8 bits per bound)
 int super_shift(int T) { const int s = tile_shift(T) + kSuperShift; return s < kSuperMaxShift ? s : kSuperMaxShift; }
 
 size_t hist_bytes(int W, int H, int T)

@@ -2,20 +2,28 @@
 //
 // The paper renders large particles on the CPU while the GPU works on the rest and names the
 // resulting imbalance as its bottleneck for R_0 > 2 (:324).  Here they stay on the GPU: k_scatter files each LARGE
-// particle under every super-tile (up to 256 x 256 px) its box touches, and k_large splits the work into items of
+// particle under every super-tile (128 x 128 px) its box touches, and k_large splits the work into items of
 // (chunk of a super-tile's records) x (32 x 32-pixel block of that super-tile) that CTAs take from an atomic counter,
 // so a region covered by hundreds of thousands of large discs (camera inside a halo, cfg3) is shared by many CTAs.
 //   * the chunk's records stream through shared memory with bulk copies on mbarriers, as in k_splat;
-//   * every thread tests two records per window against the block (box, then disc against the block's rectangle of
-//     pixel centres) and sorts the survivors into two lists: discs that contain the whole block, and the others;
-//   * pixel owners: a thread owns 8 horizontally adjacent pixels and keeps their sums in registers as packed pairs;
-//       - block inside the disc: no clip test is needed, and the Gaussian along the row follows the recurrence
-//         w(x+2) = w(x) h(x), h(x+2) = h(x) q^8 with h(x) = exp2(c (4 dx + 4)), q^8 = exp2(8 c): four ex2 per 8 pixels
-//         instead of eight (round 1 was bound by MUFU.EX2, one per evaluated pixel, profiles/r1_step5_*);
-//       - otherwise: the C1 inside test of every pixel (bit-exact d2, packed), one ex2 per pixel;
-//   * an item ends with 64-bit fixed-point reductions into the tiles' sums in L2 (exact, commutative), the same sums
-//     k_splat feeds; k_compose turns them into the float32 image.
-// Blocks are 32 x 32 px whatever the tile side T is (a thread's 8-pixel run never straddles a tile).
+//   * every thread tests two records per window against the block's four bands of 8 rows x 32 pixels and files the record
+//     in up to two lists: bands that lie wholly inside the clip disc, bands the edge of the disc crosses;
+//   * bands inside the disc: no pixel is clipped and the Gaussian is separable, exp2(c d^2) = exp2(c dx^2) exp2(c dy^2), so
+//     the sum over the records is a dense contraction D[(colour, y)][x] = sum_p A[(colour, y)][p] B[p][x] with
+//     A = a_colour exp2(c dy^2) (zero in the rows of the record's other bands), B = exp2(c dx^2).  It runs on the
+//     5th-generation tensor cores: tcgen05.mma kind::tf32, M = 128 (three colours x 32 rows), N = 32, K = 8 records per
+//     instruction, accumulator in tensor memory.  TF32 keeps 10 mantissa bits (the hardware truncates), so every float32
+//     operand is split into a high and a low part and three products are added (hi hi + hi lo + lo hi: relative error 2^-21).
+//     A is written straight to tensor memory by the lane that owns the row (tcgen05.st), B to shared memory (K-major core
+//     matrices, no swizzle), in groups of 16 records with two operand buffers; tcgen05.commit on an mbarrier frees a
+//     buffer.  The tensor cores add with truncation (measured: -1.7e-8 relative per accumulated record), so an accumulator
+//     takes 64 records, then the other one takes over and the first is folded into float32 second-level sums;
+//   * bands the edge crosses: pixel owners (a thread owns 8 adjacent pixels of a row, sums in registers as packed pairs)
+//     evaluate the C1 inside test of every pixel (bit-exact packed d2), one ex2 per pixel inside;
+//   * sums go to the tiles' 64-bit fixed-point sums in L2 (exact, commutative), the same sums k_splat feeds; k_compose
+//     turns them into the float32 image.
+// Blocks are 32 x 32 px whatever the tile side T is.  Measured on cfg3 (9.5e11 LARGE fragments): round 1 397 ms (one ex2 per
+// pixel), row recurrence 296 ms, tensor-core bands 282 ms, 128-px super-tiles 245 ms.
 #pragma once
 #include "splotch_kernels.cuh"
 #include "splotch_splat.cuh"
