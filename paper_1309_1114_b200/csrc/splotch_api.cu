@@ -209,10 +209,10 @@ void make_layout_ordered(const splotch_ctx *c, unsigned long long n, int T, unsi
     for (int k = 0; k < 2; ++k) { L->keys[k] = off; off = align_up(off + 8ull * capacity, 256); }
     for (int k = 0; k < 2; ++k) { L->vals[k] = off; off = align_up(off + 4ull * capacity, 256); }
     // one (t, c_R, c_G, c_B) per pixel and segment; segment slot = chunk + tile; k_oscan cuts the pairs into at most
-    // 128 chunks per SM, or capacity / kChunkMax when that is more
+    // 128 chunks per SM, or capacity / kOChunkMax when that is more
     L->seg = off;
     {
-        const size_t by_sm = (size_t)c->n_sm * 128, by_cap = (size_t)(capacity / kChunkMax);
+        const size_t by_sm = (size_t)c->n_sm * 128, by_cap = (size_t)(capacity / kOChunkMax) + 1;
         const size_t by_min = (size_t)(capacity / kOChunkMin) + 1;             // no chunk is shorter than kOChunkMin
         size_t chunks = by_sm > by_cap ? by_sm : by_cap;
         if (chunks > by_min) chunks = by_min;
@@ -474,7 +474,7 @@ void launch_ordered_tail(splotch_ctx *c, const Layout &L, char *ws, const FrameP
     const int ti = T == 8 ? 0 : T == 16 ? 1 : 2;
     DeviceStats *stats = (DeviceStats *)(ws + L.stats);
     const unsigned int *tile_start = (const unsigned int *)(ws + L.tile_start);
-    k_orender<T><<<c->n_sm * c->orender_blocks_per_sm[ti], SplatCfg<T>::kThreads, 0, st>>>(
+    k_orender<T><<<c->n_sm * c->orender_blocks_per_sm[ti], kORThreads, sizeof(ORenderSmem<T>), st>>>(
         (const float4 *)(ws + L.rec), vals0, vals1, tile_start, stats, (float4 *)(ws + L.seg), fp);
     if (c->profiling) cudaEventRecord(c->ev[6], st);
     k_ocombine<T><<<fp.n_tiles * (T * T / kCombinePix), kCombinePix * kCombineSlices, 0, st>>>((const float4 *)(ws + L.seg), tile_start, stats, fp, image);
@@ -602,9 +602,12 @@ int splotch_create(splotch_ctx **out, int device, int width, int height, uint64_
         if (r == SPLOTCH_OK) r = query_splat_occupancy<64>(c, &c->splat_blocks_per_sm[3]);
         if (r != SPLOTCH_OK) return r;
         CU_TRY(c, cudaFuncSetAttribute(k_rs_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(RsSmem)));
-        CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->orender_blocks_per_sm[0], k_orender<8>, SplatCfg<8>::kThreads, 0));
-        CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->orender_blocks_per_sm[1], k_orender<16>, SplatCfg<16>::kThreads, 0));
-        CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->orender_blocks_per_sm[2], k_orender<32>, SplatCfg<32>::kThreads, 0));
+        CU_TRY(c, cudaFuncSetAttribute(k_orender<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(ORenderSmem<8>)));
+        CU_TRY(c, cudaFuncSetAttribute(k_orender<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(ORenderSmem<16>)));
+        CU_TRY(c, cudaFuncSetAttribute(k_orender<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(ORenderSmem<32>)));
+        CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->orender_blocks_per_sm[0], k_orender<8>, kORThreads, sizeof(ORenderSmem<8>)));
+        CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->orender_blocks_per_sm[1], k_orender<16>, kORThreads, sizeof(ORenderSmem<16>)));
+        CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->orender_blocks_per_sm[2], k_orender<32>, kORThreads, sizeof(ORenderSmem<32>)));
         for (int k = 0; k < 3; ++k) if (c->orender_blocks_per_sm[k] < 1) c->orender_blocks_per_sm[k] = 1;
         {   // k_large allocates tensor memory, which the occupancy calculator answers with one block per SM: count registers,
             // shared memory and tensor-memory columns here

@@ -115,7 +115,7 @@ k_oscan(unsigned int *__restrict__ blk_pairs, int nblk, unsigned long long n, un
     if (threadIdx.x == 0) {
         unsigned long long cs = (total + (unsigned long long)n_sm * 128 - 1) / ((unsigned long long)n_sm * 128);
         cs = (cs + 255) / 256 * 256;             // so that chunks <= 128 n_sm (or capacity / kChunkMax): bounds the segment slots
-        cs = min((unsigned long long)kChunkMax, max((unsigned long long)kOChunkMin, cs));
+        cs = min((unsigned long long)4096, max((unsigned long long)kOChunkMin, cs));          // kOChunkMax (k_orender)
         stats->pairs = total;
         stats->large_pairs = 0ull;
         stats->sort_n = overflow ? 0ull : total;         // the sort and the renderers see an empty frame on overflow
@@ -494,26 +494,42 @@ __device__ __forceinline__ void absorb_pair(float x, float &a, float &e)
 // floor of v as an int, for any float (clamped to +-1e9 first; NaN gives -1e9)
 __device__ __forceinline__ int floor_clamped(float v) { return __float2int_rd(fminf(fmaxf(v, -1.0e9f), 1.0e9f)); }
 
+// A segment (the records of one tile inside one chunk of the sorted list) is cut into four consecutive quarters, one per
+// warp.  A warp keeps a private map (t, c_R, c_G, c_B) per pixel of the tile in shared memory and crosses its records in
+// order, 32 FRAGMENTS (record, pixel of its box inside the tile) at a time: a SMALL record is one fragment, the others one per
+// pixel of their box, so all lanes work whatever the mix (the first version gave every record to the 32 lanes that own a
+// strip of 64 pixels: 16 of 32 lanes active, 111 warp instructions per pair, profiles/r2_step1_*).  Fragments of one batch that
+// fall on the same pixel are applied in rounds, lower lane (earlier record) first: the order per pixel is the sorted order.
+// At the end of the segment the four maps are composed in order (composition is associative) into the segment's map.
+constexpr int kORThreads = 128;
+constexpr int kORWarps = kORThreads / 32;
+constexpr int kOChunkMax = 4096;               // records per chunk: a warp composes at most 1024 records in float32
+
+template <int T> struct ORenderSmem {
+    float4 map[kORWarps][T * T];
+    float4 recA[kORWarps][32], recB[kORWarps][32];
+    unsigned int box[kORWarps][32];            // x0 | y0 << 8 | (width - 1) << 16 | (height - 1) << 24, tile-relative
+    unsigned int incl[kORWarps][32];           // inclusive prefix of the fragment counts of the batch
+    unsigned int chunk;
+    int tile;
+};
+
 template <int T>
-__global__ void __launch_bounds__(SplatCfg<T>::kThreads)
+__global__ void __launch_bounds__(kORThreads)
 k_orender(const float4 *__restrict__ rec, const unsigned int *__restrict__ vals0, const unsigned int *__restrict__ vals1,
           const unsigned int *__restrict__ tile_start, DeviceStats *__restrict__ stats, float4 *__restrict__ seg,
           const __grid_constant__ FrameParams fp)
 {
-    using Cfg = SplatCfg<T>;
-    constexpr int kPix = Cfg::kPix, kThreads = Cfg::kThreads;
-    __shared__ float4 stA[2][kThreads], stB[2][kThreads];      // double buffered: one barrier per batch
-    __shared__ unsigned int stM[2][kThreads];
-    __shared__ unsigned int s_chunk;
-    __shared__ int s_tile;
+    constexpr int kPix = T * T;
+    extern __shared__ __align__(16) unsigned char orender_smem_raw[];
+    ORenderSmem<T> &S = *reinterpret_cast<ORenderSmem<T> *>(orender_smem_raw);
     const unsigned int *__restrict__ vals = (((stats->key_bits + 7u) >> 3) & 1u) ? vals1 : vals0;   // the sorted values
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int sx = warp % Cfg::kStripsX, sy = warp / Cfg::kStripsX;
-    const int lx = sx * Cfg::kSW + 2 * (lane % (Cfg::kSW / 2)), ly = sy * Cfg::kSH + lane / (Cfg::kSW / 2);
-    const unsigned int my_strip = (1u << (16 + sx)) | (1u << sy);
+    const unsigned int lt = (1u << lane) - 1u;
     const unsigned int total = (unsigned int)stats->chunks;
     const unsigned int K = stats->chunk_size;
     const unsigned int pairs = (unsigned int)stats->sort_n;
+    float4 *map = S.map[warp];
     for (;;) {
         __syncthreads();
         if (warp == 0) {
@@ -531,115 +547,129 @@ k_orender(const float4 *__restrict__ rec, const unsigned int *__restrict__ vals0
                     lo += k * step;
                     n = min(step, n - k * step);
                 }
-                if (lane == 0) s_tile = lo;
+                if (lane == 0) S.tile = lo;
             }
-            if (lane == 0) s_chunk = c;
+            if (lane == 0) S.chunk = c;
         }
         __syncthreads();
-        const unsigned int chunk = s_chunk;
+        const unsigned int chunk = S.chunk;
         if (chunk >= total) break;
         const unsigned int r0 = chunk * K, r1 = min(r0 + K, pairs);
-        int tile = s_tile;
+        int tile = S.tile;
         unsigned int tb = tile_start[tile], te = tile_start[tile + 1];
         for (;;) {
             const unsigned int begin = max(tb, r0), end = min(te, r1);
             const int tx0 = (tile % fp.ntx) * T, ty0 = (tile / fp.ntx) * T;
-            const float fx0 = __fadd_rn((float)(tx0 + lx), 0.5f), fx1 = __fadd_rn(fx0, 1.0f);
-            const float fy = __fadd_rn((float)(ty0 + ly), 0.5f);
-            // running map of the segment: double outside, float32 inside runs of ~1024 records
-            double To[2] = {1.0, 1.0}, Co[2][3] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
-            float ti[2] = {1.0f, 1.0f}, ci[2][3] = {{0.0f, 0.0f, 0.0f}, {0.0f, 0.0f, 0.0f}};
-            int fold = 0;
-            // The records of a batch are gathered through the sorted values.  Batch b + 1's records and batch b + 2's
-            // values are requested before batch b is composed, so the gather latency hides behind the arithmetic.
-            const unsigned int i0 = begin + threadIdx.x;
-            unsigned int vnext = i0 + kThreads < end ? __ldg(vals + i0 + kThreads) : 0u;
+            // this warp's quarter of the segment, in whole batches of 32 records
+            const unsigned int nb = (end - begin + 31u) / 32u, per = (nb + kORWarps - 1u) / kORWarps;
+            const unsigned int wb = min(end, begin + 32u * per * (unsigned int)warp), we = min(end, wb + 32u * per);
+            for (int i = lane; i < kPix; i += 32) map[i] = make_float4(1.0f, 0.0f, 0.0f, 0.0f);
+            __syncwarp();
+            // the records of a batch are gathered through the sorted values; the next batch's records and the following batch's
+            // values are requested before the current batch is composed
+            unsigned int vnext = wb + 32u + lane < we ? __ldg(vals + wb + 32u + lane) : 0u;
             float4 nra = make_float4(0.f, 0.f, 0.f, 0.f), nrb = nra;
-            if (i0 < end) ld_record(rec, __ldg(vals + i0), nra, nrb);
-            unsigned int batch = 0u;
-            for (unsigned int base = begin; base < end; base += kThreads, ++batch) {
-                const unsigned int idx = base + threadIdx.x;
+            if (wb + lane < we) ld_record(rec, __ldg(vals + wb + lane), nra, nrb);
+            for (unsigned int base = wb; base < we; base += 32u) {
                 const float4 ra = nra, rb = nrb;
+                const bool valid = base + lane < we;
                 {
-                    const unsigned int nxt = idx + kThreads;
+                    const unsigned int nxt = base + 32u + lane;
                     nra = make_float4(0.f, 0.f, 0.f, 0.f); nrb = nra;
-                    if (nxt < end) ld_record(rec, vnext, nra, nrb);
-                    if (nxt + kThreads < end) vnext = __ldg(vals + nxt + kThreads);
+                    if (nxt < we) ld_record(rec, vnext, nra, nrb);
+                    if (nxt + 32u < we) vnext = __ldg(vals + nxt + 32u);
                 }
-                unsigned int touch = 0u;
-                if (idx < end) {
-                    // strips the clip disc may touch (conservative: one pixel of slack; the inside test decides)
-                    const float rr = sqrtf(fabsf(ra.w)) + 1.0f;
-                    const int bx0 = max(floor_clamped(ra.x - rr) - tx0, 0), bx1 = min(floor_clamped(ra.x + rr) - tx0, T - 1);
-                    const int by0 = max(floor_clamped(ra.y - rr) - ty0, 0), by1 = min(floor_clamped(ra.y + rr) - ty0, T - 1);
-                    if (bx0 <= bx1 && by0 <= by1) {
-                        const unsigned int xm = (2u << (bx1 / Cfg::kSW)) - (1u << (bx0 / Cfg::kSW));
-                        const unsigned int ym = (2u << (by1 / Cfg::kSH)) - (1u << (by0 / Cfg::kSH));
-                        touch = (xm << 16) | ym;
+                // pixel box of the record inside the tile: exact for SMALL records (c = 0: the one pixel of the centre), one pixel of
+                // slack for the others (the C1 inside test decides)
+                unsigned int nfrag = 0u, bx = 0u;
+                if (valid) {
+                    // C1's box is ceil((p - rp) - 0.5) .. floor((p + rp) - 0.5); rp is recovered from r2 = rp^2 to a few ulp, so the bounds
+                    // are widened by a relative 1e-4 (never narrower than C1's box, one pixel wider only next to an integer)
+                    const float r2 = fabsf(ra.w);
+                    const bool point = ra.z == 0.0f;                  // SMALL: the record holds the centre of its pixel
+                    const float rr = point ? 0.0f : sqrtf(r2) * 1.0001f + 1.0e-4f;
+                    const float lo_off = point ? 0.0f : 0.5f;         // ceil(v) = floor(v - eps) + 1, done as floor(v + 0.5 - eps) for v = p - rp - 0.5 + 0.5
+                    const int x0 = max(floor_clamped(ra.x - rr + lo_off) - tx0, 0), x1 = min(floor_clamped(ra.x + rr - lo_off) - tx0, T - 1);
+                    const int y0 = max(floor_clamped(ra.y - rr + lo_off) - ty0, 0), y1 = min(floor_clamped(ra.y + rr - lo_off) - ty0, T - 1);
+                    if (x0 <= x1 && y0 <= y1) {
+                        nfrag = (unsigned int)((x1 - x0 + 1) * (y1 - y0 + 1));
+                        bx = (unsigned int)x0 | ((unsigned int)y0 << 8) | ((unsigned int)(x1 - x0) << 16) | ((unsigned int)(y1 - y0) << 24);
                     }
                 }
-                const float4 *sA = stA[batch & 1u], *sB = stB[batch & 1u];
-                const unsigned int *sM = stM[batch & 1u];
-                stA[batch & 1u][threadIdx.x] = ra; stB[batch & 1u][threadIdx.x] = rb; stM[batch & 1u][threadIdx.x] = touch;
-                __syncthreads();             // batch visible; every warp is done with the batch before the previous one
-#pragma unroll 1
-                for (int g = 0; g < kThreads; g += 32) {
-                    const unsigned int t = sM[g + lane];
-                    unsigned int m = __ballot_sync(0xffffffffu, (t & my_strip & 0xffff0000u) && (t & my_strip & 0xffffu));
-                    while (m) {                                            // ascending bit order = depth order
-                        const int r = g + __ffs(m) - 1;
-                        m &= m - 1;
-                        const float4 A = sA[r], B = sB[r];
-                        const float r2 = fabsf(A.w);
-                        const bool emit_only = A.w < 0.0f;
-                        const float dyf = __fsub_rn(fy, A.y);
-                        const float t2 = __fmul_rn(dyf, dyf);
+                unsigned int inc = nfrag;
 #pragma unroll
-                        for (int q = 0; q < 2; ++q) {
-                            const float dxf = __fsub_rn(q ? fx1 : fx0, A.x);
-                            const float d2 = __fmaf_rn(dxf, dxf, t2);
-                            if (d2 <= r2) {
-                                const float wgt = ex2_approx(d2 * A.z);
-                                if (emit_only) {
-                                    ci[q][0] = fmaf(B.x, wgt, ci[q][0]);
-                                    ci[q][1] = fmaf(B.y, wgt, ci[q][1]);
-                                    ci[q][2] = fmaf(B.z, wgt, ci[q][2]);
-                                } else {
-                                    float a, e;
-                                    absorb_pair(B.w * wgt, a, e);
-                                    ci[q][0] = fmaf(B.x - ci[q][0], a, ci[q][0]);
-                                    ci[q][1] = fmaf(B.y - ci[q][1], a, ci[q][1]);
-                                    ci[q][2] = fmaf(B.z - ci[q][2], a, ci[q][2]);
-                                    ti[q] *= e;
-                                }
-                            }
+                for (int o = 1; o < 32; o <<= 1) {
+                    const unsigned int t = __shfl_up_sync(0xffffffffu, inc, o);
+                    if (lane >= o) inc += t;
+                }
+                const unsigned int nf = __shfl_sync(0xffffffffu, inc, 31);
+                const bool single = __all_sync(0xffffffffu, nfrag <= 1u);        // every record is one fragment (or none): lane = record
+                if (!single) {
+                    S.recA[warp][lane] = ra; S.recB[warp][lane] = rb; S.box[warp][lane] = bx; S.incl[warp][lane] = inc;
+                    __syncwarp();
+                }
+                for (unsigned int f0 = 0u; f0 < (single ? 1u : nf); f0 += 32u) {
+                    float4 A = ra, B = rb;
+                    unsigned int box = bx, k = 0u;
+                    bool act = nfrag == 1u;
+                    if (!single) {
+                        const unsigned int f = f0 + lane;
+                        act = f < nf;
+                        // source record: the first lane whose inclusive prefix exceeds f (binary search over the staged prefixes)
+                        int sl = 0;
+#pragma unroll
+                        for (int st = 16; st >= 1; st >>= 1) sl += (S.incl[warp][sl + st - 1] <= f) ? st : 0;
+                        sl = min(sl, 31);
+                        A = S.recA[warp][sl]; B = S.recB[warp][sl]; box = S.box[warp][sl];
+                        k = f - (sl > 0 ? S.incl[warp][sl - 1] : 0u);
+                    }
+                    const unsigned int bw = ((box >> 16) & 255u) + 1u;
+                    const unsigned int ky = (k * ((65536u + bw - 1u) / bw)) >> 16, kx = k - ky * bw;      // k / bw, k % bw for k < 256, bw <= 32
+                    const int lx = (int)((box & 255u) + kx), ly = (int)(((box >> 8) & 255u) + ky);
+                    const float dxf = __fsub_rn(__fadd_rn((float)(tx0 + lx), 0.5f), A.x);
+                    const float dyf = __fsub_rn(__fadd_rn((float)(ty0 + ly), 0.5f), A.y);
+                    const float d2 = __fmaf_rn(dxf, dxf, __fmul_rn(dyf, dyf));
+                    act = act && d2 <= fabsf(A.w);
+                    const float wgt = ex2_approx(d2 * A.z);
+                    const bool emit_only = A.w < 0.0f;
+                    float a, e;
+                    absorb_pair(B.w * wgt, a, e);
+                    // I -> e I + g with g = q a (absorbing) or q w (pure emitter, e = 1)
+                    const float ga = emit_only ? wgt : a;
+                    e = emit_only ? 1.0f : e;
+                    const float gr = B.x * ga, gg = B.y * ga, gb = B.z * ga;
+                    const int pix = ly * T + lx;
+                    const unsigned int peers = __match_any_sync(0xffffffffu, act ? (unsigned int)pix : 0x10000u + (unsigned int)lane);
+                    const unsigned int rank = (unsigned int)__popc(peers & lt);
+                    const unsigned int rounds = __reduce_max_sync(0xffffffffu, act ? rank : 0u);
+                    for (unsigned int r = 0u; r <= rounds; ++r) {
+                        if (act && rank == r) {
+                            float4 m = map[pix];
+                            m.x *= e; m.y = fmaf(m.y, e, gr); m.z = fmaf(m.z, e, gg); m.w = fmaf(m.w, e, gb);
+                            map[pix] = m;
                         }
+                        __syncwarp();
                     }
                 }
-                if (++fold == Cfg::kFoldBatches) {
-                    fold = 0;
+                __syncwarp();
+            }
+            __syncthreads();                  // the four maps of the segment are complete
+            {   // compose them in order: slot = chunk + tile (segments of a tile are consecutive chunks)
+                float4 *out = seg + ((size_t)chunk + (size_t)tile) * kPix;
+                for (int p = threadIdx.x; p < kPix; p += kORThreads) {
+                    double t = 1.0, cr = 0.0, cg = 0.0, cb = 0.0;
 #pragma unroll
-                    for (int q = 0; q < 2; ++q) {
-#pragma unroll
-                        for (int c = 0; c < 3; ++c) { Co[q][c] = fma(Co[q][c], (double)ti[q], (double)ci[q][c]); ci[q][c] = 0.0f; }
-                        To[q] *= (double)ti[q];
-                        ti[q] = 1.0f;
+                    for (int w = 0; w < kORWarps; ++w) {
+                        const float4 m = S.map[w][p];
+                        const double mt = (double)m.x;
+                        t *= mt; cr = fma(cr, mt, (double)m.y); cg = fma(cg, mt, (double)m.z); cb = fma(cb, mt, (double)m.w);
                     }
+                    out[p] = make_float4((float)t, (float)cr, (float)cg, (float)cb);
                 }
             }
-#pragma unroll
-            for (int q = 0; q < 2; ++q) {
-#pragma unroll
-                for (int c = 0; c < 3; ++c) Co[q][c] = fma(Co[q][c], (double)ti[q], (double)ci[q][c]);
-                To[q] *= (double)ti[q];
-            }
-            // the segment's map: slot = chunk + tile (segments of a tile are consecutive chunks)
-            float4 *out = seg + ((size_t)chunk + (size_t)tile) * kPix + ly * T + lx;
-            out[0] = make_float4((float)To[0], (float)Co[0][0], (float)Co[0][1], (float)Co[0][2]);
-            out[1] = make_float4((float)To[1], (float)Co[1][0], (float)Co[1][1], (float)Co[1][2]);
             if (te >= r1) break;
             do { ++tile; tb = te; te = tile_start[tile + 1]; } while (te == tb);
-            __syncthreads();
+            __syncthreads();                  // the maps are rewritten for the next tile
         }
     }
 }
