@@ -508,8 +508,7 @@ constexpr int kOChunkMax = 4096;               // records per chunk: a warp comp
 template <int T> struct ORenderSmem {
     float4 map[kORWarps][T * T];
     float4 recA[kORWarps][32], recB[kORWarps][32];
-    unsigned int box[kORWarps][32];            // x0 | y0 << 8 | (width - 1) << 16 | (height - 1) << 24, tile-relative
-    unsigned int incl[kORWarps][32];           // inclusive prefix of the fragment counts of the batch
+    uint4 box[kORWarps][32];                   // {x0 | y0 << 8 | (width - 1) << 16 | (height - 1) << 24 (tile-relative), first fragment, 65536 / width rounded up, -}
     unsigned int chunk;
     int tile;
 };
@@ -604,27 +603,38 @@ k_orender(const float4 *__restrict__ rec, const unsigned int *__restrict__ vals0
                 }
                 const unsigned int nf = __shfl_sync(0xffffffffu, inc, 31);
                 const bool single = __all_sync(0xffffffffu, nfrag <= 1u);        // every record is one fragment (or none): lane = record
+                // otherwise the records that have fragments are staged in shared memory, packed: source c starts at fragment first_c
+                const unsigned int has = __ballot_sync(0xffffffffu, nfrag > 0u);
+                unsigned int my_first = 0xffffffffu;               // lane c: first fragment of packed source c
                 if (!single) {
-                    S.recA[warp][lane] = ra; S.recB[warp][lane] = rb; S.box[warp][lane] = bx; S.incl[warp][lane] = inc;
+                    if (nfrag > 0u) {
+                        const int c = __popc(has & lt);
+                        const unsigned int bw = ((bx >> 16) & 255u) + 1u;
+                        S.recA[warp][c] = ra; S.recB[warp][c] = rb;
+                        S.box[warp][c] = make_uint4(bx, inc - nfrag, (65536u + bw - 1u) / bw, 0u);
+                    }
                     __syncwarp();
+                    if (lane < __popc(has)) my_first = S.box[warp][lane].y;
                 }
                 for (unsigned int f0 = 0u; f0 < (single ? 1u : nf); f0 += 32u) {
                     float4 A = ra, B = rb;
-                    unsigned int box = bx, k = 0u;
+                    unsigned int box = bx, k = 0u, inv = 65536u;
                     bool act = nfrag == 1u;
                     if (!single) {
                         const unsigned int f = f0 + lane;
                         act = f < nf;
-                        // source record: the first lane whose inclusive prefix exceeds f (binary search over the staged prefixes)
-                        int sl = 0;
-#pragma unroll
-                        for (int st = 16; st >= 1; st >>= 1) sl += (S.incl[warp][sl + st - 1] <= f) ? st : 0;
-                        sl = min(sl, 31);
-                        A = S.recA[warp][sl]; B = S.recB[warp][sl]; box = S.box[warp][sl];
-                        k = f - (sl > 0 ? S.incl[warp][sl - 1] : 0u);
+                        // source of fragment f: the last packed source that starts at or before f.  `cover` sources start at or before f0;
+                        // the starts inside this window are one bit each, counted up to this lane
+                        const int cover = __popc(__ballot_sync(0xffffffffu, my_first <= f0));
+                        const unsigned int rel = my_first - f0;
+                        const unsigned int starts = __reduce_or_sync(0xffffffffu, (rel >= 1u && rel < 32u) ? (1u << rel) : 0u);
+                        const int sl = cover - 1 + __popc(starts & ((2u << lane) - 1u));
+                        const uint4 bq = S.box[warp][sl];
+                        A = S.recA[warp][sl]; B = S.recB[warp][sl];
+                        box = bq.x; k = f - bq.y; inv = bq.z;
                     }
                     const unsigned int bw = ((box >> 16) & 255u) + 1u;
-                    const unsigned int ky = (k * ((65536u + bw - 1u) / bw)) >> 16, kx = k - ky * bw;      // k / bw, k % bw for k < 256, bw <= 32
+                    const unsigned int ky = (k * inv) >> 16, kx = k - ky * bw;      // k / bw, k % bw (exact for k < 1024, bw <= 32)
                     const int lx = (int)((box & 255u) + kx), ly = (int)(((box >> 8) & 255u) + ky);
                     const float dxf = __fsub_rn(__fadd_rn((float)(tx0 + lx), 0.5f), A.x);
                     const float dyf = __fsub_rn(__fadd_rn((float)(ty0 + ly), 0.5f), A.y);
@@ -639,7 +649,15 @@ k_orender(const float4 *__restrict__ rec, const unsigned int *__restrict__ vals0
                     e = emit_only ? 1.0f : e;
                     const float gr = B.x * ga, gg = B.y * ga, gb = B.z * ga;
                     const int pix = ly * T + lx;
-                    const unsigned int peers = __match_any_sync(0xffffffffu, act ? (unsigned int)pix : 0x10000u + (unsigned int)lane);
+                    // lanes whose fragments fall on the same pixel, from one vote per bit of the pixel index (match.any takes about
+                    // 64 cycles per warp on sm_100a and was 37 % of the kernel's stall samples; votes run at full rate)
+                    unsigned int peers = __ballot_sync(0xffffffffu, act);
+#pragma unroll
+                    for (int bit = 0; (1 << bit) < kPix; ++bit) {
+                        const bool one = (pix >> bit) & 1;
+                        const unsigned int v = __ballot_sync(0xffffffffu, one);
+                        peers &= one ? v : ~v;
+                    }
                     const unsigned int rank = (unsigned int)__popc(peers & lt);
                     const unsigned int rounds = __reduce_max_sync(0xffffffffu, act ? rank : 0u);
                     for (unsigned int r = 0u; r <= rounds; ++r) {
