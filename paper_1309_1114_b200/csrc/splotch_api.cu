@@ -530,7 +530,7 @@ int render_ordered(splotch_ctx *c, const splotch_particles *p, unsigned long lon
     if (c->profiling) cudaEventRecord(c->ev[4], st);
     {
         const unsigned long long work = L.capacity > (unsigned long long)fp.n_tiles + 1 ? L.capacity : (unsigned long long)fp.n_tiles + 1;
-        k_obounds<<<(unsigned int)((work + 255) / 256), 256, 0, st>>>(keys[0], keys[1], stats, fp.n_tiles, (unsigned int *)(ws + L.tile_start));
+        k_obounds<<<(unsigned int)(((work + 3) / 4 + 255) / 256), 256, 0, st>>>(keys[0], keys[1], stats, fp.n_tiles, (unsigned int *)(ws + L.tile_start));
     }
     if (c->profiling) cudaEventRecord(c->ev[5], st);
     if (fp.T == 8) launch_ordered_tail<8>(c, L, ws, fp, vals[0], vals[1], image, st);

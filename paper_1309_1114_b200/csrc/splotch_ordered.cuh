@@ -450,19 +450,33 @@ k_obounds(const unsigned long long *__restrict__ keys0, const unsigned long long
           const DeviceStats *__restrict__ stats, int n_tiles, unsigned int *__restrict__ tile_start)
 {
     const unsigned long long P = stats->sort_n;
-    const unsigned long long p = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const unsigned long long p0 = 4ull * ((unsigned long long)blockIdx.x * blockDim.x + threadIdx.x);     // four consecutive pairs per thread
     if (P == 0ull) {
-        if (p <= (unsigned long long)n_tiles) tile_start[p] = 0u;
+        for (unsigned long long p = p0; p < p0 + 4ull; ++p) if (p <= (unsigned long long)n_tiles) tile_start[p] = 0u;
         return;
     }
-    if (p >= P) return;
+    if (p0 >= P) return;
     // the sorted pairs are in buffer (number of passes that ran) & 1
     const unsigned long long *keys = (((stats->key_bits + 7u) >> 3) & 1u) ? keys1 : keys0;
     const unsigned int zbits = stats->zbits;
-    const int t = (int)(keys[p] >> zbits);
-    const int tp = p > 0 ? (int)(keys[p - 1] >> zbits) : -1;
-    for (int u = tp + 1; u <= t; ++u) tile_start[u] = (unsigned int)p;
-    if (p == P - 1) for (int u = t + 1; u <= n_tiles; ++u) tile_start[u] = (unsigned int)P;
+    unsigned long long k[4];
+    if (p0 + 4ull <= P) {
+        const ulonglong2 a = *reinterpret_cast<const ulonglong2 *>(keys + p0), b = *reinterpret_cast<const ulonglong2 *>(keys + p0 + 2);
+        k[0] = a.x; k[1] = a.y; k[2] = b.x; k[3] = b.y;
+    } else {
+        for (int j = 0; j < 4; ++j) k[j] = p0 + j < P ? keys[p0 + j] : keys[P - 1];
+    }
+    int tp = p0 > 0 ? (int)(__ldg(keys + p0 - 1) >> zbits) : -1;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const unsigned long long p = p0 + j;
+        if (p < P) {
+            const int t = (int)(k[j] >> zbits);
+            for (int u = tp + 1; u <= t; ++u) tile_start[u] = (unsigned int)p;
+            if (p == P - 1) for (int u = t + 1; u <= n_tiles; ++u) tile_start[u] = (unsigned int)P;
+            tp = t;
+        }
+    }
 }
 
 __global__ void __launch_bounds__(256)
