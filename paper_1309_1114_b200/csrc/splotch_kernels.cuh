@@ -261,6 +261,41 @@ __device__ __forceinline__ BinWalk bin_walk(const Geo &g, int cls, const FramePa
     return w;
 }
 
+// The bins of the lanes whose box covers more than a few bins, walked by the whole warp: the lanes' bin counts are prefix-summed and the
+// warp takes 32 (lane, bin) pairs per step, whichever lanes they come from.  (One warp-uniform loop in which every lane walked its own
+// box ran as long as the largest box of the warp: 20 steps for two or three busy lanes on cfg3, where discs of 64 px cover 5 x 5 tiles
+// and LARGE discs several super-tiles; profiles/r2_step1_*: 15.7 warp instructions per particle in k_count against 5.3 on cfg2.)
+// emit(ok, source lane, bx, by, class of the source) is called by all lanes together.
+template <typename Emit>
+__device__ __forceinline__ void coop_bin_walk(bool big, const BinWalk &w, int cls, int lane, Emit emit)
+{
+    const unsigned int cnt = big ? (unsigned int)w.n : 0u;
+    unsigned int inc = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const unsigned int t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    const unsigned int total = __shfl_sync(0xffffffffu, inc, 31), excl = inc - cnt;
+    const int width = w.bx1 - w.bx0 + 1;
+#pragma unroll 1
+    for (unsigned int f0 = 0u; f0 < total; f0 += 32u) {
+        const unsigned int f = f0 + (unsigned int)lane;
+        int sl = 0;                                  // the last lane whose exclusive prefix is <= f (prefixes ascend; lanes without bins share their successor's)
+#pragma unroll
+        for (int st = 16; st >= 1; st >>= 1) {
+            const unsigned int e = __shfl_sync(0xffffffffu, excl, sl + st);
+            if (e <= f) sl += st;
+        }
+        const unsigned int se = __shfl_sync(0xffffffffu, excl, sl);
+        const int sbx0 = __shfl_sync(0xffffffffu, w.bx0, sl), sby0 = __shfl_sync(0xffffffffu, w.by0, sl);
+        const int sw = __shfl_sync(0xffffffffu, width, sl), scls = __shfl_sync(0xffffffffu, cls, sl);
+        const unsigned int k = f - se;
+        const int ky = __float2int_rz(__fdividef((float)k + 0.5f, (float)sw)), kx = (int)k - ky * sw;     // k / width, k % width (k < 2^20)
+        emit(f < total, sl, sbx0 + kx, sby0 + ky, scls);
+    }
+}
+
 template <bool ALIGNED, bool GHIST, bool BTILE>
 __global__ void __launch_bounds__(kBinThreads, 1)
 k_count(const float *__restrict__ x, const float *__restrict__ y, const float *__restrict__ z,
@@ -293,26 +328,20 @@ k_count(const float *__restrict__ x, const float *__restrict__ y, const float *_
             const int cls = (i + j < len) ? g.cls : CULLED;
             c2 += cls == MEDIUM; c3 += cls == LARGE;
             const BinWalk w = bin_walk<BTILE>(g, cls, fp);
-            // a box covers at most 2 x 2 bins unless it is wider than a bin: four predicated increments, then (rare) one
-            // warp-uniform walk over the bins beyond the first 2 x 2
+            // a box covers at most 2 x 2 bins unless it is wider than a bin: four predicated increments; the others go to the warp's
+            // common walk
             unsigned int *h00 = hist + (w.base + w.mult * (w.by0 * w.pitch + w.bx0) + w.odd);
             const bool any = w.n > 0, w2 = w.bx1 > w.bx0, h2 = w.by1 > w.by0;
-            if (any) hist_inc<GHIST>(h00);
-            if (any && w2) hist_inc<GHIST>(h00 + w.mult);
-            if (any && h2) hist_inc<GHIST>(h00 + w.mult * w.pitch);
-            if (any && w2 && h2) hist_inc<GHIST>(h00 + w.mult * w.pitch + w.mult);
             const bool big = any && (w.bx1 - w.bx0 > 1 || w.by1 - w.by0 > 1);
-            if (__any_sync(0xffffffffu, big)) {
-                const int nmax = __reduce_max_sync(0xffffffffu, big ? w.n : 0);
-                int bx = w.bx0, by = w.by0;
-#pragma unroll 1
-                for (int t = 1; t < nmax; ++t) {
-                    const bool wrap = bx == w.bx1;
-                    bx = wrap ? w.bx0 : bx + 1;
-                    by += wrap;
-                    if (big && t < w.n && (bx - w.bx0 > 1 || by - w.by0 > 1)) hist_inc<GHIST>(hist + (w.base + w.mult * (by * w.pitch + bx)));
-                }
-            }
+            const bool few = any && !big;
+            if (few) hist_inc<GHIST>(h00);
+            if (few && w2) hist_inc<GHIST>(h00 + w.mult);
+            if (few && h2) hist_inc<GHIST>(h00 + w.mult * w.pitch);
+            if (few && w2 && h2) hist_inc<GHIST>(h00 + w.mult * w.pitch + w.mult);
+            if (__any_sync(0xffffffffu, big))
+                coop_bin_walk(big, w, cls, (int)(threadIdx.x & 31u), [&](bool ok, int, int bx, int by, int scls) {
+                    if (ok) hist_inc<GHIST>(hist + (scls == LARGE ? 2 * fp.n_tiles + by * fp.nsx + bx : 2 * (by * fp.ntx + bx)));
+                });
         }
     }
     c2 = warp_sum(c2); c3 = warp_sum(c3);
@@ -795,32 +824,38 @@ k_scatter(const float *__restrict__ x, const float *__restrict__ y, const float 
                     asm volatile("st.global.v4.f32 [%0], {%1,%2,%3,%4};" :: "l"(records + u), "f"(__uint_as_float(pix)), "f"(a.x), "f"(a.y), "f"(a.z) : "memory");
                 }
             }
-            // MEDIUM and LARGE: one 32-byte record per bin of the box, one warp-uniform walk, one call site
+            // MEDIUM and LARGE: one 32-byte record per bin of the box.  A box inside one bin is written by its lane; the others are
+            // walked by the whole warp (coop_bin_walk), the record travelling from its lane by shuffles
             const int nrec = (cls == MEDIUM || cls == LARGE) ? w.n : 0;
             if (__any_sync(0xffffffffu, nrec > 0)) {
                 const float4 ra = make_float4(g.px, g.py, __fdividef(-1.4426950408889634f, sp2), __fmul_rn(g.rp, g.rp));
-                int bx = w.bx0, by = w.by0;
-                auto emit = [&]() {
+                if (nrec == 1) {
                     unsigned int box;
                     if (BTILE && cls == MEDIUM) {      // box relative to the home tile's Btile (body + boundary of r_0)
-                        const int ox = (bx << ts) - fp.btile_r0, oy = (by << ts) - fp.btile_r0;
+                        const int ox = (w.bx0 << ts) - fp.btile_r0, oy = (w.by0 << ts) - fp.btile_r0;
                         box = (unsigned int)(g.x0 - ox) | ((unsigned int)(g.y0 - oy) << 6) | ((unsigned int)(g.x1 - g.x0) << 12) | ((unsigned int)(g.y1 - g.y0) << 18);
                     } else {
-                        box = pack_box(g, bx, by, w.sh, cls == LARGE);
+                        box = pack_box(g, w.bx0, w.by0, w.sh, cls == LARGE);
                     }
-                    st_record(records, cursor_take<GHIST>(cursor + (w.base + w.mult * (by * w.pitch + bx)), 2u), ra,
+                    st_record(records, cursor_take<GHIST>(cursor + (w.base + w.mult * (w.by0 * w.pitch + w.bx0)), 2u), ra,
                               make_float4(a.x, a.y, a.z, __uint_as_float(box)));
-                };
-                if (nrec > 0) emit();                          // most particles have one bin
+                }
                 if (__any_sync(0xffffffffu, nrec > 1)) {
-                    const int nmax = __reduce_max_sync(0xffffffffu, nrec);
-#pragma unroll 1
-                    for (int t = 1; t < nmax; ++t) {
-                        const bool wrap = bx == w.bx1;
-                        bx = wrap ? w.bx0 : bx + 1;
-                        by += wrap;
-                        if (t < nrec) emit();
-                    }
+                    const unsigned int xx = (unsigned int)g.x0 | ((unsigned int)g.x1 << 16), yy = (unsigned int)g.y0 | ((unsigned int)g.y1 << 16);
+                    coop_bin_walk(nrec > 1, w, cls, (int)(threadIdx.x & 31u), [&](bool ok, int sl, int bx, int by, int scls) {
+                        const float4 sa = make_float4(__shfl_sync(0xffffffffu, ra.x, sl), __shfl_sync(0xffffffffu, ra.y, sl),
+                                                      __shfl_sync(0xffffffffu, ra.z, sl), __shfl_sync(0xffffffffu, ra.w, sl));
+                        const float s_r = __shfl_sync(0xffffffffu, a.x, sl), s_g = __shfl_sync(0xffffffffu, a.y, sl), s_b = __shfl_sync(0xffffffffu, a.z, sl);
+                        const unsigned int sxx = __shfl_sync(0xffffffffu, xx, sl), syy = __shfl_sync(0xffffffffu, yy, sl);
+                        if (ok) {
+                            Geo sg;
+                            sg.x0 = (int)(sxx & 0xffffu); sg.x1 = (int)(sxx >> 16); sg.y0 = (int)(syy & 0xffffu); sg.y1 = (int)(syy >> 16);
+                            const bool L = scls == LARGE;
+                            const unsigned int box = pack_box(sg, bx, by, L ? fp.sshift : fp.tshift, L);
+                            const int bin = L ? 2 * fp.n_tiles + by * fp.nsx + bx : 2 * (by * fp.ntx + bx);
+                            st_record(records, cursor_take<GHIST>(cursor + bin, 2u), sa, make_float4(s_r, s_g, s_b, __uint_as_float(box)));
+                        }
+                    });
                 }
             }
         }
