@@ -34,7 +34,7 @@ import torch  # noqa: E402
 
 from paper_1309_1114_b200 import workloads as wl  # noqa: E402
 
-KERNELS_ADDITIVE = 6         # k_count, k_scan, k_scatter, k_splat, k_large, k_compose (+ one memset node)
+KERNELS_ADDITIVE = 7         # k_count, k_scan, k_layout, k_scatter, k_splat, k_large, k_compose (+ memset nodes)
 L2_FLUSH_BYTES = 256 << 20   # written between frames when a config's inputs fit in the 126 MB L2
 DEFAULT_CONFIG = 3           # the largest single-GPU configuration of BASELINE.json
 
