@@ -35,7 +35,8 @@ constexpr int kChunkMin     = 256;
 constexpr int kBinThreads   = 1024;   // k_count / k_scatter block size: one CTA per SM (fewer histogram rows and write streams than 2 x 512)
 constexpr int kSuperShift   = 3;      // super-tile = 8 x 8 tiles, at most 128 px (LARGE particles are binned to super-tiles)
 constexpr int kSuperMaxShift = 7;      // 128 px: k_large tests every record of a super-tile against each of its 32-px blocks (16 instead of 64 at
-                                       // 256 px: cfg3 k_large 282 -> 245 ms for 1 ms more in k_count and 1.7 ms more in k_scatter; 64 px: no further gain)
+                                       // 256 px: cfg3 k_large 282 -> 245 ms for 1 ms more in k_count and 1.7 ms more in k_scatter; 64 px: frame 341.5 -> 335.6 ms
+                                       // but 410 M LARGE records, several GB more in the workspace: not taken)
 constexpr int kLutSmemMax   = 1024;   // colour-table entries (all species together) staged in shared memory by k_scatter
 constexpr int kFixedBits    = 30;     // the largest record amplitude maps to [2^29, 2^30) fixed-point units
 
