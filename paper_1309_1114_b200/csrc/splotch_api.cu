@@ -100,7 +100,8 @@ size_t hist_bytes(int W, int H, int T)
     const int ntx = (W + T - 1) / T, nty = (H + T - 1) / T;
     const int S = 1 << super_shift(T);
     const int nsx = (W + S - 1) / S, nsy = (H + S - 1) / S;
-    return sizeof(unsigned int) * (2 * (size_t)ntx * nty + (size_t)nsx * nsy);      // two bins per tile (MEDIUM, SMALL) + one per super-tile
+    // two bins per tile (MEDIUM, SMALL) + one per super-tile + with 32-px tiles one more per tile (wide MEDIUM discs, k_large's)
+    return sizeof(unsigned int) * (2 * (size_t)ntx * nty + (size_t)nsx * nsy + (T == 32 ? (size_t)ntx * nty : 0));
 }
 
 // dynamic shared memory of k_count / k_scatter: the block's histogram / cursors plus room for the colour tables
@@ -277,7 +278,9 @@ int check_params(splotch_ctx *c, const splotch_particles *p, unsigned long long 
     const int S = 1 << fp->sshift;
     fp->nsx = (c->width + S - 1) / S; fp->nsy = (c->height + S - 1) / S;
     fp->n_super = fp->nsx * fp->nsy;
-    fp->nbins = 2 * fp->n_tiles + fp->n_super;
+    fp->n_big = (q->tile == 32 && q->renderer == 0) ? fp->n_tiles : 0;
+    fp->r_route = kRouteRadius;
+    fp->nbins = 2 * fp->n_tiles + fp->n_super + (q->tile == 32 ? fp->n_tiles : 0);       // the bins exist with 32-px tiles (workspace layout), used when n_big > 0
     if (q->renderer != 0 && q->renderer != 1) return fail(c, SPLOTCH_EINVAL, "renderer must be 0 (default) or 1 (the paper's Btile scheme)");
     if (q->renderer == 1) {
         // the paper's constraints: additive mode (:85), r_0 <= min(t_x, t_y) (:224); the Btile must fit the 6-bit box fields
@@ -444,7 +447,7 @@ int render_device(splotch_ctx *c, const splotch_particles *p, unsigned long long
     const int bps = 1 << (fp.sshift - 5);               // 32-px blocks per super-tile side (k_large's work items)
     k_scan<<<(fp.nbins + 31) / 32, kScanThreads, 0, st>>>(counts, L.nrows, fp.nbins, fp.n_tiles, bin_count, vstart, cls_counts, 2ull * L.capacity,
                                                           c->n_sm, (unsigned int *)(ws + L.large_off), (unsigned int)kLargeChunk,
-                                                          (unsigned int)(bps * bps), stats);
+                                                          (unsigned int)(bps * bps), fp.n_super, stats);
     k_layout<<<kMaxSlabs, kLayoutThreads, 0, st>>>(counts, bin_count, L.nrows, fp.nbins, fp.n_tiles, run, stats);
     if (prof) cudaEventRecord(c->ev[2], st);
     float4 *records = (float4 *)(ws + L.records);
@@ -981,7 +984,7 @@ int splotch_debug_tile_counts(splotch_ctx *c, uint32_t *out, void *cuda_stream)
     CU_TRY(c, cudaSetDevice(c->device));
     if (c->last_additive) {
         k_tile_counts<<<(c->fp.n_tiles + 255) / 256, 256, 0, (cudaStream_t)cuda_stream>>>((const unsigned int *)(c->ws + c->lay.bin_count),
-                                                                                            c->fp.n_tiles, out);
+                                                                                            c->fp.n_tiles, c->fp.n_super, c->fp.n_big, out);
         CU_TRY(c, cudaGetLastError());
     } else {
         k_odiff<<<(c->fp.n_tiles + 255) / 256, 256, 0, (cudaStream_t)cuda_stream>>>((const unsigned int *)(c->ws + c->lay.tile_start),

@@ -37,6 +37,7 @@ constexpr int kSuperShift   = 3;      // super-tile = 8 x 8 tiles, at most 128 p
 constexpr int kSuperMaxShift = 7;      // 128 px: k_large tests every record of a super-tile against each of its 32-px blocks (16 instead of 64 at
                                        // 256 px: cfg3 k_large 282 -> 245 ms for 1 ms more in k_count and 1.7 ms more in k_scatter; 64 px: frame 341.5 -> 335.6 ms
                                        // but 410 M LARGE records, several GB more in the workspace: not taken)
+constexpr float kRouteRadius = 32.0f;  // 32-px tiles: MEDIUM discs with r(p) above this go to k_large's block renderer instead of k_splat's strips
 constexpr int kLutSmemMax   = 1024;   // colour-table entries (all species together) staged in shared memory by k_scatter
 constexpr int kFixedBits    = 30;     // the largest record amplitude maps to [2^29, 2^30) fixed-point units
 
@@ -59,6 +60,8 @@ struct FrameParams {
     int   W, H, T, tshift;
     int   ntx, nty, n_tiles;
     int   sshift, nsx, nsy, n_super, nbins;
+    int   n_big;                 // n_tiles when MEDIUM discs wider than r_route are filed in a third bin per tile (rendered by k_large), else 0
+    float r_route;
     int   additive, apply_transfer;
     int   n_species, lut_total;  // lut_total: packed entries of all colour-mapped species, 0 = read tables from global
     int   any_vector, any_auto;
@@ -182,7 +185,11 @@ __device__ __forceinline__ int2 home_tile(const Geo &g, const FrameParams &fp)
 // Bin b < 2 n_tiles: tile b >> 1; even bins hold the tile's MEDIUM records (32 bytes = 2 units of 16 bytes), odd bins
 // its SMALL records (16 bytes = 1 unit: "only their location ... has to be calculated").  Bins
 // 2 n_tiles + s hold the LARGE records of super-tile s (2 units).  A tile's two bins are neighbours, so the tile
-// renderer meets them back to back.
+// renderer meets them back to back.  With 32-px tiles there is a third bin per tile, 2 n_tiles + n_super + t: the MEDIUM records of
+// tile t whose disc is wider than kRouteRadius.  They are tile assignments like the others (the per-tile pair counts include them) but
+// k_large renders them, the tile as its 32 x 32 block: k_splat's 64-pixel strips spent 20 warp instructions per record and strip on
+// them (cfg3: 80 ms), k_large's bands 61 per 256 pixels or the tensor cores.  cfg3 frame by kRouteRadius: none 341.5 ms, 12 px 333.0,
+// 24 px 330.5, 40 px 329.9 (k_splat 80 -> 24 ms, k_large 245 -> 289 ms).
 __device__ __forceinline__ unsigned int bin_unit_size(int b, int n_tiles) { return (b < 2 * n_tiles && (b & 1)) ? 1u : 2u; }
 
 // ---- streaming loads / stores ----------------------------------------------------------------------------------
@@ -244,6 +251,7 @@ __device__ __forceinline__ unsigned int warp_sum(unsigned int v)
 // writers ran at 5 active lanes per instruction and stalled on instruction fetch on cfg3, profiles/r2_step3_*).
 struct BinWalk {
     int bx0, bx1, by0, by1, sh, pitch, base, mult, odd, n;      // bin = base + mult * (by * pitch + bx) + odd
+    int route;                                                  // 0 tile bins, 1 super-tile bins (LARGE), 2 the tile's bin for wide MEDIUM discs
 };
 
 template <bool BTILE>
@@ -251,10 +259,12 @@ __device__ __forceinline__ BinWalk bin_walk(const Geo &g, int cls, const FramePa
 {
     BinWalk w;
     const bool large = cls == LARGE;
+    const bool wide = !BTILE && cls == MEDIUM && fp.n_big > 0 && g.rp > fp.r_route;
+    w.route = large ? 1 : (wide ? 2 : 0);
     w.sh = large ? fp.sshift : fp.tshift;
     w.pitch = large ? fp.nsx : fp.ntx;
-    w.base = large ? 2 * fp.n_tiles : 0;
-    w.mult = large ? 1 : 2;
+    w.base = large ? 2 * fp.n_tiles : (wide ? 2 * fp.n_tiles + fp.n_super : 0);
+    w.mult = (large || wide) ? 1 : 2;
     w.odd = cls == SMALL ? 1 : 0;
     w.bx0 = g.x0 >> w.sh; w.bx1 = g.x1 >> w.sh; w.by0 = g.y0 >> w.sh; w.by1 = g.y1 >> w.sh;
     if (BTILE && cls == MEDIUM) { const int2 ht = home_tile(g, fp); w.bx0 = w.bx1 = ht.x; w.by0 = w.by1 = ht.y; }   // i(p): the tile of the centre
@@ -266,9 +276,14 @@ __device__ __forceinline__ BinWalk bin_walk(const Geo &g, int cls, const FramePa
 // warp takes 32 (lane, bin) pairs per step, whichever lanes they come from.  (One warp-uniform loop in which every lane walked its own
 // box ran as long as the largest box of the warp: 20 steps for two or three busy lanes on cfg3, where discs of 64 px cover 5 x 5 tiles
 // and LARGE discs several super-tiles; profiles/r2_step1_*: 15.7 warp instructions per particle in k_count against 5.3 on cfg2.)
-// emit(ok, source lane, bx, by, class of the source) is called by all lanes together.
+// emit(ok, source lane, bx, by, route of the source) is called by all lanes together.
+__device__ __forceinline__ int routed_bin(int route, int bx, int by, const FrameParams &fp)
+{
+    return route == 1 ? 2 * fp.n_tiles + by * fp.nsx + bx : (route == 2 ? 2 * fp.n_tiles + fp.n_super + by * fp.ntx + bx : 2 * (by * fp.ntx + bx));
+}
+
 template <typename Emit>
-__device__ __forceinline__ void coop_bin_walk(bool big, const BinWalk &w, int cls, int lane, Emit emit)
+__device__ __forceinline__ void coop_bin_walk(bool big, const BinWalk &w, int lane, Emit emit)
 {
     const unsigned int cnt = big ? (unsigned int)w.n : 0u;
     unsigned int inc = cnt;
@@ -290,10 +305,10 @@ __device__ __forceinline__ void coop_bin_walk(bool big, const BinWalk &w, int cl
         }
         const unsigned int se = __shfl_sync(0xffffffffu, excl, sl);
         const int sbx0 = __shfl_sync(0xffffffffu, w.bx0, sl), sby0 = __shfl_sync(0xffffffffu, w.by0, sl);
-        const int sw = __shfl_sync(0xffffffffu, width, sl), scls = __shfl_sync(0xffffffffu, cls, sl);
+        const int sw = __shfl_sync(0xffffffffu, width, sl), sroute = __shfl_sync(0xffffffffu, w.route, sl);
         const unsigned int k = f - se;
         const int ky = __float2int_rz(__fdividef((float)k + 0.5f, (float)sw)), kx = (int)k - ky * sw;     // k / width, k % width (k < 2^20)
-        emit(f < total, sl, sbx0 + kx, sby0 + ky, scls);
+        emit(f < total, sl, sbx0 + kx, sby0 + ky, sroute);
     }
 }
 
@@ -340,8 +355,8 @@ k_count(const float *__restrict__ x, const float *__restrict__ y, const float *_
             if (few && h2) hist_inc<GHIST>(h00 + w.mult * w.pitch);
             if (few && w2 && h2) hist_inc<GHIST>(h00 + w.mult * w.pitch + w.mult);
             if (__any_sync(0xffffffffu, big))
-                coop_bin_walk(big, w, cls, (int)(threadIdx.x & 31u), [&](bool ok, int, int bx, int by, int scls) {
-                    if (ok) hist_inc<GHIST>(hist + (scls == LARGE ? 2 * fp.n_tiles + by * fp.nsx + bx : 2 * (by * fp.ntx + bx)));
+                coop_bin_walk(big, w, (int)(threadIdx.x & 31u), [&](bool ok, int, int bx, int by, int route) {
+                    if (ok) hist_inc<GHIST>(hist + routed_bin(route, bx, by, fp));
                 });
         }
     }
@@ -400,7 +415,7 @@ __device__ __forceinline__ unsigned long long block_excl_scan_256(unsigned long 
 __global__ void __launch_bounds__(kScanThreads)
 k_scan(unsigned int *__restrict__ counts, int nrows, int nbins, int n_tiles, unsigned int *__restrict__ bin_count,
        unsigned int *__restrict__ vstart, const unsigned int *__restrict__ cls_counts, unsigned long long capacity_units, int n_sm,
-       unsigned int *__restrict__ large_off, unsigned int large_chunk, unsigned int large_blocks, DeviceStats *__restrict__ stats)
+       unsigned int *__restrict__ large_off, unsigned int large_chunk, unsigned int large_blocks, int n_super, DeviceStats *__restrict__ stats)
 {
     __shared__ unsigned int s_part[8][32];
     __shared__ unsigned long long s_warp[kScanThreads / 32];
@@ -463,7 +478,8 @@ k_scan(unsigned int *__restrict__ counts, int nrows, int nbins, int n_tiles, uns
             const unsigned int u = (c8[k] * bin_unit_size(b, n_tiles) + 1u) & ~1u;
             u_all += u;
             if (b < 2 * n_tiles) { u_tiles += u; n_tilerec += c8[k]; if (b & 1) n_small += c8[k]; }
-            else n_largerec += c8[k];
+            else if (b < 2 * n_tiles + n_super) n_largerec += c8[k];
+            else n_tilerec += c8[k];                 // wide MEDIUM discs: tile pairs, rendered by k_large
         }
     }
     if (threadIdx.x < 4) s_cls[threadIdx.x] = 0u;
@@ -506,17 +522,18 @@ k_scan(unsigned int *__restrict__ counts, int nrows, int nbins, int n_tiles, uns
     }
     if (threadIdx.x == kScanThreads - 1) vstart[nbins] = (unsigned int)s_tot_all;
     {   // work items of k_large: (chunk of a super-tile's records) x (block of the super-tile), exclusive prefix over the super-tiles
-        const int n_super = nbins - 2 * n_tiles;
-        const int sper = (n_super + kScanThreads - 1) / kScanThreads;
-        const int s0 = min(n_super, (int)threadIdx.x * sper), s1 = min(n_super, s0 + sper);
+        // regions: the super-tiles (large_blocks blocks each), then the tiles' bins of wide MEDIUM discs (the tile is the one block)
+        const int n_reg = nbins - 2 * n_tiles;
+        const int sper = (n_reg + kScanThreads - 1) / kScanThreads;
+        const int s0 = min(n_reg, (int)threadIdx.x * sper), s1 = min(n_reg, s0 + sper);
         unsigned long long items = 0;
-        for (int sb = s0; sb < s1; ++sb) items += (unsigned long long)((__ldcg(bin_count + 2 * n_tiles + sb) + large_chunk - 1) / large_chunk) * large_blocks;
+        for (int sb = s0; sb < s1; ++sb) items += (unsigned long long)((__ldcg(bin_count + 2 * n_tiles + sb) + large_chunk - 1) / large_chunk) * (sb < n_super ? large_blocks : 1u);
         unsigned long long irun = block_excl_scan_256(items, s_warp, &s_tot_items);
         for (int sb = s0; sb < s1; ++sb) {
             large_off[sb] = overflow ? 0u : (unsigned int)irun;
-            irun += (unsigned long long)((__ldcg(bin_count + 2 * n_tiles + sb) + large_chunk - 1) / large_chunk) * large_blocks;
+            irun += (unsigned long long)((__ldcg(bin_count + 2 * n_tiles + sb) + large_chunk - 1) / large_chunk) * (sb < n_super ? large_blocks : 1u);
         }
-        if (threadIdx.x == kScanThreads - 1) large_off[n_super] = overflow ? 0u : (unsigned int)irun;
+        if (threadIdx.x == kScanThreads - 1) large_off[n_reg] = overflow ? 0u : (unsigned int)irun;
     }
     if (threadIdx.x == 0) {
         // slabs of about 96 MB, at most 32 and at most one per row
@@ -836,14 +853,14 @@ k_scatter(const float *__restrict__ x, const float *__restrict__ y, const float 
                         const int ox = (w.bx0 << ts) - fp.btile_r0, oy = (w.by0 << ts) - fp.btile_r0;
                         box = (unsigned int)(g.x0 - ox) | ((unsigned int)(g.y0 - oy) << 6) | ((unsigned int)(g.x1 - g.x0) << 12) | ((unsigned int)(g.y1 - g.y0) << 18);
                     } else {
-                        box = pack_box(g, w.bx0, w.by0, w.sh, cls == LARGE);
+                        box = pack_box(g, w.bx0, w.by0, w.sh, w.route != 0);
                     }
                     st_record(records, cursor_take<GHIST>(cursor + (w.base + w.mult * (w.by0 * w.pitch + w.bx0)), 2u), ra,
                               make_float4(a.x, a.y, a.z, __uint_as_float(box)));
                 }
                 if (__any_sync(0xffffffffu, nrec > 1)) {
                     const unsigned int xx = (unsigned int)g.x0 | ((unsigned int)g.x1 << 16), yy = (unsigned int)g.y0 | ((unsigned int)g.y1 << 16);
-                    coop_bin_walk(nrec > 1, w, cls, (int)(threadIdx.x & 31u), [&](bool ok, int sl, int bx, int by, int scls) {
+                    coop_bin_walk(nrec > 1, w, (int)(threadIdx.x & 31u), [&](bool ok, int sl, int bx, int by, int route) {
                         const float4 sa = make_float4(__shfl_sync(0xffffffffu, ra.x, sl), __shfl_sync(0xffffffffu, ra.y, sl),
                                                       __shfl_sync(0xffffffffu, ra.z, sl), __shfl_sync(0xffffffffu, ra.w, sl));
                         const float s_r = __shfl_sync(0xffffffffu, a.x, sl), s_g = __shfl_sync(0xffffffffu, a.y, sl), s_b = __shfl_sync(0xffffffffu, a.z, sl);
@@ -851,10 +868,8 @@ k_scatter(const float *__restrict__ x, const float *__restrict__ y, const float 
                         if (ok) {
                             Geo sg;
                             sg.x0 = (int)(sxx & 0xffffu); sg.x1 = (int)(sxx >> 16); sg.y0 = (int)(syy & 0xffffu); sg.y1 = (int)(syy >> 16);
-                            const bool L = scls == LARGE;
-                            const unsigned int box = pack_box(sg, bx, by, L ? fp.sshift : fp.tshift, L);
-                            const int bin = L ? 2 * fp.n_tiles + by * fp.nsx + bx : 2 * (by * fp.ntx + bx);
-                            st_record(records, cursor_take<GHIST>(cursor + bin, 2u), sa, make_float4(s_r, s_g, s_b, __uint_as_float(box)));
+                            const unsigned int box = pack_box(sg, bx, by, route == 1 ? fp.sshift : fp.tshift, route != 0);
+                            st_record(records, cursor_take<GHIST>(cursor + routed_bin(route, bx, by, fp), 2u), sa, make_float4(s_r, s_g, s_b, __uint_as_float(box)));
                         }
                     });
                 }
@@ -983,10 +998,10 @@ k_apply_transfer(float *__restrict__ image, size_t n)
 
 // ---- test hook: per-tile pair counts (SMALL + MEDIUM bins of every tile) ---------------------------------------------
 __global__ void __launch_bounds__(256)
-k_tile_counts(const unsigned int *__restrict__ bin_count, int n_tiles, unsigned int *__restrict__ out)
+k_tile_counts(const unsigned int *__restrict__ bin_count, int n_tiles, int n_super, int n_big, unsigned int *__restrict__ out)
 {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t < n_tiles) out[t] = bin_count[2 * t] + bin_count[2 * t + 1];
+    if (t < n_tiles) out[t] = bin_count[2 * t] + bin_count[2 * t + 1] + (n_big ? bin_count[2 * n_tiles + n_super + t] : 0u);
 }
 
 // ---- test hook: per-particle classification results -----------------------------------------------------------

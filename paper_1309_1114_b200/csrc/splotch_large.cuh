@@ -101,10 +101,12 @@ k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
     extern __shared__ __align__(1024) unsigned char large_smem_raw[];
     LargeSmem &S = *reinterpret_cast<LargeSmem *>(large_smem_raw);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (stats->overflow || stats->large_pairs == 0ull) return;          // no LARGE particle in this frame
-    const int n_super = fp.n_super;
-    const unsigned int total = large_off[n_super];
-    if (total == 0u) return;
+    if (stats->overflow) return;
+    // regions: the super-tiles (LARGE records, blocks of 32 x 32 px), then, with 32-px tiles, the tiles' bins of wide MEDIUM discs (the
+    // tile is the one block); record boxes are relative to the region's origin in both
+    const int n_super = fp.n_super, n_reg = fp.n_super + fp.n_big;
+    const unsigned int total = large_off[n_reg];
+    if (total == 0u) return;                                             // nothing for this kernel in this frame
     if (threadIdx.x == 0) {
         for (int s = 0; s < kLargeStages; ++s) mbar_init(smem_u32(S.mbar + s), 1u);
         mbar_init(smem_u32(S.gbar + 0), 1u); mbar_init(smem_u32(S.gbar + 1), 1u);
@@ -169,7 +171,7 @@ k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
             if (lane == 0) it = atomicAdd(&stats->large_counter, 1u);
             it = __shfl_sync(0xffffffffu, it, 0);
             if (it < total) {
-                int lo = 0, n = n_super;
+                int lo = 0, n = n_reg;
                 while (n > 1) {
                     const int step = (n + 31) / 32;
                     const int t = lo + lane * step;
@@ -187,11 +189,13 @@ k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
         if (item >= total) break;
         const int sup = S.sup;
         const unsigned int local = item - large_off[sup];
-        const unsigned int chunk = local / (unsigned int)nblk;
-        const int blk = (int)(local % (unsigned int)nblk);
-        // block origin inside the super-tile and on the screen (record boxes are relative to the super-tile)
+        const bool in_tile = sup >= n_super;                       // region = a tile (wide MEDIUM discs): one block, the tile itself
+        const unsigned int chunk = in_tile ? local : local / (unsigned int)nblk;
+        const int blk = in_tile ? 0 : (int)(local % (unsigned int)nblk);
+        // block origin inside the region and on the screen
         const int qx0 = (blk % bps) * kLargeBlock, qy0 = (blk / bps) * kLargeBlock;
-        const int X0 = ((sup % fp.nsx) << fp.sshift) + qx0, Y0 = ((sup / fp.nsx) << fp.sshift) + qy0;
+        const int X0 = in_tile ? ((sup - n_super) % fp.ntx) << fp.tshift : ((sup % fp.nsx) << fp.sshift) + qx0;
+        const int Y0 = in_tile ? ((sup - n_super) / fp.ntx) << fp.tshift : ((sup / fp.nsx) << fp.sshift) + qy0;
         if (X0 >= fp.W || Y0 >= fp.H) continue;                  // the super-tile hangs over the image edge
         const int qx1 = qx0 + kLargeBlock - 1;
         const unsigned int le = bin_count[2 * fp.n_tiles + sup];              // records of the super-tile's bin

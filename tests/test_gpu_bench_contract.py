@@ -48,7 +48,7 @@ def test_config_1_additive_line():
     d = run_bench("--config", "1", "--no-per-config")
     check_common(d)
     assert d["config"]["workload"] == "cfg1_halos_10M" and d["config"]["mode"] == "additive"
-    assert d["gpu_launches"] == 6 * d["steps"]
+    assert d["gpu_launches"] == 7 * d["steps"]      # count, scan, layout, scatter, splat, large, compose
     assert set(d["stages"]) == {"count", "scan", "scatter", "splat", "large", "compose"}
     assert "per_config" not in d
 
