@@ -170,9 +170,13 @@ def visible_index(local_rank: int) -> int:
     return local_rank
 
 
+ROUTE_RADIUS = 32.0          # csrc kRouteRadius: with 32-px tiles k_large also renders the MEDIUM discs wider than this
+
+
 def fragments_estimate(r, fields, species, kw, chunk=1 << 26):
     """Algorithmic fragments of a frame: 1 per SMALL particle, pixel centres inside the clip disc otherwise
-    (pi r^2, at most the on-screen pixel box).  Computed once, outside the timed region, in chunks."""
+    (pi r^2, at most the on-screen pixel box); second value: the fragments k_large renders (LARGE discs and, with
+    32-px tiles, MEDIUM discs wider than ROUTE_RADIUS).  Computed once, outside the timed region, in chunks."""
     n = fields["x"].numel()
     total = large = 0.0
     for a in range(0, n, chunk):
@@ -183,7 +187,8 @@ def fragments_estimate(r, fields, species, kw, chunk=1 << 26):
         area = (box[:, 1] - box[:, 0] + 1) * (box[:, 3] - box[:, 2] + 1)
         disc = torch.minimum(torch.pi * rp * rp, area)
         total += float((cls == 1).sum() + disc[cls >= 2].sum())
-        large += float(disc[cls == 3].sum())
+        by_large = (cls == 3) | ((cls == 2) & (rp > ROUTE_RADIUS)) if kw.get("tile") == 32 and kw.get("additive", True) else (cls == 3)
+        large += float(disc[by_large].sum())
         del d, cls, rp, box, area, disc
     return total, large
 

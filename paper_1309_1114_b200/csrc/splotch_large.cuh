@@ -86,7 +86,8 @@ struct LargeSmem {
     float  acc2[32][96];                           // second-level sums of the tensor-core path: [x][(colour, y)], threads of warps 0-2
     float4 gA[kLargeWin], gB[kLargeWin];           // tensor-core list: {px, py, c, r2} {a_R, a_G, a_B, row-band mask}
     float4 cA[kLargeWin], cB[kLargeWin];           // per-pixel list
-    unsigned int cC[kLargeWin];                    // its bands: bit w set = warp w evaluates the record
+    unsigned char clist[kLargeThreads / 32][kLargeWin];   // per band (warp): the entries of the per-pixel list it evaluates
+    unsigned int ccnt[kLargeThreads / 32];
     unsigned long long mbar[kLargeStages], gbar[2];
     int cnt[kLargeThreads / 32][2];
     unsigned int item, tmem;
@@ -284,7 +285,7 @@ k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
             }
             const unsigned int mi0 = __ballot_sync(0xffffffffu, gmask[0] != 0u), mi1 = __ballot_sync(0xffffffffu, gmask[1] != 0u);
             const unsigned int mb0 = __ballot_sync(0xffffffffu, pmask[0] != 0u), mb1 = __ballot_sync(0xffffffffu, pmask[1] != 0u);
-            if (lane == 0) { S.cnt[warp][0] = __popc(mi0) + __popc(mi1); S.cnt[warp][1] = __popc(mb0) + __popc(mb1); }
+            if (lane == 0) { S.cnt[warp][0] = __popc(mi0) + __popc(mi1); S.cnt[warp][1] = __popc(mb0) + __popc(mb1); S.ccnt[warp] = 0u; }
             __syncthreads();                 // counts visible; every warp is done with the previous window's lists
             // the stage of the previous window is free now: refill it
             if (k >= 1u && warp == 0 && k - 1u + kLargeStages < nwin) issue(wbase, k - 1u + kLargeStages, r0, r1);
@@ -307,7 +308,9 @@ k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
                     const int pos = boff + (t ? __popc(mb0) : 0) + __popc((t ? mb1 : mb0) & lt);
                     S.cA[pos] = ra[t];
                     S.cB[pos] = rb[t];
-                    S.cC[pos] = pmask[t];
+#pragma unroll
+                    for (int w = 0; w < kLargeThreads / 32; ++w)         // the bands (warps) that evaluate it: one index list per band
+                        if ((pmask[t] >> w) & 1u) S.clist[w][atomicAdd(&S.ccnt[w], 1u)] = (unsigned char)pos;
                 }
             }
             __syncthreads();
@@ -388,12 +391,12 @@ k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
             // ---- bands the edge of the disc crosses: the C1 inside test of every pixel (bit-exact d2, packed), one ex2 per pixel
             //      inside.  (A row recurrence with a 0 / 1 mask per pixel was measured and dropped: its extra multiplications
             //      cost more FMA-pipe time than the ex2 they save.)
-            const float4 *pa = S.cA, *pb = S.cB;
-            const unsigned int *pc = S.cC;
+            const unsigned int n_mine = S.ccnt[warp];
+            const unsigned char *pl = S.clist[warp];
 #pragma unroll 1
-            for (int m = 0; m < n_cut; ++m, ++pa, ++pb, ++pc) {
-                if (!((*pc >> warp) & 1u)) continue;             // the same for all lanes of the warp
-                const float4 a = *pa, b = *pb;
+            for (unsigned int m = 0; m < n_mine; ++m) {
+                const unsigned int idx = pl[m];                      // the same for all lanes of the warp
+                const float4 a = S.cA[idx], b = S.cB[idx];
                 const float dyf = __fsub_rn(fyc, a.y);
                 const float t2 = __fmul_rn(dyf, dyf);
                 const f32x2 T2 = pk2(t2, t2), NX = pk2(-a.x, -a.x), C = pk2(a.z, a.z);
