@@ -842,25 +842,36 @@ k_scatter(const float *__restrict__ x, const float *__restrict__ y, const float 
                     asm volatile("st.global.v4.f32 [%0], {%1,%2,%3,%4};" :: "l"(records + u), "f"(__uint_as_float(pix)), "f"(a.x), "f"(a.y), "f"(a.z) : "memory");
                 }
             }
-            // MEDIUM and LARGE: one 32-byte record per bin of the box.  A box inside one bin is written by its lane; the others are
-            // walked by the whole warp (coop_bin_walk), the record travelling from its lane by shuffles
+            // MEDIUM and LARGE: one 32-byte record per bin of the box.  Boxes wider than 2 x 2 bins are walked by the whole warp
+            // (coop_bin_walk), the record travelling from its lane by shuffles
             const int nrec = (cls == MEDIUM || cls == LARGE) ? w.n : 0;
             if (__any_sync(0xffffffffu, nrec > 0)) {
                 const float4 ra = make_float4(g.px, g.py, __fdividef(-1.4426950408889634f, sp2), __fmul_rn(g.rp, g.rp));
-                if (nrec == 1) {
-                    unsigned int box;
-                    if (BTILE && cls == MEDIUM) {      // box relative to the home tile's Btile (body + boundary of r_0)
-                        const int ox = (w.bx0 << ts) - fp.btile_r0, oy = (w.by0 << ts) - fp.btile_r0;
-                        box = (unsigned int)(g.x0 - ox) | ((unsigned int)(g.y0 - oy) << 6) | ((unsigned int)(g.x1 - g.x0) << 12) | ((unsigned int)(g.y1 - g.y0) << 18);
-                    } else {
-                        box = pack_box(g, w.bx0, w.by0, w.sh, w.route != 0);
+                // boxes inside 2 x 2 bins (nearly all, outside cfg3): their lane writes the records, one warp-uniform loop of at most four steps
+                const bool wide = nrec > 0 && (w.bx1 - w.bx0 > 1 || w.by1 - w.by0 > 1);
+                const int nown = wide ? 0 : nrec;
+                const int nmax = __reduce_max_sync(0xffffffffu, nown);
+                int bx = w.bx0, by = w.by0;
+#pragma unroll 1
+                for (int t = 0; t < nmax; ++t) {
+                    if (t < nown) {
+                        unsigned int box;
+                        if (BTILE && cls == MEDIUM) {      // box relative to the home tile's Btile (body + boundary of r_0)
+                            const int ox = (bx << ts) - fp.btile_r0, oy = (by << ts) - fp.btile_r0;
+                            box = (unsigned int)(g.x0 - ox) | ((unsigned int)(g.y0 - oy) << 6) | ((unsigned int)(g.x1 - g.x0) << 12) | ((unsigned int)(g.y1 - g.y0) << 18);
+                        } else {
+                            box = pack_box(g, bx, by, w.sh, w.route != 0);
+                        }
+                        st_record(records, cursor_take<GHIST>(cursor + (w.base + w.mult * (by * w.pitch + bx)), 2u), ra,
+                                  make_float4(a.x, a.y, a.z, __uint_as_float(box)));
                     }
-                    st_record(records, cursor_take<GHIST>(cursor + (w.base + w.mult * (w.by0 * w.pitch + w.bx0)), 2u), ra,
-                              make_float4(a.x, a.y, a.z, __uint_as_float(box)));
+                    const bool wrap = bx == w.bx1;
+                    bx = wrap ? w.bx0 : bx + 1;
+                    by += wrap;
                 }
-                if (__any_sync(0xffffffffu, nrec > 1)) {
+                if (__any_sync(0xffffffffu, wide)) {
                     const unsigned int xx = (unsigned int)g.x0 | ((unsigned int)g.x1 << 16), yy = (unsigned int)g.y0 | ((unsigned int)g.y1 << 16);
-                    coop_bin_walk(nrec > 1, w, (int)(threadIdx.x & 31u), [&](bool ok, int sl, int bx, int by, int route) {
+                    coop_bin_walk(wide, w, (int)(threadIdx.x & 31u), [&](bool ok, int sl, int bx, int by, int route) {
                         const float4 sa = make_float4(__shfl_sync(0xffffffffu, ra.x, sl), __shfl_sync(0xffffffffu, ra.y, sl),
                                                       __shfl_sync(0xffffffffu, ra.z, sl), __shfl_sync(0xffffffffu, ra.w, sl));
                         const float s_r = __shfl_sync(0xffffffffu, a.x, sl), s_g = __shfl_sync(0xffffffffu, a.y, sl), s_b = __shfl_sync(0xffffffffu, a.z, sl);
