@@ -334,3 +334,24 @@ def test_cfg3_tile_16_integer_work_at_4096():
     assert np.array_equal(r.debug_tile_counts(16).cpu().numpy().astype(np.int64), tiles)
     check_windows(img, w, lut, kw, windows_for(img, 16, 0, 1))
     r.close()
+
+
+def test_image_of_8192_squared_with_32_and_64_px_tiles():
+    """An 8192 x 8192 image (Eq. 8: the tile grid follows the image): 65,536 tiles of 32 px (three bins per tile and
+    4,096 super-tiles: the blocks count into their rows of the count matrix in L2) and 16,384 tiles of 64 px.  Integer work
+    exhaustive, image on windows (brightest pixel, centre, ragged corner, random ones)."""
+    for tile in (32, 64):
+        w = wl.make_config(3, n=2_000_000, size=(8192, 8192), device="cuda")
+        lut = wl.palette()
+        w.fields = {k: v.contiguous() for k, v in w.fields.items()}
+        r = make_renderer(w, lut)
+        kw = dict(chi=w.chi, r_small=w.r_small, r_large=w.r_large, z_near=w.z_near, tile=tile, additive=True)
+        img = r.render(w.fields, w.species, pair_capacity=300_000_000, **kw)      # discs are twice as wide in pixels as at 4096^2
+        torch.cuda.synchronize()
+        st = r.stats()
+        counts, tiles = check_integer_work(r, w, kw, tile, geometry_every=1)
+        assert st["overflow"] == 0 and st["count"] == [int(c) for c in counts] and counts[3] > 0 and counts[2] > 0
+        assert np.array_equal(r.debug_tile_counts(tile).cpu().numpy().astype(np.int64), tiles)
+        assert st["pairs"] == int(tiles.sum())
+        check_windows(img, w, lut, kw, windows_for(img, 32, 5, seed=7 + tile))
+        r.close()
