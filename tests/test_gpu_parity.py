@@ -144,6 +144,23 @@ def test_large_particles_with_8px_tiles_and_a_disc_covering_the_image():
     assert st["count"][wl_LARGE] > 1000
 
 
+def test_many_discs_that_contain_whole_blocks_go_through_the_tensor_cores_within_tolerance():
+    """k_large's tensor-core bands: 60,000 discs of 120 .. 600 px that contain most 32-px blocks of a 160 x 128 image, so every pixel
+    sums tens of thousands of products of split TF32 operands in tensor memory (accumulators of 64 records folded into float32
+    second-level sums); the amplitudes span four decades and the colours differ per particle.  Same tolerance."""
+    w = wl.make_config(3, n=60_000, size=(160, 128))
+    w.r_large = 16.0
+    g = torch.Generator().manual_seed(5)
+    w.fields["x"] = 0.5 + 0.02 * (torch.rand(w.n, generator=g) - 0.5)
+    w.fields["y"] = 0.5 + 0.02 * (torch.rand(w.n, generator=g) - 0.5)
+    w.fields["z"] = 0.5 + 0.02 * (torch.rand(w.n, generator=g) - 0.5)
+    w.fields["h"] = 0.3 + 1.2 * torch.rand(w.n, generator=g)
+    w.fields["I"] = torch.exp(9.2 * torch.rand(w.n, generator=g) - 4.6)
+    for tile in (16, 32):
+        st, geo = full_check(w, tile)
+        assert st["count"][wl_LARGE] > 50_000
+
+
 def test_apply_transfer():
     w = wl.make_config(0, n=30_000)
     w.apply_transfer = True
