@@ -958,12 +958,13 @@ __device__ __forceinline__ void fixed_add(unsigned int *lo, unsigned int *hi, fl
                  :: "r"(alo), "r"(ahi), "r"((unsigned int)v & 0xffffu), "r"(up) : "memory");
 }
 
-// Geometry of the tile renderer: a warp owns a strip of the tile (16 x 4 pixels; 8 x 8 for T = 8; 64 x 4 for T = 64), a
+// Geometry of the tile renderer: a warp owns a strip of the tile (8 x 8 pixels; 64 x 4 for T = 64; a box of 3 x 3 pixels straddles
+// fewer square strips than 16 x 4 ones: cfg2 k_splat 2.50 -> 2.34 ms), a
 // lane owns kNP pairs of horizontally adjacent pixels of it and keeps their RGB sums in registers as packed pairs.
 template <int T> struct SplatCfg {
     static constexpr int kPix = T * T;
     static constexpr int kNP = T == 64 ? 4 : 1;          // pixel pairs per lane
-    static constexpr int kSW = T == 64 ? 64 : (T >= 16 ? 16 : 8);   // strip width
+    static constexpr int kSW = T == 64 ? 64 : 8;                     // strip width
     static constexpr int kSH = 64 * kNP / kSW;           // strip height
     static constexpr int kStripsX = T / kSW, kStripsY = T / kSH;
     static constexpr int kWarps = kStripsX * kStripsY;   // 1, 4, 16, 16 for T = 8, 16, 32, 64
