@@ -494,13 +494,16 @@ k_odiff(const unsigned int *__restrict__ tile_start, int n_tiles, unsigned int *
 // Taylor series to x^8 (relative error < 2e-8), e = 1 - a; otherwise e = 2^(-x log2 e) (ex2.approx), a = 1 - e.
 __device__ __forceinline__ void absorb_pair(float x, float &a, float &e)
 {
-    float p = fmaf(-x, 0.125f, 1.0f);
-    p = fmaf(-x * (1.0f / 7.0f), p, 1.0f);
-    p = fmaf(-x * (1.0f / 6.0f), p, 1.0f);
-    p = fmaf(-x * 0.2f, p, 1.0f);
-    p = fmaf(-x * 0.25f, p, 1.0f);
-    p = fmaf(-x * (1.0f / 3.0f), p, 1.0f);
-    p = fmaf(-x * 0.5f, p, 1.0f);
+    // (1 - exp(-x)) / x = sum_k (-x)^k / (k + 1)!, k = 0 .. 7, by Horner's rule in y = -x
+    const float y = -x;
+    float p = 2.48015873e-5f;                       // 1 / 8!
+    p = fmaf(p, y, 1.98412698e-4f);                 // 1 / 7!
+    p = fmaf(p, y, 1.38888889e-3f);                 // 1 / 6!
+    p = fmaf(p, y, 8.33333333e-3f);                 // 1 / 5!
+    p = fmaf(p, y, 4.16666667e-2f);                 // 1 / 4!
+    p = fmaf(p, y, 1.66666667e-1f);                 // 1 / 3!
+    p = fmaf(p, y, 0.5f);
+    p = fmaf(p, y, 1.0f);
     const float as = x * p;
     const float el = ex2_approx(x * -1.4426950408889634f);
     const bool small = fabsf(x) < 0.25f;
