@@ -466,6 +466,16 @@ def run_ours(args):
             del r2
             gc.collect()
             torch.cuda.empty_cache()
+        # the memory-coherent variant of the recipe: cfg1's particles contiguous by halo
+        r3 = Run(1, "additive", local)
+        perm = wl.halo_order(1, r3.w.n, f"cuda:{local}")
+        r3.fields = {k: v[perm].contiguous() for k, v in r3.fields.items()}
+        r3.w.fields = r3.fields
+        ms3, pf3, st3 = r3.timed(20, 3, barrier)
+        per["cfg1_additive_by_halo"] = r3.summary(ms3, pf3, st3, hbm_gbs, fma_peak)[0]
+        per["cfg1_additive_by_halo"]["workload"] += " (particles contiguous by halo)"
+        r3.close()
+        del r3, perm
         out["per_config"] = per
     print(json.dumps(out))
     if dist is not None:

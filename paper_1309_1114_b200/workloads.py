@@ -225,6 +225,21 @@ def _halo_set(seed: int, n: int, eta: float, device, star_begin: Optional[int] =
     return out, info
 
 
+def halo_order(cfg: int, n: int, device) -> torch.Tensor:
+    """Permutation that makes the halo set of configs[cfg] contiguous by halo (background particles last): the memory-coherent
+    variant of the recipe (the default interleaves the halos' particles, the hard case for the binning stages)."""
+    seed = 1002 if cfg == 4 else 1000 + cfg
+    mass, _, _ = halo_table(seed)
+    cum = (torch.cumsum(mass, 0) / float(mass.sum())).to(device)
+    cum[-1] = 1.0
+    key = torch.empty(n, dtype=torch.int16, device=device)
+    for s, e in _chunks(n, 1 << 22):
+        idx = torch.arange(s, e, dtype=torch.int64, device=device)
+        hk = torch.clamp(torch.searchsorted(cum, uniform(seed, idx, 1)), max=mass.numel() - 1)
+        key[s:e] = torch.where(uniform(seed, idx, 0) < 0.2, torch.full_like(hk, mass.numel()), hk).to(torch.int16)
+    return torch.sort(key, stable=True).indices
+
+
 def orbit_camera(frame: int, fov_deg: float = 45.0) -> Camera:
     """cfg4 fly-through: eye on a radius-2 circle around the box centre, 3 degrees per frame."""
     ang = math.radians(3.0 * frame)
