@@ -2,18 +2,19 @@
 //
 // Stage map (paper passages in PAPER.md):
 //   k_count    A1+A3+A4a  roto-translate, project, classify (:76, :138, :156-173) and count (particle, bin) pairs
-//   k_scan     A4b+A4c    per-bin exclusive scan down the rows of the count matrix (replaces thrust::reduce_by_key,
-//                         :203); the last block to finish scans over the bins, builds the chunk table and the frame
-//                         statistics (replaces inclusive_scan, :205)
-//   k_scatter  A1-A3+A2+A4d  recompute geometry, colourise (:76, :85), write 32-byte render records in bin order
+//   k_scan     A4b        per-bin exclusive scan down the rows of the count matrix (replaces thrust::reduce_by_key,
+//                         :203); the last block to finish builds the frame statistics, the virtual bin order, the chunk size
+//                         and k_large's item table (replaces inclusive_scan, :205)
+//   k_layout   A4b        the runs of every bin inside the slabs of the record array
+//   k_scatter  A1-A3+A2+A4c  recompute geometry, colourise (:76, :85), write render records in bin order
 //                            (replaces copy_if + sort_by_key, :196-202)
-//   k_splat    A5         SMALL + MEDIUM records of one chunk: all fragments of 32 records are spread over the 32 lanes
-//                         of a warp and accumulated into the tile's fixed-point framebuffer in shared memory (two
-//                         32-bit planes per channel, native integer atomics without return; the paper's
-//                         medium-particle kernel, :183, :224-228, without its halo copies and without idle threads
-//                         for small footprints)
-//   k_large    A6         (splotch_large.cuh) LARGE particles, which the paper renders on the CPU (:232-238): items of
-//                         (chunk of a super-tile's records) x (tile), added to the same fixed-point sums
+//   k_splat    A5         (splotch_splat.cuh) SMALL + MEDIUM records of the tile bins: a producer warp streams the records into
+//                         shared memory with bulk copies, consumer warps add SMALL records and tiny boxes straight into the
+//                         tile's fixed-point planes and evaluate the others as owners of 8 x 8-pixel strips (the paper's
+//                         medium-particle kernel, :183, :224-228, without its halo copies)
+//   k_large    A6         (splotch_large.cuh) LARGE particles, which the paper renders on the CPU (:232-238), and with 32-px tiles
+//                         the MEDIUM discs wider than 32 px: items of (chunk of a region's records) x (32 x 32-px block); bands
+//                         inside their disc are summed on the tensor cores (tcgen05), the others per pixel
 //   k_compose  A8         per tile: fixed-point sums -> float32, optional 1-exp(-S), write the image once
 //
 // Canonical float32 geometry: every operation that decides an integer (class, pixel box, tile box, the inside
