@@ -5,9 +5,12 @@
 // particle under every super-tile (128 x 128 px) its box touches, and k_large splits the work into items of
 // (chunk of a super-tile's records) x (32 x 32-pixel block of that super-tile) that CTAs take from an atomic counter,
 // so a region covered by hundreds of thousands of large discs (camera inside a halo, cfg3) is shared by many CTAs.
+// With 32-px tiles the same kernel renders the MEDIUM discs wider than kRouteRadius: they sit in a third bin of their tile
+// (splotch_kernels.cuh), a region of one block, the tile itself.
 //   * the chunk's records stream through shared memory with bulk copies on mbarriers, as in k_splat;
 //   * every thread tests two records per window against the block's four bands of 8 rows x 32 pixels and files the record
-//     in up to two lists: bands that lie wholly inside the clip disc, bands the edge of the disc crosses;
+//     in up to two lists: bands that lie wholly inside the clip disc, bands the edge of the disc crosses (with one index list
+//     per band, so a warp meets only the records that cross its band);
 //   * bands inside the disc: no pixel is clipped and the Gaussian is separable, exp2(c d^2) = exp2(c dx^2) exp2(c dy^2), so
 //     the sum over the records is a dense contraction D[(colour, y)][x] = sum_p A[(colour, y)][p] B[p][x] with
 //     A = a_colour exp2(c dy^2) (zero in the rows of the record's other bands), B = exp2(c dx^2).  It runs on the
@@ -23,7 +26,8 @@
 //   * sums go to the tiles' 64-bit fixed-point sums in L2 (exact, commutative), the same sums k_splat feeds; k_compose
 //     turns them into the float32 image.
 // Blocks are 32 x 32 px whatever the tile side T is.  Measured on cfg3 (9.5e11 LARGE fragments): round 1 397 ms (one ex2 per
-// pixel), row recurrence 296 ms, tensor-core bands 282 ms, 128-px super-tiles 245 ms.
+// pixel), row recurrence 296 ms, tensor-core bands 282 ms, 128-px super-tiles 245 ms; with the wide MEDIUM discs (1.05e12
+// fragments) 292 ms, per-band lists 274 ms.
 #pragma once
 #include "splotch_kernels.cuh"
 #include "splotch_splat.cuh"
