@@ -281,6 +281,31 @@ class Run:
         self.r.set_profiling(False)
         return ms_total / steps, per_frame, st
 
+    def timed_graph(self, steps: int):
+        """ms per frame when the frame is captured once into a CUDA graph and replayed (the library only enqueues kernels and memsets
+        on the caller's stream, so a frame can be captured): what a launch-bound frame costs without the launch gaps."""
+        self.r.set_profiling(False)
+        side = torch.cuda.Stream()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(side):
+            self.frame(0)
+            torch.cuda.synchronize()
+            with torch.cuda.graph(graph, stream=side):
+                self.frame(0)
+        torch.cuda.synchronize()
+        stream = torch.cuda.current_stream()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for i in range(3):
+            graph.replay()
+        for i in range(steps):
+            if self.flush:
+                self.fbuf.fill_(i & 255)
+            ev[i][0].record(stream)
+            graph.replay()
+            ev[i][1].record(stream)
+        torch.cuda.synchronize()
+        return sum(a.elapsed_time(b) for a, b in ev) / steps
+
     def summary(self, ms_step: float, per_frame, st, hbm_gbs: float, fma_peak: float, frags=None):
         """Per-stage roofline fractions and the frame lower bound (sum over stages)."""
         w = self.w
@@ -455,6 +480,8 @@ def run_ours(args):
                 r2 = Run(cfg, mode, local)
             ms2, pf2, st2 = r2.timed(steps, 3, barrier)
             per[key] = r2.summary(ms2, pf2, st2, hbm_gbs, fma_peak)[0]
+            if r2.flush and not r2.orbit:           # small frames are launch bound: the same frame replayed from a CUDA graph
+                per[key]["ms_per_frame_cuda_graph"] = r2.timed_graph(steps)
             keep = cfg == 4 and mode == "additive"
             if keep:
                 shared = (r2.fields, r2.w)

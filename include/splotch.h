@@ -151,7 +151,8 @@ size_t splotch_workspace_bytes(const splotch_ctx *ctx, uint64_t n, int tile, uin
  *   workspace  : DEVICE scratch of workspace_bytes bytes, 256-byte aligned, caller-owned; its contents
  *                must stay untouched until splotch_get_stats / splotch_debug_tile_counts were called
  * Errors: EINVAL, ESTATE, ENOMEM (workspace below the fixed minimum), ECUDA.  A frame whose pairs exceed the
- * record capacity is reported through splotch_stats.overflow (the image is then all zero). */
+ * record capacity is reported through splotch_stats.overflow (the image is then all zero).  * All work is enqueued on `cuda_stream` (kernels and memsets only, no synchronisation, no allocation): the call may be
+ * captured into a CUDA graph and replayed while the pointers and parameters stay the same. */
 int splotch_render(splotch_ctx *ctx, const splotch_particles *particles, uint64_t n,
                    const splotch_params *params, float *image_out,
                    void *workspace, size_t workspace_bytes, void *cuda_stream);

@@ -493,3 +493,34 @@ def test_ordered_tiny_counts(n):
         w.n = 0
         w.species[0].end = 0
     full_check(w, 16)
+
+
+def test_a_frame_captured_in_a_cuda_graph_replays_to_the_same_image():
+    """splotch_render only enqueues kernels and memsets on the caller's stream, so a frame can be captured into a CUDA graph (the
+    launch gaps of a small frame go away); the replayed image equals the directly rendered one to float32 reproducibility."""
+    b = _binding()
+    w = wl.make_config(0, n=50_000, size=(192, 160))
+    lut = wl.palette()
+    r = b.Renderer(w.width, w.height, w.n)
+    r.set_camera(w.camera)
+    r.set_colormap(0, lut)
+    f = {k: v.cuda().contiguous() for k, v in w.fields.items()}
+    kw = dict(chi=w.chi, r_small=w.r_small, r_large=8.0, z_near=w.z_near, tile=16, additive=True)      # r_large = 8: k_large takes part
+    img = torch.empty((w.height, w.width, 3), dtype=torch.float32, device="cuda")
+    r.render(f, w.species, image=img, **kw)
+    torch.cuda.synchronize()
+    ref = img.clone()
+    assert r.stats()["count"][wl_LARGE] > 0
+    side, graph = torch.cuda.Stream(), torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        r.render(f, w.species, image=img, **kw)
+        torch.cuda.synchronize()
+        with torch.cuda.graph(graph, stream=side):
+            r.render(f, w.species, image=img, **kw)
+    torch.cuda.synchronize()
+    for _ in range(3):
+        img.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert float((img - ref).abs().max()) <= 1e-6 * float(ref.max())
+    r.close()
