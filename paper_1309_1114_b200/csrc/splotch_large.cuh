@@ -88,7 +88,7 @@ struct LargeSmem {
     float4 stage[kLargeStages][kLargeWin][2];      // records of two windows (bulk copies)
     float  bop[2][2][2][256];                      // B operand: [buffer][K-step][hi, lo][(x / 8, k / 4, x % 8, k % 4)]
     float  acc2[32][96];                           // second-level sums of the tensor-core path: [x][(colour, y)], threads of warps 0-2
-    float4 gA[kLargeWin], gB[kLargeWin];           // tensor-core list: {px, py, c, r2} {a_R, a_G, a_B, row-band mask}
+    float4 gA[kLargeWin + kGemmGroup], gB[kLargeWin + kGemmGroup];   // tensor-core list (+ padding to whole groups): {px, py, c, r2} {a_R, a_G, a_B, row-band mask}
     float4 cA[kLargeWin], cB[kLargeWin];           // per-pixel list
     unsigned char clist[kLargeThreads / 32][kLargeWin];   // per band (warp): the entries of the per-pixel list it evaluates
     unsigned int ccnt[kLargeThreads / 32];
@@ -317,6 +317,11 @@ k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
                         if ((pmask[t] >> w) & 1u) S.clist[w][atomicAdd(&S.ccnt[w], 1u)] = (unsigned char)pos;
                 }
             }
+            if ((int)threadIdx.x < ((kGemmGroup - (n_in & (kGemmGroup - 1))) & (kGemmGroup - 1))) {
+                // the tensor-core list is padded to whole groups with records that add nothing (amplitudes 0, no rows; weights exp2(0) = 1)
+                S.gA[n_in + threadIdx.x] = make_float4(0.0f, 0.0f, 0.0f, 1.0f);
+                S.gB[n_in + threadIdx.x] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            }
             __syncthreads();
             // ---- bands that lie inside their disc: the sum over them is a dense contraction, D[(colour, y)][x] = sum_p A[(colour, y)][p] B[p][x]
             //      with A = a_colour exp2(c dy^2) (0 in the rows of the other bands) and B = exp2(c dx^2): the Gaussian is separable and no pixel
@@ -339,7 +344,7 @@ k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
                             const unsigned int rows = __float_as_uint(S.gB[idx].w);
                             const float dy = fyg - a.y;
                             float v = amp * ex2_approx(a.z * dy * dy);
-                            v = (idx < n_in && ((rows >> (lane >> 3)) & 1u)) ? v : 0.0f;
+                            v = ((rows >> (lane >> 3)) & 1u) ? v : 0.0f;
                             va[q] = __float_as_uint(v);
                             va[8 + q] = __float_as_uint(v - __uint_as_float(__float_as_uint(v) & 0xffffe000u));
                         }
@@ -356,8 +361,7 @@ k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
 #pragma unroll
                             for (int j = 0; j < 4; ++j) {
                                 const float dx = (fxg + (float)(8 * j)) - a.x;
-                                float w = ex2_approx(a.z * dx * dx);
-                                w = idx < n_in ? w : 0.0f;
+                                const float w = ex2_approx(a.z * dx * dx);
                                 S.bop[buf][ks][0][(j * 2 + h) * 32 + lane] = w;
                                 S.bop[buf][ks][1][(j * 2 + h) * 32 + lane] = w - __uint_as_float(__float_as_uint(w) & 0xffffe000u);
                             }
