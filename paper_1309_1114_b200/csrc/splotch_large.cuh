@@ -37,7 +37,7 @@ namespace splotch {
 constexpr int kLargeThreads = 128;
 constexpr int kLargeWin = 256;            // records per bulk copy; every thread tests two of them
 constexpr int kLargeStages = 2;
-constexpr int kLargeChunk = 4096;         // records per work item
+constexpr int kLargeChunk = 8192;         // records per work item
 constexpr int kLargeBlock = 32;           // block side in px
 constexpr int kLargePpt = 8;              // pixels per thread (one row segment) on the cutting-disc path
 constexpr int kGemmGroup = 16;            // records per operand buffer: two K-steps of 8 (tcgen05.mma kind::tf32 has K = 8)
