@@ -401,7 +401,7 @@ k_large(const float4 *__restrict__ records, const unsigned int *__restrict__ bin
             //      cost more FMA-pipe time than the ex2 they save.)
             const unsigned int n_mine = S.ccnt[warp];
             const unsigned char *pl = S.clist[warp];
-#pragma unroll 1
+#pragma unroll 4
             for (unsigned int m = 0; m < n_mine; ++m) {
                 const unsigned int idx = pl[m];                      // the same for all lanes of the warp
                 const float4 a = S.cA[idx], b = S.cB[idx];
