@@ -27,7 +27,7 @@
 //     turns them into the float32 image.
 // Blocks are 32 x 32 px whatever the tile side T is.  Measured on cfg3 (9.5e11 LARGE fragments): round 1 397 ms (one ex2 per
 // pixel), row recurrence 296 ms, tensor-core bands 282 ms, 128-px super-tiles 245 ms; with the wide MEDIUM discs (1.05e12
-// fragments) 292 ms, per-band lists 274 ms.
+// fragments) 292 ms, per-band lists 274 ms, padded list and items of 8192 records 266 ms, per-pixel loop unrolled four times 253 ms.
 #pragma once
 #include "splotch_kernels.cuh"
 #include "splotch_splat.cuh"
