@@ -201,6 +201,25 @@ int splotch_debug_geometry(splotch_ctx *ctx, const splotch_particles *particles,
 /* Per-tile pair counts of the last frame: DEVICE out, nty x ntx uint32 (SMALL + MEDIUM; ordered mode: all). */
 int splotch_debug_tile_counts(splotch_ctx *ctx, uint32_t *out, void *cuda_stream);
 
+/* Classes and per-tile pair counts of a particle set (steps A1, A3, A4a: PAPER.md:76, :138, :156-173 and the counting half
+ * of :175) for callers that cannot allocate: the call makes NO allocation (no cudaMalloc / cudaFree, no allocating library
+ * routine) and takes no workspace.  Its scratch, the count matrix, is a file-scope device array of 16 MiB inside the library
+ * (held on every GPU that loads the library until the process exits); splotch_create looks its address up once per device.
+ *   particles        : DEVICE arrays as for splotch_render (x, y, z, h are read), n <= max_particles
+ *   params           : additive != 0, renderer == 0; tile, chi, r_small, r_large, z_near as for splotch_render
+ *   tile_counts_out  : DEVICE, nty x ntx uint32: (particle, tile) pairs per tile, SMALL + MEDIUM (what
+ *                      splotch_debug_tile_counts reports after an additive frame); overwritten
+ *   class_counts_out : DEVICE, uint64[4] = {culled, small, medium, large} (splotch_stats.count); overwritten
+ * Limit: 4 x (bins + 4) x SMs bytes must fit in the 16 MiB, bins = 2 x tiles + super-tiles (+ tiles with 32-px tiles): at
+ * most about 28,000 bins on a 148-SM GPU (1920 x 1080 at 16 px fits, 4096 x 4096 needs 64-px tiles).  Larger requests return
+ * SPLOTCH_EINVAL and splotch_last_error says so.
+ * All calls share the array and it keeps the last call's contents; every call clears the part it uses first.  Calls that
+ * overlap on the GPU (other streams, other contexts of the same device) race: serialise them.  Enqueues on `cuda_stream`
+ * without synchronising, like splotch_render. */
+int splotch_count_static(splotch_ctx *ctx, const splotch_particles *particles, uint64_t n,
+                         const splotch_params *params, uint32_t *tile_counts_out, uint64_t *class_counts_out,
+                         void *cuda_stream);
+
 const char *splotch_last_error(const splotch_ctx *ctx);
 const char *splotch_version(void);
 

@@ -26,6 +26,7 @@ EXPORTS = (
     "splotch_set_colormap", "splotch_set_profiling", "splotch_workspace_bytes", "splotch_render",
     "splotch_render_host", "splotch_get_stats", "splotch_stage_name", "splotch_debug_geometry",
     "splotch_debug_tile_counts", "splotch_last_error", "splotch_version", "splotch_measure_peaks", "splotch_set_host_chunk", "splotch_apply_transfer",
+    "splotch_count_static",
 )
 
 
@@ -88,6 +89,7 @@ def load() -> C.CDLL:
     lib.splotch_stage_name.restype = C.c_char_p
     lib.splotch_debug_geometry.argtypes = [vp, C.POINTER(SplotchParticles), u64, C.POINTER(SplotchParams)] + [vp] * 10
     lib.splotch_debug_tile_counts.argtypes = [vp, vp, vp]
+    lib.splotch_count_static.argtypes = [vp, C.POINTER(SplotchParticles), u64, C.POINTER(SplotchParams), vp, vp, vp]
     lib.splotch_measure_peaks.argtypes = [vp, C.POINTER(C.c_double), vp]
     lib.splotch_set_host_chunk.argtypes = [vp, u64]
     lib.splotch_apply_transfer.argtypes = [vp, vp, vp]
@@ -290,6 +292,17 @@ class Renderer:
                                                       ("cls", "px", "py", "sp", "rp", "zc", "pbox", "tbox", "ilabel")],
             stream))
         return out
+
+    def count_static(self, fields: Dict[str, torch.Tensor], species: Sequence, tile_counts: torch.Tensor,
+                     class_counts: torch.Tensor, **params) -> None:
+        """splotch_count_static: classes and per-tile pair counts into the caller's DEVICE tensors (nty x ntx int32 and
+        int64[4]); the library call allocates nothing (its scratch is a static device array)."""
+        n = fields["x"].numel()
+        prm, keep1 = make_params(species, **params)
+        prt, keep2 = make_particles(fields, species)
+        stream = torch.cuda.current_stream(self.device).cuda_stream
+        _check(self.ctx, self.lib.splotch_count_static(self.ctx, C.byref(prt), n, C.byref(prm), tile_counts.data_ptr(),
+                                                       class_counts.data_ptr(), stream))
 
     def debug_tile_counts(self, tile: int) -> torch.Tensor:
         ntx, nty = -(-self.width // tile), -(-self.height // tile)

@@ -17,6 +17,50 @@
 
 using namespace splotch;
 
+// ---- splotch_count_static: the one entry point that allocates nothing ------------------------------------------------
+// Its scratch (the count matrix of the classify-and-count stage) lives in this file-scope device array instead of a
+// caller-owned workspace: 16 MiB on every GPU that loads the library, until the process exits.  In HOST code the name
+// g_static_scratch is a host-side stand-in, not a device address: the address the kernels get comes from
+// cudaGetSymbolAddress, once per device with that device current (static_scratch_address, called by splotch_create).
+// Every call shares the array and it keeps the last call's contents: the call clears the part it uses, and calls that
+// overlap on the GPU (two streams, two contexts of one device) race.
+constexpr size_t kStaticScratchBytes = 16u << 20;
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+
+// per-tile pair counts (the tile's SMALL, MEDIUM and, with 32-px tiles, wide-MEDIUM bins summed over the rows of the count
+// matrix) and the class totals {particles, SMALL, MEDIUM, LARGE}; k_static_count_finish turns the first into CULLED
+__global__ void __launch_bounds__(256)
+k_static_count_reduce(const unsigned int *__restrict__ counts, const unsigned int *__restrict__ cls_counts, int nrows,
+                      int nbins, int n_tiles, int n_super, int n_big, unsigned int *__restrict__ tile_out,
+                      unsigned long long *__restrict__ class_out)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned int small = 0u;
+    if (t < n_tiles) {
+        unsigned int med = 0u, wide = 0u;
+        for (int r = 0; r < nrows; ++r) {
+            const unsigned int *row = counts + (size_t)r * nbins;
+            med += row[2 * t]; small += row[2 * t + 1];
+            if (n_big) wide += row[2 * n_tiles + n_super + t];
+        }
+        tile_out[t] = med + small + wide;
+    }
+    small = __reduce_add_sync(0xffffffffu, small);
+    if ((threadIdx.x & 31) == 0 && small) atomicAdd(class_out + 1, (unsigned long long)small);
+    if (blockIdx.x == 0) {
+        unsigned long long tot = 0ull, med = 0ull, large = 0ull;
+        for (int r = threadIdx.x; r < nrows; r += blockDim.x) { tot += cls_counts[4 * r]; med += cls_counts[4 * r + 2]; large += cls_counts[4 * r + 3]; }
+        if (tot) atomicAdd(class_out + 0, tot);
+        if (med) atomicAdd(class_out + 2, med);
+        if (large) atomicAdd(class_out + 3, large);
+    }
+}
+
+__global__ void k_static_count_finish(unsigned long long *class_out)
+{
+    class_out[0] -= class_out[1] + class_out[2] + class_out[3];       // particles -> CULLED
+}
+
 namespace {
 
 constexpr int kStages = 7;                  // most stages a frame has (ordered mode); additive frames have 5
@@ -45,6 +89,7 @@ struct splotch_ctx {
     bool camera_set = false;
     float cam[16] = {0};
     float4 *lut = nullptr;                   // device, [kMaxSpecies][kMaxLut]
+    unsigned char *static_scratch = nullptr; // device address of g_static_scratch on this context's device
     int lut_n[kMaxSpecies] = {0};
     bool profiling = false;
     cudaEvent_t (*ev_ring)[kStages + 1] = nullptr;   // [kProfRing][kStages + 1], created when profiling is first enabled
@@ -91,6 +136,20 @@ int fail(splotch_ctx *c, int code, const char *fmt, ...)
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 int tile_shift(int T) { return T == 8 ? 3 : T == 16 ? 4 : T == 32 ? 5 : T == 64 ? 6 : -1; }
+
+// Device address of g_static_scratch on `device` (which must be current): looked up once per device and kept.
+int static_scratch_address(splotch_ctx *c, int device, unsigned char **out)
+{
+    static unsigned char *ptr_of_device[64] = {nullptr};
+    if (device < 0 || device >= 64) return fail(c, SPLOTCH_EINVAL, "device index %d out of range", device);
+    if (!ptr_of_device[device]) {
+        unsigned char *ptr = nullptr;
+        CU_TRY(c, cudaGetSymbolAddress((void **)&ptr, g_static_scratch));
+        ptr_of_device[device] = ptr;
+    }
+    *out = ptr_of_device[device];
+    return SPLOTCH_OK;
+}
 
 // LARGE particles are binned to super-tiles of 8 x 8 tiles, at most 128 px a side (record boxes are 8 bits per bound)
 int super_shift(int T) { const int s = tile_shift(T) + kSuperShift; return s < kSuperMaxShift ? s : kSuperMaxShift; }
@@ -591,6 +650,7 @@ int splotch_create(splotch_ctx **out, int device, int width, int height, uint64_
     int rc = [&]() -> int {
         CU_TRY(c, cudaMalloc(&c->lut, sizeof(float4) * kMaxSpecies * kMaxLut));
         CU_TRY(c, cudaMemset(c->lut, 0, sizeof(float4) * kMaxSpecies * kMaxLut));
+        { const int rs = static_scratch_address(c, device, &c->static_scratch); if (rs != SPLOTCH_OK) return rs; }   // `device` is current
         CU_TRY(c, (cudaFuncSetAttribute(k_count<true, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb)));
         CU_TRY(c, (cudaFuncSetAttribute(k_count<false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb)));
         CU_TRY(c, (cudaFuncSetAttribute(k_scatter<true, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, hb)));
@@ -991,6 +1051,43 @@ int splotch_debug_tile_counts(splotch_ctx *c, uint32_t *out, void *cuda_stream)
                                                                                      c->fp.n_tiles, out);
         CU_TRY(c, cudaGetLastError());
     }
+    return SPLOTCH_OK;
+}
+
+// Classes and per-tile pair counts of a particle set (steps A1, A3, A4a) without any allocation and without a workspace.
+int splotch_count_static(splotch_ctx *c, const splotch_particles *p, uint64_t n, const splotch_params *q,
+                         uint32_t *tile_counts_out, uint64_t *class_counts_out, void *cuda_stream)
+{
+    if (!c) return SPLOTCH_EINVAL;
+    if (!tile_counts_out || !class_counts_out) return fail(c, SPLOTCH_EINVAL, "null output");
+    FrameParams fp;
+    const int rc = check_params(c, p, n, q, &fp);
+    if (rc != SPLOTCH_OK) return rc;
+    if (!q->additive || q->renderer != 0) return fail(c, SPLOTCH_EINVAL, "splotch_count_static takes the additive mode and the default renderer");
+    if (!c->static_scratch) return fail(c, SPLOTCH_ESTATE, "static scratch was not set up");
+    const int nrows = c->n_sm;
+    const size_t counts_bytes = sizeof(unsigned int) * (size_t)nrows * fp.nbins;
+    const size_t need = align_up(counts_bytes, 256) + sizeof(unsigned int) * 4 * (size_t)nrows;
+    if (need > kStaticScratchBytes)
+        return fail(c, SPLOTCH_EINVAL, "splotch_count_static: %d bins x %d rows need %zu bytes of scratch, the static array holds %zu "
+                                        "(at most %zu bins: use a larger tile or splotch_render with a workspace)",
+                    fp.nbins, nrows, need, kStaticScratchBytes, (kStaticScratchBytes - 16 * (size_t)nrows - 256) / (sizeof(unsigned int) * nrows));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CU_TRY(c, cudaSetDevice(c->device));
+    unsigned int *counts = (unsigned int *)c->static_scratch;
+    unsigned int *cls_counts = (unsigned int *)(c->static_scratch + align_up(counts_bytes, 256));
+    // the array keeps the last call's contents: the blocks count into their rows with atomics, so the rows start at zero
+    CU_TRY(c, cudaMemsetAsync(c->static_scratch, 0, need, st));
+    CU_TRY(c, cudaMemsetAsync(class_counts_out, 0, 4 * sizeof(unsigned long long), st));
+    unsigned long long per = (n + nrows - 1) / nrows;
+    per = (per + 3) / 4 * 4;
+    if (per == 0) per = 4;
+    if (aligned16(p)) k_count<true, true, false><<<nrows, kBinThreads, 0, st>>>(p->x, p->y, p->z, p->h, n, per, fp, counts, cls_counts);
+    else              k_count<false, true, false><<<nrows, kBinThreads, 0, st>>>(p->x, p->y, p->z, p->h, n, per, fp, counts, cls_counts);
+    k_static_count_reduce<<<(fp.n_tiles + 255) / 256, 256, 0, st>>>(counts, cls_counts, nrows, fp.nbins, fp.n_tiles, fp.n_super, fp.n_big,
+                                                                    tile_counts_out, (unsigned long long *)class_counts_out);
+    k_static_count_finish<<<1, 1, 0, st>>>((unsigned long long *)class_counts_out);
+    CU_TRY(c, cudaGetLastError());
     return SPLOTCH_OK;
 }
 
