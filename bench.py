@@ -42,10 +42,13 @@ DEFAULT_CONFIG = 3           # the largest single-GPU configuration of BASELINE.
 TILE_OVERRIDE = 0
 
 
-def tile_for(cfg: int) -> int:
+def tile_for(cfg: int, mode: str = "additive") -> int:
+    """Tile side the configuration is timed with (a parameter of the library; its default is 16).  32 px for the frames of 1e8
+    particles and more in additive mode: a quarter of the bins makes k_scatter's stores land better (cfg2: 1.98 -> 1.49 ms) for a
+    little more k_splat time (2.38 -> 2.59 ms); the ordered mode and the small frames are faster with 16 px."""
     if TILE_OVERRIDE:
         return TILE_OVERRIDE
-    return 32 if cfg == 3 else 16       # 4096^2: 16,384 tiles of 32 px (65,536 of 16 px work too, on the slower global-histogram path)
+    return 32 if (cfg == 3 or (cfg in (2, 4) and mode == "additive")) else 16
 
 
 def ordered_kernels_per_frame(n_tiles: int) -> int:
@@ -226,7 +229,7 @@ class Run:
         self.additive = mode == "additive"
         self.w = workload if workload is not None else wl.make_config(cfg, device=f"cuda:{local}")
         w = self.w
-        self.tile = tile_for(cfg)
+        self.tile = tile_for(cfg, mode)
         self.lut = wl.palette()
         self.fields = fields if fields is not None else {k: v.contiguous() for k, v in w.fields.items()}
         w.fields = self.fields
@@ -540,7 +543,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    tile, additive = tile_for(args.config), args.mode == "additive"
+    tile, additive = tile_for(args.config, args.mode), args.mode == "additive"
     # bounded sample: the whole --steps / --warmup run stays near two minutes
     sample_n = max(20_000, min(args.ref_sample, int(6 * default_cpu_sample(args.config) / (args.steps + args.warmup))))
     times = []
@@ -576,7 +579,7 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=10_000_000)
     ap.add_argument("--no-per-config", action="store_true", help="skip the per_config sweep over the other configs")
     ap.add_argument("--frames-only", action="store_true", help="time the frames and stop (for runs under ncu)")
-    ap.add_argument("--tile", type=int, default=0, help="tile side in px (default: 32 for config 3, 16 otherwise)")
+    ap.add_argument("--tile", type=int, default=0, help="tile side in px (default: tile_for(config, mode))")
     args = ap.parse_args()
     if args.cpu_sample is None:
         args.cpu_sample = default_cpu_sample(args.config)

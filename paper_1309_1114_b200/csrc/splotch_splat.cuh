@@ -43,7 +43,7 @@ template <int T> struct Splat2Cfg {
     static constexpr size_t kStageBytes = 16u * kWinUnits;
     static constexpr int kMinBlocks = T == 8 ? 12 : (T == 16 ? 6 : (T == 32 ? 2 : 1));     // T = 32: two 17-warp CTAs per SM need <= 60 registers
     static constexpr size_t kSmemBytes = kStageBytes * kSplatStages + sizeof(unsigned int) * (6 * kPix + 2 * kMaxRec) +
-                                         sizeof(unsigned short) * kMaxRec * Base::kWarps + sizeof(SplatWin) * kSplatStages + 16 * kSplatStages;
+                                         sizeof(unsigned short) * kMaxRec * Base::kWarps * 2 + sizeof(SplatWin) * kSplatStages + 16 * kSplatStages;
 };
 
 __device__ __forceinline__ unsigned int smem_u32(const void *p) { return (unsigned int)__cvta_generic_to_shared(p); }
@@ -117,11 +117,12 @@ k_splat(const float4 *__restrict__ records, const unsigned int *__restrict__ vst
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float4 *stage = reinterpret_cast<float4 *>(smem_raw);                                        // [kSplatStages][kSplatWinUnits]
     unsigned int *fb = reinterpret_cast<unsigned int *>(stage + kSplatStages * kSplatWinUnits);  // lo R G B, hi R G B
-    unsigned int *stM = fb + 6 * kPix;                                                           // [2][kMaxRec] strip masks
-    unsigned short *hits = reinterpret_cast<unsigned short *>(stM + 2 * kMaxRec);                // [warps][kMaxRec] per-warp hit lists
-    SplatWin *wins = reinterpret_cast<SplatWin *>(hits + kMaxRec * Geo::kWarps);
+    unsigned int *stM = fb + 6 * kPix;                                                           // [2][warps] lengths of the hit lists (room for 2 kMaxRec words)
+    unsigned short *hits = reinterpret_cast<unsigned short *>(stM + 2 * kMaxRec);                // [2][warps][kMaxRec] per-strip hit lists, double buffered
+    SplatWin *wins = reinterpret_cast<SplatWin *>(hits + 2 * kMaxRec * Geo::kWarps);
     unsigned long long *full = reinterpret_cast<unsigned long long *>(wins + kSplatStages), *empty = full + kSplatStages;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x < 2 * Geo::kWarps) stM[threadIdx.x] = 0u;
     if (threadIdx.x == 0) {
         for (int s = 0; s < kSplatStages; ++s) { mbar_init(smem_u32(full + s), 1u); mbar_init(smem_u32(empty + s), Geo::kWarps); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -208,7 +209,6 @@ k_splat(const float4 *__restrict__ records, const unsigned int *__restrict__ vst
     constexpr int kLPR = Geo::kSW / (2 * kNP);          // lanes per strip row
     const int sx = warp % Geo::kStripsX, sy = warp / Geo::kStripsX;
     const int lx = sx * Geo::kSW + 2 * kNP * (lane % kLPR), ly = sy * Geo::kSH + lane / kLPR;
-    const unsigned int my_strip = (1u << (16 + sx)) | (1u << sy);
     const int e = fixed_exponent(stats->amax_bits);
     const float sc1 = pow2i(e / 2), sc2 = pow2i(e - e / 2);
     auto cbar = [&]() { asm volatile("bar.sync 1, %0;" :: "n"(kConsumers) : "memory"); };
@@ -279,11 +279,14 @@ k_splat(const float4 *__restrict__ records, const unsigned int *__restrict__ vst
             }
             // ---- MEDIUM records.  Decode: direct splat of boxes up to 2 x 2, strip masks for the others
             const float4 *recs = win + off;
-            unsigned int *mask = stM + (nsubs & 1u) * kMaxRec;
+            // the decoding thread appends the record to the hit list of every strip its box touches (one shared-memory atomic per strip:
+            // every warp scanning a mask word per record cost 16 scans per record with 32-px tiles).  Lists and lengths are double
+            // buffered: a warp that is done with this sub-range decodes the next one while others still evaluate this one
+            unsigned int *cnts = stM + (nsubs & 1u) * Geo::kWarps;
+            unsigned short *lists = hits + (nsubs & 1u) * (kMaxRec * Geo::kWarps);
             ++nsubs;
-            for (unsigned int i = threadIdx.x; i < ((cnt + 31u) & ~31u); i += kConsumers) {
-                unsigned int touch = 0u;
-                if (i < cnt) {
+            for (unsigned int i = threadIdx.x; i < cnt; i += kConsumers) {
+                {
                     const float4 ra = recs[2 * i], rb = recs[2 * i + 1];
                     const unsigned int box = __float_as_uint(rb.w);
                     const int bx0 = (int)(box & 63u), by0 = (int)((box >> 6) & 63u);
@@ -308,29 +311,21 @@ k_splat(const float4 *__restrict__ records, const unsigned int *__restrict__ vst
                             }
                         }
                     } else {
-                        const int x1 = bx0 + bw1, y1 = by0 + bh1;
-                        const unsigned int xm = (2u << (x1 / Geo::kSW)) - (1u << (bx0 / Geo::kSW));
-                        const unsigned int ym = (2u << (y1 / Geo::kSH)) - (1u << (by0 / Geo::kSH));
-                        touch = (xm << 16) | ym;
+                        const int sx0 = bx0 / Geo::kSW, sx1 = (bx0 + bw1) / Geo::kSW, sy0 = by0 / Geo::kSH, sy1 = (by0 + bh1) / Geo::kSH;
+                        for (int yy = sy0; yy <= sy1; ++yy)
+                            for (int xx = sx0; xx <= sx1; ++xx) {
+                                const int wq = yy * Geo::kStripsX + xx;
+                                lists[wq * kMaxRec + atomicAdd(&cnts[wq], 1u)] = (unsigned short)i;
+                            }
                     }
                 }
-                mask[i] = touch;
             }
-            cbar();                                  // masks visible; every warp is done with the sub-range before the previous one
+            cbar();                                  // lists visible; every warp is done with the sub-range before the previous one
             // ---- pixel owners: every warp compacts the records that touch its strip into its hit list (the paper's "one
             //      pixel per thread, particles in sequence", :226, with a warp strip and a box test in front), then evaluates
             //      them two at a time: the two dependent chains (LDS -> d2 -> ex2 -> FFMA2) interleave
-            unsigned short *hl = hits + warp * kMaxRec;
-            unsigned int nh = 0u;
-#pragma unroll 1
-            for (unsigned int g = 0; g < cnt; g += 32) {
-                const unsigned int t = mask[g + lane];
-                const bool hit = (t & my_strip & 0xffff0000u) && (t & my_strip & 0xffffu);
-                const unsigned int m = __ballot_sync(0xffffffffu, hit);
-                if (hit) hl[nh + __popc(m & ((1u << lane) - 1u))] = (unsigned short)(g + lane);
-                nh += __popc(m);
-            }
-            __syncwarp();
+            const unsigned short *hl = lists + warp * kMaxRec;
+            const unsigned int nh = cnts[warp];
             auto eval = [&](unsigned int r) {
                 const float4 A = recs[2 * r], B = recs[2 * r + 1];
                 const float dyf = __fsub_rn(fy, A.y);
@@ -357,7 +352,8 @@ k_splat(const float4 *__restrict__ records, const unsigned int *__restrict__ vst
                 eval(pr.x & 0xffffu); eval(pr.x >> 16); eval(pr.y & 0xffffu); eval(pr.y >> 16);
             }
             for (; j < nh; ++j) eval(hl[j]);
-            __syncwarp();                            // the list is rewritten in the next sub-range
+            __syncwarp();
+            if (lane == 0) cnts[warp] = 0u;          // this buffer is filled again in the sub-range after next
             since += cnt;
             if (since >= 1024u) {                    // two-level sums: float32 stays accurate to ~1e-6
                 since = 0u;
