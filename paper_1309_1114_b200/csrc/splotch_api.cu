@@ -916,8 +916,15 @@ int splotch_render_host(splotch_ctx *c, const splotch_particles *hp, uint64_t n,
     }
     CU_TRY(c, cudaEventRecord(c->ev_start, st));                 // the staging buffers are free once earlier work on `st` is done
     CU_TRY(c, cudaStreamWaitEvent(c->copy_stream, c->ev_start, 0));
-    for (unsigned long long k = 0; k < nchunks; ++k) {
-        const unsigned long long lo = k * ch, len = n ? (lo + ch < n ? ch : n - lo) : 0;
+    // The chunks ramp up (an eighth, a quarter, half a chunk, then whole chunks): the kernels cannot start before the first chunk has
+    // arrived, and a chunk's kernels take longer than the next chunk's copy as long as that one is not more than about 1.5 times larger
+    unsigned long long lo_next = 0, k = 0;
+    for (; k == 0 || lo_next < n; ++k) {
+        unsigned long long want = ch;
+        if (n > ch && k < 3) { want = (ch >> (3 - k)); want = want < (1ull << 20) ? (1ull << 20) : want; want = (want + 3) / 4 * 4; if (want > ch) want = ch; }
+        const unsigned long long lo = lo_next, len = n ? (lo + want < n ? want : n - lo) : 0;
+        lo_next = lo + len;
+        const bool last = lo_next >= n;
         const int b = (int)(k & 1);
         float *dst[kHostFields];
         if (k >= 2) CU_TRY(c, cudaStreamWaitEvent(c->copy_stream, c->ev_consumed[b], 0));
@@ -929,7 +936,7 @@ int splotch_render_host(splotch_ctx *c, const splotch_particles *hp, uint64_t n,
         CU_TRY(c, cudaStreamWaitEvent(st, c->ev_copied[b], 0));
         const splotch_particles dp = device_view(dst);
         const FrameParams fc = chunk_params(lo, len, dst);
-        rc = render_device(c, &dp, len, fc, L, dimg, ws, st, ChunkCtl{k == 0, k + 1 == nchunks, nchunks > 1});
+        rc = render_device(c, &dp, len, fc, L, dimg, ws, st, ChunkCtl{k == 0, last, nchunks > 1});
         if (rc != SPLOTCH_OK) return rc;
         CU_TRY(c, cudaEventRecord(c->ev_consumed[b], st));
     }
