@@ -125,13 +125,18 @@ def test_cfg2_reduced_two_species():
     assert st["count"][wl_SMALL] > 0 and st["count"][wl_MEDIUM] > 0
 
 
-@pytest.mark.parametrize("tile,r_large", [(16, 12.0), (32, 24.0), (16, 64.0)])
+@pytest.mark.parametrize("tile,r_large", [(16, 12.0), (32, 24.0), (16, 64.0), (32, 64.0), (32, 200.0)])
 def test_cfg3_reduced_large_particles(tile, r_large):
+    """(32, 64) and (32, 200): with 32-px tiles the MEDIUM discs wider than 32 px sit in the third bin of their tiles and are rendered
+    by k_large (whole image against the oracle, per-tile counts bit-exact as everywhere)."""
     w = wl.make_config(3, n=150_000, size=(512, 384))
     w.r_large = r_large
     st, g = full_check(w, tile)
-    assert st["count"][wl_LARGE] > 1000
+    assert st["count"][wl_LARGE] > (1000 if r_large < 100 else 0)
     assert st["large_pairs"] >= st["count"][wl_LARGE]
+    if tile == 32 and r_large > 32.0:
+        wide = int(((g["cls"] == wl_MEDIUM) & (g["rp"] > 32.0)).sum())
+        assert wide > 1000, wide
 
 
 def test_large_particles_with_8px_tiles_and_a_disc_covering_the_image():
