@@ -527,6 +527,7 @@ constexpr int kOChunkMax = 4096;               // records per chunk: a warp comp
 
 template <int T> struct ORenderSmem {
     float4 map[kORWarps][T * T];
+    unsigned int owner[kORWarps][T * T];       // per pixel: the lowest lane that wants it in the current round (0xffffffff: free)
     float4 recA[kORWarps][32], recB[kORWarps][32];
     uint4 box[kORWarps][32];                   // {x0 | y0 << 8 | (width - 1) << 16 | (height - 1) << 24 (tile-relative), first fragment, 65536 / width rounded up, -}
     unsigned int chunk;
@@ -582,7 +583,7 @@ k_orender(const float4 *__restrict__ rec, const unsigned int *__restrict__ vals0
             // this warp's quarter of the segment, in whole batches of 32 records
             const unsigned int nb = (end - begin + 31u) / 32u, per = (nb + kORWarps - 1u) / kORWarps;
             const unsigned int wb = min(end, begin + 32u * per * (unsigned int)warp), we = min(end, wb + 32u * per);
-            for (int i = lane; i < kPix; i += 32) map[i] = make_float4(1.0f, 0.0f, 0.0f, 0.0f);
+            for (int i = lane; i < kPix; i += 32) { map[i] = make_float4(1.0f, 0.0f, 0.0f, 0.0f); S.owner[warp][i] = 0xffffffffu; }
             __syncwarp();
             // the records of a batch are gathered through the sorted values; the next batch's records and the following batch's
             // values are requested before the current batch is composed
@@ -669,22 +670,23 @@ k_orender(const float4 *__restrict__ rec, const unsigned int *__restrict__ vals0
                     e = emit_only ? 1.0f : e;
                     const float gr = B.x * ga, gg = B.y * ga, gb = B.z * ga;
                     const int pix = ly * T + lx;
-                    // lanes whose fragments fall on the same pixel, from one vote per bit of the pixel index (match.any takes about
-                    // 64 cycles per warp on sm_100a and was 37 % of the kernel's stall samples; votes run at full rate)
-                    unsigned int peers = __ballot_sync(0xffffffffu, act);
-#pragma unroll
-                    for (int bit = 0; (1 << bit) < kPix; ++bit) {
-                        const bool one = (pix >> bit) & 1;
-                        const unsigned int v = __ballot_sync(0xffffffffu, one);
-                        peers &= one ? v : ~v;
-                    }
-                    const unsigned int rank = (unsigned int)__popc(peers & lt);
-                    const unsigned int rounds = __reduce_max_sync(0xffffffffu, act ? rank : 0u);
-                    for (unsigned int r = 0u; r <= rounds; ++r) {
-                        if (act && rank == r) {
+                    // Fragments of this step that fall on the same pixel are applied in rounds, lower lane (earlier record) first: every
+                    // pending lane bids for its pixel with a shared-memory atomicMin of its lane number, the winners apply and free the
+                    // pixel.  (First version: match.any, 37 % of the stall samples; second: one vote per bit of the pixel index, 25
+                    // instructions per step; a round of bids costs about 10 and most steps need one.)
+                    unsigned int *own = S.owner[warp];
+                    bool pending = act;
+                    while (__any_sync(0xffffffffu, pending)) {
+                        if (pending) atomicMin(own + pix, (unsigned int)lane);
+                        __syncwarp();
+                        const bool win = pending && own[pix] == (unsigned int)lane;
+                        __syncwarp();
+                        if (win) {
                             float4 m = map[pix];
                             m.x *= e; m.y = fmaf(m.y, e, gr); m.z = fmaf(m.z, e, gg); m.w = fmaf(m.w, e, gb);
                             map[pix] = m;
+                            own[pix] = 0xffffffffu;
+                            pending = false;
                         }
                         __syncwarp();
                     }
