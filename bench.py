@@ -134,12 +134,16 @@ def ncu_traffic(kernel: str, workload: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed ncu --set full capture
     (profiles/dram_traffic.csv: kernel,workload,bytes), or None."""
     path = os.path.join(ROOT, "profiles", "dram_traffic.csv")
-    best = None
+    best, src = None, None
     if os.path.exists(path):
         for line in open(path).read().splitlines()[1:]:
             parts = line.split(",")
-            if len(parts) >= 3 and parts[0] == kernel and parts[1] == workload:
-                best = float(parts[2])                # the last row for a (kernel, workload) is the newest capture
+            if len(parts) >= 4 and parts[0] == kernel and parts[1] == workload:
+                # the newest capture (last source file) counts; a kernel launched several times per frame (radix passes, some of
+                # which return at once) has several rows there: the largest is the full launch
+                if parts[3] != src:
+                    best, src = None, parts[3]
+                best = float(parts[2]) if best is None else max(best, float(parts[2]))
     return best
 
 
