@@ -201,6 +201,20 @@ int splotch_debug_geometry(splotch_ctx *ctx, const splotch_particles *particles,
 /* Per-tile pair counts of the last frame: DEVICE out, nty x ntx uint32 (SMALL + MEDIUM; ordered mode: all). */
 int splotch_debug_tile_counts(splotch_ctx *ctx, uint32_t *out, void *cuda_stream);
 
+/* The image of a particle-sharded frame ("chunks of particles among different processors, each ... producing a
+ * partial rendering, the root processor composing final renderings") from the shards' workspaces, in ONE kernel: every shard
+ * was rendered with splotch_render (additive mode, same image size and tile) into its own workspace, which then holds the tiles'
+ * exact 64-bit fixed-point sums; this call adds them per pixel (in double precision: the result does not depend on the order of
+ * the shards) and writes tiles [tile_begin, tile_end) of the image (tile_end < 0: all tiles), with the transfer 1 - exp(-S)
+ * when apply_transfer != 0.  It replaces the float32 partial images and their all-reduce.
+ *   workspaces : HOST array of n_shards (<= 16) DEVICE pointers, the workspaces the shards were rendered into, untouched since.
+ *                They may be peer-mapped memory of other GPUs (peer access enabled by the caller): the loads then cross
+ *                NVLink and a rank can compose its own share of the tiles.
+ *   image_out  : DEVICE, height x width x 3 float32 of this context's image size; only the tiles of the range are written.
+ * A shard whose frame overflowed its pair capacity makes the composed tiles zero.  Asynchronous on `cuda_stream`. */
+int splotch_compose_shards(splotch_ctx *ctx, const void *const *workspaces, int n_shards, int tile, int tile_begin,
+                           int tile_end, int apply_transfer, float *image_out, void *cuda_stream);
+
 /* Classes and per-tile pair counts of a particle set (steps A1, A3, A4a: PAPER.md:76, :138, :156-173 and the counting half
  * of :175) for callers that cannot allocate: the call makes NO allocation (no cudaMalloc / cudaFree, no allocating library
  * routine) and takes no workspace.  Its scratch, the count matrix, is a file-scope device array of 16 MiB inside the library

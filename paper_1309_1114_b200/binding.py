@@ -10,7 +10,7 @@ from __future__ import annotations
 
 import ctypes as C
 import os
-from typing import Dict, Optional, Sequence
+from typing import Dict, Optional, Sequence, Tuple
 
 import torch
 
@@ -26,7 +26,7 @@ EXPORTS = (
     "splotch_set_colormap", "splotch_set_profiling", "splotch_workspace_bytes", "splotch_render",
     "splotch_render_host", "splotch_get_stats", "splotch_stage_name", "splotch_debug_geometry",
     "splotch_debug_tile_counts", "splotch_last_error", "splotch_version", "splotch_measure_peaks", "splotch_set_host_chunk", "splotch_apply_transfer",
-    "splotch_count_static",
+    "splotch_count_static", "splotch_compose_shards",
 )
 
 
@@ -89,6 +89,7 @@ def load() -> C.CDLL:
     lib.splotch_stage_name.restype = C.c_char_p
     lib.splotch_debug_geometry.argtypes = [vp, C.POINTER(SplotchParticles), u64, C.POINTER(SplotchParams)] + [vp] * 10
     lib.splotch_debug_tile_counts.argtypes = [vp, vp, vp]
+    lib.splotch_compose_shards.argtypes = [vp, C.POINTER(vp), i32, i32, i32, i32, i32, vp, vp]
     lib.splotch_count_static.argtypes = [vp, C.POINTER(SplotchParticles), u64, C.POINTER(SplotchParams), vp, vp, vp]
     lib.splotch_measure_peaks.argtypes = [vp, C.POINTER(C.c_double), vp]
     lib.splotch_set_host_chunk.argtypes = [vp, u64]
@@ -292,6 +293,23 @@ class Renderer:
                                                       ("cls", "px", "py", "sp", "rp", "zc", "pbox", "tbox", "ilabel")],
             stream))
         return out
+
+    def compose_shards(self, workspaces: Sequence[torch.Tensor], tile: int, image: Optional[torch.Tensor] = None,
+                       tile_range: Tuple[int, int] = (0, -1), apply_transfer: bool = False) -> torch.Tensor:
+        """splotch_compose_shards: the image of a particle-sharded frame from the shards' workspaces (exact sum of their
+        fixed-point tile sums), tiles tile_range of it."""
+        if image is None:
+            image = torch.zeros((self.height, self.width, 3), dtype=torch.float32, device=f"cuda:{self.device}")
+        ptrs = (C.c_void_p * len(workspaces))(*[w.data_ptr() for w in workspaces])
+        stream = torch.cuda.current_stream(self.device).cuda_stream
+        _check(self.ctx, self.lib.splotch_compose_shards(self.ctx, ptrs, len(workspaces), tile, tile_range[0], tile_range[1],
+                                                         1 if apply_transfer else 0, image.data_ptr(), stream))
+        return image
+
+    @property
+    def last_workspace(self) -> Optional[torch.Tensor]:
+        """The workspace of the last frame (holds the tiles' fixed-point sums until the next frame)."""
+        return self._ws
 
     def count_static(self, fields: Dict[str, torch.Tensor], species: Sequence, tile_counts: torch.Tensor,
                      class_counts: torch.Tensor, **params) -> None:

@@ -993,6 +993,42 @@ int splotch_apply_transfer(splotch_ctx *c, float *image, void *cuda_stream)
     return SPLOTCH_OK;
 }
 
+int splotch_compose_shards(splotch_ctx *c, const void *const *workspaces, int n_shards, int tile, int tile_begin, int tile_end,
+                           int apply_transfer, float *image_out, void *cuda_stream)
+{
+    if (!c || !workspaces || !image_out) return SPLOTCH_EINVAL;
+    if (n_shards < 1 || n_shards > kMaxShards) return fail(c, SPLOTCH_EINVAL, "n_shards must be 1..%d", kMaxShards);
+    const int ts = tile_shift(tile);
+    if (ts < 0) return fail(c, SPLOTCH_EINVAL, "tile must be 8, 16, 32 or 64 (got %d)", tile);
+    // the offsets of the sums and of the statistics inside a workspace depend on the image size, the tile side and the SM count only
+    Layout L;
+    if (!make_layout(c, 0, tile, 1, 0, false, &L)) return fail(c, SPLOTCH_EINVAL, "no layout for this image and tile");
+    FrameParams fp;
+    memset(&fp, 0, sizeof fp);
+    fp.W = c->width; fp.H = c->height; fp.T = tile; fp.tshift = ts;
+    fp.ntx = (c->width + tile - 1) / tile; fp.nty = (c->height + tile - 1) / tile; fp.n_tiles = fp.ntx * fp.nty;
+    if (tile_end < 0) tile_end = fp.n_tiles;
+    if (tile_begin < 0 || tile_begin > tile_end || tile_end > fp.n_tiles) return fail(c, SPLOTCH_EINVAL, "bad tile range [%d, %d) of %d", tile_begin, tile_end, fp.n_tiles);
+    ShardPtrs sh;
+    memset(&sh, 0, sizeof sh);
+    sh.n = n_shards;
+    for (int k = 0; k < n_shards; ++k) {
+        if (!workspaces[k] || ((uintptr_t)workspaces[k] & 255u)) return fail(c, SPLOTCH_EINVAL, "workspace %d is null or not 256-byte aligned", k);
+        sh.accum[k] = (const unsigned long long *)((const char *)workspaces[k] + L.accum);
+        sh.stats[k] = (const DeviceStats *)((const char *)workspaces[k] + L.stats);
+    }
+    if (tile_end == tile_begin) return SPLOTCH_OK;
+    CU_TRY(c, cudaSetDevice(c->device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int grid = tile_end - tile_begin;
+    if (tile == 8) k_compose_shards<8><<<grid, 256, 0, st>>>(sh, fp, tile_begin, apply_transfer, image_out);
+    else if (tile == 16) k_compose_shards<16><<<grid, 256, 0, st>>>(sh, fp, tile_begin, apply_transfer, image_out);
+    else if (tile == 32) k_compose_shards<32><<<grid, 256, 0, st>>>(sh, fp, tile_begin, apply_transfer, image_out);
+    else k_compose_shards<64><<<grid, 256, 0, st>>>(sh, fp, tile_begin, apply_transfer, image_out);
+    CU_TRY(c, cudaGetLastError());
+    return SPLOTCH_OK;
+}
+
 int splotch_measure_peaks(splotch_ctx *c, double out[2], void *cuda_stream)
 {
     if (!c || !out) return SPLOTCH_EINVAL;

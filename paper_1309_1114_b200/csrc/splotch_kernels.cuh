@@ -1002,6 +1002,53 @@ k_compose(const unsigned long long *__restrict__ accum, const DeviceStats *__res
     }
 }
 
+// ---- A8 for a particle-sharded frame: the shards' fixed-point tile sums -> the image, in one kernel ------------------------------
+// Every shard (a GPU of a multi-GPU frame, or a part of the set rendered into its own workspace) leaves exact
+// 64-bit sums in units of its own 2^-e.  The sum over the shards is taken per pixel in double precision (integers times powers of
+// two: exact up to 2^53 units), so the result does not depend on the order of the shards; the pointers may be peer-mapped device
+// memory of other GPUs (loads over NVLink), which fuses the image reduction of the sharded frame into the epilogue: no float
+// partial images, no separate all-reduce.  Tiles [tile0, tile1): a rank may compose its share of the image only.
+constexpr int kMaxShards = 16;
+struct ShardPtrs {
+    const unsigned long long *accum[kMaxShards];
+    const DeviceStats *stats[kMaxShards];
+    int n;
+};
+
+template <int T>
+__global__ void __launch_bounds__(256)
+k_compose_shards(const __grid_constant__ ShardPtrs sh, const __grid_constant__ FrameParams fp, int tile0, int apply_transfer,
+                 float *__restrict__ image)
+{
+    constexpr int kPix = T * T;
+    __shared__ double s_unit[kMaxShards];
+    __shared__ int s_ok;
+    if (threadIdx.x == 0) {
+        int ok = 1;
+        for (int k = 0; k < sh.n; ++k) {
+            ok &= sh.stats[k]->f_overflow == 0u;
+            s_unit[k] = ldexp(1.0, -fixed_exponent(sh.stats[k]->amax_bits));
+        }
+        s_ok = ok;
+    }
+    __syncthreads();
+    const int tile = tile0 + blockIdx.x;
+    const int tx0 = (tile % fp.ntx) * T, ty0 = (tile / fp.ntx) * T;
+    for (int p = threadIdx.x; p < kPix; p += 256) {
+        const int ix = tx0 + p % T, iy = ty0 + p / T;
+        if (ix < fp.W && iy < fp.H) {
+            float *o = image + 3ull * ((size_t)iy * fp.W + ix);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                double v = 0.0;
+                for (int k = 0; k < sh.n; ++k) v += (double)(long long)__ldg(sh.accum[k] + (size_t)tile * (3 * kPix) + c * kPix + p) * s_unit[k];
+                const float f = s_ok ? (float)v : 0.0f;
+                o[c] = apply_transfer ? -expm1f(-f) : f;
+            }
+        }
+    }
+}
+
 // ---- 1 - exp(-S) on a finished image: the transfer of a frame whose partial images were summed elsewhere (multi-GPU) ----
 __global__ void __launch_bounds__(256)
 k_apply_transfer(float *__restrict__ image, size_t n)
