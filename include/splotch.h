@@ -171,7 +171,7 @@ int splotch_render_host(splotch_ctx *ctx, const splotch_particles *host_particle
                         const splotch_params *params, float *host_image_out,
                         void *workspace, size_t workspace_bytes, void *cuda_stream);
 
-/* Particles per chunk of splotch_render_host (additive mode).  0 (the default) picks about eight chunks of 2^20 ..
+/* Particles per chunk of splotch_render_host (additive mode).  0 (the default) picks about four chunks of 2^20 ..
  * 2^27 particles.  The staging buffers of the workspace are sized for this value: set it before asking
  * splotch_workspace_bytes. */
 int splotch_set_host_chunk(splotch_ctx *ctx, uint64_t particles_per_chunk);

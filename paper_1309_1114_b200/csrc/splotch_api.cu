@@ -180,12 +180,12 @@ int bin_rows(const splotch_ctx *c, int T)
 
 constexpr int kHostFields = 9;
 
-// Particles per chunk of a chunked host frame: about eight chunks, between 2^20 and 2^27 particles, a multiple of 4
+// Particles per chunk of a chunked host frame: about four chunks, between 2^20 and 2^27 particles, a multiple of 4
 unsigned long long host_chunk_particles(const splotch_ctx *c, unsigned long long n)
 {
     unsigned long long ch = c->host_chunk;
     if (ch == 0) {
-        ch = (n + 7) / 8;
+        ch = (n + 3) / 4;
         if (ch < (1ull << 20)) ch = 1ull << 20;
         if (ch > (1ull << 27)) ch = 1ull << 27;
     }
